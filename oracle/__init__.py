@@ -1,0 +1,155 @@
+"""CPU ORACLE -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+
+ctypes front-end of ``oracle/tm_oracle.c`` (plain C, double precision, full
+lattice; see that file's header for the passages it follows and its pins).
+Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline``
+/ ``--impl reference`` legs may import this package.  It imports nothing from
+``paper_1401_6750_b200`` (the CUDA path) and the CUDA path never imports it.
+
+All arrays are numpy complex128, C-contiguous, in the canonical shapes of
+``paper_1401_6750_b200/inputs.py``:
+  spinor [T,Lz,Ly,Lx,4,3], gauge [T,Lz,Ly,Lx,4,3,3]; dims = (Lx,Ly,Lz,T).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "tm_oracle.c")
+_LIB = os.path.join(_HERE, "liboracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile tm_oracle.c -> liboracle.so with gcc (OpenMP over sites)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        subprocess.check_call(
+            ["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-std=c11", "-o", _LIB, _SRC, "-lm"])
+    return _LIB
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = ctypes.CDLL(build())
+        _lib.orc_true_residual.restype = ctypes.c_double
+        _lib.orc_solve.restype = ctypes.c_int
+    return _lib
+
+
+def _c(a):
+    a = np.ascontiguousarray(a, dtype=np.complex128)
+    return a, a.ctypes.data_as(ctypes.c_void_p)
+
+
+def _dims(dims):
+    return (ctypes.c_int * 4)(*[int(d) for d in dims])
+
+
+def dims_of(field) -> tuple:
+    lt, lz, ly, lx = field.shape[:4]
+    return (lx, ly, lz, lt)
+
+
+def gamma(mu: int) -> np.ndarray:
+    """gamma_mu (mu = 0..3 = x,y,z,t; 4 = gamma5), 4x4 complex."""
+    out = np.empty((4, 4), dtype=np.complex128)
+    lib().orc_gamma(ctypes.c_int(mu), out.ctypes.data_as(ctypes.c_void_p))
+    return out
+
+
+def Gamma(n: int) -> np.ndarray:
+    """Gamma_n = g_x^b0 g_y^b1 g_z^b2 g_t^b3, n = b0+2b1+4b2+8b3."""
+    out = np.empty((4, 4), dtype=np.complex128)
+    lib().orc_Gamma(ctypes.c_int(n), out.ctypes.data_as(ctypes.c_void_p))
+    return out
+
+
+def apply_M(psi, U, kappa, mu, tb=-1, dagger=False) -> np.ndarray:
+    psi, p_psi = _c(psi)
+    U, p_U = _c(U)
+    out = np.empty_like(psi)
+    lib().orc_apply_M(out.ctypes.data_as(ctypes.c_void_p), p_psi, p_U, _dims(dims_of(psi)),
+                      ctypes.c_int(tb), ctypes.c_double(kappa), ctypes.c_double(mu),
+                      ctypes.c_int(1 if dagger else 0))
+    return out
+
+
+def solve(eta, U, kappa, mu, rho, tb=-1, max_iter=10000):
+    """Returns (s, iters, true_resid, status); status 0 = converged."""
+    eta, p_eta = _c(eta)
+    U, p_U = _c(U)
+    s = np.empty_like(eta)
+    it = ctypes.c_int(0)
+    tr = ctypes.c_double(0)
+    st = lib().orc_solve(s.ctypes.data_as(ctypes.c_void_p), p_eta, p_U, _dims(dims_of(eta)),
+                         ctypes.c_int(tb), ctypes.c_double(kappa), ctypes.c_double(mu),
+                         ctypes.c_double(rho), ctypes.c_int(max_iter),
+                         ctypes.byref(it), ctypes.byref(tr))
+    return s, it.value, tr.value, st
+
+
+def true_residual(s, eta, U, kappa, mu, tb=-1) -> float:
+    s, p_s = _c(s)
+    eta, p_eta = _c(eta)
+    U, p_U = _c(U)
+    return lib().orc_true_residual(p_s, p_eta, p_U, _dims(dims_of(eta)), ctypes.c_int(tb),
+                                   ctypes.c_double(kappa), ctypes.c_double(mu))
+
+
+def cov_deriv(psi, U, m, tb=-1) -> np.ndarray:
+    psi, p_psi = _c(psi)
+    U, p_U = _c(U)
+    out = np.empty_like(psi)
+    lib().orc_cov_deriv(out.ctypes.data_as(ctypes.c_void_p), p_psi, p_U, _dims(dims_of(psi)),
+                        ctypes.c_int(tb), ctypes.c_int(m))
+    return out
+
+
+def loops_sites(s, eta, U, kappa, mu, sites=None, tb=-1) -> np.ndarray:
+    """Per-site 160 insertions, [nsites, 2, 80]; sites = flat lexicographic indices (None = all)."""
+    s, p_s = _c(s)
+    eta, p_eta = _c(eta)
+    U, p_U = _c(U)
+    V = int(np.prod(s.shape[:4]))
+    if sites is None:
+        sites = np.arange(V)
+    sites = np.ascontiguousarray(sites, dtype=np.int64)
+    out = np.empty((len(sites), 2, 80), dtype=np.complex128)
+    lib().orc_loops_sites(out.ctypes.data_as(ctypes.c_void_p), p_s, p_eta, p_U, _dims(dims_of(s)),
+                          ctypes.c_int(tb), ctypes.c_double(kappa), ctypes.c_double(mu),
+                          sites.ctypes.data_as(ctypes.c_void_p), ctypes.c_long(len(sites)))
+    return out
+
+
+def loops_project(s, eta, U, kappa, mu, momenta, tb=-1, t0=0, t1=None) -> np.ndarray:
+    """Momentum-projected loops [2, 80, nmom, T] (timeslices outside [t0,t1) are zero)."""
+    s, p_s = _c(s)
+    eta, p_eta = _c(eta)
+    U, p_U = _c(U)
+    T = s.shape[0]
+    if t1 is None:
+        t1 = T
+    mom = np.ascontiguousarray(momenta, dtype=np.int32).reshape(-1, 3)
+    out = np.zeros((2, 80, len(mom), T), dtype=np.complex128)
+    lib().orc_loops_project(out.ctypes.data_as(ctypes.c_void_p), p_s, p_eta, p_U,
+                            _dims(dims_of(s)), ctypes.c_int(tb), ctypes.c_double(kappa),
+                            ctypes.c_double(mu), mom.ctypes.data_as(ctypes.c_void_p),
+                            ctypes.c_int(len(mom)), ctypes.c_int(t0), ctypes.c_int(t1))
+    return out
+
+
+def tsm_combine(lp, hp) -> np.ndarray:
+    """lp: [n_lp, ...], hp: [n_hp, ...] (HP sources = the first n_hp LP sources)."""
+    lp, p_lp = _c(lp)
+    hp, p_hp = _c(hp)
+    n_lp, n_hp = lp.shape[0], hp.shape[0]
+    out = np.empty(lp.shape[1:], dtype=np.complex128)
+    ln = int(np.prod(lp.shape[1:]))
+    lib().orc_tsm_combine(out.ctypes.data_as(ctypes.c_void_p), p_lp, ctypes.c_int(n_lp), p_hp,
+                          ctypes.c_int(n_hp), ctypes.c_long(ln))
+    return out
