@@ -1,0 +1,131 @@
+/* tmloops.h -- C ABI of the B200-native Truncated-Solver-Method loop estimator.
+ *
+ * One shared library (libtmloops.so, sm_100a) implementing the data-parallel hot path of
+ * arXiv:1401.6750 ("A QUDA-branch to compute disconnected diagrams in GPUs"):
+ *   eq. 2.1     M |s_r> = |eta_r>                          -> tm_cg_solve
+ *   sec 2.1  Truncated Solver Method, N_LP + N_HP        -> tsm_estimate
+ *   sec 2.1.1     one-end trick, 160 insertions, p^2 <= 9     -> loop_contract_project
+ *   sec 2.2  colour-traced contraction, covariant derivative, time-slice array
+ *   [B:ns] = BASELINE.json north_star: the operator
+ *     M = (1 + 2 i kappa mu gamma5 tau3) - kappa sum_mu [(1-gamma_mu) U_mu(x) d_{x+mu,y}
+ *                                                      + (1+gamma_mu) U_mu^dag(x-mu) d_{x-mu,y}]  -> tm_dslash
+ *
+ * No CUDA or torch types: device pointers are plain void* ("d_" prefix = device memory,
+ * "h_" = host memory), streams are void* holding a cudaStream_t (NULL = default stream).
+ *
+ * Conventions: dims = {Lx,Ly,Lz,T}, all even; canonical site index
+ * ((t*Lz+z)*Ly+y)*Lx+x; directions mu = 0..3 = x,y,z,t; parity = (x+y+z+t)&1;
+ * canonical spinor  complex128 [V][4 spin][3 colour]; canonical gauge complex128 [V][4 mu][3][3];
+ * Hermitian chiral gamma basis, gamma5 = diag(1,1,-1,-1); periodic in space,
+ * psi(t+T) = t_boundary * psi(t).  tau3 -> +1; pass mu < 0 for the other flavour.
+ *
+ * Internal fields (what tm_dslash works on, so a timed loop holds nothing but the kernel):
+ * per parity, [24/CV chunks][V/2 sites] vectors of 16 bytes (CV = 2/4/8 reals for
+ * f64/f32/16-bit); a full-lattice internal field is the even block followed by the odd block.
+ * Use tm_field_bytes / tm_field_import / tm_field_export; never index them by hand.
+ *
+ * Ownership: the caller owns every field / output buffer and the stream.  The context owns
+ * its private gauge copies (one per precision x reconstruct actually used, built lazily from
+ * the fp64 master) and solver workspaces.  Errors: every call returns tm_status; nothing
+ * throws or aborts across the ABI; text of the last error via tm_last_error.  There is NO CPU
+ * fallback: without a CUDA device tm_create fails with TM_ECUDA.
+ * Calls are stream-ordered; those that fill an *_info struct synchronise the stream at the end.
+ */
+#ifndef TMLOOPS_H
+#define TMLOOPS_H
+#include <stddef.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct tm_ctx tm_ctx;
+typedef enum { TM_OK = 0, TM_EARG = 1, TM_EDIM = 2, TM_EPREC = 3, TM_ECUDA = 4, TM_ENOCONV = 5,
+               TM_EALLOC = 6 } tm_status;
+typedef enum { TM_F64 = 0, TM_F32 = 1, TM_F16 = 2, TM_BF16 = 3 } tm_prec;
+typedef enum { TM_R18 = 18, TM_R12 = 12 } tm_recon;
+/* tm_dslash operations ([B:ns] operator; A = 1 + 2 i kappa mu gamma5 is the site-diagonal part,
+ * D the hopping sum, "p" the output parity, "q" the other one):
+ *   TM_OP_HOP        out_p = D_pq in_q
+ *   TM_OP_HOP_TWINV  out_p = A^-1 D_pq in_q
+ *   TM_OP_XPAY       out_p = A x_p - kappa^2 D_pq in_q
+ *   TM_OP_M_FULL     out = M in on the full lattice (in, out: full-lattice internal fields)
+ *   TM_OP_MHAT       out_e = (A - kappa^2 D_eo A^-1 D_oe) in_e   (even-odd Schur complement)
+ * dagger != 0 applies the adjoint (gamma_mu -> -gamma_mu in the projectors, mu -> -mu). */
+typedef enum { TM_OP_HOP = 0, TM_OP_HOP_TWINV = 1, TM_OP_XPAY = 2, TM_OP_M_FULL = 3,
+               TM_OP_MHAT = 4 } tm_op;
+
+/* dims: {Lx,Ly,Lz,T}, each even and >= 2 (TM_EDIM otherwise); t_boundary: +1 | -1;
+ * device: CUDA ordinal.  TM_ECUDA if no usable device. */
+tm_status tm_create(tm_ctx** ctx, const int dims[4], int t_boundary, int device);
+tm_status tm_destroy(tm_ctx* ctx);
+const char* tm_last_error(const tm_ctx* ctx);
+
+/* d_U: device, canonical complex128 [V][4][3][3].  Copied into the context (fp64 master);
+ * previously built reduced-precision copies are dropped. */
+tm_status tm_load_gauge(tm_ctx* ctx, const void* d_U, void* stream);
+
+/* bytes of an internal field of the given storage precision (full_lattice: 0 = one parity). */
+size_t tm_field_bytes(const tm_ctx* ctx, tm_prec prec, int full_lattice);
+/* canonical complex128 full-lattice spinor <-> internal full-lattice field (device, device). */
+tm_status tm_field_import(tm_ctx* ctx, void* d_internal, const void* d_canon, tm_prec prec, void* stream);
+tm_status tm_field_export(tm_ctx* ctx, void* d_canon, const void* d_internal, tm_prec prec, void* stream);
+
+/* One application of the operator pieces above on INTERNAL fields (device).
+ * d_out, d_in: parity fields (full-lattice fields for TM_OP_M_FULL); d_x: parity field, used by
+ * TM_OP_XPAY only (else NULL); out_parity 0 = even, 1 = odd (ignored by M_FULL / MHAT).
+ * d_out must not alias d_in.  Asynchronous on stream. */
+tm_status tm_dslash(tm_ctx* ctx, void* d_out, const void* d_in, const void* d_x, tm_op op,
+                    int out_parity, int dagger, double kappa, double mu, tm_prec prec,
+                    tm_recon recon, void* stream);
+
+/* eq. 2.1: even-odd preconditioned CG on Mhat^dag Mhat (CGLS recurrences, x0 = 0) in `sloppy`
+ * storage with reliable updates in `outer` precision (TM_F32 or TM_F64, >= sloppy).
+ * Stops when the true residual ||eta - M s|| / ||eta|| evaluated in `outer` precision is <= rho.
+ * delta: reliable-update trigger (iterated residual dropped by this factor; <= 0 -> 0.1). */
+typedef struct { tm_prec sloppy, outer; tm_recon recon; double rho; int max_iter; double delta; } tm_solve_params;
+typedef struct { int iters; int reliable_updates; double true_resid; double ms; } tm_solve_info;
+/* d_s (out), d_eta (in): device canonical complex128 full-lattice spinors.
+ * TM_ENOCONV if rho is not reached within max_iter (d_s and info are still filled). */
+tm_status tm_cg_solve(tm_ctx* ctx, void* d_s, const void* d_eta, double kappa, double mu,
+                      const tm_solve_params* params, tm_solve_info* info, void* stream);
+
+/* sec 2.1.1 / 2.2: the 160 insertions of (s, eta), momentum-projected per timeslice:
+ *   d_out[((f*80 + i)*nmom + k)*T + t] = sum_{x,y,z} exp(+2 pi i p_k.x / L) l_{f,i}(x,y,z,t)
+ *   l_{0,n} = s^dag g5 G_n s,  l_{0,16+16m+n} = s^dag g5 G_n D_m s,
+ *   l_{1,n} = s^dag g5 G_n g,  l_{1,16+16m+n} = s^dag g5 G_n D_m g,  g = g5 eta - 2 i kappa mu s,
+ *   G_n = g_x^b0 g_y^b1 g_z^b2 g_t^b3 (n = b0+2b1+4b2+8b3), D_m the symmetric covariant difference.
+ * d_s, d_eta: device canonical complex128; d_out: device complex128 [2][80][nmom][T];
+ * h_momenta: host int [nmom][3] = (px,py,pz); at most 4 distinct |px| values (TM_EARG otherwise);
+ * acc: TM_F64 or TM_F32 (arithmetic and accumulation precision of the site and DFT stages). */
+tm_status loop_contract_project(tm_ctx* ctx, void* d_out, const void* d_s, const void* d_eta,
+                                double kappa, double mu, const int* h_momenta, int nmom,
+                                tm_prec acc, void* stream);
+
+/* sec 2.1: L_TSM = (1/N_LP) sum_{r<N_LP} l_r^LP + (1/N_HP) sum_{r<N_HP} (l_r^HP - l_r^LP);
+ * the HP sources are the first n_hp of the LP sources.  Z4 noise eta_r[c] = i^k, c = (site*4+spin)*3+col:
+ * d_z4 != NULL: packed exponents, byte j of source r holds k[4j+m] in bits 2m..2m+1,
+ *               layout [n_lp][3V] bytes (device);
+ * d_z4 == NULL: generated on the device from `seed` with the counter hash of DESIGN.md
+ *               (k = h(seed, r, c) & 3). */
+typedef struct { int n_lp, n_hp; tm_solve_params lp, hp; double kappa, mu;
+                 const int* h_momenta; int nmom; tm_prec contract_acc_lp, contract_acc_hp;
+                 const unsigned char* d_z4; unsigned long long seed; } tsm_params;
+typedef struct { double ms_total, ms_lp_solve, ms_hp_solve, ms_contract; long iters_lp, iters_hp;
+                 double worst_resid_lp, worst_resid_hp; int launches; } tsm_info;
+/* d_out: device complex128 [2][80][nmom][T]; d_per_source: optional (NULL ok) device complex128
+ * [n_lp + n_hp][2][80][nmom][T] receiving every per-source array (LP first, then HP).
+ * TM_ENOCONV if any solve missed its rho (outputs still filled). */
+tm_status tsm_estimate(tm_ctx* ctx, void* d_out, void* d_per_source, const tsm_params* params,
+                       tsm_info* info, void* stream);
+/* Same with HOST buffers: h_z4 (pinned or pageable host memory, may be NULL -> seed) is copied
+ * to the device source by source and h_out is copied back, all inside the call. */
+tm_status tsm_estimate_host(tm_ctx* ctx, void* h_out, const unsigned char* h_z4,
+                            const tsm_params* params, tsm_info* info, void* stream);
+
+/* number of kernels launched by this context so far (bench.py's gpu_launches) */
+long tm_launch_count(const tm_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,172 @@
+// api.cu -- context lifetime, workspaces and the exported tm_dslash / field conversion calls.
+#include "kernels.h"
+
+static char g_last_error[512] = "";
+
+extern "C" const char* tm_last_error(const tm_ctx* ctx) { return ctx ? ctx->err : g_last_error; }
+extern "C" long tm_launch_count(const tm_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+extern "C" tm_status tm_create(tm_ctx** out, const int dims[4], int t_boundary, int device) {
+    if (!out || !dims) { snprintf(g_last_error, sizeof(g_last_error), "tm_create: null argument"); return TM_EARG; }
+    *out = nullptr;
+    for (int i = 0; i < 4; i++)
+        if (dims[i] < 2 || (dims[i] & 1)) {
+            snprintf(g_last_error, sizeof(g_last_error), "tm_create: extents must be even and >= 2");
+            return TM_EDIM;
+        }
+    if (t_boundary != 1 && t_boundary != -1) {
+        snprintf(g_last_error, sizeof(g_last_error), "tm_create: t_boundary must be +1 or -1");
+        return TM_EARG;
+    }
+    const size_t V = (size_t)dims[0] * dims[1] * dims[2] * dims[3];
+    if (V / 2 > 0x3fffffffULL) { snprintf(g_last_error, sizeof(g_last_error), "tm_create: lattice too large"); return TM_EDIM; }
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev <= 0 || device < 0 || device >= ndev) {
+        snprintf(g_last_error, sizeof(g_last_error), "tm_create: no usable CUDA device %d (%s); there is no CPU fallback",
+                 device, e != cudaSuccess ? cudaGetErrorString(e) : "device count");
+        cudaGetLastError();
+        return TM_ECUDA;
+    }
+    e = cudaSetDevice(device);
+    if (e != cudaSuccess) { snprintf(g_last_error, sizeof(g_last_error), "cudaSetDevice: %s", cudaGetErrorString(e)); return TM_ECUDA; }
+    tm_ctx* c = (tm_ctx*)calloc(1, sizeof(tm_ctx));
+    if (!c) return TM_EALLOC;
+    for (int i = 0; i < 4; i++) c->X[i] = dims[i];
+    c->Xh = dims[0] / 2;
+    c->V = V; c->Vh = V / 2;
+    c->tb = t_boundary;
+    c->device = device;
+    cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
+    bool ok = cudaMalloc((void**)&c->d_partials, sizeof(double) * (1 << 18)) == cudaSuccess
+           && cudaMalloc((void**)&c->d_counter, sizeof(unsigned int) * 4) == cudaSuccess
+           && cudaMalloc((void**)&c->d_scal, sizeof(CgScalars)) == cudaSuccess
+           && cudaMallocHost((void**)&c->h_scal, sizeof(CgScalars)) == cudaSuccess
+           && cudaMemset(c->d_counter, 0, sizeof(unsigned int) * 4) == cudaSuccess
+           && cudaMemset(c->d_scal, 0, sizeof(CgScalars)) == cudaSuccess;
+    for (int i = 0; ok && i < 4; i++) ok = cudaEventCreate(&c->ev[i]) == cudaSuccess;
+    if (!ok) {
+        snprintf(g_last_error, sizeof(g_last_error), "tm_create: device allocation failed: %s", cudaGetErrorString(cudaGetLastError()));
+        tm_destroy(c);
+        return TM_EALLOC;
+    }
+    *out = c;
+    return TM_OK;
+}
+
+static void drop_gauge_copies(tm_ctx* c) {
+    for (int p = 0; p < 4; p++)
+        for (int r = 0; r < 2; r++)
+            if (c->gauge[p][r]) { cudaFree(c->gauge[p][r]); c->gauge[p][r] = nullptr; }
+}
+
+extern "C" tm_status tm_destroy(tm_ctx* c) {
+    if (!c) return TM_OK;
+    cudaSetDevice(c->device);
+    cudaDeviceSynchronize();
+    drop_gauge_copies(c);
+    if (c->d_Ucanon) cudaFree(c->d_Ucanon);
+    if (c->d_partials) cudaFree(c->d_partials);
+    if (c->d_counter) cudaFree(c->d_counter);
+    if (c->d_scal) cudaFree(c->d_scal);
+    if (c->h_scal) cudaFreeHost(c->h_scal);
+    if (c->d_contract_tables) cudaFree(c->d_contract_tables);
+    for (int i = 0; i < TM_MAX_SCRATCH; i++)
+        if (c->scratch[i]) cudaFree(c->scratch[i]);
+    for (int i = 0; i < 4; i++)
+        if (c->ev[i]) cudaEventDestroy(c->ev[i]);
+    cudaGetLastError();
+    free(c);
+    return TM_OK;
+}
+
+tm_status tm_ws(tm_ctx* c, int slot, size_t bytes, void** out) {
+    if (slot < 0 || slot >= TM_MAX_SCRATCH) return tm_fail(c, TM_EARG, "bad workspace slot");
+    if (c->scratch_bytes[slot] < bytes) {
+        if (c->scratch[slot]) {
+            cudaDeviceSynchronize();      // a running kernel may still use the old block
+            cudaFree(c->scratch[slot]);
+            c->scratch[slot] = nullptr; c->scratch_bytes[slot] = 0;
+        }
+        cudaError_t e = cudaMalloc(&c->scratch[slot], bytes);
+        if (e != cudaSuccess) { cudaGetLastError(); c->scratch[slot] = nullptr; return tm_fail(c, TM_EALLOC, "workspace: out of device memory"); }
+        c->scratch_bytes[slot] = bytes;
+    }
+    *out = c->scratch[slot];
+    return TM_OK;
+}
+
+extern "C" tm_status tm_load_gauge(tm_ctx* c, const void* d_U, void* stream) {
+    if (!c || !d_U) return tm_fail(c, TM_EARG, "tm_load_gauge: null argument");
+    cudaStream_t st = (cudaStream_t)stream;
+    TM_CUDA(c, cudaSetDevice(c->device));
+    const size_t bytes = c->V * 4 * 9 * 16;
+    if (!c->d_Ucanon) {
+        cudaError_t e = cudaMalloc(&c->d_Ucanon, bytes);
+        if (e != cudaSuccess) { cudaGetLastError(); c->d_Ucanon = nullptr; return tm_fail(c, TM_EALLOC, "tm_load_gauge: out of device memory"); }
+    }
+    TM_CUDA(c, cudaStreamSynchronize(st));
+    drop_gauge_copies(c);
+    TM_CUDA(c, cudaMemcpyAsync(c->d_Ucanon, d_U, bytes, cudaMemcpyDeviceToDevice, st));
+    return TM_OK;
+}
+
+extern "C" size_t tm_field_bytes(const tm_ctx* c, tm_prec prec, int full_lattice) {
+    if (!c || (int)prec < 0 || (int)prec > 3) return 0;
+    return tm_parity_bytes(c, prec) * (full_lattice ? 2 : 1);
+}
+
+extern "C" tm_status tm_field_import(tm_ctx* c, void* d_internal, const void* d_canon, tm_prec prec, void* stream) {
+    if (!c || !d_internal || !d_canon) return tm_fail(c, TM_EARG, "tm_field_import: null argument");
+    TM_CUDA(c, cudaSetDevice(c->device));
+    return tm_import_launch(c, d_internal, d_canon, prec, (cudaStream_t)stream);
+}
+
+extern "C" tm_status tm_field_export(tm_ctx* c, void* d_canon, const void* d_internal, tm_prec prec, void* stream) {
+    if (!c || !d_internal || !d_canon) return tm_fail(c, TM_EARG, "tm_field_export: null argument");
+    TM_CUDA(c, cudaSetDevice(c->device));
+    return tm_export_launch(c, d_canon, d_internal, prec, (cudaStream_t)stream);
+}
+
+extern "C" tm_status tm_dslash(tm_ctx* c, void* d_out, const void* d_in, const void* d_x, tm_op op,
+                               int out_parity, int dagger, double kappa, double mu, tm_prec prec,
+                               tm_recon recon, void* stream) {
+    if (!c || !d_out || !d_in) return tm_fail(c, TM_EARG, "tm_dslash: null argument");
+    if (d_out == d_in) return tm_fail(c, TM_EARG, "tm_dslash: out must not alias in");
+    if ((int)prec < 0 || (int)prec > 3) return tm_fail(c, TM_EPREC, "tm_dslash: unknown precision");
+    if (recon != TM_R12 && recon != TM_R18) return tm_fail(c, TM_EARG, "tm_dslash: recon must be 12 or 18");
+    if (op == TM_OP_XPAY && !d_x) return tm_fail(c, TM_EARG, "tm_dslash: XPAY needs x");
+    cudaStream_t st = (cudaStream_t)stream;
+    TM_CUDA(c, cudaSetDevice(c->device));
+    const size_t pb = tm_parity_bytes(c, prec);
+    DslashCall k;
+    memset(&k, 0, sizeof(k));
+    k.out = d_out; k.in = d_in; k.x = nullptr;
+    k.out_parity = out_parity & 1; k.dagger = dagger ? 1 : 0;
+    k.kappa = kappa; k.mu = mu; k.coef = 1.0; k.red_op = RED_NONE;
+    switch (op) {
+        case TM_OP_HOP: return tm_dslash_launch(c, k, prec, recon, st);
+        case TM_OP_HOP_TWINV: k.post = 1; return tm_dslash_launch(c, k, prec, recon, st);
+        case TM_OP_XPAY: k.x = d_x; k.xmode = 2; k.coef = -kappa * kappa; return tm_dslash_launch(c, k, prec, recon, st);
+        case TM_OP_M_FULL: {
+            // out_p = A in_p - kappa D_pq in_q for both parities
+            for (int p = 0; p < 2; p++) {
+                k.out = (char*)d_out + p * pb;
+                k.in = (const char*)d_in + (1 - p) * pb;
+                k.x = (const char*)d_in + p * pb;
+                k.out_parity = p; k.xmode = 2; k.coef = -kappa;
+                TM_TRY(tm_dslash_launch(c, k, prec, recon, st));
+            }
+            return TM_OK;
+        }
+        case TM_OP_MHAT: {
+            void* tmp;
+            TM_TRY(tm_ws(c, WS_API_A, pb, &tmp));
+            k.out = tmp; k.out_parity = 1; k.post = 1;
+            TM_TRY(tm_dslash_launch(c, k, prec, recon, st));
+            k.out = d_out; k.in = tmp; k.x = d_in; k.out_parity = 0; k.post = 0; k.xmode = 2; k.coef = -kappa * kappa;
+            return tm_dslash_launch(c, k, prec, recon, st);
+        }
+    }
+    return tm_fail(c, TM_EARG, "tm_dslash: unknown op");
+}

@@ -1,0 +1,308 @@
+// blas.cu -- BLAS-1 updates and norms of the CG, fused per update step.
+// Work item = (site h, group g of 8 reals): identical (site, component) mapping in every storage
+// precision, coalesced 16-byte accesses across h, so mixed-precision updates need no reshuffle.
+#include <type_traits>
+#include "kernels.h"
+
+template <typename Fn> static tm_status dispatch_prec(tm_ctx* ctx, tm_prec p, Fn&& f) {
+    switch (p) {
+        case TM_F64:  return f((double*)nullptr);
+        case TM_F32:  return f((float*)nullptr);
+        case TM_F16:  return f((__half*)nullptr);
+        case TM_BF16: return f((__nv_bfloat16*)nullptr);
+    }
+    return tm_fail(ctx, TM_EPREC, "unknown precision");
+}
+#define TAGTYPE(tag) typename std::remove_pointer<decltype(tag)>::type
+
+static inline unsigned items_grid(const tm_ctx* ctx, int block, int nparity = 1) {
+    return (unsigned)((3 * ctx->Vh * nparity + block - 1) / block);
+}
+
+// ------------------------------------------------------------------ copy / convert
+template <typename Sd, typename Ss>
+__global__ void copy_kernel(Sd* __restrict__ dst, const Ss* __restrict__ src, int Vh) {
+    const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= 3L * Vh) return;
+    const int g = (int)(i / Vh), h = (int)(i % Vh);
+    typename Prec<Ss>::F a[8];
+    typename Prec<Sd>::F b[8];
+    load8<Ss>(src, Vh, h, g, a);
+#pragma unroll
+    for (int k = 0; k < 8; k++) b[k] = (typename Prec<Sd>::F)a[k];
+    store8<Sd>(dst, Vh, h, g, b);
+}
+
+tm_status blas_zero(tm_ctx* ctx, void* v, tm_prec p, cudaStream_t st) {
+    TM_CUDA(ctx, cudaMemsetAsync(v, 0, tm_parity_bytes(ctx, p), st));
+    return TM_OK;
+}
+
+tm_status blas_copy(tm_ctx* ctx, void* dst, tm_prec pd, const void* src, tm_prec ps, cudaStream_t st) {
+    if (pd == ps) {
+        TM_CUDA(ctx, cudaMemcpyAsync(dst, src, tm_parity_bytes(ctx, pd), cudaMemcpyDeviceToDevice, st));
+        return TM_OK;
+    }
+    return dispatch_prec(ctx, pd, [&](auto* td) {
+        return dispatch_prec(ctx, ps, [&](auto* ts) {
+            typedef TAGTYPE(td) Sd;
+            typedef TAGTYPE(ts) Ss;
+            copy_kernel<Sd, Ss><<<items_grid(ctx, 256), 256, 0, st>>>((Sd*)dst, (const Ss*)src, (int)ctx->Vh);
+            TM_LAUNCH_CHECK(ctx, "copy_kernel");
+            return TM_OK;
+        });
+    });
+}
+
+// ------------------------------------------------------------------ dst = A^-1 src
+template <typename S>
+__global__ void twist_inv_kernel(S* __restrict__ dst, const S* __restrict__ src, int Vh,
+                                 typename Prec<S>::F a) {
+    typedef typename Prec<S>::F F;
+    const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= 3L * Vh) return;
+    const int g = (int)(i / Vh), h = (int)(i % Vh);
+    F v[8];
+    load8<S>(src, Vh, h, g, v);
+    // reals 8g..8g+7: spin = (8g + k)/6 ; upper spins (0,1) are reals 0..11, lower 12..23
+    const F n = F(1) / (F(1) + a * a);
+#pragma unroll
+    for (int k = 0; k < 8; k += 2) {
+        const bool upper = (8 * g + k) < 12;
+        const F s = upper ? a : -a;                 // A^-1 = (1 - i s)/(1+a^2) on this chirality
+        const F re = v[k], im = v[k + 1];
+        v[k] = n * (re + s * im);
+        v[k + 1] = n * (im - s * re);
+    }
+    store8<S>(dst, Vh, h, g, v);
+}
+
+tm_status blas_twist_inv(tm_ctx* ctx, void* dst, const void* src, tm_prec p, double kappa, double mu,
+                         int dagger, cudaStream_t st) {
+    const double a = 2.0 * kappa * mu * (dagger ? -1.0 : 1.0);
+    return dispatch_prec(ctx, p, [&](auto* t) {
+        typedef TAGTYPE(t) S;
+        twist_inv_kernel<S><<<items_grid(ctx, 256), 256, 0, st>>>((S*)dst, (const S*)src, (int)ctx->Vh,
+                                                               (typename Prec<S>::F)a);
+        TM_LAUNCH_CHECK(ctx, "twist_inv_kernel");
+        return TM_OK;
+    });
+}
+
+// ------------------------------------------------------------------ y += x
+template <typename Sy, typename Sx>
+__global__ void axpy1_kernel(Sy* __restrict__ y, const Sx* __restrict__ x, int Vh) {
+    const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= 3L * Vh) return;
+    const int g = (int)(i / Vh), h = (int)(i % Vh);
+    typename Prec<Sx>::F a[8];
+    typename Prec<Sy>::F b[8];
+    load8<Sx>(x, Vh, h, g, a);
+    load8<Sy>(y, Vh, h, g, b);
+#pragma unroll
+    for (int k = 0; k < 8; k++) b[k] += (typename Prec<Sy>::F)a[k];
+    store8<Sy>(y, Vh, h, g, b);
+}
+
+tm_status blas_axpy1(tm_ctx* ctx, void* y, tm_prec py, const void* x, tm_prec px, cudaStream_t st) {
+    if ((py != TM_F64 && py != TM_F32) || (px != TM_F64 && px != TM_F32))
+        return tm_fail(ctx, TM_EPREC, "axpy1: f32/f64 only");
+    const unsigned grid = items_grid(ctx, 256);
+    const int Vh = (int)ctx->Vh;
+    if (py == TM_F64 && px == TM_F64) axpy1_kernel<double, double><<<grid, 256, 0, st>>>((double*)y, (const double*)x, Vh);
+    else if (py == TM_F64) axpy1_kernel<double, float><<<grid, 256, 0, st>>>((double*)y, (const float*)x, Vh);
+    else if (px == TM_F64) axpy1_kernel<float, double><<<grid, 256, 0, st>>>((float*)y, (const double*)x, Vh);
+    else axpy1_kernel<float, float><<<grid, 256, 0, st>>>((float*)y, (const float*)x, Vh);
+    TM_LAUNCH_CHECK(ctx, "axpy1_kernel");
+    return TM_OK;
+}
+
+// ------------------------------------------------------------------ r = b - m, ||r||^2
+template <typename S>
+__global__ void __launch_bounds__(256) xmy_norm_kernel(S* __restrict__ r, const S* __restrict__ b,
+                                                       const S* __restrict__ m, int Vh, int red_op,
+                                                       double* partials, unsigned int* counter, CgScalars* sc) {
+    typedef typename Prec<S>::F F;
+    __shared__ double sm[32];
+    double nrm = 0.0;
+    for (long i = (long)blockIdx.x * blockDim.x + threadIdx.x; i < 3L * Vh; i += (long)gridDim.x * blockDim.x) {
+        const int g = (int)(i / Vh), h = (int)(i % Vh);
+        F vb[8], vm[8];
+        load8<S>(b, Vh, h, g, vb);
+        load8<S>(m, Vh, h, g, vm);
+#pragma unroll
+        for (int k = 0; k < 8; k++) { vb[k] -= vm[k]; nrm += (double)vb[k] * (double)vb[k]; }
+        store8<S>(r, Vh, h, g, vb);
+    }
+    grid_reduce(nrm, partials, counter, sc, red_op, sm);
+}
+
+static inline unsigned red_grid(const tm_ctx* ctx, long items, int block) {
+    long g = (items + block - 1) / block;
+    long cap = (long)ctx->sm_count * 16;
+    return (unsigned)(g < cap ? g : cap);
+}
+
+tm_status blas_xmy_norm(tm_ctx* ctx, void* r, const void* b, const void* m, tm_prec p, int red_op, cudaStream_t st) {
+    const unsigned grid = red_grid(ctx, 3L * ctx->Vh, 256);
+    const int Vh = (int)ctx->Vh;
+    if (p == TM_F64) xmy_norm_kernel<double><<<grid, 256, 0, st>>>((double*)r, (const double*)b, (const double*)m, Vh, red_op, ctx->d_partials, ctx->d_counter, ctx->d_scal);
+    else if (p == TM_F32) xmy_norm_kernel<float><<<grid, 256, 0, st>>>((float*)r, (const float*)b, (const float*)m, Vh, red_op, ctx->d_partials, ctx->d_counter, ctx->d_scal);
+    else return tm_fail(ctx, TM_EPREC, "xmy_norm: f32/f64 only");
+    TM_LAUNCH_CHECK(ctx, "xmy_norm_kernel");
+    return TM_OK;
+}
+
+// ------------------------------------------------------------------ ||v||^2
+template <typename S>
+__global__ void __launch_bounds__(256) norm_kernel(const S* __restrict__ v, long Vh_items, int Vh, int red_op,
+                                                   double* partials, unsigned int* counter, CgScalars* sc) {
+    typedef typename Prec<S>::F F;
+    __shared__ double sm[32];
+    double nrm = 0.0;
+    // Vh_items = 3 * (number of sites in the field): a full-lattice field is two consecutive parity blocks
+    for (long i = (long)blockIdx.x * blockDim.x + threadIdx.x; i < Vh_items; i += (long)gridDim.x * blockDim.x) {
+        const long blk = i / (3L * Vh);
+        const long j = i - blk * 3L * Vh;
+        const int g = (int)(j / Vh), h = (int)(j % Vh);
+        F a[8];
+        load8<S>(v + blk * 24L * Vh, Vh, h, g, a);
+#pragma unroll
+        for (int k = 0; k < 8; k++) nrm += (double)a[k] * (double)a[k];
+    }
+    grid_reduce(nrm, partials, counter, sc, red_op, sm);
+}
+
+static tm_status norm_impl(tm_ctx* ctx, const void* v, tm_prec p, int red_op, int nparity, cudaStream_t st) {
+    const long items = 3L * ctx->Vh * nparity;
+    const unsigned grid = red_grid(ctx, items, 256);
+    return dispatch_prec(ctx, p, [&](auto* t) {
+        typedef TAGTYPE(t) S;
+        norm_kernel<S><<<grid, 256, 0, st>>>((const S*)v, items, (int)ctx->Vh, red_op, ctx->d_partials,
+                                             ctx->d_counter, ctx->d_scal);
+        TM_LAUNCH_CHECK(ctx, "norm_kernel");
+        return TM_OK;
+    });
+}
+tm_status blas_norm(tm_ctx* ctx, const void* v, tm_prec p, int red_op, cudaStream_t st) { return norm_impl(ctx, v, p, red_op, 1, st); }
+tm_status blas_norm_full(tm_ctx* ctx, const void* v, tm_prec p, int red_op, cudaStream_t st) { return norm_impl(ctx, v, p, red_op, 2, st); }
+
+// ------------------------------------------------------------------ x += alpha p ; r -= alpha w ; ||r||^2
+template <typename SA, typename SL>
+__global__ void __launch_bounds__(256) update_xr_kernel(SA* __restrict__ x, SA* __restrict__ r,
+                                                        const SL* __restrict__ p, const SL* __restrict__ w,
+                                                        SL* __restrict__ rs, int Vh, double* partials,
+                                                        unsigned int* counter, CgScalars* sc) {
+    typedef typename Prec<SA>::F FA;
+    typedef typename Prec<SL>::F FL;
+    __shared__ double sm[32];
+    if (sc->done) return;
+    const FA alpha = (FA)sc->alpha;
+    double nrm = 0.0;
+    for (long i = (long)blockIdx.x * blockDim.x + threadIdx.x; i < 3L * Vh; i += (long)gridDim.x * blockDim.x) {
+        const int g = (int)(i / Vh), h = (int)(i % Vh);
+        FA vx[8], vr[8];
+        FL vp[8], vw[8];
+        load8<SA>(x, Vh, h, g, vx);
+        load8<SA>(r, Vh, h, g, vr);
+        load8<SL>(p, Vh, h, g, vp);
+        load8<SL>(w, Vh, h, g, vw);
+#pragma unroll
+        for (int k = 0; k < 8; k++) {
+            vx[k] += alpha * (FA)vp[k];
+            vr[k] -= alpha * (FA)vw[k];
+            nrm += (double)vr[k] * (double)vr[k];
+        }
+        store8<SA>(x, Vh, h, g, vx);
+        store8<SA>(r, Vh, h, g, vr);
+        if (!std::is_same<SA, SL>::value) {
+            FL vs[8];
+#pragma unroll
+            for (int k = 0; k < 8; k++) vs[k] = (FL)vr[k];
+            store8<SL>(rs, Vh, h, g, vs);
+        }
+    }
+    grid_reduce(nrm, partials, counter, sc, RED_RR, sm);
+}
+
+tm_status blas_update_xr(tm_ctx* ctx, void* x, void* r, tm_prec pacc, const void* p, const void* w,
+                         void* rs, tm_prec psl, cudaStream_t st) {
+    const unsigned grid = red_grid(ctx, 3L * ctx->Vh, 256);
+    const int Vh = (int)ctx->Vh;
+    double* pa = ctx->d_partials; unsigned int* cn = ctx->d_counter; CgScalars* sc = ctx->d_scal;
+    if (pacc == TM_F64 && psl == TM_F64)
+        update_xr_kernel<double, double><<<grid, 256, 0, st>>>((double*)x, (double*)r, (const double*)p, (const double*)w, (double*)rs, Vh, pa, cn, sc);
+    else if (pacc == TM_F32 && psl == TM_F32)
+        update_xr_kernel<float, float><<<grid, 256, 0, st>>>((float*)x, (float*)r, (const float*)p, (const float*)w, (float*)rs, Vh, pa, cn, sc);
+    else if (pacc == TM_F32 && psl == TM_F16)
+        update_xr_kernel<float, __half><<<grid, 256, 0, st>>>((float*)x, (float*)r, (const __half*)p, (const __half*)w, (__half*)rs, Vh, pa, cn, sc);
+    else if (pacc == TM_F32 && psl == TM_BF16)
+        update_xr_kernel<float, __nv_bfloat16><<<grid, 256, 0, st>>>((float*)x, (float*)r, (const __nv_bfloat16*)p, (const __nv_bfloat16*)w, (__nv_bfloat16*)rs, Vh, pa, cn, sc);
+    else return tm_fail(ctx, TM_EPREC, "update_xr: unsupported precision pair");
+    TM_LAUNCH_CHECK(ctx, "update_xr_kernel");
+    return TM_OK;
+}
+
+// ------------------------------------------------------------------ p = z + beta p
+template <typename S>
+__global__ void update_p_kernel(S* __restrict__ p, const S* __restrict__ z, int Vh, const CgScalars* sc) {
+    typedef typename Prec<S>::F F;
+    if (sc->done) return;
+    const F beta = (F)sc->beta;
+    const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= 3L * Vh) return;
+    const int g = (int)(i / Vh), h = (int)(i % Vh);
+    F vp[8], vz[8];
+    load8<S>(p, Vh, h, g, vp);
+    load8<S>(z, Vh, h, g, vz);
+#pragma unroll
+    for (int k = 0; k < 8; k++) vp[k] = vz[k] + beta * vp[k];
+    store8<S>(p, Vh, h, g, vp);
+}
+
+tm_status blas_update_p(tm_ctx* ctx, void* p, const void* z, tm_prec psl, cudaStream_t st) {
+    return dispatch_prec(ctx, psl, [&](auto* t) {
+        typedef TAGTYPE(t) S;
+        update_p_kernel<S><<<items_grid(ctx, 256), 256, 0, st>>>((S*)p, (const S*)z, (int)ctx->Vh, ctx->d_scal);
+        TM_LAUNCH_CHECK(ctx, "update_p_kernel");
+        return TM_OK;
+    });
+}
+
+// ------------------------------------------------------------------ scalars
+tm_status scal_set(tm_ctx* ctx, const CgScalars& v, cudaStream_t st) {
+    // pinned staging: wait for earlier users of h_scal
+    TM_CUDA(ctx, cudaStreamSynchronize(st));
+    *ctx->h_scal = v;
+    TM_CUDA(ctx, cudaMemcpyAsync(ctx->d_scal, ctx->h_scal, sizeof(CgScalars), cudaMemcpyHostToDevice, st));
+    TM_CUDA(ctx, cudaStreamSynchronize(st));
+    return TM_OK;
+}
+tm_status scal_get(tm_ctx* ctx, CgScalars* v, cudaStream_t st) {
+    TM_CUDA(ctx, cudaMemcpyAsync(ctx->h_scal, ctx->d_scal, sizeof(CgScalars), cudaMemcpyDeviceToHost, st));
+    TM_CUDA(ctx, cudaStreamSynchronize(st));
+    *v = *ctx->h_scal;
+    return TM_OK;
+}
+
+__global__ void set_done_target_kernel(CgScalars* sc, int done, double target2) {
+    sc->done = done;
+    sc->target2 = target2;
+}
+tm_status scal_set_done_target(tm_ctx* ctx, int done, double target2, cudaStream_t st) {
+    set_done_target_kernel<<<1, 1, 0, st>>>(ctx->d_scal, done, target2);
+    TM_LAUNCH_CHECK(ctx, "set_done_target_kernel");
+    return TM_OK;
+}
+
+// ------------------------------------------------------------------ complex128 accumulate
+__global__ void accumulate_kernel(double* __restrict__ acc, const double* __restrict__ x, size_t n) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) acc[i] += x[i];
+}
+tm_status tm_accumulate(tm_ctx* ctx, void* d_acc, const void* d_x, size_t n, cudaStream_t st) {
+    const size_t nr = 2 * n;
+    accumulate_kernel<<<(unsigned)((nr + 255) / 256), 256, 0, st>>>((double*)d_acc, (const double*)d_x, nr);
+    TM_LAUNCH_CHECK(ctx, "accumulate_kernel");
+    return TM_OK;
+}

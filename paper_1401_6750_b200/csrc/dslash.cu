@@ -1,0 +1,226 @@
+// dslash.cu -- twisted-mass parity Dslash stencil for sm_100a.
+//
+// [B:ns]:  M = (1 + 2 i kappa mu g5) - kappa sum_mu [(1-g_mu) U_mu(x) d_{x+mu,y} + (1+g_mu) U_mu^dag(x-mu) d_{x-mu,y}]
+// One thread per output site of one parity.  For each of the 8 neighbours the spinor is projected
+// to a 2-spin half-spinor with (1 -+ g_mu) (the rank-2 "gamma-projection spin trick"), multiplied
+// by the SU(3) link (rebuilt from two rows for reconstruct-12) and reconstructed into the
+// accumulator.  HBM-bound: no tensor cores, 16-byte coalesced chunk loads, streaming (evict-first)
+// policy for links (zero reuse), default policy for spinors (8-fold reuse served by L1/L2).
+//
+// Epilogue (runtime-uniform):  res = c * (D in);  xmode 1: res += x;  xmode 2: res += A x;
+//                              post 1: res = A^-1 res;  optional ||res||^2 -> grid_reduce.
+// A = 1 + i a g5,  a = 2 kappa mu (sign flipped for dagger),  A^-1 = (1 - i a g5) / (1 + a^2).
+//
+// Chiral basis (reading 2): g_mu = [[0, B],[B^dag, 0]] with
+//   B_x = -i sigma_x, B_y = -i sigma_y, B_z = -i sigma_z, B_t = 1;
+//   (1 + s g_mu) psi = (u, s B^dag u),  u = psi_up + s B psi_low.
+#include "kernels.h"
+#include "su3.cuh"
+
+template <typename F> struct DslashArgs {
+    const void* in;
+    const void* x;
+    void* out;
+    const void* gauge;
+    Geom g;
+    int parity;        // parity of the output sites
+    F dsign;           // +1, or -1 for dagger
+    F tb;              // time boundary sign
+    F a;               // twist 2 kappa mu (already multiplied by dsign)
+    F c;               // coefficient of D in
+    int xmode, post, red_op;
+    double* partials;
+    unsigned int* counter;
+    CgScalars* sc;
+    int check_done;
+};
+
+// u (2 spins x 3 colours complex = 12 reals) = psi_up + s * B_mu psi_low
+template <int MU, typename F>
+__device__ __forceinline__ void project(const F* p, F s, F* u) {
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        const F p0r = p[2 * c], p0i = p[2 * c + 1], p1r = p[6 + 2 * c], p1i = p[6 + 2 * c + 1];
+        const F p2r = p[12 + 2 * c], p2i = p[12 + 2 * c + 1], p3r = p[18 + 2 * c], p3i = p[18 + 2 * c + 1];
+        if (MU == 0) {          // B psi_low = (-i psi3, -i psi2)
+            u[2 * c] = p0r + s * p3i;      u[2 * c + 1] = p0i - s * p3r;
+            u[6 + 2 * c] = p1r + s * p2i;  u[6 + 2 * c + 1] = p1i - s * p2r;
+        } else if (MU == 1) {   // (-psi3, psi2)
+            u[2 * c] = p0r - s * p3r;      u[2 * c + 1] = p0i - s * p3i;
+            u[6 + 2 * c] = p1r + s * p2r;  u[6 + 2 * c + 1] = p1i + s * p2i;
+        } else if (MU == 2) {   // (-i psi2, i psi3)
+            u[2 * c] = p0r + s * p2i;      u[2 * c + 1] = p0i - s * p2r;
+            u[6 + 2 * c] = p1r - s * p3i;  u[6 + 2 * c + 1] = p1i + s * p3r;
+        } else {                // (psi2, psi3)
+            u[2 * c] = p0r + s * p2r;      u[2 * c + 1] = p0i + s * p2i;
+            u[6 + 2 * c] = p1r + s * p3r;  u[6 + 2 * c + 1] = p1i + s * p3i;
+        }
+    }
+}
+
+// acc_up += v ; acc_low += s * B_mu^dag v
+template <int MU, typename F>
+__device__ __forceinline__ void reconstruct(const F* v, F s, F* acc) {
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        const F v0r = v[2 * c], v0i = v[2 * c + 1], v1r = v[6 + 2 * c], v1i = v[6 + 2 * c + 1];
+        acc[2 * c] += v0r;      acc[2 * c + 1] += v0i;
+        acc[6 + 2 * c] += v1r;  acc[6 + 2 * c + 1] += v1i;
+        if (MU == 0) {          // B^dag v = (i v1, i v0)
+            acc[12 + 2 * c] -= s * v1i;  acc[12 + 2 * c + 1] += s * v1r;
+            acc[18 + 2 * c] -= s * v0i;  acc[18 + 2 * c + 1] += s * v0r;
+        } else if (MU == 1) {   // (v1, -v0)
+            acc[12 + 2 * c] += s * v1r;  acc[12 + 2 * c + 1] += s * v1i;
+            acc[18 + 2 * c] -= s * v0r;  acc[18 + 2 * c + 1] -= s * v0i;
+        } else if (MU == 2) {   // (i v0, -i v1)
+            acc[12 + 2 * c] -= s * v0i;  acc[12 + 2 * c + 1] += s * v0r;
+            acc[18 + 2 * c] += s * v1i;  acc[18 + 2 * c + 1] -= s * v1r;
+        } else {                // (v0, v1)
+            acc[12 + 2 * c] += s * v0r;  acc[12 + 2 * c + 1] += s * v0i;
+            acc[18 + 2 * c] += s * v1r;  acc[18 + 2 * c + 1] += s * v1i;
+        }
+    }
+}
+
+template <int MU, int FWD, typename S, int R>
+__device__ __forceinline__ void hop(const S* in, const S* gauge, const Geom& g, int par_out, size_t h_out,
+                                    size_t h_nb, typename Prec<S>::F sgn, typename Prec<S>::F bsign,
+                                    bool wrap, typename Prec<S>::F* acc) {
+    typedef typename Prec<S>::F F;
+    F psi[24], u[12], v[12], U[18];
+    load_spinor<S>(in, g.Vh, h_nb, psi);
+    if (FWD) load_link<S, R>(gauge, g.Vh, par_out, MU, h_out, U);
+    else     load_link<S, R>(gauge, g.Vh, 1 - par_out, MU, h_nb, U);
+    project<MU>(psi, sgn, u);
+    if (MU == 3 && wrap) {
+#pragma unroll
+        for (int i = 0; i < 12; i++) u[i] *= bsign;
+    }
+    su3_mul_half<FWD ? 0 : 1>(U, u, v);
+    reconstruct<MU>(v, sgn, acc);
+}
+
+template <typename S, int R>
+__global__ void __launch_bounds__(128) dslash_kernel(DslashArgs<typename Prec<S>::F> A) {
+    typedef typename Prec<S>::F F;
+    __shared__ double sm[32];
+    if (A.check_done && A.sc->done) return;
+    const Geom& g = A.g;
+    const int h = blockIdx.x * blockDim.x + threadIdx.x;
+    double nrm = 0.0;
+    if (h < g.Vh) {
+        const int xh = h % g.Xh;
+        int q = h / g.Xh;
+        const int y = q % g.X1; q /= g.X1;
+        const int z = q % g.X2;
+        const int t = q / g.X2;
+        const int odd = (y + z + t + A.parity) & 1;     // x = 2*xh + odd
+        const S* in = (const S*)A.in;
+        const S* gauge = (const S*)A.gauge;
+        F acc[24];
+#pragma unroll
+        for (int i = 0; i < 24; i++) acc[i] = 0;
+        const F sf = -A.dsign, sb = A.dsign;           // forward: (1 - g), backward: (1 + g)
+        const int row = h - xh;
+        // x
+        {
+            const int xp = odd ? (xh + 1 == g.Xh ? 0 : xh + 1) : xh;
+            const int xm = odd ? xh : (xh == 0 ? g.Xh - 1 : xh - 1);
+            hop<0, 1, S, R>(in, gauge, g, A.parity, h, row + xp, sf, F(1), false, acc);
+            hop<0, 0, S, R>(in, gauge, g, A.parity, h, row + xm, sb, F(1), false, acc);
+        }
+        // y
+        {
+            const int hp = (y + 1 == g.X1) ? h - (g.X1 - 1) * g.s1 : h + g.s1;
+            const int hm = (y == 0) ? h + (g.X1 - 1) * g.s1 : h - g.s1;
+            hop<1, 1, S, R>(in, gauge, g, A.parity, h, hp, sf, F(1), false, acc);
+            hop<1, 0, S, R>(in, gauge, g, A.parity, h, hm, sb, F(1), false, acc);
+        }
+        // z
+        {
+            const int hp = (z + 1 == g.X2) ? h - (g.X2 - 1) * g.s2 : h + g.s2;
+            const int hm = (z == 0) ? h + (g.X2 - 1) * g.s2 : h - g.s2;
+            hop<2, 1, S, R>(in, gauge, g, A.parity, h, hp, sf, F(1), false, acc);
+            hop<2, 0, S, R>(in, gauge, g, A.parity, h, hm, sb, F(1), false, acc);
+        }
+        // t (boundary sign when the hop wraps around)
+        {
+            const bool wp = (t + 1 == g.X3), wm = (t == 0);
+            const int hp = wp ? h - (g.X3 - 1) * g.s3 : h + g.s3;
+            const int hm = wm ? h + (g.X3 - 1) * g.s3 : h - g.s3;
+            hop<3, 1, S, R>(in, gauge, g, A.parity, h, hp, sf, A.tb, wp, acc);
+            hop<3, 0, S, R>(in, gauge, g, A.parity, h, hm, sb, A.tb, wm, acc);
+        }
+        // epilogue
+#pragma unroll
+        for (int i = 0; i < 24; i++) acc[i] *= A.c;
+        if (A.xmode) {
+            F xv[24];
+            load_spinor<S>((const S*)A.x, g.Vh, h, xv);
+            if (A.xmode == 2) {
+#pragma unroll
+                for (int i = 0; i < 12; i += 2) {       // upper: (1 + i a) x, lower: (1 - i a) x
+                    acc[i] += xv[i] - A.a * xv[i + 1];
+                    acc[i + 1] += xv[i + 1] + A.a * xv[i];
+                    acc[12 + i] += xv[12 + i] + A.a * xv[12 + i + 1];
+                    acc[12 + i + 1] += xv[12 + i + 1] - A.a * xv[12 + i];
+                }
+            } else {
+#pragma unroll
+                for (int i = 0; i < 24; i++) acc[i] += xv[i];
+            }
+        }
+        if (A.post) {                                   // A^-1 = (1 - i a g5)/(1 + a^2)
+            const F n = F(1) / (F(1) + A.a * A.a);
+#pragma unroll
+            for (int i = 0; i < 12; i += 2) {
+                const F ur = acc[i], ui = acc[i + 1], lr = acc[12 + i], li = acc[12 + i + 1];
+                acc[i] = n * (ur + A.a * ui);
+                acc[i + 1] = n * (ui - A.a * ur);
+                acc[12 + i] = n * (lr - A.a * li);
+                acc[12 + i + 1] = n * (li + A.a * lr);
+            }
+        }
+        store_spinor<S>((S*)A.out, g.Vh, h, acc);
+        if (A.red_op != RED_NONE) {
+#pragma unroll
+            for (int i = 0; i < 24; i++) nrm += (double)acc[i] * (double)acc[i];
+        }
+    }
+    if (A.red_op != RED_NONE) grid_reduce(nrm, A.partials, A.counter, A.sc, A.red_op, sm);
+}
+
+template <typename S, int R>
+static tm_status launch_t(tm_ctx* ctx, const DslashCall& c, const void* gauge, cudaStream_t st) {
+    typedef typename Prec<S>::F F;
+    DslashArgs<F> A;
+    A.in = c.in; A.x = c.x; A.out = c.out; A.gauge = gauge;
+    A.g = tm_geom(ctx);
+    A.parity = c.out_parity;
+    A.dsign = c.dagger ? F(-1) : F(1);
+    A.tb = (F)ctx->tb;
+    A.a = (F)(2.0 * c.kappa * c.mu * (c.dagger ? -1.0 : 1.0));
+    A.c = (F)c.coef;
+    A.xmode = c.xmode; A.post = c.post; A.red_op = c.red_op;
+    A.partials = ctx->d_partials; A.counter = ctx->d_counter; A.sc = ctx->d_scal;
+    A.check_done = c.check_done;
+    const int block = 128;
+    const int grid = (int)((ctx->Vh + block - 1) / block);
+    dslash_kernel<S, R><<<grid, block, 0, st>>>(A);
+    TM_LAUNCH_CHECK(ctx, "dslash_kernel");
+    return TM_OK;
+}
+
+tm_status tm_dslash_launch(tm_ctx* ctx, const DslashCall& c, tm_prec prec, tm_recon recon, cudaStream_t st) {
+    const void* gauge = nullptr;
+    TM_TRY(tm_get_gauge(ctx, prec, recon, st, &gauge));
+    const bool r12 = (recon == TM_R12);
+    switch (prec) {
+        case TM_F64:  return r12 ? launch_t<double, 12>(ctx, c, gauge, st) : launch_t<double, 18>(ctx, c, gauge, st);
+        case TM_F32:  return r12 ? launch_t<float, 12>(ctx, c, gauge, st) : launch_t<float, 18>(ctx, c, gauge, st);
+        case TM_F16:  return r12 ? launch_t<__half, 12>(ctx, c, gauge, st) : launch_t<__half, 18>(ctx, c, gauge, st);
+        case TM_BF16: return r12 ? launch_t<__nv_bfloat16, 12>(ctx, c, gauge, st)
+                                 : launch_t<__nv_bfloat16, 18>(ctx, c, gauge, st);
+    }
+    return tm_fail(ctx, TM_EPREC, "tm_dslash: unknown precision");
+}

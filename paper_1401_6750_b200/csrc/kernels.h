@@ -1,0 +1,61 @@
+// kernels.h -- internal (non-exported) entry points shared by the translation units of libtmloops.
+#pragma once
+#include "common.cuh"
+#include "blas.cuh"
+
+// ---- dslash.cu ----------------------------------------------------------------------------
+// out_p = post( xterm(x) + coef * D_pq in ),  xmode: 0 none | 1 x | 2 A x ; post: 0 none | 1 A^-1
+struct DslashCall {
+    void* out; const void* in; const void* x;
+    int out_parity, dagger;
+    double kappa, mu, coef;
+    int xmode, post;
+    int red_op;        // RED_* applied to ||out||^2 (RED_NONE: no norm)
+    int check_done;    // skip when the running solve has converged
+};
+tm_status tm_dslash_launch(tm_ctx* ctx, const DslashCall& c, tm_prec prec, tm_recon recon, cudaStream_t st);
+
+// ---- layout.cu ----------------------------------------------------------------------------
+tm_status tm_import_launch(tm_ctx* ctx, void* d_internal, const void* d_canon, tm_prec prec, cudaStream_t st);
+tm_status tm_export_launch(tm_ctx* ctx, void* d_canon, const void* d_internal, tm_prec prec, cudaStream_t st);
+// Z4 noise into a full-lattice internal field: packed exponents (d_z4 != NULL) or counter hash
+tm_status tm_z4_expand(tm_ctx* ctx, void* d_internal, tm_prec prec, const unsigned char* d_z4,
+                       unsigned long long seed, unsigned long long r, cudaStream_t st);
+
+// ---- blas.cu ------------------------------------------------------------------------------
+// parity-vector operations (n = 24*Vh reals each); all asynchronous on st
+tm_status blas_zero(tm_ctx* ctx, void* v, tm_prec p, cudaStream_t st);
+tm_status blas_copy(tm_ctx* ctx, void* dst, tm_prec pd, const void* src, tm_prec ps, cudaStream_t st);
+// dst = post-twist-inverse? no: plain  dst = A^-1 src  (site-local twist inverse)
+tm_status blas_twist_inv(tm_ctx* ctx, void* dst, const void* src, tm_prec p, double kappa, double mu,
+                         int dagger, cudaStream_t st);
+// y += x (y: py, x: px)
+tm_status blas_axpy1(tm_ctx* ctx, void* y, tm_prec py, const void* x, tm_prec px, cudaStream_t st);
+// r = b - m ; ||r||^2 -> red_op
+tm_status blas_xmy_norm(tm_ctx* ctx, void* r, const void* b, const void* m, tm_prec p, int red_op, cudaStream_t st);
+// ||v||^2 -> red_op
+tm_status blas_norm(tm_ctx* ctx, const void* v, tm_prec p, int red_op, cudaStream_t st);
+// full-lattice norm (2 parities)
+tm_status blas_norm_full(tm_ctx* ctx, const void* v, tm_prec p, int red_op, cudaStream_t st);
+// CG updates with device-resident alpha / beta (no-ops once sc->done):
+//   x += alpha p ; r -= alpha w ; ||r||^2 -> RED_RR ; optional sloppy copy rs of r
+tm_status blas_update_xr(tm_ctx* ctx, void* x, void* r, tm_prec pacc, const void* p, const void* w,
+                         void* rs, tm_prec psl, cudaStream_t st);
+//   p = z + beta p
+tm_status blas_update_p(tm_ctx* ctx, void* p, const void* z, tm_prec psl, cudaStream_t st);
+tm_status scal_set(tm_ctx* ctx, const CgScalars& v, cudaStream_t st);    // upload whole struct
+tm_status scal_get(tm_ctx* ctx, CgScalars* v, cudaStream_t st);          // download + sync
+tm_status scal_set_done_target(tm_ctx* ctx, int done, double target2, cudaStream_t st);
+
+// ---- solver.cu ----------------------------------------------------------------------------
+// eta, s: full-lattice internal fields of precision params->outer
+tm_status tm_solve_internal(tm_ctx* ctx, void* d_s, const void* d_eta, double kappa, double mu,
+                            const tm_solve_params* params, tm_solve_info* info, cudaStream_t st);
+
+// ---- contract.cu --------------------------------------------------------------------------
+// s, eta: full-lattice internal fields of precision acc (TM_F32 | TM_F64); out: complex128 [2][80][nmom][T]
+tm_status tm_contract_internal(tm_ctx* ctx, void* d_out, const void* d_s, const void* d_eta,
+                               double kappa, double mu, const int* h_momenta, int nmom, tm_prec acc,
+                               cudaStream_t st);
+// acc += x on complex128 arrays of n complex numbers
+tm_status tm_accumulate(tm_ctx* ctx, void* d_acc, const void* d_x, size_t n, cudaStream_t st);
