@@ -1,0 +1,324 @@
+"""paper_1401_6750_b200 -- thin Python binding of libtmloops.so (hand-written CUDA, sm_100a).
+
+Argument marshalling only: every step of the hot path (Dslash, CG, contraction, projection,
+TSM combination) runs inside the CUDA library behind the C ABI of ``include/tmloops.h``.
+PyTorch is used for device memory and streams.  There is NO CPU fallback: importing works
+without a GPU (so the symbol table can be checked), but every compute entry point needs a
+CUDA device and raises ``TmError`` otherwise.  Nothing here imports ``oracle/``.
+
+Names follow the C ABI: ``tm_dslash``, ``tm_cg_solve``, ``loop_contract_project``,
+``tsm_estimate`` (methods of :class:`TmContext`).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+from . import inputs  # noqa: F401  (seeded input generators; no method arithmetic)
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libtmloops.so")
+
+TM_OK, TM_EARG, TM_EDIM, TM_EPREC, TM_ECUDA, TM_ENOCONV, TM_EALLOC = range(7)
+TM_F64, TM_F32, TM_F16, TM_BF16 = range(4)
+TM_R18, TM_R12 = 18, 12
+TM_OP_HOP, TM_OP_HOP_TWINV, TM_OP_XPAY, TM_OP_M_FULL, TM_OP_MHAT = range(5)
+PREC = {"f64": TM_F64, "f32": TM_F32, "f16": TM_F16, "bf16": TM_BF16}
+PREC_BYTES = {TM_F64: 8, TM_F32: 4, TM_F16: 2, TM_BF16: 2}
+
+EXPORTS = [
+    "tm_create", "tm_destroy", "tm_last_error", "tm_load_gauge", "tm_field_bytes",
+    "tm_field_import", "tm_field_export", "tm_dslash", "tm_cg_solve", "loop_contract_project",
+    "tsm_estimate", "tsm_estimate_host", "tm_launch_count",
+]
+
+
+class TmError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__(f"tmloops status {status}: {msg}")
+        self.status = status
+
+
+class tm_solve_params(ctypes.Structure):
+    _fields_ = [("sloppy", ctypes.c_int), ("outer", ctypes.c_int), ("recon", ctypes.c_int),
+                ("rho", ctypes.c_double), ("max_iter", ctypes.c_int), ("delta", ctypes.c_double)]
+
+
+class tm_solve_info(ctypes.Structure):
+    _fields_ = [("iters", ctypes.c_int), ("reliable_updates", ctypes.c_int),
+                ("true_resid", ctypes.c_double), ("ms", ctypes.c_double)]
+
+
+class tsm_params(ctypes.Structure):
+    _fields_ = [("n_lp", ctypes.c_int), ("n_hp", ctypes.c_int),
+                ("lp", tm_solve_params), ("hp", tm_solve_params),
+                ("kappa", ctypes.c_double), ("mu", ctypes.c_double),
+                ("h_momenta", ctypes.POINTER(ctypes.c_int)), ("nmom", ctypes.c_int),
+                ("contract_acc_lp", ctypes.c_int), ("contract_acc_hp", ctypes.c_int),
+                ("d_z4", ctypes.c_void_p), ("seed", ctypes.c_ulonglong)]
+
+
+class tsm_info(ctypes.Structure):
+    _fields_ = [("ms_total", ctypes.c_double), ("ms_lp_solve", ctypes.c_double),
+                ("ms_hp_solve", ctypes.c_double), ("ms_contract", ctypes.c_double),
+                ("iters_lp", ctypes.c_long), ("iters_hp", ctypes.c_long),
+                ("worst_resid_lp", ctypes.c_double), ("worst_resid_hp", ctypes.c_double),
+                ("launches", ctypes.c_int)]
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen libtmloops.so (built in-tree by ``python -m paper_1401_6750_b200.build``).
+
+    Fails loudly when the library is missing: there is no other implementation to fall back to."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise TmError(TM_ECUDA, f"{LIB_PATH} not built; run python -m paper_1401_6750_b200.build "
+                                "(no CPU fallback exists)")
+    L = ctypes.CDLL(LIB_PATH)
+    vp, ci, cd = ctypes.c_void_p, ctypes.c_int, ctypes.c_double
+    L.tm_create.argtypes = [ctypes.POINTER(vp), ctypes.POINTER(ci), ci, ci]
+    L.tm_destroy.argtypes = [vp]
+    L.tm_last_error.argtypes = [vp]
+    L.tm_last_error.restype = ctypes.c_char_p
+    L.tm_load_gauge.argtypes = [vp, vp, vp]
+    L.tm_field_bytes.argtypes = [vp, ci, ci]
+    L.tm_field_bytes.restype = ctypes.c_size_t
+    L.tm_field_import.argtypes = [vp, vp, vp, ci, vp]
+    L.tm_field_export.argtypes = [vp, vp, vp, ci, vp]
+    L.tm_dslash.argtypes = [vp, vp, vp, vp, ci, ci, ci, cd, cd, ci, ci, vp]
+    L.tm_cg_solve.argtypes = [vp, vp, vp, cd, cd, ctypes.POINTER(tm_solve_params),
+                              ctypes.POINTER(tm_solve_info), vp]
+    L.loop_contract_project.argtypes = [vp, vp, vp, vp, cd, cd, ctypes.POINTER(ci), ci, ci, vp]
+    L.tsm_estimate.argtypes = [vp, vp, vp, ctypes.POINTER(tsm_params), ctypes.POINTER(tsm_info), vp]
+    L.tsm_estimate_host.argtypes = [vp, vp, vp, ctypes.POINTER(tsm_params), ctypes.POINTER(tsm_info), vp]
+    L.tm_launch_count.argtypes = [vp]
+    L.tm_launch_count.restype = ctypes.c_long
+    _lib = L
+    return L
+
+
+def _torch():
+    import torch
+    return torch
+
+
+def _stream():
+    return ctypes.c_void_p(_torch().cuda.current_stream().cuda_stream)
+
+
+def _solve_params(sloppy, outer, recon, rho, max_iter, delta):
+    p = tm_solve_params()
+    p.sloppy = PREC[sloppy] if isinstance(sloppy, str) else int(sloppy)
+    p.outer = PREC[outer] if isinstance(outer, str) else int(outer)
+    p.recon = int(recon)
+    p.rho = float(rho)
+    p.max_iter = int(max_iter)
+    p.delta = float(delta)
+    return p
+
+
+class TmContext:
+    """Owns one ``tm_ctx`` (lattice geometry + private gauge copies + workspaces) on one GPU."""
+
+    def __init__(self, dims, t_boundary: int = -1, device: int = 0):
+        self.lib = load_library()
+        self.dims = tuple(int(d) for d in dims)
+        self.device = int(device)
+        self.V = int(np.prod(self.dims))
+        self.T = self.dims[3]
+        h = ctypes.c_void_p()
+        st = self.lib.tm_create(ctypes.byref(h), (ctypes.c_int * 4)(*self.dims), int(t_boundary),
+                                self.device)
+        if st != TM_OK:
+            raise TmError(st, self.lib.tm_last_error(None).decode())
+        self.h = h
+        self.tdev = _torch().device("cuda", self.device)
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.lib.tm_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    def _check(self, st, allow=()):
+        if st != TM_OK and st not in allow:
+            raise TmError(st, self.lib.tm_last_error(self.h).decode())
+        return st
+
+    def _dev(self, a, dtype=None):
+        """numpy / torch -> contiguous torch tensor on this context's device."""
+        torch = _torch()
+        if isinstance(a, np.ndarray):
+            a = torch.from_numpy(np.ascontiguousarray(a))
+        a = a.to(self.tdev)
+        if dtype is not None and a.dtype != dtype:
+            a = a.to(dtype)
+        return a.contiguous()
+
+    # ------------------------------------------------------------------ fields
+    def launch_count(self) -> int:
+        return int(self.lib.tm_launch_count(self.h))
+
+    def tm_load_gauge(self, U):
+        """U: complex128 [T,Lz,Ly,Lx,4,3,3] (numpy or torch)."""
+        torch = _torch()
+        U = self._dev(U, torch.complex128)
+        assert U.numel() == self.V * 36
+        self._check(self.lib.tm_load_gauge(self.h, U.data_ptr(), _stream()))
+        torch.cuda.current_stream().synchronize()
+
+    def tm_field_bytes(self, prec, full_lattice=True) -> int:
+        return int(self.lib.tm_field_bytes(self.h, int(prec), 1 if full_lattice else 0))
+
+    def empty_field(self, prec, full_lattice=True):
+        return _torch().empty(self.tm_field_bytes(prec, full_lattice), dtype=_torch().uint8,
+                              device=self.tdev)
+
+    def tm_field_import(self, canon, prec):
+        """canonical complex128 [T,Lz,Ly,Lx,4,3] -> internal full-lattice field (uint8 tensor)."""
+        torch = _torch()
+        canon = self._dev(canon, torch.complex128)
+        assert canon.numel() == self.V * 12
+        out = self.empty_field(prec, True)
+        self._check(self.lib.tm_field_import(self.h, out.data_ptr(), canon.data_ptr(), int(prec), _stream()))
+        return out
+
+    def tm_field_export(self, internal, prec):
+        torch = _torch()
+        lx, ly, lz, lt = self.dims
+        out = torch.empty((lt, lz, ly, lx, 4, 3), dtype=torch.complex128, device=self.tdev)
+        self._check(self.lib.tm_field_export(self.h, out.data_ptr(), internal.data_ptr(), int(prec), _stream()))
+        return out
+
+    def parity_views(self, internal):
+        """(even, odd) halves of a full-lattice internal field."""
+        n = internal.numel() // 2
+        return internal[:n], internal[n:]
+
+    # ------------------------------------------------------------------ operator
+    def tm_dslash(self, out, inp, x, op, out_parity, dagger, kappa, mu, prec, recon):
+        """One operator application on INTERNAL fields (uint8 tensors); see tmloops.h."""
+        self._check(self.lib.tm_dslash(self.h, out.data_ptr(), inp.data_ptr(),
+                                       x.data_ptr() if x is not None else None, int(op),
+                                       int(out_parity), int(bool(dagger)), float(kappa), float(mu),
+                                       int(prec), int(recon), _stream()))
+        return out
+
+    def apply_M(self, psi, kappa, mu, prec=TM_F64, recon=TM_R18, dagger=False):
+        """Convenience for tests: canonical in -> canonical out through TM_OP_M_FULL."""
+        fin = self.tm_field_import(psi, prec)
+        fout = self.empty_field(prec, True)
+        self.tm_dslash(fout, fin, None, TM_OP_M_FULL, 0, dagger, kappa, mu, prec, recon)
+        return self.tm_field_export(fout, prec)
+
+    # ------------------------------------------------------------------ solver
+    def tm_cg_solve(self, eta, kappa, mu, sloppy="f64", outer="f64", recon=TM_R18, rho=1e-10,
+                    max_iter=5000, delta=0.1, raise_on_noconv=True):
+        """eq. 2.1: returns (s canonical complex128 cuda tensor, info dict)."""
+        torch = _torch()
+        eta = self._dev(eta, torch.complex128)
+        s = torch.empty_like(eta)
+        p = _solve_params(sloppy, outer, recon, rho, max_iter, delta)
+        info = tm_solve_info()
+        st = self.lib.tm_cg_solve(self.h, s.data_ptr(), eta.data_ptr(), float(kappa), float(mu),
+                                  ctypes.byref(p), ctypes.byref(info), _stream())
+        self._check(st, allow=() if raise_on_noconv else (TM_ENOCONV,))
+        return s, dict(iters=info.iters, reliable_updates=info.reliable_updates,
+                       true_resid=info.true_resid, ms=info.ms, status=st)
+
+    # ------------------------------------------------------------------ contraction
+    def loop_contract_project(self, s, eta, kappa, mu, momenta, acc=TM_F64):
+        """sec 2.1.1/2.2: complex128 [2,80,nmom,T] cuda tensor of the 160 projected insertions."""
+        torch = _torch()
+        s = self._dev(s, torch.complex128)
+        eta = self._dev(eta, torch.complex128)
+        mom = np.ascontiguousarray(momenta, dtype=np.int32).reshape(-1, 3)
+        out = torch.empty((2, 80, len(mom), self.T), dtype=torch.complex128, device=self.tdev)
+        self._check(self.lib.loop_contract_project(
+            self.h, out.data_ptr(), s.data_ptr(), eta.data_ptr(), float(kappa), float(mu),
+            mom.ctypes.data_as(ctypes.POINTER(ctypes.c_int)), len(mom), int(acc), _stream()))
+        return out
+
+    # ------------------------------------------------------------------ TSM
+    def _tsm_params(self, n_lp, n_hp, kappa, mu, momenta, lp, hp, acc_lp, acc_hp, d_z4, seed):
+        mom = np.ascontiguousarray(momenta, dtype=np.int32).reshape(-1, 3)
+        P = tsm_params()
+        P.n_lp, P.n_hp = int(n_lp), int(n_hp)
+        P.lp = _solve_params(**lp)
+        P.hp = _solve_params(**hp)
+        P.kappa, P.mu = float(kappa), float(mu)
+        P.h_momenta = mom.ctypes.data_as(ctypes.POINTER(ctypes.c_int))
+        P.nmom = len(mom)
+        P.contract_acc_lp, P.contract_acc_hp = int(acc_lp), int(acc_hp)
+        P.d_z4 = d_z4
+        P.seed = int(seed)
+        return P, mom
+
+    @staticmethod
+    def _tsm_info(info, st):
+        return dict(ms_total=info.ms_total, ms_lp_solve=info.ms_lp_solve, ms_hp_solve=info.ms_hp_solve,
+                    ms_contract=info.ms_contract, iters_lp=info.iters_lp, iters_hp=info.iters_hp,
+                    worst_resid_lp=info.worst_resid_lp, worst_resid_hp=info.worst_resid_hp,
+                    launches=info.launches, status=st)
+
+    def tsm_estimate(self, n_lp, n_hp, kappa, mu, momenta, lp, hp, acc_lp=TM_F32, acc_hp=TM_F64,
+                     z4=None, seed=0, per_source=False, raise_on_noconv=True):
+        """sec 2.1: TSM estimate, complex128 [2,80,nmom,T] (device-resident inputs).
+
+        z4: optional uint8 cuda tensor [n_lp, 3V] of packed Z4 exponents (None: generated on the
+        device from ``seed``).  lp / hp: dicts(sloppy, outer, recon, rho, max_iter, delta)."""
+        torch = _torch()
+        d_z4 = None
+        if z4 is not None:
+            z4 = self._dev(z4, torch.uint8)
+            assert z4.numel() == n_lp * 3 * self.V
+            d_z4 = z4.data_ptr()
+        P, mom = self._tsm_params(n_lp, n_hp, kappa, mu, momenta, lp, hp, acc_lp, acc_hp, d_z4, seed)
+        out = torch.empty((2, 80, len(mom), self.T), dtype=torch.complex128, device=self.tdev)
+        ps = None
+        if per_source:
+            ps = torch.empty((n_lp + n_hp, 2, 80, len(mom), self.T), dtype=torch.complex128, device=self.tdev)
+        info = tsm_info()
+        st = self.lib.tsm_estimate(self.h, out.data_ptr(), ps.data_ptr() if ps is not None else None,
+                                   ctypes.byref(P), ctypes.byref(info), _stream())
+        self._check(st, allow=() if raise_on_noconv else (TM_ENOCONV,))
+        return out, ps, self._tsm_info(info, st)
+
+    def tsm_estimate_host(self, n_lp, n_hp, kappa, mu, momenta, lp, hp, acc_lp=TM_F32, acc_hp=TM_F64,
+                          z4_host=None, seed=0, out_host=None, raise_on_noconv=True):
+        """Same through HOST buffers: z4_host (numpy/torch CPU uint8 [n_lp,3V], pinned or not) is
+        uploaded source by source and the result is copied back inside the call."""
+        torch = _torch()
+        h_z4 = None
+        if z4_host is not None:
+            if isinstance(z4_host, np.ndarray):
+                z4_host = torch.from_numpy(z4_host)
+            assert z4_host.device.type == "cpu" and z4_host.dtype == torch.uint8 and z4_host.is_contiguous()
+            assert z4_host.numel() == n_lp * 3 * self.V
+            h_z4 = z4_host.data_ptr()
+        P, mom = self._tsm_params(n_lp, n_hp, kappa, mu, momenta, lp, hp, acc_lp, acc_hp, None, seed)
+        if out_host is None:
+            out_host = torch.empty((2, 80, len(mom), self.T), dtype=torch.complex128).pin_memory()
+        info = tsm_info()
+        st = self.lib.tsm_estimate_host(self.h, out_host.data_ptr(), h_z4, ctypes.byref(P),
+                                        ctypes.byref(info), _stream())
+        self._check(st, allow=() if raise_on_noconv else (TM_ENOCONV,))
+        return out_host, self._tsm_info(info, st)

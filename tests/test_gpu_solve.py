@@ -1,0 +1,91 @@
+"""GPU parity: eq. 2.1 solves through the C ABI vs the CPU oracle.
+
+Bar (BASELINE.json north_star): every solve reaches a TRUE residual ||eta - M s||/||eta|| <= rho,
+evaluated here by the oracle's fp64 apply_M on the exported solution (reading 8).
+HP solutions are unique: they must also agree with the oracle's own 1e-12 solution to ~cond*rho.
+"""
+import numpy as np
+import pytest
+
+from gpu_util import rel_l2, tm, to_np
+from paper_1401_6750_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+C1 = inputs.CONFIGS["c1"]
+
+
+@pytest.fixture(scope="module")
+def c1(orc):
+    dims = C1["dims"]
+    U = inputs.gauge_field(dims, C1["eps"], C1["seed"])
+    eta = inputs.z4_source(dims, C1["src_seed"], 0)
+    s_ref, _, tr, st = orc.solve(eta, U, C1["kappa"], C1["mu"], 1e-12)
+    assert st == 0 and tr < 2e-12
+    return dims, U, eta, s_ref
+
+
+@pytest.mark.parametrize("sloppy,outer,recon,rho", [
+    ("f64", "f64", 18, 1e-10),      # BASELINE c1
+    ("f64", "f64", 12, 1e-10),
+    ("f32", "f64", 12, 1e-8),       # HP: mixed precision with reliable updates
+    ("f32", "f32", 12, 1e-5),
+    ("f16", "f32", 12, 1e-2),       # LP
+    ("bf16", "f32", 12, 1e-2),
+    ("bf16", "f32", 18, 1e-2),
+    ("f16", "f64", 12, 1e-6),       # 16-bit sloppy pushed far below its own floor by reliable updates
+])
+def test_solve_c1(orc, c1, sloppy, outer, recon, rho):
+    t = tm()
+    dims, U, eta, s_ref = c1
+    with t.TmContext(dims, -1) as ctx:
+        ctx.tm_load_gauge(U)
+        s, info = ctx.tm_cg_solve(eta, C1["kappa"], C1["mu"], sloppy, outer, recon, rho, 2000)
+    s = to_np(s)
+    true = orc.true_residual(s, eta, U, C1["kappa"], C1["mu"], -1)
+    assert true <= rho, (true, info)
+    assert info["iters"] > 0
+    # reported residual is honest (outer-precision evaluation of the same quantity)
+    assert abs(info["true_resid"] - true) <= 0.05 * rho + 1e-6 * (outer == "f32")
+    # sigma_max/sigma_min(M) ~ 20 on these fields: error <= cond * residual
+    assert rel_l2(s, s_ref) <= 40 * rho
+
+
+def test_solve_medium_mixed(orc):
+    """8^3x16 (several CTAs per kernel), mixed fp32/fp64 to 1e-8 and bf16 to 1e-2."""
+    t = tm()
+    dims = (8, 8, 8, 16)
+    k, mu = 0.1565, 0.004
+    U = inputs.gauge_field(dims, 0.3, 3)
+    eta = inputs.z4_source(dims, 3, 1)
+    with t.TmContext(dims, -1) as ctx:
+        ctx.tm_load_gauge(U)
+        for sloppy, outer, rho in (("f32", "f64", 1e-8), ("bf16", "f32", 1e-2), ("f16", "f32", 1e-2)):
+            s, info = ctx.tm_cg_solve(eta, k, mu, sloppy, outer, 12, rho, 3000)
+            true = orc.true_residual(to_np(s), eta, U, k, mu, -1)
+            assert true <= rho, (sloppy, true, info)
+
+
+def test_solve_edge_cases(orc, c1):
+    t = tm()
+    dims, U, eta, _ = c1
+    with t.TmContext(dims, -1) as ctx:
+        ctx.tm_load_gauge(U)
+        # zero source -> zero solution, zero iterations
+        s, info = ctx.tm_cg_solve(np.zeros_like(eta), C1["kappa"], C1["mu"], "f32", "f64", 12, 1e-8, 100)
+        assert np.all(to_np(s) == 0) and info["iters"] == 0
+        # iteration cap -> TM_ENOCONV, solution and residual still reported
+        with pytest.raises(t.TmError) as e:
+            ctx.tm_cg_solve(eta, C1["kappa"], C1["mu"], "f64", "f64", 18, 1e-10, 3)
+        assert e.value.status == t.TM_ENOCONV
+        s, info = ctx.tm_cg_solve(eta, C1["kappa"], C1["mu"], "f64", "f64", 18, 1e-10, 3, raise_on_noconv=False)
+        true = orc.true_residual(to_np(s), eta, U, C1["kappa"], C1["mu"], -1)
+        assert info["status"] == t.TM_ENOCONV and info["iters"] == 3
+        assert abs(info["true_resid"] - true) < 1e-10 and 1e-10 < true < 1
+        # sloppy wider than outer is rejected
+        with pytest.raises(t.TmError):
+            ctx.tm_cg_solve(eta, C1["kappa"], C1["mu"], "f64", "f32", 18, 1e-5, 10)
+        # periodic time boundary and the other flavour (mu < 0)
+    with t.TmContext(dims, +1) as ctx:
+        ctx.tm_load_gauge(U)
+        s, info = ctx.tm_cg_solve(eta, C1["kappa"], -C1["mu"], "f32", "f64", 12, 1e-9, 2000)
+        assert orc.true_residual(to_np(s), eta, U, C1["kappa"], -C1["mu"], +1) <= 1e-9
