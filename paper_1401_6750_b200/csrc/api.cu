@@ -71,6 +71,7 @@ extern "C" tm_status tm_destroy(tm_ctx* c) {
     if (c->d_scal) cudaFree(c->d_scal);
     if (c->h_scal) cudaFreeHost(c->h_scal);
     if (c->d_contract_tables) cudaFree(c->d_contract_tables);
+    free(c->h_contract_tables);
     for (int i = 0; i < TM_MAX_SCRATCH; i++)
         if (c->scratch[i]) cudaFree(c->scratch[i]);
     for (int i = 0; i < 4; i++)

@@ -40,6 +40,7 @@ struct tm_ctx {
     size_t scratch_bytes[TM_MAX_SCRATCH];
     // contraction tables
     void* d_contract_tables;
+    void* h_contract_tables;        // host mirror (rebuild only when the momentum list changes)
     size_t contract_tables_bytes;
     cudaEvent_t ev[4];
 };

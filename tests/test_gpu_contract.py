@@ -1,0 +1,102 @@
+"""GPU parity: fused contraction + momentum projection vs the oracle.
+
+Bar (BASELINE.json north_star): contractions of a given s agree within 1e-12 relative (fp64) and
+1e-5 (fp32 accumulate).  Norm (reading 17): relative L2 per (f, ultra-local | derivative)
+block so a small block cannot hide behind a large one.
+"""
+import numpy as np
+import pytest
+
+from gpu_util import rel_l2, tm, to_np
+from paper_1401_6750_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+TOL = {"f64": 1e-12, "f32": 1e-5}
+
+
+def check_blocks(got, ref, tol):
+    for f in (0, 1):
+        for name, sl in (("local", slice(0, 16)), ("deriv", slice(16, 80))):
+            e = rel_l2(got[f, sl], ref[f, sl])
+            assert e <= tol, (f, name, e)
+
+
+def case(dims, eps, seed):
+    U = inputs.gauge_field(dims, eps, seed)
+    s = inputs.random_spinor(dims, seed + 100)      # any s: the contraction does not need M s = eta
+    eta = inputs.z4_source(dims, seed + 200, 0)
+    return U, s, eta
+
+
+@pytest.mark.parametrize("acc", ["f64", "f32"])
+@pytest.mark.parametrize("tb", [-1, 1])
+def test_contract_c1(orc, acc, tb):
+    """BASELINE c1: 4^3x8, 160 insertions, p = 0 only -- and all 33 momenta with p^2 <= 4."""
+    t = tm()
+    c = inputs.CONFIGS["c1"]
+    U, s, eta = case(c["dims"], c["eps"], c["seed"])
+    with t.TmContext(c["dims"], tb) as ctx:
+        ctx.tm_load_gauge(U)
+        for mom in (np.zeros((1, 3), dtype=np.int32), inputs.momentum_list(4)):
+            ref = orc.loops_project(s, eta, U, c["kappa"], c["mu"], mom, tb)
+            got = to_np(ctx.loop_contract_project(s, eta, c["kappa"], c["mu"], mom, t.PREC[acc]))
+            assert got.shape == ref.shape == (2, 80, len(mom), c["dims"][3])
+            check_blocks(got, ref, TOL[acc])
+
+
+@pytest.mark.parametrize("acc", ["f64", "f32"])
+@pytest.mark.parametrize("dims,p2", [
+    ((6, 4, 6, 10), 4),      # unequal extents, lanes beyond Lx idle
+    ((8, 8, 8, 4), 9),       # all 123 momenta
+    ((40, 4, 2, 2), 9),      # Lx > 32: two x-chunks per row, ragged second chunk
+])
+def test_contract_shapes(orc, acc, dims, p2):
+    t = tm()
+    U, s, eta = case(dims, 0.25, 7)
+    k, mu = 0.1563, 0.0055
+    mom = inputs.momentum_list(p2)
+    ref = orc.loops_project(s, eta, U, k, mu, mom, -1)
+    with t.TmContext(dims, -1) as ctx:
+        ctx.tm_load_gauge(U)
+        got = to_np(ctx.loop_contract_project(s, eta, k, mu, mom, t.PREC[acc]))
+    check_blocks(got, ref, TOL[acc])
+
+
+def test_contract_unpruned_momenta_and_large_twist(orc):
+    """px^2 + py^2 > 9 selects the unpruned accumulator set; big mu exposes the g = g5 eta - 2 i kappa mu s term."""
+    t = tm()
+    dims = (8, 8, 8, 4)
+    U, s, eta = case(dims, 0.3, 9)
+    k, mu = 0.15, 0.7
+    mom = np.array([[3, 3, 3], [-3, 3, -2], [2, -3, 1], [0, 0, 0], [-1, -2, -3], [3, -1, 0]], dtype=np.int32)
+    ref = orc.loops_project(s, eta, U, k, mu, mom, -1)
+    with t.TmContext(dims, -1) as ctx:
+        ctx.tm_load_gauge(U)
+        got = to_np(ctx.loop_contract_project(s, eta, k, mu, mom, t.TM_F64))
+        check_blocks(got, ref, 1e-12)
+        # momentum list changes between calls on one context (tables are rebuilt)
+        mom2 = mom[::-1].copy()
+        got2 = to_np(ctx.loop_contract_project(s, eta, k, mu, mom2, t.TM_F64))
+        assert np.array_equal(got2, got[:, :, ::-1, :])
+        with pytest.raises(t.TmError) as e:
+            ctx.loop_contract_project(s, eta, k, mu, np.array([[4, 0, 0]]), t.TM_F64)
+        assert e.value.status == t.TM_EARG
+        with pytest.raises(t.TmError):
+            ctx.loop_contract_project(s, eta, k, mu, mom, t.TM_F16)
+
+
+def test_contract_of_a_solution(orc):
+    """End of the per-source chain: GPU solve -> GPU contraction vs oracle loops of the GPU's own s."""
+    t = tm()
+    c = inputs.CONFIGS["c1"]
+    U = inputs.gauge_field(c["dims"], c["eps"], c["seed"])
+    eta = inputs.z4_source(c["dims"], c["src_seed"], 0)
+    mom = inputs.momentum_list(1)
+    with t.TmContext(c["dims"], -1) as ctx:
+        ctx.tm_load_gauge(U)
+        s, _ = ctx.tm_cg_solve(eta, c["kappa"], c["mu"], "f64", "f64", 18, 1e-10)
+        got = to_np(ctx.loop_contract_project(s, eta, c["kappa"], c["mu"], mom, t.TM_F64))
+    ref = orc.loops_project(to_np(s), eta, U, c["kappa"], c["mu"], mom, -1)
+    check_blocks(got, ref, 1e-12)
+    # gamma5 insertion at p = 0 summed over t is ||s||^2 (oracle pin (ii), now on the GPU result)
+    assert abs(got[0, 15, 0, :].sum() - np.vdot(to_np(s), to_np(s))) <= 1e-10 * np.vdot(to_np(s), to_np(s)).real

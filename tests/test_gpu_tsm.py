@@ -1,0 +1,95 @@
+"""GPU parity: the TSM estimator loop through the C ABI.
+
+LP solutions are not unique, so the end-to-end check is by decomposition:
+per-source arrays vs the oracle, the oracle's combiner on the GPU's per-source arrays, the
+N_LP = N_HP identity (BASELINE.json north_star: within 1e-10), and path equivalences.
+"""
+import numpy as np
+import pytest
+
+from gpu_util import rel_l2, tm, to_np
+from paper_1401_6750_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+C1 = inputs.CONFIGS["c1"]
+LP = dict(sloppy="bf16", outer="f32", recon=12, rho=1e-2, max_iter=500, delta=0.1)
+HP = dict(sloppy="f32", outer="f64", recon=12, rho=1e-8, max_iter=2000, delta=0.1)
+
+
+def packed_z4(dims, seed, n):
+    return np.stack([inputs.pack_z4(inputs.z4_exponents(dims, seed, r)) for r in range(n)])
+
+
+@pytest.fixture(scope="module")
+def setup():
+    dims = C1["dims"]
+    return dims, inputs.gauge_field(dims, C1["eps"], C1["seed"]), inputs.momentum_list(2)
+
+
+def test_tsm_decomposition(orc, setup):
+    t = tm()
+    dims, U, mom = setup
+    k, mu = C1["kappa"], C1["mu"]
+    n_lp, n_hp = 5, 2
+    z4 = packed_z4(dims, C1["src_seed"], n_lp)
+    with t.TmContext(dims, -1) as ctx:
+        ctx.tm_load_gauge(U)
+        out, ps, info = ctx.tsm_estimate(n_lp, n_hp, k, mu, mom, LP, HP, t.TM_F32, t.TM_F64, z4=z4, per_source=True)
+        out, ps = to_np(out), to_np(ps)
+        assert info["worst_resid_lp"] <= LP["rho"] and info["worst_resid_hp"] <= HP["rho"]
+        assert info["iters_lp"] > 0 and info["iters_hp"] > info["iters_lp"] / n_lp and info["launches"] > 0
+        # (3) oracle combiner applied to the GPU's per-source arrays
+        ref = orc.tsm_combine(ps[:n_lp], ps[n_lp:])
+        assert rel_l2(out, ref) <= 1e-12
+        # (4) HP per-source arrays vs the oracle end to end (unique solution): error ~ cond * rho
+        for r in range(n_hp):
+            eta = inputs.z4_source(dims, C1["src_seed"], r)
+            s_ref, _, _, st = orc.solve(eta, U, k, mu, 1e-12)
+            assert st == 0
+            l_ref = orc.loops_project(s_ref, eta, U, k, mu, mom, -1)
+            assert rel_l2(ps[n_lp + r], l_ref) <= 100 * HP["rho"]
+            # LP arrays are only O(rho_LP) close
+            assert rel_l2(ps[r], l_ref) <= 20 * LP["rho"]
+        # device-generated noise (counter hash) == packed noise from the host generator
+        out2, _, _ = ctx.tsm_estimate(n_lp, n_hp, k, mu, mom, LP, HP, t.TM_F32, t.TM_F64, z4=None, seed=C1["src_seed"])
+        assert np.array_equal(to_np(out2), out)
+        # host-buffer entry point == device entry point
+        out3, _ = ctx.tsm_estimate_host(n_lp, n_hp, k, mu, mom, LP, HP, t.TM_F32, t.TM_F64, z4_host=z4)
+        assert np.array_equal(out3.numpy(), out)
+
+
+def test_tsm_identity_nlp_equals_nhp(orc, setup):
+    """N_LP = N_HP with identical sources equals the plain (HP-only) estimator within 1e-10."""
+    t = tm()
+    dims, U, mom = setup
+    k, mu = C1["kappa"], C1["mu"]
+    n = 3
+    with t.TmContext(dims, -1) as ctx:
+        ctx.tm_load_gauge(U)
+        out, _, _ = ctx.tsm_estimate(n, n, k, mu, mom, LP, HP, t.TM_F32, t.TM_F64, seed=C1["src_seed"])
+        plain = 0
+        for r in range(n):
+            eta = inputs.z4_source(dims, C1["src_seed"], r)
+            s, _ = ctx.tm_cg_solve(eta, k, mu, **{kk: HP[kk] for kk in ("sloppy", "outer", "recon", "rho", "max_iter", "delta")})
+            plain = plain + to_np(ctx.loop_contract_project(s, eta, k, mu, mom, t.TM_F64))
+        plain = plain / n
+    assert rel_l2(to_np(out), plain) <= 1e-10
+
+
+def test_tsm_edge_cases(setup):
+    t = tm()
+    dims, U, mom = setup
+    k, mu = C1["kappa"], C1["mu"]
+    with t.TmContext(dims, -1) as ctx:
+        ctx.tm_load_gauge(U)
+        # n_hp = 0: plain LP mean
+        out, ps, _ = ctx.tsm_estimate(2, 0, k, mu, mom, LP, HP, seed=1, per_source=True)
+        assert rel_l2(to_np(out), to_np(ps).mean(axis=0)) <= 1e-14
+        with pytest.raises(t.TmError):
+            ctx.tsm_estimate(1, 2, k, mu, mom, LP, HP, seed=1)          # n_hp > n_lp
+        with pytest.raises(t.TmError):
+            ctx.tsm_estimate(0, 0, k, mu, mom, LP, HP, seed=1)
+        bad = dict(LP, max_iter=1)
+        with pytest.raises(t.TmError) as e:
+            ctx.tsm_estimate(1, 0, k, mu, mom, bad, HP, seed=1)
+        assert e.value.status == t.TM_ENOCONV
