@@ -277,9 +277,9 @@ __device__ __forceinline__ void load_link(const S* g, size_t Vh, int par, int mu
             const int i = (c + 1) % 3, j = (c + 2) % 3;
             F ar = u[2 * i], ai = u[2 * i + 1], br = u[6 + 2 * j], bi = u[6 + 2 * j + 1];
             F cr = u[2 * j], ci = u[2 * j + 1], dr = u[6 + 2 * i], di = u[6 + 2 * i + 1];
-            // a_i b_j - a_j b_i
-            F re = ar * br - ai * bi - (cr * dr - ci * di);
-            F im = ar * bi + ai * br - (cr * di + ci * dr);
+            // a_i b_j - a_j b_i, one FMA per statement
+            F re = ar * br; re -= ai * bi; re -= cr * dr; re += ci * di;
+            F im = ar * bi; im += ai * br; im -= cr * di; im -= ci * dr;
             u[12 + 2 * c] = re;
             u[12 + 2 * c + 1] = -im;
         }

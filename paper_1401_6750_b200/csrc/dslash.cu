@@ -190,6 +190,224 @@ __global__ void __launch_bounds__(128) dslash_kernel(DslashArgs<typename Prec<S>
     if (A.red_op != RED_NONE) grid_reduce(nrm, A.partials, A.counter, A.sc, A.red_op, sm);
 }
 
+
+// =====================================================================================================
+// 16-bit storage path (fp16 / bf16), reconstruct-12.  Blackwell's mixed-precision FMA
+// (PTX fma.rn.f32.f16 / .bf16 -> SASS FHFMA with .H0/.H1 operand selects) multiplies two 16-bit
+// operands straight out of the packed registers and accumulates in fp32, so neither the links nor
+// the neighbour spinors are ever unpacked: one 32-bit register = one complex number (re, im).
+//   project     packed half2 arithmetic on the loaded spinor (result rounded to storage precision)
+//   row 2       conj(row0 x row1) by FHFMA in fp32, packed back to 16 bit
+//   SU(3) * u   FHFMA, fp32 accumulate
+//   reconstruct / epilogue / norm   fp32 (as in the generic kernel)
+template <typename S> struct Pk;
+template <> struct Pk<__half> {
+    typedef __half2 V2;
+    template <int HA, int HB, int NEG> static __device__ __forceinline__ float fma(unsigned a, unsigned b, float c) {
+        const unsigned short ah = HA ? (unsigned short)(a >> 16) : (unsigned short)(a & 0xffffu);
+        const unsigned short bh = HB ? (unsigned short)(b >> 16) : (unsigned short)(b & 0xffffu);
+        if (NEG) asm("{ .reg .b16 t; neg.f16 t, %1; fma.rn.f32.f16 %0, t, %2, %0; }" : "+f"(c) : "h"(ah), "h"(bh));
+        else     asm("fma.rn.f32.f16 %0, %1, %2, %0;" : "+f"(c) : "h"(ah), "h"(bh));
+        return c;
+    }
+    static __device__ __forceinline__ V2 make(float lo, float hi) { return __floats2half2_rn(lo, hi); }
+};
+template <> struct Pk<__nv_bfloat16> {
+    typedef __nv_bfloat162 V2;
+    template <int HA, int HB, int NEG> static __device__ __forceinline__ float fma(unsigned a, unsigned b, float c) {
+        const unsigned short ah = HA ? (unsigned short)(a >> 16) : (unsigned short)(a & 0xffffu);
+        const unsigned short bh = HB ? (unsigned short)(b >> 16) : (unsigned short)(b & 0xffffu);
+        if (NEG) asm("{ .reg .b16 t; neg.bf16 t, %1; fma.rn.f32.bf16 %0, t, %2, %0; }" : "+f"(c) : "h"(ah), "h"(bh));
+        else     asm("fma.rn.f32.bf16 %0, %1, %2, %0;" : "+f"(c) : "h"(ah), "h"(bh));
+        return c;
+    }
+    static __device__ __forceinline__ V2 make(float lo, float hi) { return __floats2bfloat162_rn(lo, hi); }
+};
+template <typename V2> __device__ __forceinline__ V2 as_v2(unsigned w) { return *reinterpret_cast<V2*>(&w); }
+template <typename V2> __device__ __forceinline__ unsigned as_u(V2 v) { return *reinterpret_cast<unsigned*>(&v); }
+
+// acc += (CONJ ? conj(a) : a) * b for packed complex a, b
+template <typename S, int CONJ>
+__device__ __forceinline__ void cmadd16(unsigned a, unsigned b, float& re, float& im) {
+    re = Pk<S>::template fma<0, 0, 0>(a, b, re);
+    re = Pk<S>::template fma<1, 1, CONJ ? 0 : 1>(a, b, re);
+    im = Pk<S>::template fma<0, 1, 0>(a, b, im);
+    im = Pk<S>::template fma<1, 0, CONJ ? 1 : 0>(a, b, im);
+}
+
+// packed half-spinor u[sp*3 + c] = psi_up + s * B_mu psi_low, s = SGN (compile time)
+template <int MU, int SGN, typename S>
+__device__ __forceinline__ void project16(const unsigned* p, unsigned* u) {
+    typedef typename Pk<S>::V2 V2;
+    const V2 mi = Pk<S>::make((float)SGN, (float)-SGN);      // multiply by -i*s after a (re,im) swap
+    const V2 pi = Pk<S>::make((float)-SGN, (float)SGN);      // multiply by +i*s after a swap
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        const V2 p0 = as_v2<V2>(p[c]), p1 = as_v2<V2>(p[3 + c]), p2 = as_v2<V2>(p[6 + c]), p3 = as_v2<V2>(p[9 + c]);
+        V2 u0, u1;
+        if (MU == 0) {          // (-i psi3, -i psi2)
+            u0 = __hfma2(__lowhigh2highlow(p3), mi, p0);
+            u1 = __hfma2(__lowhigh2highlow(p2), mi, p1);
+        } else if (MU == 1) {   // (-psi3, psi2)
+            u0 = SGN > 0 ? __hsub2(p0, p3) : __hadd2(p0, p3);
+            u1 = SGN > 0 ? __hadd2(p1, p2) : __hsub2(p1, p2);
+        } else if (MU == 2) {   // (-i psi2, i psi3)
+            u0 = __hfma2(__lowhigh2highlow(p2), mi, p0);
+            u1 = __hfma2(__lowhigh2highlow(p3), pi, p1);
+        } else {                // (psi2, psi3)
+            u0 = SGN > 0 ? __hadd2(p0, p2) : __hsub2(p0, p2);
+            u1 = SGN > 0 ? __hadd2(p1, p3) : __hsub2(p1, p3);
+        }
+        u[c] = as_u(u0);
+        u[3 + c] = as_u(u1);
+    }
+}
+
+template <int MU, int FWD, int DAGGER, typename S>
+__device__ __forceinline__ void hop16(const S* in, const S* gauge, size_t Vh, int par_out, size_t h_out, size_t h_nb,
+                                      float bsign, bool wrap, float* acc) {
+    typedef typename Pk<S>::V2 V2;
+    constexpr int SGN = (FWD ? -1 : 1) * (DAGGER ? -1 : 1);       // forward: (1 - g), backward: (1 + g)
+    unsigned p[12], U[9], u[6];
+    {
+        const uint4* f = reinterpret_cast<const uint4*>(in) + h_nb;
+#pragma unroll
+        for (int k = 0; k < 3; k++) {
+            const uint4 q = __ldg(f + (size_t)k * Vh);
+            p[4 * k] = q.x; p[4 * k + 1] = q.y; p[4 * k + 2] = q.z; p[4 * k + 3] = q.w;
+        }
+    }
+    {
+        const size_t hl = FWD ? h_out : h_nb;
+        const int pl = FWD ? par_out : 1 - par_out;
+        const uint2* g = reinterpret_cast<const uint2*>(gauge) + ((size_t)(pl * 4 + MU) * 3 * Vh + hl);
+#pragma unroll
+        for (int k = 0; k < 3; k++) {
+            const uint2 q = __ldcs(g + (size_t)k * Vh);
+            U[2 * k] = q.x; U[2 * k + 1] = q.y;
+        }
+    }
+    project16<MU, SGN, S>(p, u);
+    if (MU == 3 && wrap) {
+        const V2 b2 = Pk<S>::make(bsign, bsign);
+#pragma unroll
+        for (int i = 0; i < 6; i++) u[i] = as_u(__hmul2(as_v2<V2>(u[i]), b2));
+    }
+    // row 2 = conj(row0 x row1)
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        const int i = (c + 1) % 3, j = (c + 2) % 3;
+        float re = 0.f, im = 0.f, re2 = 0.f, im2 = 0.f;
+        cmadd16<S, 0>(U[i], U[3 + j], re, im);          // a_i b_j
+        cmadd16<S, 0>(U[j], U[3 + i], re2, im2);        // a_j b_i
+        U[6 + c] = as_u(Pk<S>::make(re - re2, im2 - im));
+    }
+    float v[12];
+#pragma unroll
+    for (int sp = 0; sp < 2; sp++)
+#pragma unroll
+        for (int a = 0; a < 3; a++) {
+            float re = 0.f, im = 0.f;
+#pragma unroll
+            for (int b = 0; b < 3; b++) {
+                if (FWD) cmadd16<S, 0>(U[a * 3 + b], u[sp * 3 + b], re, im);       // U u
+                else     cmadd16<S, 1>(U[b * 3 + a], u[sp * 3 + b], re, im);       // U^dag u
+            }
+            v[sp * 6 + 2 * a] = re;
+            v[sp * 6 + 2 * a + 1] = im;
+        }
+    reconstruct<MU>(v, (float)SGN, acc);
+}
+
+template <typename S, int DAGGER>
+__global__ void __launch_bounds__(128) dslash16_kernel(DslashArgs<float> A) {
+    __shared__ double sm[32];
+    if (A.check_done && A.sc->done) return;
+    const Geom& g = A.g;
+    const int h = blockIdx.x * blockDim.x + threadIdx.x;
+    double nrm = 0.0;
+    if (h < g.Vh) {
+        const int xh = h % g.Xh;
+        int q = h / g.Xh;
+        const int y = q % g.X1; q /= g.X1;
+        const int z = q % g.X2;
+        const int t = q / g.X2;
+        const int odd = (y + z + t + A.parity) & 1;
+        const S* in = (const S*)A.in;
+        const S* gauge = (const S*)A.gauge;
+        const size_t Vh = g.Vh;
+        float acc[24];
+#pragma unroll
+        for (int i = 0; i < 24; i++) acc[i] = 0.f;
+        const int row = h - xh;
+        {
+            const int xp = odd ? (xh + 1 == g.Xh ? 0 : xh + 1) : xh;
+            const int xm = odd ? xh : (xh == 0 ? g.Xh - 1 : xh - 1);
+            hop16<0, 1, DAGGER, S>(in, gauge, Vh, A.parity, h, row + xp, 1.f, false, acc);
+            hop16<0, 0, DAGGER, S>(in, gauge, Vh, A.parity, h, row + xm, 1.f, false, acc);
+        }
+        {
+            const int hp = (y + 1 == g.X1) ? h - (g.X1 - 1) * g.s1 : h + g.s1;
+            const int hm = (y == 0) ? h + (g.X1 - 1) * g.s1 : h - g.s1;
+            hop16<1, 1, DAGGER, S>(in, gauge, Vh, A.parity, h, hp, 1.f, false, acc);
+            hop16<1, 0, DAGGER, S>(in, gauge, Vh, A.parity, h, hm, 1.f, false, acc);
+        }
+        {
+            const int hp = (z + 1 == g.X2) ? h - (g.X2 - 1) * g.s2 : h + g.s2;
+            const int hm = (z == 0) ? h + (g.X2 - 1) * g.s2 : h - g.s2;
+            hop16<2, 1, DAGGER, S>(in, gauge, Vh, A.parity, h, hp, 1.f, false, acc);
+            hop16<2, 0, DAGGER, S>(in, gauge, Vh, A.parity, h, hm, 1.f, false, acc);
+        }
+        {
+            const bool wp = (t + 1 == g.X3), wm = (t == 0);
+            const int hp = wp ? h - (g.X3 - 1) * g.s3 : h + g.s3;
+            const int hm = wm ? h + (g.X3 - 1) * g.s3 : h - g.s3;
+            hop16<3, 1, DAGGER, S>(in, gauge, Vh, A.parity, h, hp, A.tb, wp, acc);
+            hop16<3, 0, DAGGER, S>(in, gauge, Vh, A.parity, h, hm, A.tb, wm, acc);
+        }
+        // epilogue: res = c * acc (+ x | + A x), optional A^-1, store, optional norm
+        const float cf = A.c, a = A.a;
+        if (A.xmode) {
+            float xv[24];
+            load_spinor<S>((const S*)A.x, g.Vh, h, xv);
+            if (A.xmode == 2) {
+#pragma unroll
+                for (int i = 0; i < 12; i += 2) {
+                    float t0 = xv[i]; t0 -= a * xv[i + 1];              acc[i] = fmaf(cf, acc[i], t0);
+                    float t1 = xv[i + 1]; t1 += a * xv[i];              acc[i + 1] = fmaf(cf, acc[i + 1], t1);
+                    float t2 = xv[12 + i]; t2 += a * xv[12 + i + 1];    acc[12 + i] = fmaf(cf, acc[12 + i], t2);
+                    float t3 = xv[12 + i + 1]; t3 -= a * xv[12 + i];    acc[12 + i + 1] = fmaf(cf, acc[12 + i + 1], t3);
+                }
+            } else {
+#pragma unroll
+                for (int i = 0; i < 24; i++) acc[i] = fmaf(cf, acc[i], xv[i]);
+            }
+        } else {
+#pragma unroll
+            for (int i = 0; i < 24; i++) acc[i] *= cf;
+        }
+        if (A.post) {
+            const float n = 1.f / (1.f + a * a);
+#pragma unroll
+            for (int i = 0; i < 12; i += 2) {
+                const float ur = acc[i], ui = acc[i + 1], lr = acc[12 + i], li = acc[12 + i + 1];
+                acc[i] = n * (ur + a * ui);
+                acc[i + 1] = n * (ui - a * ur);
+                acc[12 + i] = n * (lr - a * li);
+                acc[12 + i + 1] = n * (li + a * lr);
+            }
+        }
+        store_spinor<S>((S*)A.out, g.Vh, h, acc);
+        if (A.red_op != RED_NONE) {
+            float n2 = 0.f;      // 24 terms in fp32, then fp64 across sites
+#pragma unroll
+            for (int i = 0; i < 24; i++) n2 = fmaf(acc[i], acc[i], n2);
+            nrm = (double)n2;
+        }
+    }
+    if (A.red_op != RED_NONE) grid_reduce(nrm, A.partials, A.counter, A.sc, A.red_op, sm);
+}
+
 template <typename S, int R>
 static tm_status launch_t(tm_ctx* ctx, const DslashCall& c, const void* gauge, cudaStream_t st) {
     typedef typename Prec<S>::F F;
@@ -211,6 +429,27 @@ static tm_status launch_t(tm_ctx* ctx, const DslashCall& c, const void* gauge, c
     return TM_OK;
 }
 
+template <typename S>
+static tm_status launch16(tm_ctx* ctx, const DslashCall& c, const void* gauge, cudaStream_t st) {
+    DslashArgs<float> A;
+    A.in = c.in; A.x = c.x; A.out = c.out; A.gauge = gauge;
+    A.g = tm_geom(ctx);
+    A.parity = c.out_parity;
+    A.dsign = c.dagger ? -1.f : 1.f;
+    A.tb = (float)ctx->tb;
+    A.a = (float)(2.0 * c.kappa * c.mu * (c.dagger ? -1.0 : 1.0));
+    A.c = (float)c.coef;
+    A.xmode = c.xmode; A.post = c.post; A.red_op = c.red_op;
+    A.partials = ctx->d_partials; A.counter = ctx->d_counter; A.sc = ctx->d_scal;
+    A.check_done = c.check_done;
+    const int block = 128;
+    const int grid = (int)((ctx->Vh + block - 1) / block);
+    if (c.dagger) dslash16_kernel<S, 1><<<grid, block, 0, st>>>(A);
+    else          dslash16_kernel<S, 0><<<grid, block, 0, st>>>(A);
+    TM_LAUNCH_CHECK(ctx, "dslash16_kernel");
+    return TM_OK;
+}
+
 tm_status tm_dslash_launch(tm_ctx* ctx, const DslashCall& c, tm_prec prec, tm_recon recon, cudaStream_t st) {
     const void* gauge = nullptr;
     TM_TRY(tm_get_gauge(ctx, prec, recon, st, &gauge));
@@ -218,8 +457,8 @@ tm_status tm_dslash_launch(tm_ctx* ctx, const DslashCall& c, tm_prec prec, tm_re
     switch (prec) {
         case TM_F64:  return r12 ? launch_t<double, 12>(ctx, c, gauge, st) : launch_t<double, 18>(ctx, c, gauge, st);
         case TM_F32:  return r12 ? launch_t<float, 12>(ctx, c, gauge, st) : launch_t<float, 18>(ctx, c, gauge, st);
-        case TM_F16:  return r12 ? launch_t<__half, 12>(ctx, c, gauge, st) : launch_t<__half, 18>(ctx, c, gauge, st);
-        case TM_BF16: return r12 ? launch_t<__nv_bfloat16, 12>(ctx, c, gauge, st)
+        case TM_F16:  return r12 ? launch16<__half>(ctx, c, gauge, st) : launch_t<__half, 18>(ctx, c, gauge, st);
+        case TM_BF16: return r12 ? launch16<__nv_bfloat16>(ctx, c, gauge, st)
                                  : launch_t<__nv_bfloat16, 18>(ctx, c, gauge, st);
     }
     return tm_fail(ctx, TM_EPREC, "tm_dslash: unknown precision");

@@ -14,8 +14,9 @@ __device__ __forceinline__ void su3_mul_half(const F* U, const F* u, F* v) {
                 const F ur = DAG ? U[(b * 3 + a) * 2] : U[(a * 3 + b) * 2];
                 const F ui = DAG ? -U[(b * 3 + a) * 2 + 1] : U[(a * 3 + b) * 2 + 1];
                 const F xr = u[sp * 6 + 2 * b], xi = u[sp * 6 + 2 * b + 1];
-                re += ur * xr - ui * xi;
-                im += ur * xi + ui * xr;
+                // one FMA per statement (a single expression would cost FMUL + FFMA + FADD)
+                re += ur * xr; re -= ui * xi;
+                im += ur * xi; im += ui * xr;
             }
             v[sp * 6 + 2 * a] = re;
             v[sp * 6 + 2 * a + 1] = im;

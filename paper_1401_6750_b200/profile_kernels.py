@@ -1,0 +1,86 @@
+"""Run one hot kernel family a few times on paper-sized fields (for ncu captures).
+
+    python -m paper_1401_6750_b200.profile_kernels --what dslash --prec f16 --recon 12 --dims 32 32 32 64 --napp 6
+    python -m paper_1401_6750_b200.profile_kernels --what contract --prec f32 --dims 32 32 32 64
+    python -m paper_1401_6750_b200.profile_kernels --what solve --prec f16 --dims 32 32 32 64
+
+Prints CUDA-event timings; meant to be wrapped as `<cmd> && ncu ... <cmd>` (B200_PROFILING.md).
+"""
+from __future__ import annotations
+
+import argparse
+
+import torch
+
+import paper_1401_6750_b200 as tmod
+from paper_1401_6750_b200 import inputs, inputs_torch
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--what", default="dslash", choices=["dslash", "contract", "solve"])
+    ap.add_argument("--prec", default="f16")
+    ap.add_argument("--recon", type=int, default=12)
+    ap.add_argument("--dims", type=int, nargs=4, default=[32, 32, 32, 64])
+    ap.add_argument("--napp", type=int, default=6)
+    ap.add_argument("--op", default="XPAY")
+    ap.add_argument("--eps", type=float, default=0.2)
+    ap.add_argument("--kappa", type=float, default=0.161231)
+    ap.add_argument("--mu", type=float, default=0.004)
+    ap.add_argument("--p2max", type=int, default=9)
+    a = ap.parse_args()
+    dims = tuple(a.dims)
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(0)
+    U = inputs_torch.gauge_field(dims, a.eps, 5, dev)
+    ctx = tmod.TmContext(dims, -1, 0)
+    ctx.tm_load_gauge(U)
+    del U
+    P = tmod.PREC[a.prec]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if a.what == "dslash":
+        tdt = {"f64": torch.float64, "f32": torch.float32, "f16": torch.float16, "bf16": torch.bfloat16}[a.prec]
+        nb = 3
+        ins = [ctx.empty_field(P, False) for _ in range(nb)]
+        outs = [ctx.empty_field(P, False) for _ in range(nb)]
+        xs = ctx.empty_field(P, False)
+        for b in ins + [xs]:
+            v = b.view(tdt)
+            v.copy_((torch.rand(v.shape, device=dev, dtype=torch.float32) - 0.5).to(tdt))
+        op = getattr(tmod, "TM_OP_" + a.op)
+        for i in range(3):
+            ctx.tm_dslash(outs[i % nb], ins[i % nb], xs, op, 0, False, a.kappa, a.mu, P, a.recon)
+        torch.cuda.synchronize()
+        e0.record()
+        for i in range(a.napp):
+            ctx.tm_dslash(outs[i % nb], ins[i % nb], xs, op, 0, False, a.kappa, a.mu, P, a.recon)
+        e1.record()
+        torch.cuda.synchronize()
+        V = inputs.volume(dims)
+        us = e0.elapsed_time(e1) * 1e3 / a.napp
+        nbytes = (48 + 8 * a.recon + (24 if a.op == "XPAY" else 0)) * tmod.PREC_BYTES[P] * (V // 2)
+        print("dslash %s r%d %s: %.1f us/launch, %.0f GB/s algorithmic" % (a.prec, a.recon, a.op, us, nbytes / us / 1e3))
+    elif a.what == "contract":
+        s = inputs_torch.z4_source(dims, 11, 0, dev)
+        eta = inputs_torch.z4_source(dims, 11, 1, dev)
+        mom = inputs.momentum_list(a.p2max)
+        ctx.loop_contract_project(s, eta, a.kappa, a.mu, mom, P)
+        torch.cuda.synchronize()
+        e0.record()
+        for i in range(a.napp):
+            ctx.loop_contract_project(s, eta, a.kappa, a.mu, mom, P)
+        e1.record()
+        torch.cuda.synchronize()
+        print("contract %s: %.3f ms/call (includes 2 canonical->internal imports)" % (a.prec, e0.elapsed_time(e1) / a.napp))
+    else:
+        eta = inputs_torch.z4_source(dims, 11, 0, dev)
+        outer = "f32" if a.prec in ("f16", "bf16") else "f64"
+        rho = 1e-2 if outer == "f32" else 1e-8
+        for i in range(2):
+            s, info = ctx.tm_cg_solve(eta, a.kappa, a.mu, a.prec, outer, a.recon, rho, 5000)
+        print("solve %s/%s rho=%g: %s" % (a.prec, outer, rho, info))
+    ctx.close()
+
+
+if __name__ == "__main__":
+    main()
