@@ -263,30 +263,32 @@ __device__ __forceinline__ void project16(const unsigned* p, unsigned* u) {
     }
 }
 
+template <int MU, int FWD, typename S>
+__device__ __forceinline__ void load16(const S* in, const S* gauge, size_t Vh, int par_out, size_t h_out, size_t h_nb,
+                                       unsigned* p, unsigned* U) {
+    const uint4* f = reinterpret_cast<const uint4*>(in) + h_nb;
+#pragma unroll
+    for (int k = 0; k < 3; k++) {
+        const uint4 q = __ldg(f + (size_t)k * Vh);
+        p[4 * k] = q.x; p[4 * k + 1] = q.y; p[4 * k + 2] = q.z; p[4 * k + 3] = q.w;
+    }
+    const size_t hl = FWD ? h_out : h_nb;
+    const int pl = FWD ? par_out : 1 - par_out;
+    const uint2* g = reinterpret_cast<const uint2*>(gauge) + ((size_t)(pl * 4 + MU) * 3 * Vh + hl);
+#pragma unroll
+    for (int k = 0; k < 3; k++) {
+        const uint2 q = __ldcs(g + (size_t)k * Vh);
+        U[2 * k] = q.x; U[2 * k + 1] = q.y;
+    }
+}
+
 template <int MU, int FWD, int DAGGER, typename S>
-__device__ __forceinline__ void hop16(const S* in, const S* gauge, size_t Vh, int par_out, size_t h_out, size_t h_nb,
-                                      float bsign, bool wrap, float* acc) {
+__device__ __forceinline__ void compute16(const unsigned* p, const unsigned* Uin, float bsign, bool wrap, float* acc) {
     typedef typename Pk<S>::V2 V2;
     constexpr int SGN = (FWD ? -1 : 1) * (DAGGER ? -1 : 1);       // forward: (1 - g), backward: (1 + g)
-    unsigned p[12], U[9], u[6];
-    {
-        const uint4* f = reinterpret_cast<const uint4*>(in) + h_nb;
+    unsigned U[9], u[6];
 #pragma unroll
-        for (int k = 0; k < 3; k++) {
-            const uint4 q = __ldg(f + (size_t)k * Vh);
-            p[4 * k] = q.x; p[4 * k + 1] = q.y; p[4 * k + 2] = q.z; p[4 * k + 3] = q.w;
-        }
-    }
-    {
-        const size_t hl = FWD ? h_out : h_nb;
-        const int pl = FWD ? par_out : 1 - par_out;
-        const uint2* g = reinterpret_cast<const uint2*>(gauge) + ((size_t)(pl * 4 + MU) * 3 * Vh + hl);
-#pragma unroll
-        for (int k = 0; k < 3; k++) {
-            const uint2 q = __ldcs(g + (size_t)k * Vh);
-            U[2 * k] = q.x; U[2 * k + 1] = q.y;
-        }
-    }
+    for (int i = 0; i < 6; i++) U[i] = Uin[i];
     project16<MU, SGN, S>(p, u);
     if (MU == 3 && wrap) {
         const V2 b2 = Pk<S>::make(bsign, bsign);
@@ -319,8 +321,8 @@ __device__ __forceinline__ void hop16(const S* in, const S* gauge, size_t Vh, in
     reconstruct<MU>(v, (float)SGN, acc);
 }
 
-template <typename S, int DAGGER>
-__global__ void __launch_bounds__(128) dslash16_kernel(DslashArgs<float> A) {
+template <typename S, int DAGGER, int PIPE, int MINB>
+__global__ void __launch_bounds__(128, MINB) dslash16_kernel(DslashArgs<float> A) {
     __shared__ double sm[32];
     if (A.check_done && A.sc->done) return;
     const Geom& g = A.g;
@@ -340,30 +342,45 @@ __global__ void __launch_bounds__(128) dslash16_kernel(DslashArgs<float> A) {
 #pragma unroll
         for (int i = 0; i < 24; i++) acc[i] = 0.f;
         const int row = h - xh;
-        {
-            const int xp = odd ? (xh + 1 == g.Xh ? 0 : xh + 1) : xh;
-            const int xm = odd ? xh : (xh == 0 ? g.Xh - 1 : xh - 1);
-            hop16<0, 1, DAGGER, S>(in, gauge, Vh, A.parity, h, row + xp, 1.f, false, acc);
-            hop16<0, 0, DAGGER, S>(in, gauge, Vh, A.parity, h, row + xm, 1.f, false, acc);
-        }
-        {
-            const int hp = (y + 1 == g.X1) ? h - (g.X1 - 1) * g.s1 : h + g.s1;
-            const int hm = (y == 0) ? h + (g.X1 - 1) * g.s1 : h - g.s1;
-            hop16<1, 1, DAGGER, S>(in, gauge, Vh, A.parity, h, hp, 1.f, false, acc);
-            hop16<1, 0, DAGGER, S>(in, gauge, Vh, A.parity, h, hm, 1.f, false, acc);
-        }
-        {
-            const int hp = (z + 1 == g.X2) ? h - (g.X2 - 1) * g.s2 : h + g.s2;
-            const int hm = (z == 0) ? h + (g.X2 - 1) * g.s2 : h - g.s2;
-            hop16<2, 1, DAGGER, S>(in, gauge, Vh, A.parity, h, hp, 1.f, false, acc);
-            hop16<2, 0, DAGGER, S>(in, gauge, Vh, A.parity, h, hm, 1.f, false, acc);
-        }
-        {
-            const bool wp = (t + 1 == g.X3), wm = (t == 0);
-            const int hp = wp ? h - (g.X3 - 1) * g.s3 : h + g.s3;
-            const int hm = wm ? h + (g.X3 - 1) * g.s3 : h - g.s3;
-            hop16<3, 1, DAGGER, S>(in, gauge, Vh, A.parity, h, hp, A.tb, wp, acc);
-            hop16<3, 0, DAGGER, S>(in, gauge, Vh, A.parity, h, hm, A.tb, wm, acc);
+        const int xp = row + (odd ? (xh + 1 == g.Xh ? 0 : xh + 1) : xh);
+        const int xm = row + (odd ? xh : (xh == 0 ? g.Xh - 1 : xh - 1));
+        const int yp = (y + 1 == g.X1) ? h - (g.X1 - 1) * g.s1 : h + g.s1;
+        const int ym = (y == 0) ? h + (g.X1 - 1) * g.s1 : h - g.s1;
+        const int zp = (z + 1 == g.X2) ? h - (g.X2 - 1) * g.s2 : h + g.s2;
+        const int zm = (z == 0) ? h + (g.X2 - 1) * g.s2 : h - g.s2;
+        const bool wp = (t + 1 == g.X3), wm = (t == 0);
+        const int tp = wp ? h - (g.X3 - 1) * g.s3 : h + g.s3;
+        const int tm = wm ? h + (g.X3 - 1) * g.s3 : h - g.s3;
+        const int par = A.parity;
+        unsigned pa[12], ua[6];
+        if (PIPE) {
+            // software pipeline: the loads of hop k+1 are in flight while hop k is computed
+            unsigned pb[12], ub[6];
+            load16<0, 1, S>(in, gauge, Vh, par, h, xp, pa, ua);
+            load16<0, 0, S>(in, gauge, Vh, par, h, xm, pb, ub);
+            compute16<0, 1, DAGGER, S>(pa, ua, 1.f, false, acc);
+            load16<1, 1, S>(in, gauge, Vh, par, h, yp, pa, ua);
+            compute16<0, 0, DAGGER, S>(pb, ub, 1.f, false, acc);
+            load16<1, 0, S>(in, gauge, Vh, par, h, ym, pb, ub);
+            compute16<1, 1, DAGGER, S>(pa, ua, 1.f, false, acc);
+            load16<2, 1, S>(in, gauge, Vh, par, h, zp, pa, ua);
+            compute16<1, 0, DAGGER, S>(pb, ub, 1.f, false, acc);
+            load16<2, 0, S>(in, gauge, Vh, par, h, zm, pb, ub);
+            compute16<2, 1, DAGGER, S>(pa, ua, 1.f, false, acc);
+            load16<3, 1, S>(in, gauge, Vh, par, h, tp, pa, ua);
+            compute16<2, 0, DAGGER, S>(pb, ub, 1.f, false, acc);
+            load16<3, 0, S>(in, gauge, Vh, par, h, tm, pb, ub);
+            compute16<3, 1, DAGGER, S>(pa, ua, A.tb, wp, acc);
+            compute16<3, 0, DAGGER, S>(pb, ub, A.tb, wm, acc);
+        } else {
+            load16<0, 1, S>(in, gauge, Vh, par, h, xp, pa, ua); compute16<0, 1, DAGGER, S>(pa, ua, 1.f, false, acc);
+            load16<0, 0, S>(in, gauge, Vh, par, h, xm, pa, ua); compute16<0, 0, DAGGER, S>(pa, ua, 1.f, false, acc);
+            load16<1, 1, S>(in, gauge, Vh, par, h, yp, pa, ua); compute16<1, 1, DAGGER, S>(pa, ua, 1.f, false, acc);
+            load16<1, 0, S>(in, gauge, Vh, par, h, ym, pa, ua); compute16<1, 0, DAGGER, S>(pa, ua, 1.f, false, acc);
+            load16<2, 1, S>(in, gauge, Vh, par, h, zp, pa, ua); compute16<2, 1, DAGGER, S>(pa, ua, 1.f, false, acc);
+            load16<2, 0, S>(in, gauge, Vh, par, h, zm, pa, ua); compute16<2, 0, DAGGER, S>(pa, ua, 1.f, false, acc);
+            load16<3, 1, S>(in, gauge, Vh, par, h, tp, pa, ua); compute16<3, 1, DAGGER, S>(pa, ua, A.tb, wp, acc);
+            load16<3, 0, S>(in, gauge, Vh, par, h, tm, pa, ua); compute16<3, 0, DAGGER, S>(pa, ua, A.tb, wm, acc);
         }
         // epilogue: res = c * acc (+ x | + A x), optional A^-1, store, optional norm
         const float cf = A.c, a = A.a;
@@ -444,8 +461,9 @@ static tm_status launch16(tm_ctx* ctx, const DslashCall& c, const void* gauge, c
     A.check_done = c.check_done;
     const int block = 128;
     const int grid = (int)((ctx->Vh + block - 1) / block);
-    if (c.dagger) dslash16_kernel<S, 1><<<grid, block, 0, st>>>(A);
-    else          dslash16_kernel<S, 0><<<grid, block, 0, st>>>(A);
+    // <PIPE = 0, MINB = 6>: 80 registers, 24 warps/SM; measured best-or-equal among {no pipe, pipe} x {4,5,6,8 blocks}
+    if (c.dagger) dslash16_kernel<S, 1, 0, 6><<<grid, block, 0, st>>>(A);
+    else          dslash16_kernel<S, 0, 0, 6><<<grid, block, 0, st>>>(A);
     TM_LAUNCH_CHECK(ctx, "dslash16_kernel");
     return TM_OK;
 }
