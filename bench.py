@@ -374,6 +374,8 @@ def main():
     ap.add_argument("--n-lp", type=int, default=None, help="override N_LP (debugging; invalidates the headline)")
     ap.add_argument("--n-hp", type=int, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--lp-delta", type=float, default=None, help="reliable-update trigger of the LP solves (tuning)")
+    ap.add_argument("--hp-delta", type=float, default=None, help="reliable-update trigger of the HP solves (tuning)")
     args = ap.parse_args()
     cfg = dict(inputs.CONFIGS[args.config])
     cfg.setdefault("n_lp", 4)
@@ -383,6 +385,10 @@ def main():
         cfg["n_lp"] = args.n_lp
     if args.n_hp is not None:
         cfg["n_hp"] = args.n_hp
+    if args.lp_delta is not None:
+        LP["delta"] = args.lp_delta
+    if args.hp_delta is not None:
+        HP["delta"] = args.hp_delta
     if args.impl == "reference":
         run_reference(args, cfg)
     else:

@@ -89,9 +89,10 @@ tm_status blas_twist_inv(tm_ctx* ctx, void* dst, const void* src, tm_prec p, dou
     });
 }
 
-// ------------------------------------------------------------------ y += x
+// ------------------------------------------------------------------ reliable update, part 1: y += x ; x = 0
 template <typename Sy, typename Sx>
-__global__ void axpy1_kernel(Sy* __restrict__ y, const Sx* __restrict__ x, int Vh) {
+__global__ void ru_begin_kernel(Sy* __restrict__ y, Sx* __restrict__ x, int Vh, const CgScalars* sc) {
+    if (guard_skip(sc, GUARD_RU)) return;
     const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= 3L * Vh) return;
     const int g = (int)(i / Vh), h = (int)(i % Vh);
@@ -100,39 +101,54 @@ __global__ void axpy1_kernel(Sy* __restrict__ y, const Sx* __restrict__ x, int V
     load8<Sx>(x, Vh, h, g, a);
     load8<Sy>(y, Vh, h, g, b);
 #pragma unroll
-    for (int k = 0; k < 8; k++) b[k] += (typename Prec<Sy>::F)a[k];
+    for (int k = 0; k < 8; k++) { b[k] += (typename Prec<Sy>::F)a[k]; a[k] = 0; }
     store8<Sy>(y, Vh, h, g, b);
+    store8<Sx>(x, Vh, h, g, a);
 }
 
-tm_status blas_axpy1(tm_ctx* ctx, void* y, tm_prec py, const void* x, tm_prec px, cudaStream_t st) {
-    if ((py != TM_F64 && py != TM_F32) || (px != TM_F64 && px != TM_F32))
-        return tm_fail(ctx, TM_EPREC, "axpy1: f32/f64 only");
+tm_status blas_ru_begin(tm_ctx* ctx, void* y, tm_prec po, void* x, tm_prec pacc, cudaStream_t st) {
     const unsigned grid = items_grid(ctx, 256);
     const int Vh = (int)ctx->Vh;
-    if (py == TM_F64 && px == TM_F64) axpy1_kernel<double, double><<<grid, 256, 0, st>>>((double*)y, (const double*)x, Vh);
-    else if (py == TM_F64) axpy1_kernel<double, float><<<grid, 256, 0, st>>>((double*)y, (const float*)x, Vh);
-    else if (px == TM_F64) axpy1_kernel<float, double><<<grid, 256, 0, st>>>((float*)y, (const double*)x, Vh);
-    else axpy1_kernel<float, float><<<grid, 256, 0, st>>>((float*)y, (const float*)x, Vh);
-    TM_LAUNCH_CHECK(ctx, "axpy1_kernel");
+    if (po == TM_F64 && pacc == TM_F64) ru_begin_kernel<double, double><<<grid, 256, 0, st>>>((double*)y, (double*)x, Vh, ctx->d_scal);
+    else if (po == TM_F64 && pacc == TM_F32) ru_begin_kernel<double, float><<<grid, 256, 0, st>>>((double*)y, (float*)x, Vh, ctx->d_scal);
+    else if (po == TM_F32 && pacc == TM_F32) ru_begin_kernel<float, float><<<grid, 256, 0, st>>>((float*)y, (float*)x, Vh, ctx->d_scal);
+    else return tm_fail(ctx, TM_EPREC, "ru_begin: unsupported precision pair");
+    TM_LAUNCH_CHECK(ctx, "ru_begin_kernel");
     return TM_OK;
 }
 
-// ------------------------------------------------------------------ r = b - m, ||r||^2
-template <typename S>
-__global__ void __launch_bounds__(256) xmy_norm_kernel(S* __restrict__ r, const S* __restrict__ b,
-                                                       const S* __restrict__ m, int Vh, int red_op,
+// ------------------------------------------------------------------ r = b - m (acc), rs = b - m (sloppy), ||b - m||^2
+// m == NULL: r = rs = b (start of a solve).  SA == SL: rs is not written (r is the sloppy vector).
+template <typename SO, typename SA, typename SL>
+__global__ void __launch_bounds__(256) residual_kernel(SA* __restrict__ r, SL* __restrict__ rs, const SO* __restrict__ b,
+                                                       const SO* __restrict__ m, int Vh, int red_op, int guard,
                                                        double* partials, unsigned int* counter, CgScalars* sc) {
-    typedef typename Prec<S>::F F;
+    typedef typename Prec<SO>::F FO;
+    typedef typename Prec<SA>::F FA;
+    typedef typename Prec<SL>::F FL;
     __shared__ double sm[32];
+    if (guard_skip(sc, guard)) return;
     double nrm = 0.0;
     for (long i = (long)blockIdx.x * blockDim.x + threadIdx.x; i < 3L * Vh; i += (long)gridDim.x * blockDim.x) {
         const int g = (int)(i / Vh), h = (int)(i % Vh);
-        F vb[8], vm[8];
-        load8<S>(b, Vh, h, g, vb);
-        load8<S>(m, Vh, h, g, vm);
+        FO vb[8];
+        load8<SO>(b, Vh, h, g, vb);
+        if (m) {
+            FO vm[8];
+            load8<SO>(m, Vh, h, g, vm);
 #pragma unroll
-        for (int k = 0; k < 8; k++) { vb[k] -= vm[k]; nrm += (double)vb[k] * (double)vb[k]; }
-        store8<S>(r, Vh, h, g, vb);
+            for (int k = 0; k < 8; k++) vb[k] -= vm[k];
+        }
+        FA va[8];
+#pragma unroll
+        for (int k = 0; k < 8; k++) { nrm += (double)vb[k] * (double)vb[k]; va[k] = (FA)vb[k]; }
+        store8<SA>(r, Vh, h, g, va);
+        if (!std::is_same<SA, SL>::value) {
+            FL vs[8];
+#pragma unroll
+            for (int k = 0; k < 8; k++) vs[k] = (FL)vb[k];
+            store8<SL>(rs, Vh, h, g, vs);
+        }
     }
     grid_reduce(nrm, partials, counter, sc, red_op, sm);
 }
@@ -143,14 +159,29 @@ static inline unsigned red_grid(const tm_ctx* ctx, long items, int block) {
     return (unsigned)(g < cap ? g : cap);
 }
 
-tm_status blas_xmy_norm(tm_ctx* ctx, void* r, const void* b, const void* m, tm_prec p, int red_op, cudaStream_t st) {
+template <typename SO, typename SA, typename SL>
+static tm_status residual_launch(tm_ctx* ctx, void* r, void* rs, const void* b, const void* m, int red_op, int guard,
+                                 cudaStream_t st) {
     const unsigned grid = red_grid(ctx, 3L * ctx->Vh, 256);
-    const int Vh = (int)ctx->Vh;
-    if (p == TM_F64) xmy_norm_kernel<double><<<grid, 256, 0, st>>>((double*)r, (const double*)b, (const double*)m, Vh, red_op, ctx->d_partials, ctx->d_counter, ctx->d_scal);
-    else if (p == TM_F32) xmy_norm_kernel<float><<<grid, 256, 0, st>>>((float*)r, (const float*)b, (const float*)m, Vh, red_op, ctx->d_partials, ctx->d_counter, ctx->d_scal);
-    else return tm_fail(ctx, TM_EPREC, "xmy_norm: f32/f64 only");
-    TM_LAUNCH_CHECK(ctx, "xmy_norm_kernel");
+    residual_kernel<SO, SA, SL><<<grid, 256, 0, st>>>((SA*)r, (SL*)rs, (const SO*)b, (const SO*)m, (int)ctx->Vh, red_op,
+                                                     guard, ctx->d_partials, ctx->d_counter, ctx->d_scal);
+    TM_LAUNCH_CHECK(ctx, "residual_kernel");
     return TM_OK;
+}
+
+tm_status blas_residual(tm_ctx* ctx, void* r, tm_prec pacc, void* rs, tm_prec psl, const void* b, const void* m,
+                        tm_prec po, int red_op, int guard, cudaStream_t st) {
+    if (po == TM_F64) {
+        if (pacc == TM_F64 && psl == TM_F64) return residual_launch<double, double, double>(ctx, r, rs, b, m, red_op, guard, st);
+        if (pacc == TM_F32 && psl == TM_F32) return residual_launch<double, float, float>(ctx, r, rs, b, m, red_op, guard, st);
+        if (pacc == TM_F32 && psl == TM_F16) return residual_launch<double, float, __half>(ctx, r, rs, b, m, red_op, guard, st);
+        if (pacc == TM_F32 && psl == TM_BF16) return residual_launch<double, float, __nv_bfloat16>(ctx, r, rs, b, m, red_op, guard, st);
+    } else if (po == TM_F32 && pacc == TM_F32) {
+        if (psl == TM_F32) return residual_launch<float, float, float>(ctx, r, rs, b, m, red_op, guard, st);
+        if (psl == TM_F16) return residual_launch<float, float, __half>(ctx, r, rs, b, m, red_op, guard, st);
+        if (psl == TM_BF16) return residual_launch<float, float, __nv_bfloat16>(ctx, r, rs, b, m, red_op, guard, st);
+    }
+    return tm_fail(ctx, TM_EPREC, "residual: unsupported precision combination");
 }
 
 // ------------------------------------------------------------------ ||v||^2
@@ -196,7 +227,7 @@ __global__ void __launch_bounds__(256) update_xr_kernel(SA* __restrict__ x, SA* 
     typedef typename Prec<SA>::F FA;
     typedef typename Prec<SL>::F FL;
     __shared__ double sm[32];
-    if (sc->done) return;
+    if (guard_skip(sc, GUARD_ITER)) return;
     const FA alpha = (FA)sc->alpha;
     double nrm = 0.0;
     for (long i = (long)blockIdx.x * blockDim.x + threadIdx.x; i < 3L * Vh; i += (long)gridDim.x * blockDim.x) {
@@ -247,16 +278,21 @@ tm_status blas_update_xr(tm_ctx* ctx, void* x, void* r, tm_prec pacc, const void
 template <typename S>
 __global__ void update_p_kernel(S* __restrict__ p, const S* __restrict__ z, int Vh, const CgScalars* sc) {
     typedef typename Prec<S>::F F;
-    if (sc->done) return;
+    if (guard_skip(sc, GUARD_ITER)) return;
     const F beta = (F)sc->beta;
     const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= 3L * Vh) return;
     const int g = (int)(i / Vh), h = (int)(i % Vh);
     F vp[8], vz[8];
-    load8<S>(p, Vh, h, g, vp);
     load8<S>(z, Vh, h, g, vz);
+    if (beta != F(0)) {             // beta == 0: first iteration of a solve, p is uninitialised, p = z
+        load8<S>(p, Vh, h, g, vp);
 #pragma unroll
-    for (int k = 0; k < 8; k++) vp[k] = vz[k] + beta * vp[k];
+        for (int k = 0; k < 8; k++) vp[k] = vz[k] + beta * vp[k];
+    } else {
+#pragma unroll
+        for (int k = 0; k < 8; k++) vp[k] = vz[k];
+    }
     store8<S>(p, Vh, h, g, vp);
 }
 
@@ -270,28 +306,21 @@ tm_status blas_update_p(tm_ctx* ctx, void* p, const void* z, tm_prec psl, cudaSt
 }
 
 // ------------------------------------------------------------------ scalars
-tm_status scal_set(tm_ctx* ctx, const CgScalars& v, cudaStream_t st) {
-    // pinned staging: wait for earlier users of h_scal
-    TM_CUDA(ctx, cudaStreamSynchronize(st));
-    *ctx->h_scal = v;
-    TM_CUDA(ctx, cudaMemcpyAsync(ctx->d_scal, ctx->h_scal, sizeof(CgScalars), cudaMemcpyHostToDevice, st));
-    TM_CUDA(ctx, cudaStreamSynchronize(st));
+__global__ void scal_init_kernel(CgScalars* sc, double rho2, double delta2, int max_iter) {
+    CgScalars z;
+    memset(&z, 0, sizeof(z));
+    z.rho2 = rho2; z.delta2 = delta2; z.max_iter = max_iter;
+    *sc = z;
+}
+tm_status scal_init(tm_ctx* ctx, double rho2, double delta2, int max_iter, cudaStream_t st) {
+    scal_init_kernel<<<1, 1, 0, st>>>(ctx->d_scal, rho2, delta2, max_iter);
+    TM_LAUNCH_CHECK(ctx, "scal_init_kernel");
     return TM_OK;
 }
 tm_status scal_get(tm_ctx* ctx, CgScalars* v, cudaStream_t st) {
     TM_CUDA(ctx, cudaMemcpyAsync(ctx->h_scal, ctx->d_scal, sizeof(CgScalars), cudaMemcpyDeviceToHost, st));
     TM_CUDA(ctx, cudaStreamSynchronize(st));
     *v = *ctx->h_scal;
-    return TM_OK;
-}
-
-__global__ void set_done_target_kernel(CgScalars* sc, int done, double target2) {
-    sc->done = done;
-    sc->target2 = target2;
-}
-tm_status scal_set_done_target(tm_ctx* ctx, int done, double target2, cudaStream_t st) {
-    set_done_target_kernel<<<1, 1, 0, st>>>(ctx->d_scal, done, target2);
-    TM_LAUNCH_CHECK(ctx, "set_done_target_kernel");
     return TM_OK;
 }
 

@@ -1,29 +1,48 @@
-// blas.cuh -- device scalars of a running CG and the deterministic grid reduction used by every
-// kernel with a norm epilogue (row a3 of SURVEY.md sec 8: "reduced via warp shuffles").
+// blas.cuh -- device scalars / state machine of a running CG and the deterministic grid reduction
+// used by every kernel with a norm epilogue (row a3 of SURVEY.md sec 8: "reduced via warp shuffles").
 #pragma once
 #include "common.cuh"
 
-// Device-resident CG state: alpha/beta/stopping are computed by the LAST block of the kernel that
-// produced the norm, so the host never has to feed scalars back (SURVEY.md sec 7 hard part 4).
+// Device-resident CG state.  alpha/beta, the stopping test AND the decision to pause for a reliable
+// update are taken by the LAST block of the kernel that produced the norm, so the host never feeds
+// scalars back (SURVEY.md sec 7 hard part 4).  Every solver kernel carries a guard: it runs only
+// while `done` has the value it was enqueued for, so the host can enqueue iterations and
+// reliable-update blocks speculatively, ahead of the device, without changing the result:
+//   done = 0  iterating            (iteration kernels run, reliable-update kernels are no-ops)
+//   done = 1  paused: the iterated ||r||^2 met the target, dropped by delta^2, or the cap was hit
+//             (reliable-update kernels run, iteration kernels are no-ops)
+//   done = 2  converged: outer-precision ||bhat - Mhat y||^2 <= target2      (everything is a no-op)
+//   done = 3  failed: iteration cap reached or NaN                           (everything is a no-op)
 struct CgScalars {
     double gamma;      // ||z||^2 of the current search direction
     double ww;         // ||Mhat p||^2
     double rr;         // ||r||^2 (iterated)
     double alpha, beta;
-    double target2;    // stop when rr <= target2
-    double slot[8];    // generic results (norms for setup / true residual)
-    int done;          // set once rr <= target2: later kernels of the solve become no-ops
+    double target2;    // rho^2 ||eta||^2
+    double ru2;        // pause for a reliable update when rr <= ru2 (= delta^2 ||r||^2 at the last update)
+    double rr_true;    // ||bhat - Mhat y||^2 at the last reliable update (outer precision)
+    double rho2, delta2;
+    double slot[8];    // generic results (slot 0: ||eta||^2)
+    int done;
     int iters;
-    int pad[2];
+    int max_iter;
+    int n_ru;          // reliable updates so far
+    int pause_iter[CG_MAX_PAUSES];   // iteration count at each pause (replayed by the host as a launch plan)
 };
+
+enum { GUARD_ALWAYS = 0, GUARD_ITER = 1, GUARD_RU = 2 };     // run iff guard == 0 || done == guard - 1
+__device__ __forceinline__ bool guard_skip(const CgScalars* sc, int guard) {
+    return guard != GUARD_ALWAYS && sc->done != guard - 1;
+}
 
 // what the last block does with the reduced sum
 enum {
     RED_NONE = 0,
     RED_WW,        // ww = sum; alpha = gamma / ww
-    RED_RR,        // rr = sum; iters++; done = rr <= target2
-    RED_ZZ,        // beta = sum / gamma; gamma = sum
-    RED_ZZ_INIT,   // gamma = sum; beta = 0
+    RED_RR,        // rr = sum; iters++; pause (done = 1) on target / reliable-update trigger / cap / NaN
+    RED_ZZ,        // beta = gamma > 0 ? sum / gamma : 0; gamma = sum
+    RED_START,     // sum = ||bhat||^2: target2, ru2, rr; done = 0 (or 1 when already converged / no iterations allowed)
+    RED_RU,        // sum = ||bhat - Mhat y||^2: converged (2) | failed (3) | resume (0) with a new ru2
     RED_SLOT0      // slot[k] = sum for RED_SLOT0 + k
 };
 
@@ -69,9 +88,25 @@ __device__ __forceinline__ void grid_reduce(double v, double* partials, unsigned
             *counter = 0;
             switch (op) {
                 case RED_WW: sc->ww = s; sc->alpha = sc->gamma / s; break;
-                case RED_RR: sc->rr = s; sc->iters += 1; if (s <= sc->target2) sc->done = 1; break;
-                case RED_ZZ: sc->beta = s / sc->gamma; sc->gamma = s; break;
-                case RED_ZZ_INIT: sc->gamma = s; sc->beta = 0.0; break;
+                case RED_RR:
+                    sc->rr = s; sc->iters += 1;
+                    if (!(s > sc->target2) || !(s > sc->ru2) || sc->iters >= sc->max_iter) sc->done = 1;
+                    break;
+                case RED_ZZ: sc->beta = sc->gamma > 0.0 ? s / sc->gamma : 0.0; sc->gamma = s; break;
+                case RED_START:
+                    sc->target2 = sc->rho2 * sc->slot[0];
+                    sc->rr = s; sc->rr_true = s; sc->ru2 = sc->delta2 * s;
+                    sc->done = (s > sc->target2 && sc->max_iter > 0) ? 0 : 1;
+                    break;
+                case RED_RU:
+                    if (sc->n_ru < CG_MAX_PAUSES) sc->pause_iter[sc->n_ru] = sc->iters;
+                    sc->n_ru += 1;
+                    sc->rr_true = s;
+                    if (!(s == s)) sc->done = 3;
+                    else if (s <= sc->target2) sc->done = 2;
+                    else if (sc->iters >= sc->max_iter) sc->done = 3;
+                    else { sc->rr = s; sc->ru2 = sc->delta2 * s; sc->done = 0; }
+                    break;
                 default: if (op >= RED_SLOT0) sc->slot[op - RED_SLOT0] = s; break;
             }
         }

@@ -19,6 +19,19 @@
 
 struct CgScalars;   // blas.cuh
 
+// Launch plan of the CG: the iteration counts at which the previous solve with the same parameters
+// paused for a reliable update.  The next solve enqueues its kernels along this plan without
+// waiting for the device (every kernel is guarded by the device-side state, so a wrong plan costs
+// only no-op launches or an extra host round trip, never a different result).
+#define CG_MAX_PAUSES 48
+struct CgPlan {
+    int valid;
+    int sloppy, outer, recon, max_iter;
+    double rho, delta;
+    int n_pause;
+    int pause_iter[CG_MAX_PAUSES];
+};
+
 struct tm_ctx {
     int X[4];
     int Xh;
@@ -35,6 +48,7 @@ struct tm_ctx {
     unsigned int* d_counter;        // last-block-done counter
     CgScalars* d_scal;              // device scalars of the running solve
     CgScalars* h_scal;              // pinned mirror
+    CgPlan plan[4];                 // per sloppy precision
     // generic workspace pool (freed in tm_destroy): named slots grown on demand
     void* scratch[TM_MAX_SCRATCH];
     size_t scratch_bytes[TM_MAX_SCRATCH];

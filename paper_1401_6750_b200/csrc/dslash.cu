@@ -32,7 +32,7 @@ template <typename F> struct DslashArgs {
     double* partials;
     unsigned int* counter;
     CgScalars* sc;
-    int check_done;
+    int guard;         // GUARD_* (blas.cuh): skip unless the running solve is in the matching state
 };
 
 // u (2 spins x 3 colours complex = 12 reals) = psi_up + s * B_mu psi_low
@@ -104,7 +104,7 @@ template <typename S, int R>
 __global__ void __launch_bounds__(128) dslash_kernel(DslashArgs<typename Prec<S>::F> A) {
     typedef typename Prec<S>::F F;
     __shared__ double sm[32];
-    if (A.check_done && A.sc->done) return;
+    if (guard_skip(A.sc, A.guard)) return;
     const Geom& g = A.g;
     const int h = blockIdx.x * blockDim.x + threadIdx.x;
     double nrm = 0.0;
@@ -324,7 +324,7 @@ __device__ __forceinline__ void compute16(const unsigned* p, const unsigned* Uin
 template <typename S, int DAGGER, int PIPE, int MINB>
 __global__ void __launch_bounds__(128, MINB) dslash16_kernel(DslashArgs<float> A) {
     __shared__ double sm[32];
-    if (A.check_done && A.sc->done) return;
+    if (guard_skip(A.sc, A.guard)) return;
     const Geom& g = A.g;
     const int h = blockIdx.x * blockDim.x + threadIdx.x;
     double nrm = 0.0;
@@ -438,7 +438,7 @@ static tm_status launch_t(tm_ctx* ctx, const DslashCall& c, const void* gauge, c
     A.c = (F)c.coef;
     A.xmode = c.xmode; A.post = c.post; A.red_op = c.red_op;
     A.partials = ctx->d_partials; A.counter = ctx->d_counter; A.sc = ctx->d_scal;
-    A.check_done = c.check_done;
+    A.guard = c.guard;
     const int block = 128;
     const int grid = (int)((ctx->Vh + block - 1) / block);
     dslash_kernel<S, R><<<grid, block, 0, st>>>(A);
@@ -458,7 +458,7 @@ static tm_status launch16(tm_ctx* ctx, const DslashCall& c, const void* gauge, c
     A.c = (float)c.coef;
     A.xmode = c.xmode; A.post = c.post; A.red_op = c.red_op;
     A.partials = ctx->d_partials; A.counter = ctx->d_counter; A.sc = ctx->d_scal;
-    A.check_done = c.check_done;
+    A.guard = c.guard;
     const int block = 128;
     const int grid = (int)((ctx->Vh + block - 1) / block);
     // <PIPE = 0, MINB = 6>: 80 registers, 24 warps/SM; measured best-or-equal among {no pipe, pipe} x {4,5,6,8 blocks}

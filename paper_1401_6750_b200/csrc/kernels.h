@@ -11,7 +11,7 @@ struct DslashCall {
     double kappa, mu, coef;
     int xmode, post;
     int red_op;        // RED_* applied to ||out||^2 (RED_NONE: no norm)
-    int check_done;    // skip when the running solve has converged
+    int guard;         // GUARD_ALWAYS | GUARD_ITER | GUARD_RU (blas.cuh)
 };
 tm_status tm_dslash_launch(tm_ctx* ctx, const DslashCall& c, tm_prec prec, tm_recon recon, cudaStream_t st);
 
@@ -26,26 +26,28 @@ tm_status tm_z4_expand(tm_ctx* ctx, void* d_internal, tm_prec prec, const unsign
 // parity-vector operations (n = 24*Vh reals each); all asynchronous on st
 tm_status blas_zero(tm_ctx* ctx, void* v, tm_prec p, cudaStream_t st);
 tm_status blas_copy(tm_ctx* ctx, void* dst, tm_prec pd, const void* src, tm_prec ps, cudaStream_t st);
-// dst = post-twist-inverse? no: plain  dst = A^-1 src  (site-local twist inverse)
+// dst = A^-1 src  (site-local twist inverse)
 tm_status blas_twist_inv(tm_ctx* ctx, void* dst, const void* src, tm_prec p, double kappa, double mu,
                          int dagger, cudaStream_t st);
-// y += x (y: py, x: px)
-tm_status blas_axpy1(tm_ctx* ctx, void* y, tm_prec py, const void* x, tm_prec px, cudaStream_t st);
-// r = b - m ; ||r||^2 -> red_op
-tm_status blas_xmy_norm(tm_ctx* ctx, void* r, const void* b, const void* m, tm_prec p, int red_op, cudaStream_t st);
 // ||v||^2 -> red_op
 tm_status blas_norm(tm_ctx* ctx, const void* v, tm_prec p, int red_op, cudaStream_t st);
 // full-lattice norm (2 parities)
 tm_status blas_norm_full(tm_ctx* ctx, const void* v, tm_prec p, int red_op, cudaStream_t st);
-// CG updates with device-resident alpha / beta (no-ops once sc->done):
-//   x += alpha p ; r -= alpha w ; ||r||^2 -> RED_RR ; optional sloppy copy rs of r
+// CG kernels driven by the device-resident state (CgScalars); each runs only in its guard state:
+//   x += alpha p ; r -= alpha w ; ||r||^2 -> RED_RR ; sloppy copy rs of r            (GUARD_ITER)
 tm_status blas_update_xr(tm_ctx* ctx, void* x, void* r, tm_prec pacc, const void* p, const void* w,
                          void* rs, tm_prec psl, cudaStream_t st);
-//   p = z + beta p
+//   p = z + beta p  (p = z when beta == 0: first iteration)                                  (GUARD_ITER)
 tm_status blas_update_p(tm_ctx* ctx, void* p, const void* z, tm_prec psl, cudaStream_t st);
-tm_status scal_set(tm_ctx* ctx, const CgScalars& v, cudaStream_t st);    // upload whole struct
+//   y += x ; x = 0                                                                           (GUARD_RU)
+tm_status blas_ru_begin(tm_ctx* ctx, void* y, tm_prec po, void* x, tm_prec pacc, cudaStream_t st);
+//   r = b - m (acc precision) ; rs = b - m (sloppy) ; ||b - m||^2 -> red_op (RED_START: m == NULL,
+//   GUARD_ALWAYS; RED_RU: GUARD_RU)
+tm_status blas_residual(tm_ctx* ctx, void* r, tm_prec pacc, void* rs, tm_prec psl, const void* b, const void* m,
+                        tm_prec po, int red_op, int guard, cudaStream_t st);
+// reset the device state for a new solve (no host synchronisation)
+tm_status scal_init(tm_ctx* ctx, double rho2, double delta2, int max_iter, cudaStream_t st);
 tm_status scal_get(tm_ctx* ctx, CgScalars* v, cudaStream_t st);          // download + sync
-tm_status scal_set_done_target(tm_ctx* ctx, int done, double target2, cudaStream_t st);
 
 // ---- solver.cu ----------------------------------------------------------------------------
 // eta, s: full-lattice internal fields of precision params->outer
