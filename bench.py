@@ -33,8 +33,8 @@ sys.path.insert(0, ROOT)
 
 from paper_1401_6750_b200 import inputs  # noqa: E402
 
-LP = dict(sloppy="f16", outer="f32", recon=12, rho=1e-2, max_iter=2000, delta=0.1)
-HP = dict(sloppy="f32", outer="f64", recon=12, rho=1e-8, max_iter=5000, delta=0.1)
+LP = dict(sloppy="f16", outer="f32", recon=12, rho=1e-2, max_iter=2000, delta=0.01)
+HP = dict(sloppy="f32", outer="f64", recon=12, rho=1e-8, max_iter=5000, delta=0.01)
 
 
 def peaks():

@@ -16,17 +16,20 @@
 //     l_{1,n} = sum_a ph_n(a) g5(perm_n(a)) C_{eta,d}[a][perm_n(a)] - 2 i kappa mu l_{0,n}
 // (g = g5 eta - 2 i kappa mu s, reading 5), times 1/2 for the derivative insertions.
 //
-// Kernel 1 thread roles (320 threads = 10 warps per CTA):
-//   phase A: warp g = fam*5 + d, lane = x: computes the 32 reals of C_{fam,d}(x) -> shared memory
-//   phase B: thread jr = one of the 320 real components: x-sum with 7 real weights, then the y-stage
-//            update of its NQ register accumulators Q[(m,n),(cos|sin)x,(cos|sin)y].
+// Kernel 1 is warp-specialised (see contract_xy_kernel): producer warps (lane = x) compute the 16
+// complex numbers of C_{fam,d}(x) into a shared-memory ring of row buffers, consumer warps (thread =
+// one complex component) do the x-sum with 7 real weights and the y-stage update of their NQ register
+// accumulators Q[(m,n),(cos|sin)x,(cos|sin)y].
 #include <math.h>
 #include <complex>
 #include <vector>
 #include "kernels.h"
 #include "su3.cuh"
 
-#define CT_THREADS 320
+#define CT_THREADS 320          // real components per site: 10 (fam, d) x 16 complex x 2
+#define CT_NCC 160              // complex components per site
+#define CT_NC 5                 // consumer warps: one thread per complex component
+#define CT_BSC 34               // row-buffer stride in complex numbers (32 x-values + 2 pad: conflict-free 16-byte reads)
 
 template <int PRUNE> struct QLayout { static constexpr int NQ = PRUNE ? 29 : 49; };
 
@@ -41,157 +44,263 @@ struct ContractArgs {
     double tb;
 };
 
-template <typename F> struct BufStride;
-template <> struct BufStride<float>  { static constexpr int V = 36; };
-template <> struct BufStride<double> { static constexpr int V = 34; };
-
-// full 4-spin SU(3) multiply
-template <int DAG, typename F>
-__device__ __forceinline__ void su3_mul_full(const F* U, const F* in, F* out) {
-    su3_mul_half<DAG>(U, in, out);
-    su3_mul_half<DAG>(U, in + 12, out + 12);
+// ---- pair arithmetic: one complex number (re, im) per pair.  fp32 pairs live in one 64-bit register
+// and use Blackwell's packed FFMA2 / FADD2 (PTX fma.rn.f32x2): one issue slot per complex FMA with a
+// broadcast real scalar; ptxas folds the (re, im) swap into the operand swizzle.
+template <typename F> struct P2;
+template <> struct P2<float> {
+    typedef unsigned long long T;
+    static __device__ __forceinline__ T make(float re, float im) { T r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(re), "f"(im)); return r; }
+    static __device__ __forceinline__ void get(T v, float& re, float& im) { asm("mov.b64 {%0, %1}, %2;" : "=f"(re), "=f"(im) : "l"(v)); }
+    static __device__ __forceinline__ T fma_s(float s, T b, T c) {      // c + s * b
+        T d; const T ss = make(s, s);
+        asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(ss), "l"(b), "l"(c));
+        return d;
+    }
+    static __device__ __forceinline__ T add(T a, T b) { T d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+    static __device__ __forceinline__ T mul_s(float s, T b) { T d; const T ss = make(s, s); asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(ss), "l"(b)); return d; }
+};
+template <> struct P2<double> {
+    typedef double2 T;
+    static __device__ __forceinline__ T make(double re, double im) { return make_double2(re, im); }
+    static __device__ __forceinline__ void get(T v, double& re, double& im) { re = v.x; im = v.y; }
+    static __device__ __forceinline__ T fma_s(double s, T b, T c) { return make_double2(fma(s, b.x, c.x), fma(s, b.y, c.y)); }
+    static __device__ __forceinline__ T add(T a, T b) { return make_double2(a.x + b.x, a.y + b.y); }
+    static __device__ __forceinline__ T mul_s(double s, T b) { return make_double2(s * b.x, s * b.y); }
+};
+// i * v = (-im, re)
+template <typename F> __device__ __forceinline__ typename P2<F>::T times_i(typename P2<F>::T v) {
+    F re, im;
+    P2<F>::get(v, re, im);
+    return P2<F>::make(-im, re);
 }
 
-template <typename S, int R, int PRUNE, int NBUF>
-__global__ void __launch_bounds__(CT_THREADS) contract_xy_kernel(ContractArgs A) {
+// out[sp][a] (+|-)= sum_b U[a][b] in[sp][b]  (DAG: U^dag), 4 spins x 3 colours as 12 pairs; NEG subtracts
+template <int DAG, int NEG, typename F>
+__device__ __forceinline__ void su3_macc(const F* U, const typename P2<F>::T* in, typename P2<F>::T* out) {
+    typedef typename P2<F>::T T;
+#pragma unroll
+    for (int sp = 0; sp < 4; sp++) {
+        T ib[3];
+#pragma unroll
+        for (int b = 0; b < 3; b++) ib[b] = times_i<F>(in[sp * 3 + b]);
+#pragma unroll
+        for (int a = 0; a < 3; a++) {
+            T acc = out[sp * 3 + a];
+#pragma unroll
+            for (int b = 0; b < 3; b++) {
+                F ur = DAG ? U[(b * 3 + a) * 2] : U[(a * 3 + b) * 2];
+                F ui = DAG ? -U[(b * 3 + a) * 2 + 1] : U[(a * 3 + b) * 2 + 1];
+                if (NEG) { ur = -ur; ui = -ui; }
+                acc = P2<F>::fma_s(ur, in[sp * 3 + b], acc);       // (ur + i ui) * in = ur * in + ui * (i in)
+                acc = P2<F>::fma_s(ui, ib[b], acc);
+            }
+            out[sp * 3 + a] = acc;
+        }
+    }
+}
+
+template <typename S>
+__device__ __forceinline__ void load_spinor_pairs(const S* f, size_t Vh, size_t h, typename P2<S>::T* v) {
+    S t[24];
+    load_spinor<S>(f, Vh, h, t);
+#pragma unroll
+    for (int i = 0; i < 12; i++) v[i] = P2<S>::make(t[2 * i], t[2 * i + 1]);
+}
+
+__device__ __forceinline__ void named_bar_sync(int id, int count) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory"); }
+__device__ __forceinline__ void named_bar_arrive(int id, int count) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(count) : "memory"); }
+
+// C[a][b] = sum_c conj(s_ac) psi_bc for the (fam, d) slot `slot` of site column `lane` -> row buffer
+template <typename F>
+__device__ __forceinline__ void outer_store(const typename P2<F>::T* sv, const typename P2<F>::T* psi,
+                                            typename P2<F>::T* rowbuf, int slot, int lane) {
+    typedef typename P2<F>::T T;
+    F sre[12], sim[12];
+#pragma unroll
+    for (int i = 0; i < 12; i++) { P2<F>::get(sv[i], sre[i], sim[i]); sim[i] = -sim[i]; }
+    T* out = rowbuf + (size_t)(slot * 16) * CT_BSC + lane;
+#pragma unroll
+    for (int bb = 0; bb < 4; bb++) {
+        T ip[3];
+#pragma unroll
+        for (int c = 0; c < 3; c++) ip[c] = times_i<F>(psi[bb * 3 + c]);
+#pragma unroll
+        for (int a = 0; a < 4; a++) {
+            T acc = P2<F>::make(0, 0);
+#pragma unroll
+            for (int c = 0; c < 3; c++) {       // conj(s) psi = s.re * psi - s.im * (i psi)
+                acc = P2<F>::fma_s(sre[a * 3 + c], psi[bb * 3 + c], acc);
+                acc = P2<F>::fma_s(sim[a * 3 + c], ip[c], acc);
+            }
+            out[(size_t)(a * 4 + bb) * CT_BSC] = acc;
+        }
+    }
+}
+
+// Warp-specialised CTA, one (z,t) plane per CTA:
+//   NP producer warps (lane = x): jobs (fam, d) of one row chunk -> psi_{fam,d}(x), colour-traced outer
+//     product with s(x) -> row buffer (NS-stage ring in shared memory)
+//   CT_NC consumer warps (thread = complex component): x-sum of the row buffer with the 7 real weights,
+//     y-stage update of the NQ register accumulators; written to qbuf at the end of the plane.
+// Producers never hold the Q accumulators and consumers never hold spinors, so neither role pays the
+// other's registers; the ring lets the global loads of row y+1 overlap the DFT of row y.
+template <typename S, int R, int PRUNE, int NP, int NS>
+__global__ void __launch_bounds__((NP + CT_NC) * 32, 1) contract_xy_kernel(ContractArgs A) {
     typedef S F;
-    constexpr int BS = BufStride<F>::V;
+    typedef typename P2<F>::T T;
     constexpr int NQ = QLayout<PRUNE>::NQ;
+    constexpr int NTHREADS = (NP + CT_NC) * 32;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    F* buf = reinterpret_cast<F*>(smem_raw);                 // [NBUF][320][BS]
-    F* swx = buf + (size_t)NBUF * CT_THREADS * BS;           // [Lx][8]
-    F* swy = swx + (size_t)A.g.X0 * 8;                       // [Ly][8]
+    T* buf = reinterpret_cast<T*>(smem_raw);                     // [NS][160][CT_BSC]
+    F* swx = reinterpret_cast<F*>(buf + (size_t)NS * CT_NCC * CT_BSC);   // [Lx][8]
+    F* swy = swx + (size_t)A.g.X0 * 8;                           // [Ly][8]
     const Geom& g = A.g;
     const int zt = blockIdx.x;
     const int z = zt % g.X2, t = zt / g.X2;
-    const int lane = threadIdx.x & 31, grp = threadIdx.x >> 5;
-    const int fam = grp / 5, d = grp % 5;
-    const int jr = threadIdx.x;
-    for (int i = threadIdx.x; i < g.X0 * 8; i += CT_THREADS) swx[i] = ((const F*)A.wx)[i];
-    for (int i = threadIdx.x; i < g.X1 * 8; i += CT_THREADS) swy[i] = ((const F*)A.wy)[i];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int i = threadIdx.x; i < g.X0 * 8; i += NTHREADS) swx[i] = ((const F*)A.wx)[i];
+    for (int i = threadIdx.x; i < g.X1 * 8; i += NTHREADS) swy[i] = ((const F*)A.wy)[i];
     __syncthreads();
 
-    const S* sfield = (const S*)A.s;
-    const S* pfield = fam ? (const S*)A.eta : (const S*)A.s;
-    const S* gauge = (const S*)A.gauge;
-    const size_t Vh = g.Vh;
-    const size_t pblk = Vh * 24;
-
-    F Q[NQ];
-#pragma unroll
-    for (int q = 0; q < NQ; q++) Q[q] = 0;
-    int b = 0;
     const int nxc = (g.X0 + 31) / 32;
-    for (int y = 0; y < g.X1; y++) {
-        F xc_[4], xs_[4];
-#pragma unroll
-        for (int m = 0; m < 4; m++) { xc_[m] = 0; xs_[m] = 0; }
-        for (int xc = 0; xc < nxc; xc++) {
+    const int niter = g.X1 * nxc;
+    // barrier ids: full[st] = 1 + st, empty[st] = 1 + NS + st
+    if (warp < NP) {
+        // ================================================================ producers
+        const S* sfield = (const S*)A.s;
+        const S* efield = (const S*)A.eta;
+        const S* gauge = (const S*)A.gauge;
+        const size_t Vh = g.Vh;
+        const size_t pblk = Vh * 24;
+        for (int it = 0; it < niter; it++) {
+            const int st = it % NS;
+            const int y = it / nxc, xc = it - y * nxc;
             const int x = xc * 32 + lane;
-            F* mybuf = buf + (size_t)b * CT_THREADS * BS;
-            // ---------------------------------------------------------------- phase A
+            T* rowbuf = buf + (size_t)st * CT_NCC * CT_BSC;
+            if (it >= NS) named_bar_sync(1 + NS + st, NTHREADS);
             if (x < g.X0) {
                 const int par = (x + y + z + t) & 1;
                 const int row = ((t * g.X2 + z) * g.X1 + y) * g.X0;      // lex index of x = 0
                 const size_t h = (size_t)(row + x) >> 1;
-                F sv[24], psi[24];
-                load_spinor<S>(sfield + par * pblk, Vh, h, sv);
-                if (d == 0) {
-                    if (fam) load_spinor<S>(pfield + par * pblk, Vh, h, psi);
-                    else {
-#pragma unroll
-                        for (int i = 0; i < 24; i++) psi[i] = sv[i];
-                    }
-                } else {
-                    const int mu = d - 1;
-                    // neighbour lex indices and boundary signs
+                T sv[12];
+                load_spinor_pairs<S>(sfield + par * pblk, Vh, h, sv);
+                // ---- heavy jobs: derivative directions
+#pragma unroll 1
+                for (int job = warp; job < 8; job += NP) {
+                    const int fam = job >> 2, mu = job & 3;
+                    const S* pfield = fam ? efield : sfield;
                     int lf, lb;
-                    F sf = 1, sb = 1;
+                    bool wf = false, wb = false;
                     if (mu == 0) {
                         lf = row + (x + 1 == g.X0 ? 0 : x + 1);
                         lb = row + (x == 0 ? g.X0 - 1 : x - 1);
                     } else if (mu == 1) {
-                        const int st = g.X0;
-                        lf = (y + 1 == g.X1) ? row + x - (g.X1 - 1) * st : row + x + st;
-                        lb = (y == 0) ? row + x + (g.X1 - 1) * st : row + x - st;
+                        const int sd = g.X0;
+                        lf = (y + 1 == g.X1) ? row + x - (g.X1 - 1) * sd : row + x + sd;
+                        lb = (y == 0) ? row + x + (g.X1 - 1) * sd : row + x - sd;
                     } else if (mu == 2) {
-                        const int st = g.X0 * g.X1;
-                        lf = (z + 1 == g.X2) ? row + x - (g.X2 - 1) * st : row + x + st;
-                        lb = (z == 0) ? row + x + (g.X2 - 1) * st : row + x - st;
+                        const int sd = g.X0 * g.X1;
+                        lf = (z + 1 == g.X2) ? row + x - (g.X2 - 1) * sd : row + x + sd;
+                        lb = (z == 0) ? row + x + (g.X2 - 1) * sd : row + x - sd;
                     } else {
-                        const int st = g.X0 * g.X1 * g.X2;
-                        if (t + 1 == g.X3) { lf = row + x - (g.X3 - 1) * st; sf = (F)A.tb; } else lf = row + x + st;
-                        if (t == 0) { lb = row + x + (g.X3 - 1) * st; sb = (F)A.tb; } else lb = row + x - st;
+                        const int sd = g.X0 * g.X1 * g.X2;
+                        if (t + 1 == g.X3) { lf = row + x - (g.X3 - 1) * sd; wf = true; } else lf = row + x + sd;
+                        if (t == 0) { lb = row + x + (g.X3 - 1) * sd; wb = true; } else lb = row + x - sd;
                     }
                     const size_t hf = (size_t)lf >> 1, hb = (size_t)lb >> 1;
-                    F nb[24], U[18], tmp[24];
-                    load_spinor<S>(pfield + (1 - par) * pblk, Vh, hf, nb);
+                    T nb[12], psi[12];
+                    F U[18];
+#pragma unroll
+                    for (int i = 0; i < 12; i++) psi[i] = P2<F>::make(0, 0);
+                    load_spinor_pairs<S>(pfield + (1 - par) * pblk, Vh, hf, nb);
                     load_link<S, R, LD_DEFAULT>(gauge, Vh, par, mu, h, U);
-                    su3_mul_full<0>(U, nb, psi);
-                    load_spinor<S>(pfield + (1 - par) * pblk, Vh, hb, nb);
+                    if (wf) {
+#pragma unroll
+                        for (int i = 0; i < 12; i++) nb[i] = P2<F>::mul_s((F)A.tb, nb[i]);
+                    }
+                    su3_macc<0, 0, F>(U, nb, psi);
+                    load_spinor_pairs<S>(pfield + (1 - par) * pblk, Vh, hb, nb);
                     load_link<S, R, LD_DEFAULT>(gauge, Vh, 1 - par, mu, hb, U);
-                    su3_mul_full<1>(U, nb, tmp);
+                    if (wb) {
 #pragma unroll
-                    for (int i = 0; i < 24; i++) psi[i] = sf * psi[i] - sb * tmp[i];
+                        for (int i = 0; i < 12; i++) nb[i] = P2<F>::mul_s((F)A.tb, nb[i]);
+                    }
+                    su3_macc<1, 1, F>(U, nb, psi);
+                    outer_store<F>(sv, psi, rowbuf, fam * 5 + 1 + mu, lane);
                 }
-                // C[a][b] = sum_c conj(s_ac) psi_bc
-                F* out = mybuf + (size_t)(grp * 32) * BS + lane;
+                // ---- light jobs (d = 0), rotated over the producer warps
+                const int lw = (2 * it) % NP;
+                if (warp == lw) outer_store<F>(sv, sv, rowbuf, 0, lane);
+                if (warp == (lw + 1) % NP) {
+                    T ev[12];
+                    load_spinor_pairs<S>(efield + par * pblk, Vh, h, ev);
+                    outer_store<F>(sv, ev, rowbuf, 5, lane);
+                }
+            }
+            __syncwarp();
+            named_bar_arrive(1 + st, NTHREADS);
+        }
+    } else {
+        // ================================================================ consumers
+        const int cc = threadIdx.x - NP * 32;        // 0..159
+        T Q[NQ];
 #pragma unroll
-                for (int a = 0; a < 4; a++)
+        for (int q = 0; q < NQ; q++) Q[q] = P2<F>::make(0, 0);
+        T a0 = P2<F>::make(0, 0), ac[3], as[3];
 #pragma unroll
-                    for (int bb = 0; bb < 4; bb++) {
-                        F re = 0, im = 0;
+        for (int m = 0; m < 3; m++) { ac[m] = P2<F>::make(0, 0); as[m] = P2<F>::make(0, 0); }
+        for (int it = 0; it < niter; it++) {
+            const int st = it % NS;
+            const int y = it / nxc, xc = it - y * nxc;
+            const T* v = buf + ((size_t)st * CT_NCC + cc) * CT_BSC;
+            const F* w = swx + (size_t)xc * 32 * 8;
+            const int nvalid = min(32, g.X0 - xc * 32);
+            named_bar_sync(1 + st, NTHREADS);
+#pragma unroll 4
+            for (int l = 0; l < nvalid; l++) {
+                const T val = v[l];
+                const F* wl = w + l * 8;
+                a0 = P2<F>::add(a0, val);
 #pragma unroll
-                        for (int c = 0; c < 3; c++) {
-                            const F sr = sv[(a * 3 + c) * 2], si = sv[(a * 3 + c) * 2 + 1];
-                            const F pr = psi[(bb * 3 + c) * 2], pi = psi[(bb * 3 + c) * 2 + 1];
-                            re += sr * pr + si * pi;
-                            im += sr * pi - si * pr;
+                for (int m = 0; m < 3; m++) {
+                    ac[m] = P2<F>::fma_s(wl[2 * m + 1], val, ac[m]);
+                    as[m] = P2<F>::fma_s(wl[2 * m + 2], val, as[m]);
+                }
+            }
+            if (it + NS < niter) named_bar_arrive(1 + NS + st, NTHREADS);
+            if (xc == nxc - 1) {
+                // ---------------------------------------------------------------- y-stage
+                const F* wl = swy + y * 8;
+                F cy[4], sy[4];
+                cy[0] = 1; sy[0] = 0;
+                cy[1] = wl[1]; sy[1] = wl[2]; cy[2] = wl[3]; sy[2] = wl[4]; cy[3] = wl[5]; sy[3] = wl[6];
+                int q = 0;
+#pragma unroll
+                for (int m = 0; m < 4; m++)
+#pragma unroll
+                    for (int n = 0; n < 4; n++) {
+                        if (!PRUNE || m * m + n * n <= 9) {
+                            const T xcm = m ? ac[m - 1] : a0;
+                            if (n == 0) Q[q] = P2<F>::add(Q[q], xcm); else Q[q] = P2<F>::fma_s(cy[n], xcm, Q[q]);
+                            q++;
+                            if (n > 0) { Q[q] = P2<F>::fma_s(sy[n], xcm, Q[q]); q++; }
+                            if (m > 0) {
+                                if (n == 0) Q[q] = P2<F>::add(Q[q], as[m - 1]); else Q[q] = P2<F>::fma_s(cy[n], as[m - 1], Q[q]);
+                                q++;
+                            }
+                            if (m > 0 && n > 0) { Q[q] = P2<F>::fma_s(sy[n], as[m - 1], Q[q]); q++; }
                         }
-                        out[(size_t)((a * 4 + bb) * 2) * BS] = re;
-                        out[(size_t)((a * 4 + bb) * 2 + 1) * BS] = im;
                     }
-            }
-            __syncthreads();
-            // ---------------------------------------------------------------- phase B: x-sum
-            {
-                const int nvalid = min(32, g.X0 - xc * 32);
-                const F* v = mybuf + (size_t)jr * BS;
-                const F* w = swx + (size_t)xc * 32 * 8;
-                for (int l = 0; l < nvalid; l++) {
-                    const F val = v[l];
-                    const F* wl = w + l * 8;
-                    xc_[0] += val;
-                    xc_[1] += wl[1] * val; xs_[1] += wl[2] * val;
-                    xc_[2] += wl[3] * val; xs_[2] += wl[4] * val;
-                    xc_[3] += wl[5] * val; xs_[3] += wl[6] * val;
-                }
-            }
-            if (NBUF == 2) b ^= 1; else __syncthreads();
-        }
-        // -------------------------------------------------------------------- y-stage
-        {
-            const F* wl = swy + y * 8;
-            F cy[4], sy[4];
-            cy[0] = 1; sy[0] = 0;
-            cy[1] = wl[1]; sy[1] = wl[2]; cy[2] = wl[3]; sy[2] = wl[4]; cy[3] = wl[5]; sy[3] = wl[6];
-            int q = 0;
+                a0 = P2<F>::make(0, 0);
 #pragma unroll
-            for (int m = 0; m < 4; m++)
-#pragma unroll
-                for (int n = 0; n < 4; n++) {
-                    if (!PRUNE || m * m + n * n <= 9) {
-                        Q[q++] += cy[n] * xc_[m];
-                        if (n > 0) Q[q++] += sy[n] * xc_[m];
-                        if (m > 0) Q[q++] += cy[n] * xs_[m];
-                        if (m > 0 && n > 0) Q[q++] += sy[n] * xs_[m];
-                    }
-                }
+                for (int m = 0; m < 3; m++) { ac[m] = P2<F>::make(0, 0); as[m] = P2<F>::make(0, 0); }
+            }
         }
+        T* qb = reinterpret_cast<T*>((F*)A.qbuf + (size_t)zt * NQ * CT_THREADS) + cc;
+#pragma unroll
+        for (int q = 0; q < NQ; q++) qb[(size_t)q * CT_NCC] = Q[q];
     }
-    F* qb = (F*)A.qbuf + (size_t)zt * NQ * CT_THREADS + jr;
-#pragma unroll
-    for (int q = 0; q < NQ; q++) qb[(size_t)q * CT_THREADS] = Q[q];
 }
 
 // ------------------------------------------------------------------ kernel 2: z-sum + assembly
@@ -366,19 +475,23 @@ static void build_qidx(short* qidx, int prune, int* nq) {
     *nq = q;
 }
 
+template <typename S> struct XyConfig;
+template <> struct XyConfig<float>  { static constexpr int NP = 8, NS = 3; };
+template <> struct XyConfig<double> { static constexpr int NP = 4, NS = 2; };
+
 template <typename S, int R>
 static tm_status launch_xy(tm_ctx* ctx, const ContractArgs& A, int prune, cudaStream_t st) {
-    constexpr int BS = BufStride<S>::V;
-    constexpr int NBUF = sizeof(S) == 4 ? 2 : 1;
-    const size_t smem = (size_t)NBUF * CT_THREADS * BS * sizeof(S) + (size_t)(ctx->X[0] + ctx->X[1]) * 8 * sizeof(S);
+    constexpr int NP = XyConfig<S>::NP, NS = XyConfig<S>::NS;
+    constexpr int NT = (NP + CT_NC) * 32;
+    const size_t smem = (size_t)NS * CT_NCC * CT_BSC * 2 * sizeof(S) + (size_t)(ctx->X[0] + ctx->X[1]) * 8 * sizeof(S);
     if (smem > 227 * 1024) return tm_fail(ctx, TM_EDIM, "contract: Lx + Ly too large for the shared-memory weight tables");
     const unsigned grid = (unsigned)(ctx->X[2] * ctx->X[3]);
     if (prune) {
-        TM_CUDA(ctx, cudaFuncSetAttribute(contract_xy_kernel<S, R, 1, NBUF>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        contract_xy_kernel<S, R, 1, NBUF><<<grid, CT_THREADS, smem, st>>>(A);
+        TM_CUDA(ctx, cudaFuncSetAttribute(contract_xy_kernel<S, R, 1, NP, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        contract_xy_kernel<S, R, 1, NP, NS><<<grid, NT, smem, st>>>(A);
     } else {
-        TM_CUDA(ctx, cudaFuncSetAttribute(contract_xy_kernel<S, R, 0, NBUF>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        contract_xy_kernel<S, R, 0, NBUF><<<grid, CT_THREADS, smem, st>>>(A);
+        TM_CUDA(ctx, cudaFuncSetAttribute(contract_xy_kernel<S, R, 0, NP, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        contract_xy_kernel<S, R, 0, NP, NS><<<grid, NT, smem, st>>>(A);
     }
     TM_LAUNCH_CHECK(ctx, "contract_xy_kernel");
     return TM_OK;
