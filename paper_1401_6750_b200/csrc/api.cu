@@ -1,4 +1,5 @@
 // api.cu -- context lifetime, workspaces and the exported tm_dslash / field conversion calls.
+#include <stdlib.h>
 #include "kernels.h"
 
 static char g_last_error[512] = "";
@@ -37,6 +38,7 @@ extern "C" tm_status tm_create(tm_ctx** out, const int dims[4], int t_boundary, 
     c->V = V; c->Vh = V / 2;
     c->tb = t_boundary;
     c->device = device;
+    { const char* e = getenv("TMLOOPS_NO_TMA"); c->no_tma = (e && e[0] == '1'); }
     cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
     bool ok = cudaMalloc((void**)&c->d_partials, sizeof(double) * (1 << 18)) == cudaSuccess
            && cudaMalloc((void**)&c->d_counter, sizeof(unsigned int) * 4) == cudaSuccess

@@ -57,6 +57,7 @@ struct tm_ctx {
     void* h_contract_tables;        // host mirror (rebuild only when the momentum list changes)
     size_t contract_tables_bytes;
     cudaEvent_t ev[4];
+    int no_tma;                     // TMLOOPS_NO_TMA=1: force the generic contraction kernel (testing)
 };
 
 static inline tm_status tm_fail(tm_ctx* c, tm_status s, const char* msg) {

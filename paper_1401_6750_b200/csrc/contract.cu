@@ -23,120 +23,7 @@
 #include <math.h>
 #include <complex>
 #include <vector>
-#include "kernels.h"
-#include "su3.cuh"
-
-#define CT_THREADS 320          // real components per site: 10 (fam, d) x 16 complex x 2
-#define CT_NCC 160              // complex components per site
-#define CT_NC 5                 // consumer warps: one thread per complex component
-#define CT_BSC 34               // row-buffer stride in complex numbers (32 x-values + 2 pad: conflict-free 16-byte reads)
-
-template <int PRUNE> struct QLayout { static constexpr int NQ = PRUNE ? 29 : 49; };
-
-struct ContractArgs {
-    const void* s;         // full-lattice internal field (even block, odd block)
-    const void* eta;
-    const void* gauge;
-    void* qbuf;            // [T*Lz][NQ][320]
-    const void* wx;        // [Lx][8]: 1, c1, s1, c2, s2, c3, s3, 0   (F precision)
-    const void* wy;        // [Ly][8]
-    Geom g;
-    double tb;
-};
-
-// ---- pair arithmetic: one complex number (re, im) per pair.  fp32 pairs live in one 64-bit register
-// and use Blackwell's packed FFMA2 / FADD2 (PTX fma.rn.f32x2): one issue slot per complex FMA with a
-// broadcast real scalar; ptxas folds the (re, im) swap into the operand swizzle.
-template <typename F> struct P2;
-template <> struct P2<float> {
-    typedef unsigned long long T;
-    static __device__ __forceinline__ T make(float re, float im) { T r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(re), "f"(im)); return r; }
-    static __device__ __forceinline__ void get(T v, float& re, float& im) { asm("mov.b64 {%0, %1}, %2;" : "=f"(re), "=f"(im) : "l"(v)); }
-    static __device__ __forceinline__ T fma_s(float s, T b, T c) {      // c + s * b
-        T d; const T ss = make(s, s);
-        asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(ss), "l"(b), "l"(c));
-        return d;
-    }
-    static __device__ __forceinline__ T add(T a, T b) { T d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
-    static __device__ __forceinline__ T mul_s(float s, T b) { T d; const T ss = make(s, s); asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(ss), "l"(b)); return d; }
-};
-template <> struct P2<double> {
-    typedef double2 T;
-    static __device__ __forceinline__ T make(double re, double im) { return make_double2(re, im); }
-    static __device__ __forceinline__ void get(T v, double& re, double& im) { re = v.x; im = v.y; }
-    static __device__ __forceinline__ T fma_s(double s, T b, T c) { return make_double2(fma(s, b.x, c.x), fma(s, b.y, c.y)); }
-    static __device__ __forceinline__ T add(T a, T b) { return make_double2(a.x + b.x, a.y + b.y); }
-    static __device__ __forceinline__ T mul_s(double s, T b) { return make_double2(s * b.x, s * b.y); }
-};
-// i * v = (-im, re)
-template <typename F> __device__ __forceinline__ typename P2<F>::T times_i(typename P2<F>::T v) {
-    F re, im;
-    P2<F>::get(v, re, im);
-    return P2<F>::make(-im, re);
-}
-
-// out[sp][a] (+|-)= sum_b U[a][b] in[sp][b]  (DAG: U^dag), 4 spins x 3 colours as 12 pairs; NEG subtracts
-template <int DAG, int NEG, typename F>
-__device__ __forceinline__ void su3_macc(const F* U, const typename P2<F>::T* in, typename P2<F>::T* out) {
-    typedef typename P2<F>::T T;
-#pragma unroll
-    for (int sp = 0; sp < 4; sp++) {
-        T ib[3];
-#pragma unroll
-        for (int b = 0; b < 3; b++) ib[b] = times_i<F>(in[sp * 3 + b]);
-#pragma unroll
-        for (int a = 0; a < 3; a++) {
-            T acc = out[sp * 3 + a];
-#pragma unroll
-            for (int b = 0; b < 3; b++) {
-                F ur = DAG ? U[(b * 3 + a) * 2] : U[(a * 3 + b) * 2];
-                F ui = DAG ? -U[(b * 3 + a) * 2 + 1] : U[(a * 3 + b) * 2 + 1];
-                if (NEG) { ur = -ur; ui = -ui; }
-                acc = P2<F>::fma_s(ur, in[sp * 3 + b], acc);       // (ur + i ui) * in = ur * in + ui * (i in)
-                acc = P2<F>::fma_s(ui, ib[b], acc);
-            }
-            out[sp * 3 + a] = acc;
-        }
-    }
-}
-
-template <typename S>
-__device__ __forceinline__ void load_spinor_pairs(const S* f, size_t Vh, size_t h, typename P2<S>::T* v) {
-    S t[24];
-    load_spinor<S>(f, Vh, h, t);
-#pragma unroll
-    for (int i = 0; i < 12; i++) v[i] = P2<S>::make(t[2 * i], t[2 * i + 1]);
-}
-
-__device__ __forceinline__ void named_bar_sync(int id, int count) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory"); }
-__device__ __forceinline__ void named_bar_arrive(int id, int count) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(count) : "memory"); }
-
-// C[a][b] = sum_c conj(s_ac) psi_bc for the (fam, d) slot `slot` of site column `lane` -> row buffer
-template <typename F>
-__device__ __forceinline__ void outer_store(const typename P2<F>::T* sv, const typename P2<F>::T* psi,
-                                            typename P2<F>::T* rowbuf, int slot, int lane) {
-    typedef typename P2<F>::T T;
-    F sre[12], sim[12];
-#pragma unroll
-    for (int i = 0; i < 12; i++) { P2<F>::get(sv[i], sre[i], sim[i]); sim[i] = -sim[i]; }
-    T* out = rowbuf + (size_t)(slot * 16) * CT_BSC + lane;
-#pragma unroll
-    for (int bb = 0; bb < 4; bb++) {
-        T ip[3];
-#pragma unroll
-        for (int c = 0; c < 3; c++) ip[c] = times_i<F>(psi[bb * 3 + c]);
-#pragma unroll
-        for (int a = 0; a < 4; a++) {
-            T acc = P2<F>::make(0, 0);
-#pragma unroll
-            for (int c = 0; c < 3; c++) {       // conj(s) psi = s.re * psi - s.im * (i psi)
-                acc = P2<F>::fma_s(sre[a * 3 + c], psi[bb * 3 + c], acc);
-                acc = P2<F>::fma_s(sim[a * 3 + c], ip[c], acc);
-            }
-            out[(size_t)(a * 4 + bb) * CT_BSC] = acc;
-        }
-    }
-}
+#include "contract.cuh"
 
 // Warp-specialised CTA, one (z,t) plane per CTA:
 //   NP producer warps (lane = x): jobs (fam, d) of one row chunk -> psi_{fam,d}(x), colour-traced outer
@@ -312,7 +199,8 @@ struct GammaTable {
 __constant__ GammaTable c_gamma;
 
 struct AssembleArgs {
-    const void* qbuf;
+    const void* qbuf;          // [T*Lz][NQ][320] (F precision): x/y partial sums per (z,t) plane
+    double* zbuf;              // [T][NQ][7][320]: z-stage sums with weights 1, c1, s1, c2, s2, c3, s3
     void* out;                 // complex128 [2][80][nmom][T]
     const int* mom;            // [nmom][3]
     const short* qidx;         // [4][4][4]: index of Qcc, Qcs, Qsc, Qss for (m,n), -1 if absent
@@ -321,7 +209,28 @@ struct AssembleArgs {
     double twokmu;             // 2 kappa mu
 };
 
+// z-stage: every x/y partial sum is read exactly once and reduced against the 7 real z-weights
 template <typename F>
+__global__ void __launch_bounds__(CT_THREADS) contract_zsum_kernel(AssembleArgs A) {
+    const int q = blockIdx.x, t = blockIdx.y, jr = threadIdx.x;
+    const F* qb = (const F*)A.qbuf + ((size_t)t * A.Lz * A.NQ + q) * CT_THREADS + jr;
+    double acc[7];
+#pragma unroll
+    for (int k = 0; k < 7; k++) acc[k] = 0.0;
+    for (int z = 0; z < A.Lz; z++) {
+        const double v = (double)qb[(size_t)z * A.NQ * CT_THREADS];
+        const double* w = A.wz + z * 8;
+        acc[0] += v;
+#pragma unroll
+        for (int k = 1; k < 7; k++) acc[k] += w[k] * v;
+    }
+    double* zb = A.zbuf + (((size_t)t * A.NQ + q) * 7) * CT_THREADS + jr;
+#pragma unroll
+    for (int k = 0; k < 7; k++) zb[(size_t)k * CT_THREADS] = acc[k];
+}
+
+// assembly of exp(+2 pi i p.x / L) for every requested momentum from the (cos|sin)^3 sums, then the
+// site-independent Gamma change of basis
 __global__ void __launch_bounds__(CT_THREADS) contract_assemble_kernel(AssembleArgs A) {
     __shared__ double zre[CT_THREADS], zim[CT_THREADS];
     const int k = blockIdx.x, t = blockIdx.y;
@@ -330,22 +239,24 @@ __global__ void __launch_bounds__(CT_THREADS) contract_assemble_kernel(AssembleA
     const int m = abs(px), n = abs(py), l = abs(pz);
     const double sx = px < 0 ? -1.0 : 1.0, sy = py < 0 ? -1.0 : 1.0, sz = pz < 0 ? -1.0 : 1.0;
     const short* qi = A.qidx + (m * 4 + n) * 4;
-    const int icc = qi[0], ics = qi[1], isc = qi[2], iss = qi[3];
-    const F* qb = (const F*)A.qbuf + (size_t)t * A.Lz * A.NQ * CT_THREADS + jr;
-    double ar = 0, ai = 0;
-    for (int z = 0; z < A.Lz; z++) {
-        const F* q = qb + (size_t)z * A.NQ * CT_THREADS;
-        const double cc = (double)q[(size_t)icc * CT_THREADS];
-        const double cs = ics >= 0 ? (double)q[(size_t)ics * CT_THREADS] : 0.0;
-        const double sc = isc >= 0 ? (double)q[(size_t)isc * CT_THREADS] : 0.0;
-        const double ss = iss >= 0 ? (double)q[(size_t)iss * CT_THREADS] : 0.0;
-        // (cos mx + i sx sin mx)(cos ny + i sy sin ny)
-        const double wr = cc - sx * sy * ss, wi = sx * sc + sy * cs;
-        const double cz = l ? A.wz[z * 8 + 2 * l - 1] : 1.0, szv = l ? sz * A.wz[z * 8 + 2 * l] : 0.0;
-        ar += cz * wr - szv * wi;
-        ai += cz * wi + szv * wr;
+    const double* zb = A.zbuf + (size_t)t * A.NQ * 7 * CT_THREADS + jr;
+    // X[c] = sum_z cos(2 pi l z / L) Q_X(z), X[s] = sum_z sin(...) Q_X(z) for X in cc, cs, sc, ss
+    double C[4], S[4];
+#pragma unroll
+    for (int x = 0; x < 4; x++) {
+        const int iq = qi[x];
+        C[x] = 0.0; S[x] = 0.0;
+        if (iq >= 0) {
+            const double* e = zb + (size_t)iq * 7 * CT_THREADS;
+            C[x] = l ? e[(size_t)(2 * l - 1) * CT_THREADS] : e[0];
+            S[x] = l ? e[(size_t)(2 * l) * CT_THREADS] : 0.0;
+        }
     }
-    zre[jr] = ar; zim[jr] = ai;
+    // (cos mx + i sx sin mx)(cos ny + i sy sin ny)(cos lz + i sz sin lz)
+    const double wrC = C[0] - sx * sy * C[3], wiC = sx * C[2] + sy * C[1];
+    const double wrS = S[0] - sx * sy * S[3], wiS = sx * S[2] + sy * S[1];
+    zre[jr] = wrC - sz * wiS;
+    zim[jr] = wiC + sz * wrS;
     __syncthreads();
     if (jr < 160) {
         const int f = jr / 80, i = jr % 80;
@@ -558,18 +469,23 @@ tm_status tm_contract_internal(tm_ctx* ctx, void* d_out, const void* d_s, const 
     A.g = tm_geom(ctx);
     A.tb = (double)ctx->tb;
     if (acc == TM_F64) TM_TRY((launch_xy<double, 18>(ctx, A, prune, st)));
+    else if (!ctx->no_tma && tm_contract_tma_usable(ctx)) TM_TRY(tm_contract_xy_tma(ctx, qbuf, d_s, d_eta, gauge, A.wx, A.wy, prune, st));
     else TM_TRY((launch_xy<float, 12>(ctx, A, prune, st)));
 
     AssembleArgs B;
     B.qbuf = qbuf; B.out = d_out;
+    TM_TRY(tm_ws(ctx, WS_CT_OUT, (size_t)ctx->X[3] * nq * 7 * CT_THREADS * sizeof(double), (void**)&B.zbuf));
     B.mom = (const int*)(tb + L.off_mom);
     B.qidx = (const short*)(tb + L.off_qidx);
     B.wz = (const double*)(tb + L.off_wz);
     B.nmom = nmom; B.T = ctx->X[3]; B.Lz = ctx->X[2]; B.NQ = nq;
     B.twokmu = 2.0 * kappa * mu;
+    dim3 zgrid((unsigned)nq, (unsigned)ctx->X[3]);
+    if (acc == TM_F64) contract_zsum_kernel<double><<<zgrid, CT_THREADS, 0, st>>>(B);
+    else contract_zsum_kernel<float><<<zgrid, CT_THREADS, 0, st>>>(B);
+    TM_LAUNCH_CHECK(ctx, "contract_zsum_kernel");
     dim3 grid((unsigned)nmom, (unsigned)ctx->X[3]);
-    if (acc == TM_F64) contract_assemble_kernel<double><<<grid, CT_THREADS, 0, st>>>(B);
-    else contract_assemble_kernel<float><<<grid, CT_THREADS, 0, st>>>(B);
+    contract_assemble_kernel<<<grid, CT_THREADS, 0, st>>>(B);
     TM_LAUNCH_CHECK(ctx, "contract_assemble_kernel");
     return TM_OK;
 }

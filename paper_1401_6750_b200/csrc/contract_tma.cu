@@ -1,0 +1,473 @@
+// contract_tma.cu -- TMA-staged fast path of the fused contraction + projection kernel (fp32, Lx <= 32).
+//
+// Same mathematics and the same output (qbuf) as contract_xy_kernel in contract.cu (SURVEY.md sec 8
+// rows a6-a8); what changes is how operands reach the SM.  One CTA per (z,t)
+// plane, 14 warps:
+//   warp 13      loader: one thread issues, per y-row, 18 TMA tensor copies (cp.async.bulk.tensor) that
+//                land the 7 rows of s and eta the row needs (centre, y+-1, z+-1, t+-1), the row's 4
+//                forward links and the 3 backward links of the y-1, z-1, t-1 rows in shared memory,
+//                completion signalled on an mbarrier (2-stage ring)
+//   warps 0..7   producers, one fixed (fam, mu) derivative job each (+ the rotating d = 0 jobs): operands
+//                come from shared memory with compile-time offsets (no global address arithmetic, no
+//                long-scoreboard stalls), FFMA2 complex arithmetic, 16 complex outer-product values per
+//                site -> row buffer
+//   warps 8..12  consumers: thread = complex component; x-sum with 7 real weights, y-stage accumulators
+// Lane l of a producer handles the site of parity p = l / Xh with in-row half index idx = l % Xh
+// (x = 2 idx + (p ^ row parity)), so that every shared-memory operand read is a contiguous run of
+// 16-byte vectors; the consumers use the correspondingly permuted x-weight table.
+#include <cuda.h>
+#include "contract.cuh"
+
+#define TX_NP 8
+#define TX_NTHREADS ((TX_NP + CT_NC + 1) * 32)
+#define TX_NCOMP ((TX_NP + CT_NC) * 32)       // threads taking part in the row-buffer barriers
+#define TX_NSI 2                               // input stages
+#define TX_NSC 2                               // row-buffer stages
+#ifndef TX_PF
+#define TX_PF 1000                                // L2 prefetch distance in rows
+#endif
+
+struct TmaContractArgs {
+    void* qbuf;            // [T*Lz][NQ][320] float
+    const float* wx;       // [Lx][8]
+    const float* wy;       // [Ly][8]
+    Geom g;
+    float tb;
+};
+
+// shared-memory plan (bytes), every TMA destination 128-byte aligned
+struct TxPlan {
+    int seg;               // bytes of one segment: Xh float4
+    int row;               // one spinor row block: 12 segments, padded to 128
+    int gf, gb;            // forward-link block (24 segments), one backward-link block (6 segments)
+    int stage;             // one input stage: 14 rows + gf + 3 gb
+    int off_c, off_wx, off_wy, off_bar, total;
+};
+__host__ __device__ inline int tx_pad128(int b) { return (b + 127) & ~127; }
+__host__ __device__ inline TxPlan tx_plan(int Lx, int Ly) {
+    TxPlan P;
+    P.seg = (Lx / 2) * 16;
+    P.row = tx_pad128(12 * P.seg);
+    P.gf = tx_pad128(24 * P.seg);
+    P.gb = tx_pad128(6 * P.seg);
+    P.stage = 14 * P.row + P.gf + 3 * P.gb;
+    P.off_c = TX_NSI * P.stage;
+    P.off_wx = P.off_c + TX_NSC * CT_NCC * CT_BSC * 8;
+    P.off_wy = P.off_wx + 2 * 32 * 8 * 4;
+    P.off_bar = tx_pad128(P.off_wy + Ly * 8 * 4);
+    P.total = P.off_bar + 64;
+    return P;
+}
+
+// ------------------------------------------------------------------ mbarrier / TMA primitives
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
+    unsigned ok;
+    do {
+        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                     : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    } while (!ok);
+}
+__device__ __forceinline__ void tma_load_2d(unsigned dst, const CUtensorMap* map, unsigned bar, int c0, int c1) {
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+                 ::"r"(dst), "l"(map), "r"(bar), "r"(c0), "r"(c1) : "memory");
+}
+__device__ __forceinline__ void tma_load_4d(unsigned dst, const CUtensorMap* map, unsigned bar, int c0, int c1, int c2, int c3) {
+    asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
+                 ::"r"(dst), "l"(map), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
+}
+__device__ __forceinline__ void tma_prefetch_2d(const CUtensorMap* map, int c0, int c1) {
+    asm volatile("cp.async.bulk.prefetch.tensor.2d.L2.global [%0, {%1, %2}];" ::"l"(map), "r"(c0), "r"(c1) : "memory");
+}
+__device__ __forceinline__ void tma_prefetch_4d(const CUtensorMap* map, int c0, int c1, int c2, int c3) {
+    asm volatile("cp.async.bulk.prefetch.tensor.4d.L2.global [%0, {%1, %2, %3, %4}];"
+                 ::"l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
+}
+
+// ------------------------------------------------------------------ shared-memory operand reads
+typedef P2<float>::T T2;
+
+// 12 complex numbers of the site (parity q, in-row index idx) of a staged spinor row
+__device__ __forceinline__ void lds_spinor(const float4* rowblk, int Xh, int q, int idx, T2* v) {
+#pragma unroll
+    for (int k = 0; k < 6; k++) {
+        const float4 f = rowblk[(q * 6 + k) * Xh + idx];
+        v[2 * k] = P2<float>::make(f.x, f.y);
+        v[2 * k + 1] = P2<float>::make(f.z, f.w);
+    }
+}
+// link stored as 3 segments starting at segment `seg0` of a link block; row 2 = conj(row0 x row1)
+__device__ __forceinline__ void lds_link(const float4* blk, int Xh, int seg0, int idx, float* u) {
+#pragma unroll
+    for (int k = 0; k < 3; k++) {
+        const float4 f = blk[(seg0 + k) * Xh + idx];
+        u[4 * k] = f.x; u[4 * k + 1] = f.y; u[4 * k + 2] = f.z; u[4 * k + 3] = f.w;
+    }
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        const int i = (c + 1) % 3, j = (c + 2) % 3;
+        const float ar = u[2 * i], ai = u[2 * i + 1], br = u[6 + 2 * j], bi = u[6 + 2 * j + 1];
+        const float cr = u[2 * j], ci = u[2 * j + 1], dr = u[6 + 2 * i], di = u[6 + 2 * i + 1];
+        float re = ar * br; re -= ai * bi; re -= cr * dr; re += ci * di;
+        float im = ar * bi; im += ai * br; im -= cr * di; im -= ci * dr;
+        u[12 + 2 * c] = re;
+        u[12 + 2 * c + 1] = -im;
+    }
+}
+
+// row blocks of one input stage, in the order the loader fills them
+enum { ROW_C = 0, ROW_YP, ROW_YM, ROW_ZP, ROW_ZM, ROW_TP, ROW_TM };
+
+struct TxShared {             // resolved shared-memory pointers of the CTA
+    unsigned char* in;        // [TX_NSI] input stages
+    T2* cbuf;                 // [TX_NSC][160][CT_BSC]
+    float* swx;               // [2 row parities][32 columns][8]
+    float* swy;               // [Ly][8]
+    unsigned bar_full, bar_empty;   // shared-space addresses of in_full[0], in_empty[0] (8 bytes apart per stage)
+};
+
+// producer warp: fixed derivative job (fam, mu) for every row of the plane, plus the rotating d = 0 jobs.
+// One copy of the code for all directions (the direction only selects loop-invariant shared-memory
+// offsets), so the 8 producer warps share the instruction cache.
+__device__ __forceinline__ void producer_rows(const TxShared& sh, const TxPlan& P, const Geom& g, int z, int t,
+                                              int warp, int lane, float tb) {
+    const int Xh = g.Xh;
+    const int fam = warp >> 2, mu = warp & 3;
+    const int p = lane / Xh, idx = lane - p * Xh;
+    const bool active = lane < g.X0;
+    const float sgn_f = (mu == 3 && t + 1 == g.X3) ? tb : 1.f;
+    const float sgn_b = (mu == 3 && t == 0) ? tb : 1.f;
+    // byte offsets inside an input stage (float4 index = segment * Xh + idx)
+    const int fam_off = fam ? 7 * P.row : 0;
+    const int rf = mu == 0 ? ROW_C : mu == 1 ? ROW_YP : mu == 2 ? ROW_ZP : ROW_TP;
+    const int rb = mu == 0 ? ROW_C : mu == 1 ? ROW_YM : mu == 2 ? ROW_ZM : ROW_TM;
+    const int idx_up = idx + 1 == Xh ? 0 : idx + 1, idx_dn = idx == 0 ? Xh - 1 : idx - 1;
+    const int off_sv = ((p * 6) * Xh + idx) * 16;                                   // centre s
+    const int off_ev = 7 * P.row + off_sv;                                          // centre eta
+    const int off_uf = 14 * P.row + (((p * 4 + mu) * 3) * Xh + idx) * 16;           // U_mu(x)
+    // backward link U_mu(x - mu): mu = 0 from the row's own forward block, else from the staged neighbour row
+    const int ub_blk = mu == 0 ? 14 * P.row + (((1 - p) * 4) * 3) * Xh * 16
+                               : 14 * P.row + P.gf + (mu - 1) * P.gb + ((1 - p) * 3) * Xh * 16;
+    const int nbf_blk = fam_off + rf * P.row + ((1 - p) * 6) * Xh * 16;
+    const int nbb_blk = fam_off + rb * P.row + ((1 - p) * 6) * Xh * 16;
+    const int seg = Xh * 16;
+    for (int y = 0; y < g.X1; y++) {
+        const int si = y % TX_NSI, sc = y % TX_NSC;
+        const unsigned char* stage = sh.in + (size_t)si * P.stage;
+        T2* rowbuf = sh.cbuf + (size_t)sc * CT_NCC * CT_BSC;
+        mbar_wait(sh.bar_full + 8 * si, (y / TX_NSI) & 1);
+        if (y >= TX_NSC) named_bar_sync(1 + TX_NSC + sc, TX_NCOMP);
+        if (active) {
+            const int xo = (p ^ (y + z + t)) & 1;                 // x = 2 idx + xo
+            const int idx_f = mu == 0 ? (xo ? idx_up : idx) : idx;
+            const int idx_b = mu == 0 ? (xo ? idx : idx_dn) : idx;
+            T2 sv[12];
+#pragma unroll
+            for (int k = 0; k < 6; k++) {
+                const float4 f = *reinterpret_cast<const float4*>(stage + off_sv + k * seg);
+                sv[2 * k] = P2<float>::make(f.x, f.y);
+                sv[2 * k + 1] = P2<float>::make(f.z, f.w);
+            }
+            {
+                // psi = U_mu(x) f(x+mu) - U_mu^dag(x-mu) f(x-mu)
+                T2 psi[12], nb[12];
+                float U[18];
+#pragma unroll
+                for (int i = 0; i < 12; i++) psi[i] = P2<float>::make(0.f, 0.f);
+                const unsigned char* nf = stage + nbf_blk + idx_f * 16;
+#pragma unroll
+                for (int k = 0; k < 6; k++) {
+                    const float4 f = *reinterpret_cast<const float4*>(nf + k * seg);
+                    nb[2 * k] = P2<float>::make(f.x, f.y);
+                    nb[2 * k + 1] = P2<float>::make(f.z, f.w);
+                }
+                if (sgn_f != 1.f) {
+#pragma unroll
+                    for (int i = 0; i < 12; i++) nb[i] = P2<float>::mul_s(sgn_f, nb[i]);
+                }
+                lds_link(reinterpret_cast<const float4*>(stage + off_uf), Xh, 0, 0, U);
+                su3_macc<0, 0, float>(U, nb, psi);
+                const unsigned char* nbk = stage + nbb_blk + idx_b * 16;
+#pragma unroll
+                for (int k = 0; k < 6; k++) {
+                    const float4 f = *reinterpret_cast<const float4*>(nbk + k * seg);
+                    nb[2 * k] = P2<float>::make(f.x, f.y);
+                    nb[2 * k + 1] = P2<float>::make(f.z, f.w);
+                }
+                if (sgn_b != 1.f) {
+#pragma unroll
+                    for (int i = 0; i < 12; i++) nb[i] = P2<float>::mul_s(sgn_b, nb[i]);
+                }
+                lds_link(reinterpret_cast<const float4*>(stage + ub_blk + idx_b * 16), Xh, 0, 0, U);
+                su3_macc<1, 1, float>(U, nb, psi);
+                outer_store<float>(sv, psi, rowbuf, fam * 5 + 1 + mu, lane);
+            }
+            {
+                // this warp's quarter of a d = 0 job: column bb = mu of C_{fam,0}[a][bb] = sum_c conj(s_ac) f_{bb,c}
+                // (splitting the two light jobs 8 ways keeps the producer warps in step)
+                const int bb = mu;
+                T2 f3[3];
+                if (fam == 0) {
+#pragma unroll
+                    for (int c = 0; c < 3; c++) f3[c] = bb == 0 ? sv[c] : bb == 1 ? sv[3 + c] : bb == 2 ? sv[6 + c] : sv[9 + c];
+                } else {
+                    const int k0 = (6 * bb) >> 2;
+                    const float4 f0 = *reinterpret_cast<const float4*>(stage + off_ev + k0 * seg);
+                    const float4 f1 = *reinterpret_cast<const float4*>(stage + off_ev + (k0 + 1) * seg);
+                    if (bb & 1) { f3[0] = P2<float>::make(f0.z, f0.w); f3[1] = P2<float>::make(f1.x, f1.y); f3[2] = P2<float>::make(f1.z, f1.w); }
+                    else        { f3[0] = P2<float>::make(f0.x, f0.y); f3[1] = P2<float>::make(f0.z, f0.w); f3[2] = P2<float>::make(f1.x, f1.y); }
+                }
+                T2 acc[4];
+#pragma unroll
+                for (int a = 0; a < 4; a++) acc[a] = P2<float>::make(0.f, 0.f);
+#pragma unroll
+                for (int c = 0; c < 3; c++) {
+                    const T2 ip = times_i<float>(f3[c]);
+                    float sre[4], sim[4];
+#pragma unroll
+                    for (int a = 0; a < 4; a++) { P2<float>::get(sv[a * 3 + c], sre[a], sim[a]); }
+#pragma unroll
+                    for (int a = 0; a < 4; a++) acc[a] = P2<float>::fma_s(sre[a], f3[c], acc[a]);
+#pragma unroll
+                    for (int a = 0; a < 4; a++) acc[a] = P2<float>::fma_s(-sim[a], ip, acc[a]);
+                }
+                T2* out = rowbuf + (size_t)(fam * 5 * 16 + bb) * CT_BSC + lane;
+#pragma unroll
+                for (int a = 0; a < 4; a++) out[(size_t)(a * 4) * CT_BSC] = acc[a];
+            }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(sh.bar_empty + 8 * si);        // this warp is done reading the input stage
+        named_bar_arrive(1 + sc, TX_NCOMP);
+    }
+}
+
+template <int PRUNE>
+__global__ void __launch_bounds__(TX_NTHREADS, 1)
+contract_xy_tma_kernel(const __grid_constant__ CUtensorMap tm_s, const __grid_constant__ CUtensorMap tm_e,
+                       const __grid_constant__ CUtensorMap tm_gf, const __grid_constant__ CUtensorMap tm_gb,
+                       TmaContractArgs A) {
+    constexpr int NQ = QLayout<PRUNE>::NQ;
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    const Geom& g = A.g;
+    const TxPlan P = tx_plan(g.X0, g.X1);
+    TxShared sh;
+    sh.in = smem_raw;
+    sh.cbuf = reinterpret_cast<T2*>(smem_raw + P.off_c);
+    sh.swx = reinterpret_cast<float*>(smem_raw + P.off_wx);
+    sh.swy = reinterpret_cast<float*>(smem_raw + P.off_wy);
+    sh.bar_full = smem_u32(smem_raw + P.off_bar);
+    sh.bar_empty = sh.bar_full + 8 * TX_NSI;
+    const int zt = blockIdx.x;
+    const int z = zt % g.X2, t = zt / g.X2;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int Xh = g.Xh;
+
+    // x-weight tables in column order: column l <-> x = 2 (l % Xh) + ((l / Xh) ^ row parity)
+    for (int i = threadIdx.x; i < 2 * 32 * 8; i += TX_NTHREADS) {
+        const int rp = i >> 8, l = (i >> 3) & 31, k = i & 7;
+        float w = 0.f;
+        if (l < g.X0) {
+            const int x = 2 * (l % Xh) + ((l / Xh) ^ rp);
+            w = A.wx[x * 8 + k];
+        }
+        sh.swx[i] = w;
+    }
+    for (int i = threadIdx.x; i < g.X1 * 8; i += TX_NTHREADS) sh.swy[i] = A.wy[i];
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < TX_NSI; s++) {
+            mbar_init(sh.bar_full + 8 * s, 1);
+            mbar_init(sh.bar_empty + 8 * s, TX_NP);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    if (warp == TX_NP + CT_NC) {
+        // ================================================================ loader
+        if (lane == 0) {
+            asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_s) : "memory");
+            asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_e) : "memory");
+            asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_gf) : "memory");
+            asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_gb) : "memory");
+            const unsigned in0 = smem_u32(sh.in);
+            const int zp = z + 1 == g.X2 ? 0 : z + 1, zm = z == 0 ? g.X2 - 1 : z - 1;
+            const int tp = t + 1 == g.X3 ? 0 : t + 1, tm = t == 0 ? g.X3 - 1 : t - 1;
+            const unsigned bytes = (unsigned)(14 * 12 + 24 + 18) * (unsigned)P.seg;
+            for (int y = 0; y < g.X1; y++) {
+                const int si = y % TX_NSI;
+                const unsigned full = sh.bar_full + 8 * si;
+                if (y >= TX_NSI) mbar_wait(sh.bar_empty + 8 * si, ((y / TX_NSI) - 1) & 1);
+                mbar_expect_tx(full, bytes);
+                const int yp = y + 1 == g.X1 ? 0 : y + 1, ym = y == 0 ? g.X1 - 1 : y - 1;
+                // float coordinate of the first site of row (yy, zz, tt) inside a parity block: 4 * (lex / 2)
+                auto c0 = [&](int yy, int zz, int tt) { return 2 * (((tt * g.X2 + zz) * g.X1 + yy) * g.X0); };
+                const int rc[7] = {c0(y, z, t), c0(yp, z, t), c0(ym, z, t), c0(y, zp, t), c0(y, zm, t), c0(y, z, tp), c0(y, z, tm)};
+                const unsigned st0 = in0 + (unsigned)si * (unsigned)P.stage;
+#pragma unroll
+                for (int r = 0; r < 7; r++) {
+                    tma_load_2d(st0 + (unsigned)(r * P.row), &tm_s, full, rc[r], 0);
+                    tma_load_2d(st0 + (unsigned)((7 + r) * P.row), &tm_e, full, rc[r], 0);
+                }
+                const unsigned gbase = st0 + (unsigned)(14 * P.row);
+                tma_load_4d(gbase, &tm_gf, full, rc[0], 0, 0, 0);
+                tma_load_4d(gbase + (unsigned)P.gf, &tm_gb, full, rc[2], 0, 1, 0);
+                tma_load_4d(gbase + (unsigned)(P.gf + P.gb), &tm_gb, full, rc[4], 0, 2, 0);
+                tma_load_4d(gbase + (unsigned)(P.gf + 2 * P.gb), &tm_gb, full, rc[6], 0, 3, 0);
+                // pull the rows a few iterations ahead into L2 (costs no shared memory): the y+1 row of
+                // iteration y + TX_PF is the only one of its y-window not requested before
+                const int ya = y + TX_PF;
+                if (ya < g.X1) {
+                    const int yb = ya + 1 == g.X1 ? 0 : ya + 1;
+                    const int pc[5] = {c0(yb, z, t), c0(ya, zp, t), c0(ya, zm, t), c0(ya, z, tp), c0(ya, z, tm)};
+#pragma unroll
+                    for (int r = 0; r < 5; r++) { tma_prefetch_2d(&tm_s, pc[r], 0); tma_prefetch_2d(&tm_e, pc[r], 0); }
+                    tma_prefetch_4d(&tm_gf, pc[0], 0, 0, 0);
+                    tma_prefetch_4d(&tm_gb, pc[2], 0, 2, 0);
+                    tma_prefetch_4d(&tm_gb, pc[4], 0, 3, 0);
+                }
+            }
+        }
+    } else if (warp < TX_NP) {
+        // ================================================================ producers
+        producer_rows(sh, P, g, z, t, warp, lane, A.tb);
+    } else {
+        // ================================================================ consumers
+        typedef P2<float> PP;
+        const int cc = threadIdx.x - TX_NP * 32;        // 0..159
+        T2 Q[NQ];
+#pragma unroll
+        for (int q = 0; q < NQ; q++) Q[q] = PP::make(0.f, 0.f);
+        for (int y = 0; y < g.X1; y++) {
+            const int sc = y % TX_NSC;
+            const T2* v = sh.cbuf + ((size_t)sc * CT_NCC + cc) * CT_BSC;
+            const float* w = sh.swx + ((y + z + t) & 1) * 256;
+            T2 a0 = PP::make(0.f, 0.f), ac[3], as[3];
+#pragma unroll
+            for (int m = 0; m < 3; m++) { ac[m] = PP::make(0.f, 0.f); as[m] = PP::make(0.f, 0.f); }
+            named_bar_sync(1 + sc, TX_NCOMP);
+#pragma unroll 4
+            for (int l = 0; l < g.X0; l++) {
+                const T2 val = v[l];
+                const float* wl = w + l * 8;
+                a0 = PP::add(a0, val);
+#pragma unroll
+                for (int m = 0; m < 3; m++) {
+                    ac[m] = PP::fma_s(wl[2 * m + 1], val, ac[m]);
+                    as[m] = PP::fma_s(wl[2 * m + 2], val, as[m]);
+                }
+            }
+            if (y + TX_NSC < g.X1) named_bar_arrive(1 + TX_NSC + sc, TX_NCOMP);
+            const float* wl = sh.swy + y * 8;
+            float cy[4], sy[4];
+            cy[0] = 1.f; sy[0] = 0.f;
+            cy[1] = wl[1]; sy[1] = wl[2]; cy[2] = wl[3]; sy[2] = wl[4]; cy[3] = wl[5]; sy[3] = wl[6];
+            int q = 0;
+#pragma unroll
+            for (int m = 0; m < 4; m++)
+#pragma unroll
+                for (int n = 0; n < 4; n++) {
+                    if (!PRUNE || m * m + n * n <= 9) {
+                        const T2 xcm = m ? ac[m - 1] : a0;
+                        if (n == 0) Q[q] = PP::add(Q[q], xcm); else Q[q] = PP::fma_s(cy[n], xcm, Q[q]);
+                        q++;
+                        if (n > 0) { Q[q] = PP::fma_s(sy[n], xcm, Q[q]); q++; }
+                        if (m > 0) {
+                            if (n == 0) Q[q] = PP::add(Q[q], as[m - 1]); else Q[q] = PP::fma_s(cy[n], as[m - 1], Q[q]);
+                            q++;
+                        }
+                        if (m > 0 && n > 0) { Q[q] = PP::fma_s(sy[n], as[m - 1], Q[q]); q++; }
+                    }
+                }
+        }
+        T2* qb = reinterpret_cast<T2*>((float*)A.qbuf + (size_t)zt * NQ * CT_THREADS) + cc;
+#pragma unroll
+        for (int q = 0; q < NQ; q++) qb[(size_t)q * CT_NCC] = Q[q];
+    }
+}
+
+// ------------------------------------------------------------------ host side
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn get_encode_fn() {
+    static EncodeTiledFn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess
+            && qres == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+        else
+            cudaGetLastError();
+    }
+    return fn;
+}
+
+static bool encode_map(CUtensorMap* m, const void* base, int rank, const cuuint64_t* dims, const cuuint64_t* strides,
+                       const cuuint32_t* box) {
+    EncodeTiledFn fn = get_encode_fn();
+    if (!fn) return false;
+    cuuint32_t estr[4] = {1, 1, 1, 1};
+    return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, (cuuint32_t)rank, const_cast<void*>(base), dims, strides, box, estr,
+              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+bool tm_contract_tma_usable(const tm_ctx* ctx) {
+    if (ctx->X[0] > 32) return false;
+    if (4 * ctx->Vh >= (size_t)1 << 31) return false;             // TMA coordinates are int32
+    const TxPlan P = tx_plan(ctx->X[0], ctx->X[1]);
+    if (P.total > 227 * 1024) return false;
+    return get_encode_fn() != nullptr;
+}
+
+// s, eta: fp32 full-lattice internal fields; gauge: fp32 reconstruct-12 internal copy; wx, wy: float tables
+tm_status tm_contract_xy_tma(tm_ctx* ctx, void* qbuf, const void* d_s, const void* d_eta, const void* gauge,
+                             const void* wx, const void* wy, int prune, cudaStream_t st) {
+    const int Xh = ctx->Xh;
+    const cuuint64_t Vh = ctx->Vh;
+    CUtensorMap ms, me, mgf, mgb;
+    {
+        const cuuint64_t dims[2] = {4 * Vh, 12};
+        const cuuint64_t strides[1] = {Vh * 16};
+        const cuuint32_t box[2] = {(cuuint32_t)(4 * Xh), 12};
+        if (!encode_map(&ms, d_s, 2, dims, strides, box) || !encode_map(&me, d_eta, 2, dims, strides, box))
+            return tm_fail(ctx, TM_ECUDA, "contract: cuTensorMapEncodeTiled failed (spinor)");
+    }
+    {
+        const cuuint64_t dims[4] = {4 * Vh, 3, 4, 2};
+        const cuuint64_t strides[3] = {Vh * 16, 3 * Vh * 16, 12 * Vh * 16};
+        const cuuint32_t boxf[4] = {(cuuint32_t)(4 * Xh), 3, 4, 2};
+        const cuuint32_t boxb[4] = {(cuuint32_t)(4 * Xh), 3, 1, 2};
+        if (!encode_map(&mgf, gauge, 4, dims, strides, boxf) || !encode_map(&mgb, gauge, 4, dims, strides, boxb))
+            return tm_fail(ctx, TM_ECUDA, "contract: cuTensorMapEncodeTiled failed (gauge)");
+    }
+    TmaContractArgs A;
+    A.qbuf = qbuf; A.wx = (const float*)wx; A.wy = (const float*)wy;
+    A.g = tm_geom(ctx);
+    A.tb = (float)ctx->tb;
+    const TxPlan P = tx_plan(ctx->X[0], ctx->X[1]);
+    const unsigned grid = (unsigned)(ctx->X[2] * ctx->X[3]);
+    if (prune) {
+        TM_CUDA(ctx, cudaFuncSetAttribute(contract_xy_tma_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, P.total));
+        contract_xy_tma_kernel<1><<<grid, TX_NTHREADS, P.total, st>>>(ms, me, mgf, mgb, A);
+    } else {
+        TM_CUDA(ctx, cudaFuncSetAttribute(contract_xy_tma_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, P.total));
+        contract_xy_tma_kernel<0><<<grid, TX_NTHREADS, P.total, st>>>(ms, me, mgf, mgb, A);
+    }
+    TM_LAUNCH_CHECK(ctx, "contract_xy_tma_kernel");
+    return TM_OK;
+}

@@ -59,5 +59,9 @@ tm_status tm_solve_internal(tm_ctx* ctx, void* d_s, const void* d_eta, double ka
 tm_status tm_contract_internal(tm_ctx* ctx, void* d_out, const void* d_s, const void* d_eta,
                                double kappa, double mu, const int* h_momenta, int nmom, tm_prec acc,
                                cudaStream_t st);
+// contract_tma.cu: TMA-staged fast path of the site + x/y-DFT stage (fp32, Lx <= 32)
+bool tm_contract_tma_usable(const tm_ctx* ctx);
+tm_status tm_contract_xy_tma(tm_ctx* ctx, void* qbuf, const void* d_s, const void* d_eta, const void* gauge,
+                             const void* wx, const void* wy, int prune, cudaStream_t st);
 // acc += x on complex128 arrays of n complex numbers
 tm_status tm_accumulate(tm_ctx* ctx, void* d_acc, const void* d_x, size_t n, cudaStream_t st);
