@@ -45,6 +45,19 @@ def peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
+def ncu_traffic(prec):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
+    `ncu --set full` summary (text) of the same kernel, or None when no capture of it is committed."""
+    import re
+    p = os.path.join(ROOT, "profiles", "r01_dslash16_%s.md" % prec)
+    if not os.path.exists(p):
+        return None, None
+    tot, scale = 0.0, {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+    for m in re.finditer(r"`dram__bytes_(?:read|write)\.sum` \| ([0-9.,]+) \| (\w+)", open(p).read()):
+        tot += float(m.group(1).replace(",", "")) * scale[m.group(2)]
+    return (tot or None), "profiles/" + os.path.basename(p)
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
     Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
@@ -324,12 +337,7 @@ def run_b200(args, cfg):
                 "traffic": None, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": dslash_bytes_per_site(LP["sloppy"], 12, True) * Vh,
                 "how": "CUDA events around %d back-to-back launches on the current stream, 4 rotating field pairs" % napp}
-    prof = os.path.join(ROOT, "profiles", "dslash_traffic.json")
-    if os.path.exists(prof):
-        try:
-            roofline["traffic"] = json.load(open(prof)).get(LP["sloppy"] + "_r12_xpay_bytes_per_launch")
-        except Exception:
-            pass
+    roofline["traffic"], roofline["traffic_source"] = ncu_traffic(LP["sloppy"])
 
     it_lp = np.mean([i["iters_lp"] for i in infos])
     it_hp = np.mean([i["iters_hp"] for i in infos])
