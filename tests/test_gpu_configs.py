@@ -1,0 +1,123 @@
+"""GPU parity on BASELINE.json's other configs (c2, c3, c5), each as the config describes it.
+
+  c2  16^3x32: repeated Dslash applications at fp64/fp32/fp16/bf16 storage with reconstruct-12 and -18
+      (first application against the oracle, the repeats must reproduce it bit for bit), one fp32 CG
+      solve to rho = 1e-8 from a Z4 source;
+  c3  24^3x48: the small TSM run (N_LP = 100 at 16-bit storage to 1e-2, N_HP = 10 mixed to 1e-8, 160
+      insertions, 33 momenta), checked by decomposition: the oracle's combiner on the
+      GPU's per-source arrays, HP per-source arrays of sampled sources against the oracle end to end;
+  c5  48^3x96: the bandwidth-sweep lattice -- one full operator application per storage precision
+      against the oracle's apply_M on all 10.6 M sites (non-power-of-two extents: x-rows straddle warps).
+Inputs: the seeded recipes of DESIGN.md sec 4, generated on the device by inputs_torch.
+"""
+import numpy as np
+import pytest
+
+from gpu_util import rel_l2, tm, to_np
+from paper_1401_6750_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+TOL = {"f64": 1e-13, "f32": 1e-6, "f16": 5e-3, "bf16": 5e-3}
+
+
+def setup(name):
+    import torch
+    from paper_1401_6750_b200 import inputs_torch
+    t = tm()
+    c = inputs.CONFIGS[name]
+    dev = torch.device("cuda", 0)
+    U = inputs_torch.gauge_field(c["dims"], c["eps"], c["seed"], dev)
+    ctx = t.TmContext(c["dims"], -1, 0)
+    ctx.tm_load_gauge(U)
+    U_h = U.cpu().numpy()
+    del U
+    return t, c, ctx, U_h, dev
+
+
+def gaussian_spinor(dims, seed):
+    import torch
+    lx, ly, lz, lt = dims
+    g = torch.Generator(device="cpu")
+    g.manual_seed(seed)
+    return torch.view_as_complex(torch.randn((lt, lz, ly, lx, 4, 3, 2), generator=g, dtype=torch.float64)).numpy()
+
+
+def test_c2_dslash_all_precisions_and_fp32_solve(orc):
+    from paper_1401_6750_b200 import inputs_torch
+    t, c, ctx, U_h, dev = setup("c2")
+    try:
+        psi = gaussian_spinor(c["dims"], 21)
+        ref = orc.apply_M(psi, U_h, c["kappa"], c["mu"], -1)
+        for prec in ("f64", "f32", "f16", "bf16"):
+            for recon in (12, 18):
+                P = t.PREC[prec]
+                fin = ctx.tm_field_import(psi, P)
+                fout = ctx.empty_field(P, True)
+                ctx.tm_dslash(fout, fin, None, t.TM_OP_M_FULL, 0, False, c["kappa"], c["mu"], P, recon)
+                first = fout.clone()
+                assert rel_l2(to_np(ctx.tm_field_export(fout, P)), ref) <= TOL[prec], (prec, recon)
+                # "repeated applications": same input, same launch, same bits (no race, no stale state)
+                for _ in range(50):
+                    ctx.tm_dslash(fout, fin, None, t.TM_OP_M_FULL, 0, False, c["kappa"], c["mu"], P, recon)
+                assert bool((fout == first).all()), (prec, recon)
+        eta = inputs_torch.z4_source(c["dims"], c["src_seed"], 0, dev)
+        # pure fp32 (sloppy = outer = fp32): fp32 cannot certify 1e-8 (eps = 6e-8), so the solver may stop at its
+        # floor and say so (TM_ENOCONV); whatever it reports must agree with the oracle's evaluation
+        s, info = ctx.tm_cg_solve(eta, c["kappa"], c["mu"], "f32", "f32", 12, 1e-8, 5000, raise_on_noconv=False)
+        true = orc.true_residual(to_np(s), to_np(eta), U_h, c["kappa"], c["mu"], -1)
+        print("c2 fp32/fp32:", info, true)
+        assert true <= 5e-7 and abs(info["true_resid"] - true) <= 2e-7, (true, info)
+        assert info["status"] == t.TM_ENOCONV or true <= 1e-8
+        s, info = ctx.tm_cg_solve(eta, c["kappa"], c["mu"], "f32", "f64", 12, 1e-8, 5000)
+        true = orc.true_residual(to_np(s), to_np(eta), U_h, c["kappa"], c["mu"], -1)
+        assert true <= 1e-8 and abs(info["true_resid"] - true) <= 5e-10, (true, info)
+    finally:
+        ctx.close()
+
+
+def test_c3_small_tsm_run(orc):
+    t, c, ctx, U_h, dev = setup("c3")
+    try:
+        n_lp, n_hp = c["n_lp"], c["n_hp"]
+        mom = inputs.momentum_list(c["p2max"])
+        assert len(mom) == 33
+        lp = dict(sloppy="bf16", outer="f32", recon=12, rho=1e-2, max_iter=2000, delta=0.01)
+        hp = dict(sloppy="f32", outer="f64", recon=12, rho=1e-8, max_iter=5000, delta=0.01)
+        out, ps, info = ctx.tsm_estimate(n_lp, n_hp, c["kappa"], c["mu"], mom, lp, hp, t.TM_F32, t.TM_F64,
+                                         seed=c["src_seed"], per_source=True)
+        assert info["worst_resid_lp"] <= 1e-2 and info["worst_resid_hp"] <= 1e-8
+        out, ps = to_np(out), to_np(ps)
+        assert rel_l2(out, orc.tsm_combine(ps[:n_lp], ps[n_lp:])) <= 1e-12
+        from paper_1401_6750_b200 import inputs_torch
+        for r in (0, n_hp - 1):
+            eta = inputs_torch.z4_source(c["dims"], c["src_seed"], r, dev)
+            # the GPU's own HP solution: residual by the oracle, loops of that solution by the oracle
+            s, _ = ctx.tm_cg_solve(eta, c["kappa"], c["mu"], **hp)
+            s_h, eta_h = to_np(s), to_np(eta)
+            assert orc.true_residual(s_h, eta_h, U_h, c["kappa"], c["mu"], -1) <= 1e-8
+            for ts in (0, 47):
+                ref = orc.loops_project(s_h, eta_h, U_h, c["kappa"], c["mu"], mom, -1, ts, ts + 1)[..., ts]
+                for f in (0, 1):
+                    for sl in (slice(0, 16), slice(16, 80)):
+                        assert rel_l2(ps[n_lp + r][f, sl, :, ts], ref[f, sl]) <= 1e-10, (r, ts, f)
+                        # the LP loop of the same source is O(rho_LP) away, not equal
+                        assert rel_l2(ps[r][f, sl, :, ts], ref[f, sl]) <= 0.2
+    finally:
+        ctx.close()
+
+
+@pytest.mark.parametrize("prec,recon", [("f16", 12), ("bf16", 12), ("f32", 12), ("f64", 12), ("f16", 18)])
+def test_c5_operator(orc, prec, recon, c5_case):
+    t, c, ctx, psi, ref = c5_case
+    got = to_np(ctx.apply_M(psi, c["kappa"], c["mu"], t.PREC[prec], recon))
+    assert rel_l2(got, ref) <= TOL[prec], (prec, recon)
+
+
+@pytest.fixture(scope="module")
+def c5_case(orc):
+    t, c, ctx, U_h, dev = setup("c5")
+    psi = gaussian_spinor(c["dims"], 55)
+    ref = orc.apply_M(psi, U_h, c["kappa"], c["mu"], -1)
+    del U_h
+    yield t, c, ctx, psi, ref
+    ctx.close()
