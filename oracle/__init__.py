@@ -153,3 +153,36 @@ def tsm_combine(lp, hp) -> np.ndarray:
     lib().orc_tsm_combine(out.ctypes.data_as(ctypes.c_void_p), p_lp, ctypes.c_int(n_lp), p_hp,
                           ctypes.c_int(n_hp), ctypes.c_long(ln))
     return out
+
+
+def binary_nfiles(n: int) -> int:
+    """Number of files n sources touch: the smallest K with 2^K - 1 >= n."""
+    k = 0
+    while (1 << k) - 1 < n:
+        k += 1
+    return k
+
+
+def binary_store(per_source):
+    """sec 2.1.1 / Fig. 2: per_source [n, ...] -> (files [K, ...], counts [K]); file k sums sources 2^k-1 .. 2^(k+1)-2."""
+    ps, p_ps = _c(per_source)
+    n = ps.shape[0]
+    ln = int(np.prod(ps.shape[1:]))
+    K = binary_nfiles(n)
+    files = np.empty((K,) + ps.shape[1:], dtype=np.complex128)
+    counts = np.zeros(K, dtype=np.int32)
+    lib().orc_binary_store(files.ctypes.data_as(ctypes.c_void_p), counts.ctypes.data_as(ctypes.c_void_p), p_ps,
+                           ctypes.c_int(n), ctypes.c_long(ln))
+    return files, counts
+
+
+def binary_recover(files, counts, N: int):
+    """Estimator from N sources = sum of the files named by the binary digits of N, / N (None if not recoverable)."""
+    f, p_f = _c(files)
+    counts = np.ascontiguousarray(counts, dtype=np.int32)
+    out = np.empty(f.shape[1:], dtype=np.complex128)
+    ln = int(np.prod(f.shape[1:]))
+    lib().orc_binary_recover.restype = ctypes.c_int
+    st = lib().orc_binary_recover(out.ctypes.data_as(ctypes.c_void_p), p_f, counts.ctypes.data_as(ctypes.c_void_p),
+                                  ctypes.c_int(f.shape[0]), ctypes.c_int(N), ctypes.c_long(ln))
+    return out if st == 0 else None

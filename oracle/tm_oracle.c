@@ -16,6 +16,7 @@
  *                               [(1-g_mu) U_mu(x) d_{x+mu,y} + (1+g_mu) U_mu^dag(x-mu) d_{x-mu,y}]
  *                                                                   -> orc_apply_M
  *   sec 2.1  PAPER.md:56-58     TSM: N_LP low precision + N_HP correction -> orc_tsm_combine
+ *   sec 2.1.1, Fig. 2  binary storage of partial sums       -> orc_binary_store / _recover
  *   sec 2.1.1 PAPER.md:72       one-end trick, 16 ultra-local + 64 one-derivative
  *                               insertions, with/without tau3 = 160  -> orc_loops_sites
  *   sec 2.2  PAPER.md:86        colour trace, Dirac indices open; covariant derivative
@@ -27,7 +28,8 @@
  * hermiticity; free-field plane waves vs the momentum-space closed form;
  * gauge covariance / invariance; dense assembly + LU on 2^4; full-dilution
  * loops vs traces of dense inverses; summation by parts; numpy.fft cross-check
- * of the projection; TSM identity.  No function here is "parity unpinned".
+ * of the projection; TSM identity; Fig. 2's 13-source example of the binary
+ * storage.  No function here is "parity unpinned".
  *
  * Conventions (readings 1-7,15,16): dims = {Lx,Ly,Lz,T}; site index
  * ((t*Lz+z)*Ly+y)*Lx+x; directions mu = 0,1,2,3 = x,y,z,t; spinor
@@ -408,4 +410,44 @@ void orc_tsm_combine(cplx *out, const cplx *lp, int n_lp, const cplx *hp, int n_
         for (int r = 0; r < n_hp; r++) b += hp[(long)r * len + j] - lp[(long)r * len + j];
         out[j] = a / n_lp + (n_hp > 0 ? b / n_hp : 0);
     }
+}
+
+/* sec 2.1.1 (Fig. 2) + DESIGN.md reading 21: binary storage of partial sums.
+ * "in File.1 we store the contractions generated with one stochastic source, in File.2 we store the
+ * sum of the contractions coming from the second and the third stochastic source, and so on":
+ * file k = 0,1,2,... (the paper's File.2^k) holds the sum over the 2^k sources r = 2^k - 1 ... 2^(k+1) - 2.
+ * per_source: [n][len]; files: [nfiles][len] with nfiles = floor(log2(n)) + 1 (the last file may be
+ * incomplete when n + 1 is not a power of two); counts[k] = number of sources summed into file k. */
+void orc_binary_store(cplx *files, int *counts, const cplx *per_source, int n, long len)
+{
+    int nfiles = 0;
+    while (((1L << nfiles) - 1) < n) nfiles++;          /* smallest K with 2^K - 1 >= n */
+    for (int k = 0; k < nfiles; k++) {
+        counts[k] = 0;
+        for (long j = 0; j < len; j++) files[(long)k * len + j] = 0;
+    }
+    for (int r = 0; r < n; r++) {
+        int k = 0;
+        while (((1L << (k + 1)) - 1) <= r) k++;          /* 2^k - 1 <= r < 2^(k+1) - 1 */
+        counts[k] += 1;
+        for (long j = 0; j < len; j++) files[(long)k * len + j] += per_source[(long)r * len + j];
+    }
+}
+
+/* "Reconstruction is straightforward, taking into account the base-2 structure": the estimator from N
+ * sources is the sum of the files whose weight 2^k is a binary digit of N, divided by N (Fig. 2:
+ * N = 13 = 1101b -> the files with 1, 4 and 8 sources).  Returns 0, or -1 when a needed file does not
+ * exist or is incomplete (counts[k] != 2^k). */
+int orc_binary_recover(cplx *out, const cplx *files, const int *counts, int nfiles, int N, long len)
+{
+    if (N < 1) return -1;
+    for (int k = 0; (1L << k) <= N; k++)
+        if ((N >> k) & 1)
+            if (k >= nfiles || counts[k] != (1 << k)) return -1;
+    for (long j = 0; j < len; j++) out[j] = 0;
+    for (int k = 0; (1L << k) <= N; k++)
+        if ((N >> k) & 1)
+            for (long j = 0; j < len; j++) out[j] += files[(long)k * len + j];
+    for (long j = 0; j < len; j++) out[j] /= N;
+    return 0;
 }

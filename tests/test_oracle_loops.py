@@ -189,3 +189,36 @@ def test_tsm_combine(orc):
     assert np.allclose(orc.tsm_combine(lp, hp[:0]), lp.mean(axis=0), atol=1e-14)  # no correction
     hp3 = hp[:3]
     assert np.allclose(orc.tsm_combine(lp, hp3), lp.mean(0) + (hp3 - lp[:3]).mean(0), atol=1e-14)
+
+
+def test_binary_storage_fig2(orc):
+    """sec 2.1.1 / Fig. 2: the 13-source example, hand-worked in tests/golden/binary_storage_example.txt."""
+    v = (np.arange(15) + 1.0).astype(np.complex128).reshape(15, 1)
+    files, counts = orc.binary_store(v)
+    assert list(counts) == [1, 2, 4, 8]
+    assert np.allclose(files[:, 0], [1, 5, 22, 92])
+    golden = np.loadtxt(os.path.join(os.path.dirname(__file__), "golden", "binary_storage_example.txt"))
+    for N, tot in golden:
+        got = orc.binary_recover(files, counts, int(N))
+        assert got is not None and abs(got[0] - tot / N) < 1e-14, (N, got)
+    # 13 = 1101b uses exactly the sources {0} + {3..6} + {7..14}: brute force over those subsets
+    rng = np.random.default_rng(3)
+    ps = rng.normal(size=(15, 4, 3)) + 1j * rng.normal(size=(15, 4, 3))
+    files, counts = orc.binary_store(ps)
+    sel = [0] + list(range(3, 7)) + list(range(7, 15))
+    assert len(sel) == 13
+    assert np.allclose(orc.binary_recover(files, counts, 13), ps[sel].mean(axis=0), atol=1e-14)
+    # any N <= 15 is recoverable and is a mean over N distinct sources; a full set is the plain mean
+    for N in range(1, 16):
+        sel = [r for k in range(4) if (N >> k) & 1 for r in range(2 ** k - 1, 2 ** (k + 1) - 1)]
+        assert len(sel) == N
+        assert np.allclose(orc.binary_recover(files, counts, N), ps[sel].mean(axis=0), atol=1e-14)
+    assert np.allclose(orc.binary_recover(files, counts, 15), ps.mean(axis=0), atol=1e-14)
+    # an incomplete last file (13 sources generated) cannot serve N = 8..15, the complete ones still serve N <= 7
+    files, counts = orc.binary_store(ps[:13])
+    assert list(counts) == [1, 2, 4, 6]
+    assert orc.binary_recover(files, counts, 13) is None and orc.binary_recover(files, counts, 16) is None
+    assert np.allclose(orc.binary_recover(files, counts, 7), ps[:7].mean(axis=0), atol=1e-14)
+    assert np.allclose(files.sum(axis=0) / 13, ps[:13].mean(axis=0), atol=1e-14)      # nothing is lost
+    # O(log2 N) files
+    assert [orc.binary_nfiles(n) for n in (1, 2, 3, 4, 7, 8, 500, 1023)] == [1, 2, 2, 3, 3, 4, 9, 10]
