@@ -122,6 +122,29 @@ tm_status tsm_estimate(tm_ctx* ctx, void* d_out, void* d_per_source, const tsm_p
 tm_status tsm_estimate_host(tm_ctx* ctx, void* h_out, const unsigned char* h_z4,
                             const tsm_params* params, tsm_info* info, void* stream);
 
+/* sec 2.1.1 (Fig. 2): binary storage of partial sums, on the device, in momentum space.
+ * File k = 0, 1, 2, ... (the paper's File.2^k) holds the SUM of the per-source arrays of the 2^k sources
+ * r = 2^k - 1 ... 2^(k+1) - 2, so n sources need loop_binary_nfiles(n) = ceil(log2(n + 1)) arrays instead of n.
+ *   loop_binary_accumulate: d_files[k(r)] += d_loop   (k(r) = floor(log2(r + 1)))
+ *   loop_binary_recover:    d_out = (sum of the files named by the binary digits of N) / N
+ *                           ("Reconstruction is straightforward, taking into account the base-2 structure";
+ *                           Fig. 2: N = 13 = 1101b -> the files holding 8, 4 and 1 sources).
+ * d_files: device complex128 [nfiles][len], zeroed by the caller before the first source; d_loop, d_out:
+ * device complex128 [len]; len = number of complex entries of one per-source array (160 * nmom * T).
+ * n_stored = number of sources accumulated so far: recover returns TM_EARG when N needs a file that is
+ * missing or not yet complete.  Asynchronous on stream. */
+int loop_binary_nfiles(int n_sources);
+tm_status loop_binary_accumulate(tm_ctx* ctx, void* d_files, const void* d_loop, int r, size_t len, void* stream);
+tm_status loop_binary_recover(tm_ctx* ctx, void* d_out, const void* d_files, int n_stored, int N, size_t len,
+                              void* stream);
+/* tsm_estimate that also fills the binary-storage files (either may be NULL):
+ *   d_files_lp   [loop_binary_nfiles(n_lp)][2][80][nmom][T]: file k += l_r^LP              for every r < n_lp
+ *   d_files_corr [loop_binary_nfiles(n_hp)][2][80][nmom][T]: file k += l_r^HP - l_r^LP     for every r < n_hp
+ * so that the TSM estimate of any (N_LP', N_HP') with complete files is
+ *   recover(files_lp, N_LP') + recover(files_corr, N_HP').  Both are zeroed inside the call. */
+tm_status tsm_estimate_binary(tm_ctx* ctx, void* d_out, void* d_files_lp, void* d_files_corr,
+                              const tsm_params* params, tsm_info* info, void* stream);
+
 /* number of kernels launched by this context so far (bench.py's gpu_launches) */
 long tm_launch_count(const tm_ctx* ctx);
 

@@ -32,6 +32,7 @@ EXPORTS = [
     "tm_create", "tm_destroy", "tm_last_error", "tm_load_gauge", "tm_field_bytes",
     "tm_field_import", "tm_field_export", "tm_dslash", "tm_cg_solve", "loop_contract_project",
     "tsm_estimate", "tsm_estimate_host", "tm_launch_count",
+    "loop_binary_nfiles", "loop_binary_accumulate", "loop_binary_recover", "tsm_estimate_binary",
 ]
 
 
@@ -98,6 +99,11 @@ def load_library():
     L.loop_contract_project.argtypes = [vp, vp, vp, vp, cd, cd, ctypes.POINTER(ci), ci, ci, vp]
     L.tsm_estimate.argtypes = [vp, vp, vp, ctypes.POINTER(tsm_params), ctypes.POINTER(tsm_info), vp]
     L.tsm_estimate_host.argtypes = [vp, vp, vp, ctypes.POINTER(tsm_params), ctypes.POINTER(tsm_info), vp]
+    L.loop_binary_nfiles.argtypes = [ci]
+    L.loop_binary_nfiles.restype = ci
+    L.loop_binary_accumulate.argtypes = [vp, vp, vp, ci, ctypes.c_size_t, vp]
+    L.loop_binary_recover.argtypes = [vp, vp, vp, ci, ci, ctypes.c_size_t, vp]
+    L.tsm_estimate_binary.argtypes = [vp, vp, vp, vp, ctypes.POINTER(tsm_params), ctypes.POINTER(tsm_info), vp]
     L.tm_launch_count.argtypes = [vp]
     L.tm_launch_count.restype = ctypes.c_long
     _lib = L
@@ -301,6 +307,42 @@ class TmContext:
                                    ctypes.byref(P), ctypes.byref(info), _stream())
         self._check(st, allow=() if raise_on_noconv else (TM_ENOCONV,))
         return out, ps, self._tsm_info(info, st)
+
+    # ------------------------------------------------------------------ binary storage (sec 2.1.1, Fig. 2)
+    def loop_binary_nfiles(self, n_sources: int) -> int:
+        return int(self.lib.loop_binary_nfiles(int(n_sources)))
+
+    def loop_binary_accumulate(self, files, loop, r: int):
+        """files: complex128 cuda tensor [nfiles, ...] (zeroed by the caller); loop: one per-source array."""
+        self._check(self.lib.loop_binary_accumulate(self.h, files.data_ptr(), loop.data_ptr(), int(r),
+                                                    loop.numel(), _stream()))
+
+    def loop_binary_recover(self, files, n_stored: int, N: int):
+        torch = _torch()
+        out = torch.empty(files.shape[1:], dtype=torch.complex128, device=self.tdev)
+        self._check(self.lib.loop_binary_recover(self.h, out.data_ptr(), files.data_ptr(), int(n_stored), int(N),
+                                                 out.numel(), _stream()))
+        return out
+
+    def tsm_estimate_binary(self, n_lp, n_hp, kappa, mu, momenta, lp, hp, acc_lp=TM_F32, acc_hp=TM_F64,
+                            z4=None, seed=0, raise_on_noconv=True):
+        """tsm_estimate that also returns the binary-storage files: (out, files_lp, files_corr, info)."""
+        torch = _torch()
+        d_z4 = None
+        if z4 is not None:
+            z4 = self._dev(z4, torch.uint8)
+            assert z4.numel() == n_lp * 3 * self.V
+            d_z4 = z4.data_ptr()
+        P, mom = self._tsm_params(n_lp, n_hp, kappa, mu, momenta, lp, hp, acc_lp, acc_hp, d_z4, seed)
+        shape = (2, 80, len(mom), self.T)
+        out = torch.empty(shape, dtype=torch.complex128, device=self.tdev)
+        f_lp = torch.empty((self.loop_binary_nfiles(n_lp),) + shape, dtype=torch.complex128, device=self.tdev)
+        f_co = torch.empty((max(1, self.loop_binary_nfiles(n_hp)),) + shape, dtype=torch.complex128, device=self.tdev)
+        info = tsm_info()
+        st = self.lib.tsm_estimate_binary(self.h, out.data_ptr(), f_lp.data_ptr(), f_co.data_ptr() if n_hp else None,
+                                          ctypes.byref(P), ctypes.byref(info), _stream())
+        self._check(st, allow=() if raise_on_noconv else (TM_ENOCONV,))
+        return out, f_lp, (f_co if n_hp else None), self._tsm_info(info, st)
 
     def tsm_estimate_host(self, n_lp, n_hp, kappa, mu, momenta, lp, hp, acc_lp=TM_F32, acc_hp=TM_F64,
                           z4_host=None, seed=0, out_host=None, raise_on_noconv=True):

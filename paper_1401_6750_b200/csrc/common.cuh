@@ -92,7 +92,7 @@ enum {
     WS_OU_Y, WS_OU_B, WS_OU_R, WS_OU_TMP, WS_OU_TMP2,           // outer precision parity vectors
     WS_OU_ETA, WS_OU_S,                                         // outer precision full-lattice fields
     WS_CT_S, WS_CT_ETA, WS_CT_PLANES, WS_CT_OUT,                // contraction
-    WS_TSM_ACC, WS_TSM_ETA32, WS_TSM_ETA64, WS_TSM_S32, WS_TSM_S64, WS_TSM_Z4,
+    WS_TSM_ACC, WS_TSM_ETA32, WS_TSM_ETA64, WS_TSM_S32, WS_TSM_S64, WS_TSM_Z4, WS_TSM_KEEP,
     WS_API_A, WS_API_B, WS_API_C
 };
 tm_status tm_ws(tm_ctx* c, int slot, size_t bytes, void** out);     // api.cu

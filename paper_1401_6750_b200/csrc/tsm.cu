@@ -29,6 +29,63 @@ __global__ void tsm_combine_kernel(double* __restrict__ out, const double* __res
     out[i] = slp[i] * inv_lp + (shp[i] - slpc[i]) * inv_hp;
 }
 
+// binary storage (sec 2.1.1): file += x  |  file += x - y
+__global__ void binary_add_kernel(double* __restrict__ file, const double* __restrict__ x,
+                                  const double* __restrict__ y, size_t n) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    file[i] += y ? x[i] - y[i] : x[i];
+}
+// out = (sum of the files whose bit is set in mask) / N, summed in ascending file order
+__global__ void binary_recover_kernel(double* __restrict__ out, const double* __restrict__ files, unsigned mask,
+                                      double inv_n, size_t n) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    double s = 0.0;
+    for (int k = 0; k < 32; k++)
+        if ((mask >> k) & 1u) s += files[(size_t)k * n + i];
+    out[i] = s * inv_n;
+}
+
+static inline int binary_file_of(int r) {       // 2^k - 1 <= r < 2^(k+1) - 1
+    int k = 0;
+    while (((1L << (k + 1)) - 1) <= r) k++;
+    return k;
+}
+
+extern "C" int loop_binary_nfiles(int n_sources) {
+    int k = 0;
+    while (((1L << k) - 1) < n_sources) k++;
+    return k;
+}
+
+extern "C" tm_status loop_binary_accumulate(tm_ctx* ctx, void* d_files, const void* d_loop, int r, size_t len,
+                                            void* stream) {
+    if (!ctx || !d_files || !d_loop || r < 0 || len == 0) return tm_fail(ctx, TM_EARG, "loop_binary_accumulate: bad argument");
+    TM_CUDA(ctx, cudaSetDevice(ctx->device));
+    const size_t nr = 2 * len;
+    binary_add_kernel<<<(unsigned)((nr + 255) / 256), 256, 0, (cudaStream_t)stream>>>(
+        (double*)d_files + (size_t)binary_file_of(r) * nr, (const double*)d_loop, nullptr, nr);
+    TM_LAUNCH_CHECK(ctx, "binary_add_kernel");
+    return TM_OK;
+}
+
+extern "C" tm_status loop_binary_recover(tm_ctx* ctx, void* d_out, const void* d_files, int n_stored, int N,
+                                         size_t len, void* stream) {
+    if (!ctx || !d_out || !d_files || len == 0) return tm_fail(ctx, TM_EARG, "loop_binary_recover: bad argument");
+    if (N < 1 || N > n_stored) return tm_fail(ctx, TM_EARG, "loop_binary_recover: need 1 <= N <= n_stored");
+    // file k is complete when all of its 2^k sources are in: 2^(k+1) - 1 <= n_stored
+    for (int k = 0; (1L << k) <= N; k++)
+        if (((N >> k) & 1) && ((1L << (k + 1)) - 1) > n_stored)
+            return tm_fail(ctx, TM_EARG, "loop_binary_recover: N needs a file that is not complete yet");
+    TM_CUDA(ctx, cudaSetDevice(ctx->device));
+    const size_t nr = 2 * len;
+    binary_recover_kernel<<<(unsigned)((nr + 255) / 256), 256, 0, (cudaStream_t)stream>>>(
+        (double*)d_out, (const double*)d_files, (unsigned)N, 1.0 / N, nr);
+    TM_LAUNCH_CHECK(ctx, "binary_recover_kernel");
+    return TM_OK;
+}
+
 // full-lattice field precision conversion (two parity blocks)
 static tm_status convert_full(tm_ctx* ctx, void* dst, tm_prec pd, const void* src, tm_prec ps, cudaStream_t st) {
     for (int p = 0; p < 2; p++)
@@ -38,7 +95,8 @@ static tm_status convert_full(tm_ctx* ctx, void* dst, tm_prec pd, const void* sr
 }
 
 static tm_status tsm_core(tm_ctx* ctx, void* d_out, void* d_per_source, const tsm_params* P, tsm_info* info,
-                          const unsigned char* z4, int z4_on_host, cudaStream_t st) {
+                          const unsigned char* z4, int z4_on_host, cudaStream_t st,
+                          void* d_files_lp = nullptr, void* d_files_corr = nullptr) {
     if (!P || !d_out) return tm_fail(ctx, TM_EARG, "tsm_estimate: null argument");
     if (P->n_lp < 1 || P->n_hp < 0 || P->n_hp > P->n_lp)
         return tm_fail(ctx, TM_EARG, "tsm_estimate: need 1 <= n_lp and 0 <= n_hp <= n_lp");
@@ -58,6 +116,12 @@ static tm_status tsm_core(tm_ctx* ctx, void* d_out, void* d_per_source, const ts
     TM_TRY(tm_ws(ctx, WS_TSM_ACC, 4 * nr * sizeof(double), (void**)&acc));
     double *S_lp = acc, *S_lpc = acc + nr, *S_hp = acc + 2 * nr, *tmp = acc + 3 * nr;
     TM_CUDA(ctx, cudaMemsetAsync(acc, 0, 3 * nr * sizeof(double), st));
+    double* lp_keep = nullptr;          // l_r^LP kept until l_r^HP is known (binary files of the correction)
+    if (d_files_lp) TM_CUDA(ctx, cudaMemsetAsync(d_files_lp, 0, (size_t)loop_binary_nfiles(P->n_lp) * nr * sizeof(double), st));
+    if (d_files_corr && P->n_hp) {
+        TM_CUDA(ctx, cudaMemsetAsync(d_files_corr, 0, (size_t)loop_binary_nfiles(P->n_hp) * nr * sizeof(double), st));
+        TM_TRY(tm_ws(ctx, WS_TSM_KEEP, nr * sizeof(double), (void**)&lp_keep));
+    }
     void *eta32 = nullptr, *eta64 = nullptr, *s32 = nullptr, *s64 = nullptr, *z4dev = nullptr;
     const bool need32 = po_lp == TM_F32 || ac_lp == TM_F32 || (P->n_hp && (po_hp == TM_F32 || ac_hp == TM_F32));
     const bool need64 = po_lp == TM_F64 || ac_lp == TM_F64 || (P->n_hp && (po_hp == TM_F64 || ac_hp == TM_F64));
@@ -124,6 +188,17 @@ static tm_status tsm_core(tm_ctx* ctx, void* d_out, void* d_per_source, const ts
             if (pass) tsm_accumulate_kernel<<<agrid, 256, 0, st>>>(S_hp, nullptr, copy, tmp, nr);
             else      tsm_accumulate_kernel<<<agrid, 256, 0, st>>>(S_lp, do_hp ? S_lpc : nullptr, copy, tmp, nr);
             TM_LAUNCH_CHECK(ctx, "tsm_accumulate_kernel");
+            if (!pass && d_files_lp) {
+                binary_add_kernel<<<agrid, 256, 0, st>>>((double*)d_files_lp + (size_t)binary_file_of(r) * nr, tmp, nullptr, nr);
+                TM_LAUNCH_CHECK(ctx, "binary_add_kernel");
+            }
+            if (lp_keep && do_hp) {
+                if (!pass) TM_CUDA(ctx, cudaMemcpyAsync(lp_keep, tmp, nr * sizeof(double), cudaMemcpyDeviceToDevice, st));
+                else {
+                    binary_add_kernel<<<agrid, 256, 0, st>>>((double*)d_files_corr + (size_t)binary_file_of(r) * nr, tmp, lp_keep, nr);
+                    TM_LAUNCH_CHECK(ctx, "binary_add_kernel");
+                }
+            }
         }
     }
     tsm_combine_kernel<<<agrid, 256, 0, st>>>((double*)d_out, S_lp, S_lpc, S_hp, 1.0 / P->n_lp,
@@ -152,6 +227,12 @@ extern "C" tm_status tsm_estimate(tm_ctx* ctx, void* d_out, void* d_per_source, 
                                   tsm_info* info, void* stream) {
     if (!ctx) return TM_EARG;
     return tsm_core(ctx, d_out, d_per_source, P, info, P ? P->d_z4 : nullptr, 0, (cudaStream_t)stream);
+}
+
+extern "C" tm_status tsm_estimate_binary(tm_ctx* ctx, void* d_out, void* d_files_lp, void* d_files_corr,
+                                         const tsm_params* P, tsm_info* info, void* stream) {
+    if (!ctx) return TM_EARG;
+    return tsm_core(ctx, d_out, nullptr, P, info, P ? P->d_z4 : nullptr, 0, (cudaStream_t)stream, d_files_lp, d_files_corr);
 }
 
 extern "C" tm_status tsm_estimate_host(tm_ctx* ctx, void* h_out, const unsigned char* h_z4, const tsm_params* P,

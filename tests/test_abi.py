@@ -12,7 +12,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 def _declared():
     src = open(os.path.join(ROOT, "include", "tmloops.h")).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    names = re.findall(r"\b(?:tm_status|size_t|const char\*|long)\s+(\w+)\s*\(", src)
+    names = re.findall(r"\b(?:tm_status|size_t|const char\*|long|int)\s+(\w+)\s*\(", src)
     return sorted(set(names))
 
 
