@@ -7,6 +7,50 @@ static char g_last_error[512] = "";
 extern "C" const char* tm_last_error(const tm_ctx* ctx) { return ctx ? ctx->err : g_last_error; }
 extern "C" long tm_launch_count(const tm_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
+// allocate the private resources of a lane into the context's active fields
+static bool lane_alloc(tm_ctx* c, int lane) {
+    bool ok = cudaMalloc((void**)&c->d_partials, sizeof(double) * (1 << 18)) == cudaSuccess
+           && cudaMalloc((void**)&c->d_counter, sizeof(unsigned int) * 4) == cudaSuccess
+           && cudaMalloc((void**)&c->d_scal, sizeof(CgScalars)) == cudaSuccess
+           && cudaMallocHost((void**)&c->h_scal, sizeof(CgScalars)) == cudaSuccess
+           && cudaMemset(c->d_counter, 0, sizeof(unsigned int) * 4) == cudaSuccess
+           && cudaMemset(c->d_scal, 0, sizeof(CgScalars)) == cudaSuccess;
+    for (int i = 0; ok && i < TM_NEVENTS; i++) ok = cudaEventCreate(&c->ev[i]) == cudaSuccess;
+    if (ok && lane > 0) ok = cudaStreamCreateWithFlags(&c->lane_stream, cudaStreamNonBlocking) == cudaSuccess;
+    return ok;
+}
+
+static void lane_park(tm_ctx* c, TmLane* L) {          // active fields -> L
+    L->ready = 1;
+    L->d_partials = c->d_partials; L->d_counter = c->d_counter; L->d_scal = c->d_scal; L->h_scal = c->h_scal;
+    memcpy(L->scratch, c->scratch, sizeof(c->scratch));
+    memcpy(L->scratch_bytes, c->scratch_bytes, sizeof(c->scratch_bytes));
+    memcpy(L->ev, c->ev, sizeof(c->ev));
+    L->stream = c->lane_stream;
+}
+static void lane_load(tm_ctx* c, const TmLane* L) {    // L -> active fields
+    c->d_partials = L->d_partials; c->d_counter = L->d_counter; c->d_scal = L->d_scal; c->h_scal = L->h_scal;
+    memcpy(c->scratch, L->scratch, sizeof(c->scratch));
+    memcpy(c->scratch_bytes, L->scratch_bytes, sizeof(c->scratch_bytes));
+    memcpy(c->ev, L->ev, sizeof(c->ev));
+    c->lane_stream = L->stream;
+}
+
+tm_status tm_lane_use(tm_ctx* c, int lane) {
+    if (lane < 0 || lane >= TM_NLANES) return tm_fail(c, TM_EARG, "bad lane");
+    if (lane == c->cur_lane) return TM_OK;
+    lane_park(c, &c->lanes[c->cur_lane]);
+    c->cur_lane = lane;
+    if (c->lanes[lane].ready) { lane_load(c, &c->lanes[lane]); return TM_OK; }
+    c->d_partials = nullptr; c->d_counter = nullptr; c->d_scal = nullptr; c->h_scal = nullptr;
+    memset(c->scratch, 0, sizeof(c->scratch));
+    memset(c->scratch_bytes, 0, sizeof(c->scratch_bytes));
+    memset(c->ev, 0, sizeof(c->ev));
+    c->lane_stream = nullptr;
+    if (!lane_alloc(c, lane)) { cudaGetLastError(); return tm_fail(c, TM_EALLOC, "lane: device allocation failed"); }
+    return TM_OK;
+}
+
 extern "C" tm_status tm_create(tm_ctx** out, const int dims[4], int t_boundary, int device) {
     if (!out || !dims) { snprintf(g_last_error, sizeof(g_last_error), "tm_create: null argument"); return TM_EARG; }
     *out = nullptr;
@@ -40,13 +84,7 @@ extern "C" tm_status tm_create(tm_ctx** out, const int dims[4], int t_boundary, 
     c->device = device;
     { const char* e = getenv("TMLOOPS_NO_TMA"); c->no_tma = (e && e[0] == '1'); }
     cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
-    bool ok = cudaMalloc((void**)&c->d_partials, sizeof(double) * (1 << 18)) == cudaSuccess
-           && cudaMalloc((void**)&c->d_counter, sizeof(unsigned int) * 4) == cudaSuccess
-           && cudaMalloc((void**)&c->d_scal, sizeof(CgScalars)) == cudaSuccess
-           && cudaMallocHost((void**)&c->h_scal, sizeof(CgScalars)) == cudaSuccess
-           && cudaMemset(c->d_counter, 0, sizeof(unsigned int) * 4) == cudaSuccess
-           && cudaMemset(c->d_scal, 0, sizeof(CgScalars)) == cudaSuccess;
-    for (int i = 0; ok && i < 4; i++) ok = cudaEventCreate(&c->ev[i]) == cudaSuccess;
+    bool ok = lane_alloc(c, 0);
     if (!ok) {
         snprintf(g_last_error, sizeof(g_last_error), "tm_create: device allocation failed: %s", cudaGetErrorString(cudaGetLastError()));
         tm_destroy(c);
@@ -68,16 +106,22 @@ extern "C" tm_status tm_destroy(tm_ctx* c) {
     cudaDeviceSynchronize();
     drop_gauge_copies(c);
     if (c->d_Ucanon) cudaFree(c->d_Ucanon);
-    if (c->d_partials) cudaFree(c->d_partials);
-    if (c->d_counter) cudaFree(c->d_counter);
-    if (c->d_scal) cudaFree(c->d_scal);
-    if (c->h_scal) cudaFreeHost(c->h_scal);
+    lane_park(c, &c->lanes[c->cur_lane]);
+    for (int l = 0; l < TM_NLANES; l++) {
+        TmLane* L = &c->lanes[l];
+        if (!L->ready) continue;
+        if (L->d_partials) cudaFree(L->d_partials);
+        if (L->d_counter) cudaFree(L->d_counter);
+        if (L->d_scal) cudaFree(L->d_scal);
+        if (L->h_scal) cudaFreeHost(L->h_scal);
+        for (int i = 0; i < TM_MAX_SCRATCH; i++)
+            if (L->scratch[i]) cudaFree(L->scratch[i]);
+        for (int i = 0; i < TM_NEVENTS; i++)
+            if (L->ev[i]) cudaEventDestroy(L->ev[i]);
+        if (L->stream) cudaStreamDestroy(L->stream);
+    }
     if (c->d_contract_tables) cudaFree(c->d_contract_tables);
     free(c->h_contract_tables);
-    for (int i = 0; i < TM_MAX_SCRATCH; i++)
-        if (c->scratch[i]) cudaFree(c->scratch[i]);
-    for (int i = 0; i < 4; i++)
-        if (c->ev[i]) cudaEventDestroy(c->ev[i]);
     cudaGetLastError();
     free(c);
     return TM_OK;

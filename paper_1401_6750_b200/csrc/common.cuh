@@ -32,6 +32,24 @@ struct CgPlan {
     int pause_iter[CG_MAX_PAUSES];
 };
 
+// A lane = everything one in-flight solve + contraction needs privately: reduction scratch, the device state
+// of the CG, workspaces, events and (lanes >= 1) a stream.  The context's own fields of the same names are
+// the ACTIVE lane's (tm_lane_use swaps them), so kernels and helpers never see lanes; tsm.cu keeps
+// TM_NLANES sources in flight so that the tail of one kernel overlaps the next kernel of another source.
+#define TM_NLANES 2
+#define TM_NEVENTS 6
+struct TmLane {
+    int ready;
+    double* d_partials;
+    unsigned int* d_counter;
+    CgScalars* d_scal;
+    CgScalars* h_scal;
+    void* scratch[TM_MAX_SCRATCH];
+    size_t scratch_bytes[TM_MAX_SCRATCH];
+    cudaEvent_t ev[TM_NEVENTS];
+    cudaStream_t stream;            // owned side stream (lane 0: none, it runs on the caller's stream)
+};
+
 struct tm_ctx {
     int X[4];
     int Xh;
@@ -56,7 +74,10 @@ struct tm_ctx {
     void* d_contract_tables;
     void* h_contract_tables;        // host mirror (rebuild only when the momentum list changes)
     size_t contract_tables_bytes;
-    cudaEvent_t ev[4];
+    cudaEvent_t ev[TM_NEVENTS];     // 0,1: solve; 2,3: tsm; 4: solver state download; 5: lane join
+    int cur_lane;
+    TmLane lanes[TM_NLANES];        // parked state of the inactive lanes (the active one lives in the fields above)
+    cudaStream_t lane_stream;       // stream owned by the active lane (0 for lane 0)
     int no_tma;                     // TMLOOPS_NO_TMA=1: force the generic contraction kernel (testing)
 };
 
@@ -96,6 +117,7 @@ enum {
     WS_API_A, WS_API_B, WS_API_C
 };
 tm_status tm_ws(tm_ctx* c, int slot, size_t bytes, void** out);     // api.cu
+tm_status tm_lane_use(tm_ctx* c, int lane);                          // api.cu: make `lane` the active one
 tm_status tm_get_gauge(tm_ctx* c, tm_prec prec, tm_recon recon, cudaStream_t st, const void** out);  // layout.cu
 
 static inline size_t tm_prec_size(tm_prec p) { return p == TM_F64 ? 8 : p == TM_F32 ? 4 : 2; }

@@ -51,6 +51,20 @@ tm_status scal_get(tm_ctx* ctx, CgScalars* v, cudaStream_t st);          // down
 
 // ---- solver.cu ----------------------------------------------------------------------------
 // eta, s: full-lattice internal fields of precision params->outer
+struct SolveJob {                       // one solve in flight (solver.cu: tm_solve_begin / tm_solve_end)
+    tm_solve_params P;
+    tm_prec po, ps, pa; tm_recon rc;
+    double kappa, mu, delta;
+    cudaStream_t st;
+    void *p, *w, *z, *tmp, *rs, *x, *r, *b, *tmpo, *mo;
+    char *y, *s_o; const char* eta_o;
+    cudaEvent_t e0, e1, e_scal;
+    CgScalars* h_scal;
+    bool tail_valid; long enq;
+};
+tm_status tm_solve_begin(tm_ctx* ctx, SolveJob* job, void* d_s, const void* d_eta, double kappa, double mu,
+                         const tm_solve_params* params, cudaStream_t st);
+tm_status tm_solve_end(tm_ctx* ctx, SolveJob* job, tm_solve_info* info);
 tm_status tm_solve_internal(tm_ctx* ctx, void* d_s, const void* d_eta, double kappa, double mu,
                             const tm_solve_params* params, tm_solve_info* info, cudaStream_t st);
 

@@ -33,8 +33,36 @@ static tm_status apply_mhat(tm_ctx* ctx, void* out, const void* in, void* tmp, i
     return tm_dslash_launch(ctx, k, prec, recon, st);
 }
 
-tm_status tm_solve_internal(tm_ctx* ctx, void* d_s, const void* d_eta, double kappa, double mu,
-                            const tm_solve_params* P, tm_solve_info* info, cudaStream_t st) {
+// One solve in two host phases, so that several solves can be in flight on different lanes (tsm.cu):
+//   tm_solve_begin  enqueues setup + the planned iteration / update blocks + tail + an asynchronous
+//                   download of the device state, without any host synchronisation;
+//   tm_solve_end    waits for that download, continues off plan if the state machine has not finished,
+//                   records the plan of the next solve and fills `info`.
+// Both must be called with the same lane of the context active (tm_lane_use).
+static tm_status job_iteration(tm_ctx* ctx, const SolveJob& J) {
+    TM_TRY(apply_mhat(ctx, J.z, J.rs, J.tmp, 1, J.kappa, J.mu, J.ps, J.rc, RED_ZZ, GUARD_ITER, J.st));
+    TM_TRY(blas_update_p(ctx, J.p, J.z, J.ps, J.st));
+    TM_TRY(apply_mhat(ctx, J.w, J.p, J.tmp, 0, J.kappa, J.mu, J.ps, J.rc, RED_WW, GUARD_ITER, J.st));
+    return blas_update_xr(ctx, J.x, J.r, J.pa, J.p, J.w, J.rs, J.ps, J.st);
+}
+static tm_status job_update(tm_ctx* ctx, const SolveJob& J) {
+    TM_TRY(blas_ru_begin(ctx, J.y, J.po, J.x, J.pa, J.st));
+    TM_TRY(apply_mhat(ctx, J.mo, J.y, J.tmpo, 0, J.kappa, J.mu, J.po, J.rc, RED_NONE, GUARD_RU, J.st));
+    return blas_residual(ctx, J.r, J.pa, J.rs, J.ps, J.b, J.mo, J.po, RED_RU, GUARD_RU, J.st);
+}
+static tm_status job_tail(tm_ctx* ctx, const SolveJob& J) {
+    DslashCall k;
+    memset(&k, 0, sizeof(k));
+    k.out = J.s_o; k.in = J.y; k.x = J.eta_o; k.out_parity = 1; k.kappa = J.kappa; k.mu = J.mu;
+    k.xmode = 1; k.post = 1; k.coef = J.kappa; k.red_op = RED_NONE;
+    TM_TRY(tm_dslash_launch(ctx, k, J.po, J.rc, J.st));
+    TM_CUDA(ctx, cudaEventRecord(J.e1, J.st));
+    return TM_OK;
+}
+
+tm_status tm_solve_begin(tm_ctx* ctx, SolveJob* Jp, void* d_s, const void* d_eta, double kappa, double mu,
+                         const tm_solve_params* P, cudaStream_t st) {
+    SolveJob& J = *Jp;
     if (!P) return tm_fail(ctx, TM_EARG, "solve: null params");
     const tm_prec po = P->outer, ps = P->sloppy;
     if (po != TM_F64 && po != TM_F32) return tm_fail(ctx, TM_EPREC, "solve: outer precision must be f32 or f64");
@@ -42,107 +70,99 @@ tm_status tm_solve_internal(tm_ctx* ctx, void* d_s, const void* d_eta, double ka
     if (tm_prec_size(ps) > tm_prec_size(po)) return tm_fail(ctx, TM_EPREC, "solve: sloppy precision wider than outer");
     if (P->recon != TM_R12 && P->recon != TM_R18) return tm_fail(ctx, TM_EARG, "solve: recon must be 12 or 18");
     if (!(P->rho > 0) || P->max_iter < 0) return tm_fail(ctx, TM_EARG, "solve: rho must be > 0, max_iter >= 0");
-    const tm_prec pa = (ps == TM_F64) ? TM_F64 : TM_F32;        // accumulate precision of x, r
-    const tm_recon rc = P->recon;
-    const double delta = (P->delta > 0 && P->delta < 1) ? P->delta : 0.1;
-    const size_t bo = tm_parity_bytes(ctx, po), bs = tm_parity_bytes(ctx, ps), ba = tm_parity_bytes(ctx, pa);
+    J.P = *P;
+    J.po = po; J.ps = ps;
+    J.pa = (ps == TM_F64) ? TM_F64 : TM_F32;        // accumulate precision of x, r
+    J.rc = P->recon;
+    J.delta = (P->delta > 0 && P->delta < 1) ? P->delta : 0.1;
+    J.kappa = kappa; J.mu = mu; J.st = st;
+    const size_t bo = tm_parity_bytes(ctx, po), bs = tm_parity_bytes(ctx, ps), ba = tm_parity_bytes(ctx, J.pa);
 
-    cudaEvent_t e0 = ctx->ev[0], e1 = ctx->ev[1];
-    TM_CUDA(ctx, cudaEventRecord(e0, st));
+    J.e0 = ctx->ev[0]; J.e1 = ctx->ev[1];
+    TM_CUDA(ctx, cudaEventRecord(J.e0, st));
 
-    void *p, *w, *z, *tmp, *rs, *x, *r, *b, *tmpo, *mo;
-    TM_TRY(tm_ws(ctx, WS_SL_P, bs, &p));
-    TM_TRY(tm_ws(ctx, WS_SL_W, bs, &w));
-    TM_TRY(tm_ws(ctx, WS_SL_Z, bs, &z));
-    TM_TRY(tm_ws(ctx, WS_SL_TMP, bs, &tmp));
-    TM_TRY(tm_ws(ctx, WS_AC_X, ba, &x));
-    TM_TRY(tm_ws(ctx, WS_AC_R, ba, &r));
-    if (pa != ps) TM_TRY(tm_ws(ctx, WS_SL_R, bs, &rs)); else rs = r;
-    TM_TRY(tm_ws(ctx, WS_OU_B, bo, &b));
-    TM_TRY(tm_ws(ctx, WS_OU_TMP, bo, &tmpo));
-    TM_TRY(tm_ws(ctx, WS_OU_TMP2, bo, &mo));
+    TM_TRY(tm_ws(ctx, WS_SL_P, bs, &J.p));
+    TM_TRY(tm_ws(ctx, WS_SL_W, bs, &J.w));
+    TM_TRY(tm_ws(ctx, WS_SL_Z, bs, &J.z));
+    TM_TRY(tm_ws(ctx, WS_SL_TMP, bs, &J.tmp));
+    TM_TRY(tm_ws(ctx, WS_AC_X, ba, &J.x));
+    TM_TRY(tm_ws(ctx, WS_AC_R, ba, &J.r));
+    if (J.pa != ps) TM_TRY(tm_ws(ctx, WS_SL_R, bs, &J.rs)); else J.rs = J.r;
+    TM_TRY(tm_ws(ctx, WS_OU_B, bo, &J.b));
+    TM_TRY(tm_ws(ctx, WS_OU_TMP, bo, &J.tmpo));
+    TM_TRY(tm_ws(ctx, WS_OU_TMP2, bo, &J.mo));
 
     const char* eta_e = (const char*)d_eta;
-    const char* eta_o = eta_e + bo;
-    char* y = (char*)d_s;                  // the even half of the solution is accumulated in place
-    char* s_o = y + bo;
+    J.eta_o = eta_e + bo;
+    J.y = (char*)d_s;                      // the even half of the solution is accumulated in place
+    J.s_o = J.y + bo;
 
     // ---- setup (no host synchronisation): state, ||eta||^2, bhat, y = x = 0, r = rs = bhat
-    TM_TRY(scal_init(ctx, P->rho * P->rho, delta * delta, P->max_iter, st));
+    TM_TRY(scal_init(ctx, P->rho * P->rho, J.delta * J.delta, P->max_iter, st));
     TM_TRY(blas_norm_full(ctx, d_eta, po, RED_SLOT0 + 0, st));
-    TM_TRY(blas_twist_inv(ctx, tmpo, eta_o, po, kappa, mu, 0, st));
+    TM_TRY(blas_twist_inv(ctx, J.tmpo, J.eta_o, po, kappa, mu, 0, st));
     {
         DslashCall k;
         memset(&k, 0, sizeof(k));
-        k.out = b; k.in = tmpo; k.x = eta_e; k.out_parity = 0; k.kappa = kappa; k.mu = mu;
+        k.out = J.b; k.in = J.tmpo; k.x = eta_e; k.out_parity = 0; k.kappa = kappa; k.mu = mu;
         k.xmode = 1; k.coef = kappa; k.red_op = RED_NONE;
-        TM_TRY(tm_dslash_launch(ctx, k, po, rc, st));
+        TM_TRY(tm_dslash_launch(ctx, k, po, J.rc, st));
     }
-    TM_TRY(blas_zero(ctx, y, po, st));
-    TM_TRY(blas_zero(ctx, x, pa, st));
-    TM_TRY(blas_residual(ctx, r, pa, rs, ps, b, nullptr, po, RED_START, GUARD_ALWAYS, st));
+    TM_TRY(blas_zero(ctx, J.y, po, st));
+    TM_TRY(blas_zero(ctx, J.x, J.pa, st));
+    TM_TRY(blas_residual(ctx, J.r, J.pa, J.rs, ps, J.b, nullptr, po, RED_START, GUARD_ALWAYS, st));
 
-    auto iteration = [&]() -> tm_status {
-        TM_TRY(apply_mhat(ctx, z, rs, tmp, 1, kappa, mu, ps, rc, RED_ZZ, GUARD_ITER, st));
-        TM_TRY(blas_update_p(ctx, p, z, ps, st));
-        TM_TRY(apply_mhat(ctx, w, p, tmp, 0, kappa, mu, ps, rc, RED_WW, GUARD_ITER, st));
-        return blas_update_xr(ctx, x, r, pa, p, w, rs, ps, st);
-    };
-    auto update = [&]() -> tm_status {
-        TM_TRY(blas_ru_begin(ctx, y, po, x, pa, st));
-        TM_TRY(apply_mhat(ctx, mo, y, tmpo, 0, kappa, mu, po, rc, RED_NONE, GUARD_RU, st));
-        return blas_residual(ctx, r, pa, rs, ps, b, mo, po, RED_RU, GUARD_RU, st);
-    };
-    auto tail = [&]() -> tm_status {
-        DslashCall k;
-        memset(&k, 0, sizeof(k));
-        k.out = s_o; k.in = y; k.x = eta_o; k.out_parity = 1; k.kappa = kappa; k.mu = mu;
-        k.xmode = 1; k.post = 1; k.coef = kappa; k.red_op = RED_NONE;
-        TM_TRY(tm_dslash_launch(ctx, k, po, rc, st));
-        TM_CUDA(ctx, cudaEventRecord(e1, st));
-        return TM_OK;
-    };
-
-    CgPlan& plan = ctx->plan[(int)ps];
-    const bool have_plan = plan.valid && plan.sloppy == (int)ps && plan.outer == (int)po && plan.recon == (int)rc
-                        && plan.max_iter == P->max_iter && plan.rho == P->rho && plan.delta == delta;
-    CgScalars sc;
-    bool tail_valid = false;
-    long enq = 0;                                   // iteration blocks enqueued so far
+    const CgPlan& plan = ctx->plan[(int)ps];
+    const bool have_plan = plan.valid && plan.sloppy == (int)ps && plan.outer == (int)po && plan.recon == (int)J.rc
+                        && plan.max_iter == P->max_iter && plan.rho == P->rho && plan.delta == J.delta;
+    J.tail_valid = false;
+    J.enq = 0;                                      // iteration blocks enqueued so far
     if (have_plan) {
         for (int k = 0; k < plan.n_pause; k++) {
-            for (; enq < plan.pause_iter[k]; enq++) TM_TRY(iteration());
-            TM_TRY(update());
+            for (; J.enq < plan.pause_iter[k]; J.enq++) TM_TRY(job_iteration(ctx, J));
+            TM_TRY(job_update(ctx, J));
         }
-        TM_TRY(tail());
-        tail_valid = true;
+        TM_TRY(job_tail(ctx, J));
+        J.tail_valid = true;
     } else {
-        TM_TRY(update());                           // covers "already converged at x = 0" (state 1 after RED_START)
+        TM_TRY(job_update(ctx, J));                 // covers "already converged at x = 0" (state 1 after RED_START)
     }
-    TM_TRY(scal_get(ctx, &sc, st));
+    J.h_scal = ctx->h_scal;
+    J.e_scal = ctx->ev[4];
+    TM_CUDA(ctx, cudaMemcpyAsync(ctx->h_scal, ctx->d_scal, sizeof(CgScalars), cudaMemcpyDeviceToHost, st));
+    TM_CUDA(ctx, cudaEventRecord(J.e_scal, st));
+    return TM_OK;
+}
+
+tm_status tm_solve_end(tm_ctx* ctx, SolveJob* Jp, tm_solve_info* info) {
+    SolveJob& J = *Jp;
+    const tm_solve_params* P = &J.P;
+    cudaStream_t st = J.st;
+    CgScalars sc;
+    TM_CUDA(ctx, cudaEventSynchronize(J.e_scal));
+    sc = *J.h_scal;
     while (sc.done < 2) {
         // off plan (first solve with these parameters, or this source behaves differently):
         // [iteration, update] pairs, polled every few pairs
         const int burst = 4;
-        for (int k = 0; k < burst; k++) { TM_TRY(iteration()); TM_TRY(update()); enq++; }
-        tail_valid = false;
+        for (int k = 0; k < burst; k++) { TM_TRY(job_iteration(ctx, J)); TM_TRY(job_update(ctx, J)); J.enq++; }
+        J.tail_valid = false;
         TM_TRY(scal_get(ctx, &sc, st));
-        if (enq > (long)P->max_iter + 8 * (long)CG_MAX_PAUSES + 64 && sc.done < 2)
+        if (J.enq > (long)P->max_iter + 8 * (long)CG_MAX_PAUSES + 64 && sc.done < 2)
             return tm_fail(ctx, TM_ECUDA, "solve: device state machine did not terminate");
     }
-    if (!tail_valid) {
-        TM_TRY(tail());
-        TM_CUDA(ctx, cudaEventSynchronize(e1));
-    }
+    if (!J.tail_valid) TM_TRY(job_tail(ctx, J));
+    TM_CUDA(ctx, cudaEventSynchronize(J.e1));
     // remember where this solve paused: the launch plan of the next one
+    CgPlan& plan = ctx->plan[(int)J.ps];
     plan.valid = sc.n_ru <= CG_MAX_PAUSES;
-    plan.sloppy = (int)ps; plan.outer = (int)po; plan.recon = (int)rc; plan.max_iter = P->max_iter;
-    plan.rho = P->rho; plan.delta = delta;
+    plan.sloppy = (int)J.ps; plan.outer = (int)J.po; plan.recon = (int)J.rc; plan.max_iter = P->max_iter;
+    plan.rho = P->rho; plan.delta = J.delta;
     plan.n_pause = sc.n_ru < CG_MAX_PAUSES ? sc.n_ru : CG_MAX_PAUSES;
     for (int k = 0; k < plan.n_pause; k++) plan.pause_iter[k] = sc.pause_iter[k];
 
     float ms = 0;
-    cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventElapsedTime(&ms, J.e0, J.e1);
     const double eta2 = sc.slot[0];
     const double resid = eta2 > 0 ? sqrt(sc.rr_true / eta2) : 0.0;
     if (info) {
@@ -157,6 +177,13 @@ tm_status tm_solve_internal(tm_ctx* ctx, void* d_s, const void* d_eta, double ka
         return TM_ENOCONV;
     }
     return TM_OK;
+}
+
+tm_status tm_solve_internal(tm_ctx* ctx, void* d_s, const void* d_eta, double kappa, double mu,
+                            const tm_solve_params* P, tm_solve_info* info, cudaStream_t st) {
+    SolveJob J;
+    TM_TRY(tm_solve_begin(ctx, &J, d_s, d_eta, kappa, mu, P, st));
+    return tm_solve_end(ctx, &J, info);
 }
 
 extern "C" tm_status tm_cg_solve(tm_ctx* ctx, void* d_s, const void* d_eta, double kappa, double mu,

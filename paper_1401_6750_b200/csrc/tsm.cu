@@ -1,11 +1,13 @@
-// tsm.cu -- Truncated Solver Method estimator loop (sec 2.1).
+// tsm.cu -- Truncated Solver Method estimator loop (sec 2.1) and the
+// binary storage of partial sums (sec 2.1.1, Fig. 2; row f2).
 //
 //   L_TSM = (1/N_LP) sum_{r<N_LP} l_r^LP + (1/N_HP) sum_{r<N_HP} (l_r^HP - l_r^LP)
-// with the HP sources = the first N_HP of the LP sources (reading 14).  Per source:
-// Z4 noise expanded on the device -> tm_solve_internal (LP, and HP for r < N_HP) -> fused
-// contraction + projection -> momentum-space accumulators S_LP, S_LPc, S_HP (device, complex128).
-// Nothing crosses to the host per source except the solver's convergence scalars (and, in
-// tsm_estimate_host, the packed noise of that source).
+// with the HP sources = the first N_HP of the LP sources (reading 14).  Per (source, pass) job:
+// Z4 noise expanded on the device -> solve (LP, and HP for r < N_HP) -> fused contraction + projection ->
+// momentum-space accumulators S_LP, S_LPc, S_HP (device, complex128).  TM_NLANES jobs are in flight at a
+// time, each on its own lane (private workspaces, CG state and stream; common.cuh), so that the draining
+// tail and the launch gap of every kernel are covered by another source's kernels.  Nothing crosses to the
+// host per source except the solver's convergence scalars (and, in tsm_estimate_host, the packed noise).
 #include <math.h>
 #include "kernels.h"
 
@@ -20,13 +22,16 @@ __global__ void tsm_accumulate_kernel(double* __restrict__ acc0, double* __restr
     if (copy) copy[i] = v;
 }
 
-// out = S_LP / n_lp + (S_HP - S_LPc) / n_hp
-__global__ void tsm_combine_kernel(double* __restrict__ out, const double* __restrict__ slp,
-                                   const double* __restrict__ slpc, const double* __restrict__ shp,
-                                   double inv_lp, double inv_hp, size_t n) {
+// out = S_LP / n_lp + (S_HP - S_LPc) / n_hp, the three sums taken over the lanes in lane order
+struct TsmLaneAcc { int n; const double* acc[TM_NLANES]; };
+__global__ void tsm_combine_kernel(double* __restrict__ out, TsmLaneAcc L, double inv_lp, double inv_hp, size_t n) {
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    out[i] = slp[i] * inv_lp + (shp[i] - slpc[i]) * inv_hp;
+    double slp = 0.0, slpc = 0.0, shp = 0.0;
+    for (int l = 0; l < L.n; l++) {
+        slp += L.acc[l][i]; slpc += L.acc[l][n + i]; shp += L.acc[l][2 * n + i];
+    }
+    out[i] = slp * inv_lp + (shp - slpc) * inv_hp;
 }
 
 // binary storage (sec 2.1.1): file += x  |  file += x - y
@@ -94,6 +99,156 @@ static tm_status convert_full(tm_ctx* ctx, void* dst, tm_prec pd, const void* sr
     return TM_OK;
 }
 
+// one (source, pass) unit of work in flight on a lane
+struct TsmJob {
+    int r, pass;
+    SolveJob sj;
+    void *eta_o, *s_o;
+    tm_prec po, ac;
+    cudaStream_t st;
+};
+
+struct TsmRun {
+    tm_ctx* ctx; const tsm_params* P; void* d_per_source; void* d_files_lp; void* d_files_corr;
+    const unsigned char* z4; int z4_on_host;
+    size_t nr, z4_bytes; unsigned agrid;
+    double ms_lp, ms_hp, worst_lp, worst_hp; long it_lp, it_hp; int noconv;
+    double* acc[TM_NLANES];         // per lane: S_lp, S_lpc, S_hp, tmp (nr doubles each)
+    double* lp_keep;
+};
+
+// lane-private buffers of the active lane
+static tm_status lane_buffers(TsmRun& R, int lane, cudaStream_t st) {
+    tm_ctx* ctx = R.ctx;
+    if (R.acc[lane]) return TM_OK;
+    TM_TRY(tm_ws(ctx, WS_TSM_ACC, 4 * R.nr * sizeof(double), (void**)&R.acc[lane]));
+    TM_CUDA(ctx, cudaMemsetAsync(R.acc[lane], 0, 3 * R.nr * sizeof(double), st));
+    return TM_OK;
+}
+
+// noise of source r in precision p into the active lane's buffer
+static tm_status job_noise(TsmRun& R, int r, tm_prec p, cudaStream_t st, void** out) {
+    tm_ctx* ctx = R.ctx;
+    const unsigned char* zsrc = nullptr;
+    if (R.z4) {
+        if (R.z4_on_host) {
+            // staged per lane: the previous user of this lane's slot (its z4_expand) finished before that
+            // lane's solve was waited for
+            void* slot;
+            TM_TRY(tm_ws(ctx, WS_TSM_Z4, R.z4_bytes, &slot));
+            TM_CUDA(ctx, cudaMemcpyAsync(slot, R.z4 + (size_t)r * R.z4_bytes, R.z4_bytes, cudaMemcpyHostToDevice, st));
+            zsrc = (const unsigned char*)slot;
+        } else zsrc = R.z4 + (size_t)r * R.z4_bytes;
+    }
+    TM_TRY(tm_ws(ctx, p == TM_F32 ? WS_TSM_ETA32 : WS_TSM_ETA64, 2 * tm_parity_bytes(ctx, p), out));
+    return tm_z4_expand(ctx, *out, p, zsrc, R.P->seed, (unsigned long long)r, st);
+}
+
+static tm_status job_start(TsmRun& R, TsmJob& J, int r, int pass, cudaStream_t st) {
+    tm_ctx* ctx = R.ctx;
+    const tsm_params* P = R.P;
+    J.r = r; J.pass = pass; J.st = st;
+    J.po = pass ? P->hp.outer : P->lp.outer;
+    J.ac = pass ? P->contract_acc_hp : P->contract_acc_lp;
+    TM_TRY(job_noise(R, r, J.po, st, &J.eta_o));
+    TM_TRY(tm_ws(ctx, J.po == TM_F32 ? WS_TSM_S32 : WS_TSM_S64, 2 * tm_parity_bytes(ctx, J.po), &J.s_o));
+    return tm_solve_begin(ctx, &J.sj, J.s_o, J.eta_o, P->kappa, P->mu, pass ? &P->hp : &P->lp, st);
+}
+
+static tm_status job_finish(TsmRun& R, TsmJob& J, int lane) {
+    tm_ctx* ctx = R.ctx;
+    const tsm_params* P = R.P;
+    cudaStream_t st = J.st;
+    tm_solve_info si;
+    tm_status s = tm_solve_end(ctx, &J.sj, &si);
+    if (s == TM_ENOCONV) R.noconv++;
+    else if (s != TM_OK) return s;
+    if (J.pass) { R.ms_hp += si.ms; R.it_hp += si.iters; R.worst_hp = fmax(R.worst_hp, si.true_resid); }
+    else        { R.ms_lp += si.ms; R.it_lp += si.iters; R.worst_lp = fmax(R.worst_lp, si.true_resid); }
+    void *s_c = J.s_o, *eta_c = J.eta_o;
+    if (J.ac != J.po) {
+        TM_TRY(tm_ws(ctx, J.ac == TM_F32 ? WS_TSM_S32 : WS_TSM_S64, 2 * tm_parity_bytes(ctx, J.ac), &s_c));
+        TM_TRY(convert_full(ctx, s_c, J.ac, J.s_o, J.po, st));
+        TM_TRY(job_noise(R, J.r, J.ac, st, &eta_c));
+    }
+    double* A = R.acc[lane];
+    const size_t nr = R.nr;
+    double *S_lp = A, *S_lpc = A + nr, *S_hp = A + 2 * nr, *tmp = A + 3 * nr;
+    TM_TRY(tm_contract_internal(ctx, tmp, s_c, eta_c, P->kappa, P->mu, P->h_momenta, P->nmom, J.ac, st));
+    const int do_hp = J.r < P->n_hp;
+    double* copy = R.d_per_source ? (double*)R.d_per_source + (size_t)(J.pass ? P->n_lp + J.r : J.r) * nr : nullptr;
+    if (J.pass) tsm_accumulate_kernel<<<R.agrid, 256, 0, st>>>(S_hp, nullptr, copy, tmp, nr);
+    else        tsm_accumulate_kernel<<<R.agrid, 256, 0, st>>>(S_lp, do_hp ? S_lpc : nullptr, copy, tmp, nr);
+    TM_LAUNCH_CHECK(ctx, "tsm_accumulate_kernel");
+    if (!J.pass && R.d_files_lp) {
+        binary_add_kernel<<<R.agrid, 256, 0, st>>>((double*)R.d_files_lp + (size_t)binary_file_of(J.r) * nr, tmp, nullptr, nr);
+        TM_LAUNCH_CHECK(ctx, "binary_add_kernel");
+    }
+    if (R.lp_keep && do_hp) {
+        if (!J.pass) TM_CUDA(ctx, cudaMemcpyAsync(R.lp_keep, tmp, nr * sizeof(double), cudaMemcpyDeviceToDevice, st));
+        else {
+            binary_add_kernel<<<R.agrid, 256, 0, st>>>((double*)R.d_files_corr + (size_t)binary_file_of(J.r) * nr, tmp, R.lp_keep, nr);
+            TM_LAUNCH_CHECK(ctx, "binary_add_kernel");
+        }
+    }
+    return TM_OK;
+}
+
+// Software pipeline over the (source, pass) jobs: TM_NLANES jobs are in flight, each on its own lane (private
+// workspaces, device CG state and stream), so the draining tail and launch gap of every kernel of one source
+// are filled by kernels of another.  Lane l accumulates into its own S_lp / S_lpc / S_hp; the lanes are joined
+// and summed by the final combine kernel.  Job j runs on lane j % NL: results do not depend on timing.
+static tm_status tsm_pipeline(TsmRun& R, int NL, cudaStream_t st, void* d_out) {
+    tm_ctx* ctx = R.ctx;
+    const tsm_params* P = R.P;
+    // everything shared between lanes is built on the caller's stream before the lanes fork
+    const void* g;
+    TM_TRY(tm_get_gauge(ctx, P->lp.sloppy, P->lp.recon, st, &g));
+    TM_TRY(tm_get_gauge(ctx, P->lp.outer, P->lp.recon, st, &g));
+    TM_TRY(tm_get_gauge(ctx, P->contract_acc_lp, P->contract_acc_lp == TM_F64 ? TM_R18 : TM_R12, st, &g));
+    if (P->n_hp) {
+        TM_TRY(tm_get_gauge(ctx, P->hp.sloppy, P->hp.recon, st, &g));
+        TM_TRY(tm_get_gauge(ctx, P->hp.outer, P->hp.recon, st, &g));
+        TM_TRY(tm_get_gauge(ctx, P->contract_acc_hp, P->contract_acc_hp == TM_F64 ? TM_R18 : TM_R12, st, &g));
+    }
+    cudaEvent_t fork = ctx->ev[5];                 // lane 0's
+    TM_CUDA(ctx, cudaEventRecord(fork, st));
+    cudaStream_t lst[TM_NLANES];
+    for (int l = 0; l < NL; l++) {
+        TM_TRY(tm_lane_use(ctx, l));
+        lst[l] = l ? ctx->lane_stream : st;
+        if (l) TM_CUDA(ctx, cudaStreamWaitEvent(lst[l], fork, 0));
+        TM_TRY(lane_buffers(R, l, lst[l]));
+    }
+    const int njobs = P->n_lp + P->n_hp;
+    TsmJob jobs[TM_NLANES];
+    int jr = 0, jpass = 0;                          // next job to start: r = 0: LP, HP; r = 1: LP, HP; ...
+    for (int j = 0; j < njobs + NL; j++) {
+        const int l = j % NL;
+        TM_TRY(tm_lane_use(ctx, l));
+        if (j >= NL) TM_TRY(job_finish(R, jobs[l], l));
+        if (j < njobs) {
+            TM_TRY(job_start(R, jobs[l], jr, jpass, lst[l]));
+            if (!jpass && jr < P->n_hp) jpass = 1; else { jpass = 0; jr++; }
+        }
+    }
+    // join
+    cudaEvent_t joined[TM_NLANES];
+    for (int l = 1; l < NL; l++) {
+        TM_TRY(tm_lane_use(ctx, l));
+        joined[l] = ctx->ev[5];
+        TM_CUDA(ctx, cudaEventRecord(joined[l], lst[l]));
+    }
+    TM_TRY(tm_lane_use(ctx, 0));
+    for (int l = 1; l < NL; l++) TM_CUDA(ctx, cudaStreamWaitEvent(st, joined[l], 0));
+    TsmLaneAcc LA;
+    LA.n = NL;
+    for (int l = 0; l < TM_NLANES; l++) LA.acc[l] = l < NL ? R.acc[l] : nullptr;
+    tsm_combine_kernel<<<R.agrid, 256, 0, st>>>((double*)d_out, LA, 1.0 / P->n_lp, P->n_hp ? 1.0 / P->n_hp : 0.0, R.nr);
+    TM_LAUNCH_CHECK(ctx, "tsm_combine_kernel");
+    return TM_OK;
+}
+
 static tm_status tsm_core(tm_ctx* ctx, void* d_out, void* d_per_source, const tsm_params* P, tsm_info* info,
                           const unsigned char* z4, int z4_on_host, cudaStream_t st,
                           void* d_files_lp = nullptr, void* d_files_corr = nullptr) {
@@ -107,117 +262,56 @@ static tm_status tsm_core(tm_ctx* ctx, void* d_out, void* d_per_source, const ts
         return tm_fail(ctx, TM_EPREC, "tsm_estimate: outer precisions must be f32 or f64");
     if ((ac_lp != TM_F32 && ac_lp != TM_F64) || (ac_hp != TM_F32 && ac_hp != TM_F64))
         return tm_fail(ctx, TM_EPREC, "tsm_estimate: contraction precisions must be f32 or f64");
+    if ((int)P->lp.sloppy < 0 || (int)P->lp.sloppy > 3 || (int)P->hp.sloppy < 0 || (int)P->hp.sloppy > 3)
+        return tm_fail(ctx, TM_EPREC, "tsm_estimate: unknown sloppy precision");
+    if ((P->lp.recon != TM_R12 && P->lp.recon != TM_R18) || (P->hp.recon != TM_R12 && P->hp.recon != TM_R18))
+        return tm_fail(ctx, TM_EARG, "tsm_estimate: recon must be 12 or 18");
     TM_CUDA(ctx, cudaSetDevice(ctx->device));
+    TM_TRY(tm_lane_use(ctx, 0));
     const long launches0 = ctx->launches;
-    const size_t nout = (size_t)160 * P->nmom * ctx->X[3];       // complex entries
-    const size_t nr = 2 * nout;                                  // doubles
-    const size_t z4_bytes = 3 * ctx->V;
-    double* acc;
-    TM_TRY(tm_ws(ctx, WS_TSM_ACC, 4 * nr * sizeof(double), (void**)&acc));
-    double *S_lp = acc, *S_lpc = acc + nr, *S_hp = acc + 2 * nr, *tmp = acc + 3 * nr;
-    TM_CUDA(ctx, cudaMemsetAsync(acc, 0, 3 * nr * sizeof(double), st));
-    double* lp_keep = nullptr;          // l_r^LP kept until l_r^HP is known (binary files of the correction)
-    if (d_files_lp) TM_CUDA(ctx, cudaMemsetAsync(d_files_lp, 0, (size_t)loop_binary_nfiles(P->n_lp) * nr * sizeof(double), st));
+    TsmRun R;
+    memset(&R, 0, sizeof(R));
+    R.ctx = ctx; R.P = P; R.d_per_source = d_per_source; R.d_files_lp = d_files_lp; R.d_files_corr = d_files_corr;
+    R.z4 = z4; R.z4_on_host = z4_on_host;
+    R.nr = 2 * (size_t)160 * P->nmom * ctx->X[3];                // doubles per per-source array
+    R.z4_bytes = 3 * ctx->V;
+    R.agrid = (unsigned)((R.nr + 255) / 256);
+    // the binary-storage files are shared accumulators: one lane keeps their additions ordered
+    const int NL = (d_files_lp || d_files_corr || P->n_lp + P->n_hp < 2) ? 1 : TM_NLANES;
+    if (d_files_lp) TM_CUDA(ctx, cudaMemsetAsync(d_files_lp, 0, (size_t)loop_binary_nfiles(P->n_lp) * R.nr * sizeof(double), st));
     if (d_files_corr && P->n_hp) {
-        TM_CUDA(ctx, cudaMemsetAsync(d_files_corr, 0, (size_t)loop_binary_nfiles(P->n_hp) * nr * sizeof(double), st));
-        TM_TRY(tm_ws(ctx, WS_TSM_KEEP, nr * sizeof(double), (void**)&lp_keep));
+        TM_CUDA(ctx, cudaMemsetAsync(d_files_corr, 0, (size_t)loop_binary_nfiles(P->n_hp) * R.nr * sizeof(double), st));
+        TM_TRY(tm_ws(ctx, WS_TSM_KEEP, R.nr * sizeof(double), (void**)&R.lp_keep));
     }
-    void *eta32 = nullptr, *eta64 = nullptr, *s32 = nullptr, *s64 = nullptr, *z4dev = nullptr;
-    const bool need32 = po_lp == TM_F32 || ac_lp == TM_F32 || (P->n_hp && (po_hp == TM_F32 || ac_hp == TM_F32));
-    const bool need64 = po_lp == TM_F64 || ac_lp == TM_F64 || (P->n_hp && (po_hp == TM_F64 || ac_hp == TM_F64));
-    if (need32) {
-        TM_TRY(tm_ws(ctx, WS_TSM_ETA32, 2 * tm_parity_bytes(ctx, TM_F32), &eta32));
-        TM_TRY(tm_ws(ctx, WS_TSM_S32, 2 * tm_parity_bytes(ctx, TM_F32), &s32));
-    }
-    if (need64) {
-        TM_TRY(tm_ws(ctx, WS_TSM_ETA64, 2 * tm_parity_bytes(ctx, TM_F64), &eta64));
-        TM_TRY(tm_ws(ctx, WS_TSM_S64, 2 * tm_parity_bytes(ctx, TM_F64), &s64));
-    }
-    if (z4 && z4_on_host) TM_TRY(tm_ws(ctx, WS_TSM_Z4, 2 * z4_bytes, &z4dev));
-
     cudaEvent_t e0 = ctx->ev[2], e1 = ctx->ev[3];
     TM_CUDA(ctx, cudaEventRecord(e0, st));
-    double ms_lp = 0, ms_hp = 0;
-    long it_lp = 0, it_hp = 0;
-    double worst_lp = 0, worst_hp = 0;
-    int noconv = 0;
-    const unsigned agrid = (unsigned)((nr + 255) / 256);
-
-    for (int r = 0; r < P->n_lp; r++) {
-        const unsigned char* zsrc = nullptr;
-        if (z4) {
-            if (z4_on_host) {
-                // double-buffered staging: the copy of source r is stream-ordered behind the work of r-1
-                unsigned char* slot = (unsigned char*)z4dev + (size_t)(r & 1) * z4_bytes;
-                TM_CUDA(ctx, cudaMemcpyAsync(slot, z4 + (size_t)r * z4_bytes, z4_bytes, cudaMemcpyHostToDevice, st));
-                zsrc = slot;
-            } else zsrc = z4 + (size_t)r * z4_bytes;
-        }
-        const int do_hp = r < P->n_hp;
-        // noise in every precision this source needs
-        bool have32 = false, have64 = false;
-        auto eta_in = [&](tm_prec p, void** out) -> tm_status {
-            if (p == TM_F32) {
-                if (!have32) { TM_TRY(tm_z4_expand(ctx, eta32, TM_F32, zsrc, P->seed, (unsigned long long)r, st)); have32 = true; }
-                *out = eta32;
-            } else {
-                if (!have64) { TM_TRY(tm_z4_expand(ctx, eta64, TM_F64, zsrc, P->seed, (unsigned long long)r, st)); have64 = true; }
-                *out = eta64;
-            }
-            return TM_OK;
-        };
-        for (int pass = 0; pass < 1 + do_hp; pass++) {
-            const tm_solve_params* sp = pass ? &P->hp : &P->lp;
-            const tm_prec po = pass ? po_hp : po_lp, ac = pass ? ac_hp : ac_lp;
-            void *eta_o, *eta_c, *s_o = po == TM_F32 ? s32 : s64, *s_c;
-            TM_TRY(eta_in(po, &eta_o));
-            tm_solve_info si;
-            tm_status s = tm_solve_internal(ctx, s_o, eta_o, P->kappa, P->mu, sp, &si, st);
-            if (s == TM_ENOCONV) noconv++;
-            else if (s != TM_OK) return s;
-            if (pass) { ms_hp += si.ms; it_hp += si.iters; worst_hp = fmax(worst_hp, si.true_resid); }
-            else      { ms_lp += si.ms; it_lp += si.iters; worst_lp = fmax(worst_lp, si.true_resid); }
-            if (ac == po) { s_c = s_o; eta_c = eta_o; }
-            else {
-                s_c = ac == TM_F32 ? s32 : s64;
-                TM_TRY(convert_full(ctx, s_c, ac, s_o, po, st));
-                TM_TRY(eta_in(ac, &eta_c));
-            }
-            TM_TRY(tm_contract_internal(ctx, tmp, s_c, eta_c, P->kappa, P->mu, P->h_momenta, P->nmom, ac, st));
-            double* copy = d_per_source ? (double*)d_per_source + (size_t)(pass ? P->n_lp + r : r) * nr : nullptr;
-            if (pass) tsm_accumulate_kernel<<<agrid, 256, 0, st>>>(S_hp, nullptr, copy, tmp, nr);
-            else      tsm_accumulate_kernel<<<agrid, 256, 0, st>>>(S_lp, do_hp ? S_lpc : nullptr, copy, tmp, nr);
-            TM_LAUNCH_CHECK(ctx, "tsm_accumulate_kernel");
-            if (!pass && d_files_lp) {
-                binary_add_kernel<<<agrid, 256, 0, st>>>((double*)d_files_lp + (size_t)binary_file_of(r) * nr, tmp, nullptr, nr);
-                TM_LAUNCH_CHECK(ctx, "binary_add_kernel");
-            }
-            if (lp_keep && do_hp) {
-                if (!pass) TM_CUDA(ctx, cudaMemcpyAsync(lp_keep, tmp, nr * sizeof(double), cudaMemcpyDeviceToDevice, st));
-                else {
-                    binary_add_kernel<<<agrid, 256, 0, st>>>((double*)d_files_corr + (size_t)binary_file_of(r) * nr, tmp, lp_keep, nr);
-                    TM_LAUNCH_CHECK(ctx, "binary_add_kernel");
-                }
-            }
-        }
+    tm_status s = tsm_pipeline(R, NL, st, d_out);
+    if (s != TM_OK) {
+        // leave no lane running behind the caller's back
+        for (int l = 1; l < NL; l++)
+            if (tm_lane_use(ctx, l) == TM_OK && ctx->lane_stream) cudaStreamSynchronize(ctx->lane_stream);
+        char keep[sizeof(ctx->err)];
+        memcpy(keep, ctx->err, sizeof(keep));
+        tm_lane_use(ctx, 0);
+        memcpy(ctx->err, keep, sizeof(keep));
+        cudaGetLastError();
+        return s;
     }
-    tsm_combine_kernel<<<agrid, 256, 0, st>>>((double*)d_out, S_lp, S_lpc, S_hp, 1.0 / P->n_lp,
-                                             P->n_hp ? 1.0 / P->n_hp : 0.0, nr);
-    TM_LAUNCH_CHECK(ctx, "tsm_combine_kernel");
     TM_CUDA(ctx, cudaEventRecord(e1, st));
     TM_CUDA(ctx, cudaEventSynchronize(e1));
     float ms = 0;
     cudaEventElapsedTime(&ms, e0, e1);
     if (info) {
-        info->ms_total = ms; info->ms_lp_solve = ms_lp; info->ms_hp_solve = ms_hp;
-        info->ms_contract = ms - ms_lp - ms_hp;      // contraction + noise expansion + accumulation
-        info->iters_lp = it_lp; info->iters_hp = it_hp;
-        info->worst_resid_lp = worst_lp; info->worst_resid_hp = worst_hp;
+        // with NL solves in flight the per-solve elapsed times overlap: their sums are divided by NL
+        info->ms_total = ms; info->ms_lp_solve = R.ms_lp / NL; info->ms_hp_solve = R.ms_hp / NL;
+        info->ms_contract = ms - info->ms_lp_solve - info->ms_hp_solve;   // contraction + noise expansion + accumulation
+        info->iters_lp = R.it_lp; info->iters_hp = R.it_hp;
+        info->worst_resid_lp = R.worst_lp; info->worst_resid_hp = R.worst_hp;
         info->launches = (int)(ctx->launches - launches0);
     }
-    if (noconv) {
+    if (R.noconv) {
         snprintf(ctx->err, sizeof(ctx->err), "tsm_estimate: %d solve(s) missed their rho (worst LP %g, HP %g)",
-                 noconv, worst_lp, worst_hp);
+                 R.noconv, R.worst_lp, R.worst_hp);
         return TM_ENOCONV;
     }
     return TM_OK;

@@ -50,7 +50,7 @@ def test_tsm_with_binary_files(orc):
         ctx.tm_load_gauge(U)
         out, ps, _ = ctx.tsm_estimate(n_lp, n_hp, k, mu, mom, LP, HP, t.TM_F32, t.TM_F64, seed=9, per_source=True)
         out2, f_lp, f_co, _ = ctx.tsm_estimate_binary(n_lp, n_hp, k, mu, mom, LP, HP, t.TM_F32, t.TM_F64, seed=9)
-        assert np.array_equal(to_np(out2), to_np(out))
+        assert rel_l2(to_np(out2), to_np(out)) <= 1e-13      # one lane instead of two: another summation order
         ps = to_np(ps)
         ref_lp, c_lp = orc.binary_store(ps[:n_lp])
         ref_co, c_co = orc.binary_store(ps[n_lp:] - ps[:n_hp])
