@@ -142,7 +142,7 @@ __global__ void __launch_bounds__(256) residual_kernel(SA* __restrict__ r, SL* _
         FA va[8];
 #pragma unroll
         for (int k = 0; k < 8; k++) { nrm += (double)vb[k] * (double)vb[k]; va[k] = (FA)vb[k]; }
-        store8<SA>(r, Vh, h, g, va);
+        if (r) store8<SA>(r, Vh, h, g, va);          // r == NULL: the residual lives in sloppy storage only
         if (!std::is_same<SA, SL>::value) {
             FL vs[8];
 #pragma unroll
@@ -235,7 +235,13 @@ __global__ void __launch_bounds__(256) update_xr_kernel(SA* __restrict__ x, SA* 
         FA vx[8], vr[8];
         FL vp[8], vw[8];
         load8<SA>(x, Vh, h, g, vx);
-        load8<SA>(r, Vh, h, g, vr);
+        if (r) load8<SA>(r, Vh, h, g, vr);
+        else {                                       // r == NULL: the residual lives in sloppy storage only
+            FL vs[8];
+            load8<SL>(rs, Vh, h, g, vs);
+#pragma unroll
+            for (int k = 0; k < 8; k++) vr[k] = (FA)vs[k];
+        }
         load8<SL>(p, Vh, h, g, vp);
         load8<SL>(w, Vh, h, g, vw);
 #pragma unroll
@@ -245,7 +251,7 @@ __global__ void __launch_bounds__(256) update_xr_kernel(SA* __restrict__ x, SA* 
             nrm += (double)vr[k] * (double)vr[k];
         }
         store8<SA>(x, Vh, h, g, vx);
-        store8<SA>(r, Vh, h, g, vr);
+        if (r) store8<SA>(r, Vh, h, g, vr);
         if (!std::is_same<SA, SL>::value) {
             FL vs[8];
 #pragma unroll
@@ -306,14 +312,15 @@ tm_status blas_update_p(tm_ctx* ctx, void* p, const void* z, tm_prec psl, cudaSt
 }
 
 // ------------------------------------------------------------------ scalars
-__global__ void scal_init_kernel(CgScalars* sc, double rho2, double delta2, int max_iter) {
+__global__ void scal_init_kernel(CgScalars* sc, double rho2, double delta2, int max_iter, double eta2) {
     CgScalars z;
     memset(&z, 0, sizeof(z));
     z.rho2 = rho2; z.delta2 = delta2; z.max_iter = max_iter;
+    z.slot[0] = eta2;               // ||eta||^2 when the caller knows it (else 0, filled by the norm kernel)
     *sc = z;
 }
-tm_status scal_init(tm_ctx* ctx, double rho2, double delta2, int max_iter, cudaStream_t st) {
-    scal_init_kernel<<<1, 1, 0, st>>>(ctx->d_scal, rho2, delta2, max_iter);
+tm_status scal_init(tm_ctx* ctx, double rho2, double delta2, int max_iter, double eta2, cudaStream_t st) {
+    scal_init_kernel<<<1, 1, 0, st>>>(ctx->d_scal, rho2, delta2, max_iter, eta2);
     TM_LAUNCH_CHECK(ctx, "scal_init_kernel");
     return TM_OK;
 }

@@ -46,7 +46,8 @@ tm_status blas_ru_begin(tm_ctx* ctx, void* y, tm_prec po, void* x, tm_prec pacc,
 tm_status blas_residual(tm_ctx* ctx, void* r, tm_prec pacc, void* rs, tm_prec psl, const void* b, const void* m,
                         tm_prec po, int red_op, int guard, cudaStream_t st);
 // reset the device state for a new solve (no host synchronisation)
-tm_status scal_init(tm_ctx* ctx, double rho2, double delta2, int max_iter, cudaStream_t st);
+// eta2 > 0: ||eta||^2 known to the caller (Z4 noise: 12 V exactly), no norm kernel needed
+tm_status scal_init(tm_ctx* ctx, double rho2, double delta2, int max_iter, double eta2, cudaStream_t st);
 tm_status scal_get(tm_ctx* ctx, CgScalars* v, cudaStream_t st);          // download + sync
 
 // ---- solver.cu ----------------------------------------------------------------------------
@@ -62,8 +63,9 @@ struct SolveJob {                       // one solve in flight (solver.cu: tm_so
     CgScalars* h_scal;
     bool tail_valid; long enq;
 };
+// eta_norm2 > 0: ||eta||^2 known exactly to the caller (skips the norm kernel); 0: computed
 tm_status tm_solve_begin(tm_ctx* ctx, SolveJob* job, void* d_s, const void* d_eta, double kappa, double mu,
-                         const tm_solve_params* params, cudaStream_t st);
+                         const tm_solve_params* params, cudaStream_t st, double eta_norm2 = 0.0);
 tm_status tm_solve_end(tm_ctx* ctx, SolveJob* job, tm_solve_info* info);
 tm_status tm_solve_internal(tm_ctx* ctx, void* d_s, const void* d_eta, double kappa, double mu,
                             const tm_solve_params* params, tm_solve_info* info, cudaStream_t st);

@@ -61,7 +61,7 @@ static tm_status job_tail(tm_ctx* ctx, const SolveJob& J) {
 }
 
 tm_status tm_solve_begin(tm_ctx* ctx, SolveJob* Jp, void* d_s, const void* d_eta, double kappa, double mu,
-                         const tm_solve_params* P, cudaStream_t st) {
+                         const tm_solve_params* P, cudaStream_t st, double eta_norm2) {
     SolveJob& J = *Jp;
     if (!P) return tm_fail(ctx, TM_EARG, "solve: null params");
     const tm_prec po = P->outer, ps = P->sloppy;
@@ -86,7 +86,9 @@ tm_status tm_solve_begin(tm_ctx* ctx, SolveJob* Jp, void* d_s, const void* d_eta
     TM_TRY(tm_ws(ctx, WS_SL_Z, bs, &J.z));
     TM_TRY(tm_ws(ctx, WS_SL_TMP, bs, &J.tmp));
     TM_TRY(tm_ws(ctx, WS_AC_X, ba, &J.x));
-    TM_TRY(tm_ws(ctx, WS_AC_R, ba, &J.r));
+    // fp16 sloppy storage: the iterated residual lives in fp16 only (11-bit mantissa: 2.4e-4 relative rounding per
+    // update, far below what a reliable update corrects); bf16 (8 bits) keeps an fp32 copy
+    if (ps == TM_F16) J.r = nullptr; else TM_TRY(tm_ws(ctx, WS_AC_R, ba, &J.r));
     if (J.pa != ps) TM_TRY(tm_ws(ctx, WS_SL_R, bs, &J.rs)); else J.rs = J.r;
     TM_TRY(tm_ws(ctx, WS_OU_B, bo, &J.b));
     TM_TRY(tm_ws(ctx, WS_OU_TMP, bo, &J.tmpo));
@@ -98,8 +100,8 @@ tm_status tm_solve_begin(tm_ctx* ctx, SolveJob* Jp, void* d_s, const void* d_eta
     J.s_o = J.y + bo;
 
     // ---- setup (no host synchronisation): state, ||eta||^2, bhat, y = x = 0, r = rs = bhat
-    TM_TRY(scal_init(ctx, P->rho * P->rho, J.delta * J.delta, P->max_iter, st));
-    TM_TRY(blas_norm_full(ctx, d_eta, po, RED_SLOT0 + 0, st));
+    TM_TRY(scal_init(ctx, P->rho * P->rho, J.delta * J.delta, P->max_iter, eta_norm2 > 0 ? eta_norm2 : 0.0, st));
+    if (!(eta_norm2 > 0)) TM_TRY(blas_norm_full(ctx, d_eta, po, RED_SLOT0 + 0, st));
     TM_TRY(blas_twist_inv(ctx, J.tmpo, J.eta_o, po, kappa, mu, 0, st));
     {
         DslashCall k;

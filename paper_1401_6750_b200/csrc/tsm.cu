@@ -152,7 +152,8 @@ static tm_status job_start(TsmRun& R, TsmJob& J, int r, int pass, cudaStream_t s
     J.ac = pass ? P->contract_acc_hp : P->contract_acc_lp;
     TM_TRY(job_noise(R, r, J.po, st, &J.eta_o));
     TM_TRY(tm_ws(ctx, J.po == TM_F32 ? WS_TSM_S32 : WS_TSM_S64, 2 * tm_parity_bytes(ctx, J.po), &J.s_o));
-    return tm_solve_begin(ctx, &J.sj, J.s_o, J.eta_o, P->kappa, P->mu, pass ? &P->hp : &P->lp, st);
+    // Z4 noise: |eta_c| = 1 for each of the 12 V components, so ||eta||^2 = 12 V exactly (no norm kernel)
+    return tm_solve_begin(ctx, &J.sj, J.s_o, J.eta_o, P->kappa, P->mu, pass ? &P->hp : &P->lp, st, 12.0 * (double)ctx->V);
 }
 
 static tm_status job_finish(TsmRun& R, TsmJob& J, int lane) {

@@ -18,7 +18,7 @@ from paper_1401_6750_b200 import inputs, inputs_torch
 
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("--what", default="dslash", choices=["dslash", "contract", "solve"])
+    ap.add_argument("--what", default="dslash", choices=["dslash", "contract", "solve", "sweep"])
     ap.add_argument("--prec", default="f16")
     ap.add_argument("--recon", type=int, default=12)
     ap.add_argument("--dims", type=int, nargs=4, default=[32, 32, 32, 64])
@@ -60,6 +60,47 @@ def main():
         us = e0.elapsed_time(e1) * 1e3 / a.napp
         nbytes = (48 + 8 * a.recon + (24 if a.op == "XPAY" else 0)) * tmod.PREC_BYTES[P] * (V // 2)
         print("dslash %s r%d %s: %.1f us/launch, %.0f GB/s algorithmic" % (a.prec, a.recon, a.op, us, nbytes / us / 1e3))
+    elif a.what == "sweep":
+        # BASELINE.json configs[4] (bandwidth sweep): standalone parity Dslash (XPAY epilogue) and one CG iteration
+        # (4 Dslash + fused BLAS-1) per storage precision / reconstruct; a.napp applications each
+        import json
+        import os
+        V = inputs.volume(dims)
+        Vh = V // 2
+        pk = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "MEASURED_PEAKS.json")
+        peak = json.load(open(pk))["hbm_gbs"] if os.path.exists(pk) else 6650.0
+        print("| storage | recon | us / Dslash | GB/s (algorithmic) | frac of %.0f GB/s | GFLOP/s | CG it/s | us / CG iteration |" % peak)
+        print("|---|---|---|---|---|---|---|---|")
+        eta = inputs_torch.z4_source(dims, 11, 0, dev)
+        for prec in ("f64", "f32", "f16", "bf16"):
+            for recon in (12, 18):
+                Pq = tmod.PREC[prec]
+                tdt = {"f64": torch.float64, "f32": torch.float32, "f16": torch.float16, "bf16": torch.bfloat16}[prec]
+                nb = 3
+                ins = [ctx.empty_field(Pq, False) for _ in range(nb)]
+                outs = [ctx.empty_field(Pq, False) for _ in range(nb)]
+                xs = ctx.empty_field(Pq, False)
+                for b in ins + [xs]:
+                    v = b.view(tdt)
+                    v.copy_((torch.rand(v.shape, device=dev, dtype=torch.float32) - 0.5).to(tdt))
+                for i in range(5):
+                    ctx.tm_dslash(outs[i % nb], ins[i % nb], xs, tmod.TM_OP_XPAY, 0, False, a.kappa, a.mu, Pq, recon)
+                torch.cuda.synchronize()
+                e0.record()
+                for i in range(a.napp):
+                    ctx.tm_dslash(outs[i % nb], ins[i % nb], xs, tmod.TM_OP_XPAY, 0, False, a.kappa, a.mu, Pq, recon)
+                e1.record()
+                torch.cuda.synchronize()
+                us = e0.elapsed_time(e1) * 1e3 / a.napp
+                gbs = (48 + 8 * recon + 24) * tmod.PREC_BYTES[Pq] * Vh / us / 1e3
+                del ins, outs, xs
+                # CG: a fixed number of iterations (rho unreachable, max_iter = 40) so that it/s is per iteration
+                outer = "f32" if prec in ("f16", "bf16") else prec
+                for i in range(2):
+                    s, info = ctx.tm_cg_solve(eta, a.kappa, a.mu, prec, outer, recon, 1e-30, 40, 1e-30, raise_on_noconv=False)
+                it_us = info["ms"] * 1e3 / max(1, info["iters"])
+                print("| %s | %d | %.1f | %.0f | %.2f | %.0f | %.0f | %.1f |" % (
+                    prec, recon, us, gbs, gbs / peak, 1416.0 * Vh / us / 1e3, 1e6 / it_us, it_us))
     elif a.what == "contract":
         s = inputs_torch.z4_source(dims, 11, 0, dev)
         eta = inputs_torch.z4_source(dims, 11, 1, dev)
