@@ -81,8 +81,20 @@ __device__ __forceinline__ void grid_reduce(double v, double* partials, unsigned
     __syncthreads();
     if (is_last) {
         __threadfence();
-        double s = 0.0;
-        for (unsigned int i = threadIdx.x; i < gridDim.x; i += blockDim.x) s += __ldcg(partials + i);
+        // fixed-order sum of the per-block partials, 16 independent loads in flight per thread (a dependent
+        // one-load-per-round loop over 8192 partials costs ~10 us of L2 latency at the tail of every Dslash)
+        double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+        const unsigned int n = gridDim.x, bd = blockDim.x;
+        unsigned int i = threadIdx.x;
+        for (; i + 15u * bd < n; i += 16u * bd) {
+            double v[16];
+#pragma unroll
+            for (int k = 0; k < 16; k++) v[k] = __ldcg(partials + i + (unsigned)k * bd);
+#pragma unroll
+            for (int k = 0; k < 16; k += 4) { s0 += v[k]; s1 += v[k + 1]; s2 += v[k + 2]; s3 += v[k + 3]; }
+        }
+        for (; i < n; i += bd) s0 += __ldcg(partials + i);
+        double s = (s0 + s1) + (s2 + s3);
         s = block_sum(s, sm);
         if (threadIdx.x == 0) {
             *counter = 0;
