@@ -331,6 +331,28 @@ tm_status scal_get(tm_ctx* ctx, CgScalars* v, cudaStream_t st) {
     return TM_OK;
 }
 
+// ------------------------------------------------------------------ second stage of the Dslash norm epilogue
+// one block: fixed-order sum of the n per-block partials a Dslash kernel left behind, then the op on the CG state
+__global__ void __launch_bounds__(1024) reduce_finish_kernel(const double* __restrict__ partials, unsigned int n,
+                                                             CgScalars* sc, int op, int guard) {
+    __shared__ double sm[32];
+    if (guard_skip(sc, guard)) return;
+    double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+    unsigned int i = threadIdx.x;
+    for (; i + 3u * 1024u < n; i += 4u * 1024u) {
+        s0 += partials[i]; s1 += partials[i + 1024u]; s2 += partials[i + 2048u]; s3 += partials[i + 3072u];
+    }
+    for (; i < n; i += 1024u) s0 += partials[i];
+    double s = (s0 + s1) + (s2 + s3);
+    s = block_sum(s, sm);
+    if (threadIdx.x == 0) apply_red_op(sc, op, s);
+}
+tm_status tm_reduce_finish(tm_ctx* ctx, unsigned int nblocks, int op, int guard, cudaStream_t st) {
+    reduce_finish_kernel<<<1, 1024, 0, st>>>(ctx->d_partials, nblocks, ctx->d_scal, op, guard);
+    TM_LAUNCH_CHECK(ctx, "reduce_finish_kernel");
+    return TM_OK;
+}
+
 // ------------------------------------------------------------------ complex128 accumulate
 __global__ void accumulate_kernel(double* __restrict__ acc, const double* __restrict__ x, size_t n) {
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;

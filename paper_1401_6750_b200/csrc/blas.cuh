@@ -66,6 +66,42 @@ __device__ __forceinline__ double block_sum(double v, double* sm /* >= 32 double
     return v;
 }
 
+// what the reduced sum `s` does to the CG state (one thread)
+__device__ __forceinline__ void apply_red_op(CgScalars* sc, int op, double s) {
+    switch (op) {
+        case RED_WW: sc->ww = s; sc->alpha = sc->gamma / s; break;
+        case RED_RR:
+            sc->rr = s; sc->iters += 1;
+            if (!(s > sc->target2) || !(s > sc->ru2) || sc->iters >= sc->max_iter) sc->done = 1;
+            break;
+        case RED_ZZ: sc->beta = sc->gamma > 0.0 ? s / sc->gamma : 0.0; sc->gamma = s; break;
+        case RED_START:
+            sc->target2 = sc->rho2 * sc->slot[0];
+            sc->rr = s; sc->rr_true = s; sc->ru2 = sc->delta2 * s;
+            sc->done = (s > sc->target2 && sc->max_iter > 0) ? 0 : 1;
+            break;
+        case RED_RU:
+            if (sc->n_ru < CG_MAX_PAUSES) sc->pause_iter[sc->n_ru] = sc->iters;
+            sc->n_ru += 1;
+            sc->rr_true = s;
+            if (!(s == s)) sc->done = 3;
+            else if (s <= sc->target2) sc->done = 2;
+            else if (sc->iters >= sc->max_iter) sc->done = 3;
+            else { sc->rr = s; sc->ru2 = sc->delta2 * s; sc->done = 0; }
+            break;
+        default: if (op >= RED_SLOT0) sc->slot[op - RED_SLOT0] = s; break;
+    }
+}
+
+// Per-block partial only (no fence, no atomic, no last-block tail): used by the Dslash kernels, whose 8192
+// short-lived CTAs would each hold their SM slot ~1 us longer for the fence + atomic of grid_reduce (measured:
+// +13.5 us on a 66 us launch).  reduce_finish_kernel (blas.cu), enqueued right behind, sums the partials in
+// a fixed order and applies the op.  Must be reached by all threads of the block.
+__device__ __forceinline__ void block_partial(double v, double* partials, double* sm) {
+    v = block_sum(v, sm);
+    if (threadIdx.x == 0) partials[blockIdx.x] = v;
+}
+
 // Deterministic grid reduction: every block deposits its partial, the last one to arrive sums all
 // partials in a fixed order and applies `op` to the CG scalars.  Must be reached by all threads.
 __device__ __forceinline__ void grid_reduce(double v, double* partials, unsigned int* counter,
@@ -98,29 +134,7 @@ __device__ __forceinline__ void grid_reduce(double v, double* partials, unsigned
         s = block_sum(s, sm);
         if (threadIdx.x == 0) {
             *counter = 0;
-            switch (op) {
-                case RED_WW: sc->ww = s; sc->alpha = sc->gamma / s; break;
-                case RED_RR:
-                    sc->rr = s; sc->iters += 1;
-                    if (!(s > sc->target2) || !(s > sc->ru2) || sc->iters >= sc->max_iter) sc->done = 1;
-                    break;
-                case RED_ZZ: sc->beta = sc->gamma > 0.0 ? s / sc->gamma : 0.0; sc->gamma = s; break;
-                case RED_START:
-                    sc->target2 = sc->rho2 * sc->slot[0];
-                    sc->rr = s; sc->rr_true = s; sc->ru2 = sc->delta2 * s;
-                    sc->done = (s > sc->target2 && sc->max_iter > 0) ? 0 : 1;
-                    break;
-                case RED_RU:
-                    if (sc->n_ru < CG_MAX_PAUSES) sc->pause_iter[sc->n_ru] = sc->iters;
-                    sc->n_ru += 1;
-                    sc->rr_true = s;
-                    if (!(s == s)) sc->done = 3;
-                    else if (s <= sc->target2) sc->done = 2;
-                    else if (sc->iters >= sc->max_iter) sc->done = 3;
-                    else { sc->rr = s; sc->ru2 = sc->delta2 * s; sc->done = 0; }
-                    break;
-                default: if (op >= RED_SLOT0) sc->slot[op - RED_SLOT0] = s; break;
-            }
+            apply_red_op(sc, op, s);
         }
     }
 }

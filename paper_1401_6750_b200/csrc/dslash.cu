@@ -8,7 +8,7 @@
 // policy for links (zero reuse), default policy for spinors (8-fold reuse served by L1/L2).
 //
 // Epilogue (runtime-uniform):  res = c * (D in);  xmode 1: res += x;  xmode 2: res += A x;
-//                              post 1: res = A^-1 res;  optional ||res||^2 -> grid_reduce.
+//                              post 1: res = A^-1 res;  optional ||res||^2 -> per-block partials + reduce_finish_kernel.
 // A = 1 + i a g5,  a = 2 kappa mu (sign flipped for dagger),  A^-1 = (1 - i a g5) / (1 + a^2).
 //
 // Chiral basis (reading 2): g_mu = [[0, B],[B^dag, 0]] with
@@ -187,7 +187,7 @@ __global__ void __launch_bounds__(128) dslash_kernel(DslashArgs<typename Prec<S>
             for (int i = 0; i < 24; i++) nrm += (double)acc[i] * (double)acc[i];
         }
     }
-    if (A.red_op != RED_NONE) grid_reduce(nrm, A.partials, A.counter, A.sc, A.red_op, sm);
+    if (A.red_op != RED_NONE) block_partial(nrm, A.partials, sm);
 }
 
 
@@ -518,7 +518,7 @@ __global__ void __launch_bounds__(128, MINB) dslash16_kernel(DslashArgs<float> A
             nrm = (double)n2;
         }
     }
-    if (A.red_op != RED_NONE) grid_reduce(nrm, A.partials, A.counter, A.sc, A.red_op, sm);
+    if (A.red_op != RED_NONE) block_partial(nrm, A.partials, sm);
 }
 
 template <typename S, int R>
@@ -539,6 +539,7 @@ static tm_status launch_t(tm_ctx* ctx, const DslashCall& c, const void* gauge, c
     const int grid = (int)((ctx->Vh + block - 1) / block);
     dslash_kernel<S, R><<<grid, block, 0, st>>>(A);
     TM_LAUNCH_CHECK(ctx, "dslash_kernel");
+    if (c.red_op != RED_NONE) TM_TRY(tm_reduce_finish(ctx, (unsigned)grid, c.red_op, c.guard, st));
     return TM_OK;
 }
 
@@ -562,6 +563,7 @@ static tm_status launch16(tm_ctx* ctx, const DslashCall& c, const void* gauge, c
     if (c.dagger) dslash16_kernel<S, 1, 2, 5><<<grid, block, 0, st>>>(A);
     else          dslash16_kernel<S, 0, 2, 5><<<grid, block, 0, st>>>(A);
     TM_LAUNCH_CHECK(ctx, "dslash16_kernel");
+    if (c.red_op != RED_NONE) TM_TRY(tm_reduce_finish(ctx, (unsigned)grid, c.red_op, c.guard, st));
     return TM_OK;
 }
 

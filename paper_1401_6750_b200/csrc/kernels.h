@@ -45,6 +45,8 @@ tm_status blas_ru_begin(tm_ctx* ctx, void* y, tm_prec po, void* x, tm_prec pacc,
 //   GUARD_ALWAYS; RED_RU: GUARD_RU)
 tm_status blas_residual(tm_ctx* ctx, void* r, tm_prec pacc, void* rs, tm_prec psl, const void* b, const void* m,
                         tm_prec po, int red_op, int guard, cudaStream_t st);
+// second stage of a Dslash norm epilogue: sum the nblocks per-block partials, apply red_op (same guard as the Dslash)
+tm_status tm_reduce_finish(tm_ctx* ctx, unsigned int nblocks, int op, int guard, cudaStream_t st);
 // reset the device state for a new solve (no host synchronisation)
 // eta2 > 0: ||eta||^2 known to the caller (Z4 noise: 12 V exactly), no norm kernel needed
 tm_status scal_init(tm_ctx* ctx, double rho2, double delta2, int max_iter, double eta2, cudaStream_t st);
