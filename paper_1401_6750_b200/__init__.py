@@ -19,7 +19,7 @@ import numpy as np
 from . import inputs  # noqa: F401  (seeded input generators; no method arithmetic)
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libtmloops.so")
+LIB_PATH = os.environ.get("TMLOOPS_LIB") or os.path.join(_HERE, "libtmloops.so")
 
 TM_OK, TM_EARG, TM_EDIM, TM_EPREC, TM_ECUDA, TM_ENOCONV, TM_EALLOC = range(7)
 TM_F64, TM_F32, TM_F16, TM_BF16 = range(4)

@@ -77,6 +77,40 @@ __global__ void twist_inv_kernel(S* __restrict__ dst, const S* __restrict__ src,
     store8<S>(dst, Vh, h, g, v);
 }
 
+// dst = A^-1 src + c * add   (odd-site reconstruction s_o = A^-1 eta_o + kappa [A^-1 D_oe y], solver.cu)
+template <typename S>
+__global__ void twist_inv_axpy_kernel(S* __restrict__ dst, const S* __restrict__ src, const S* __restrict__ add, int Vh,
+                                      typename Prec<S>::F a, typename Prec<S>::F c) {
+    typedef typename Prec<S>::F F;
+    const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= 3L * Vh) return;
+    const int g = (int)(i / Vh), h = (int)(i % Vh);
+    F v[8], w[8];
+    load8<S>(src, Vh, h, g, v);
+    load8<S>(add, Vh, h, g, w);
+    const F n = F(1) / (F(1) + a * a);
+#pragma unroll
+    for (int k = 0; k < 8; k += 2) {
+        const bool upper = (8 * g + k) < 12;
+        const F s = upper ? a : -a;
+        const F re = v[k], im = v[k + 1];
+        v[k] = n * (re + s * im) + c * w[k];
+        v[k + 1] = n * (im - s * re) + c * w[k + 1];
+    }
+    store8<S>(dst, Vh, h, g, v);
+}
+tm_status blas_twist_inv_axpy(tm_ctx* ctx, void* dst, const void* src, const void* add, tm_prec p, double kappa,
+                              double mu, double c, cudaStream_t st) {
+    const double a = 2.0 * kappa * mu;
+    return dispatch_prec(ctx, p, [&](auto* t) {
+        typedef TAGTYPE(t) S;
+        typedef typename Prec<S>::F F;
+        twist_inv_axpy_kernel<S><<<items_grid(ctx, 256), 256, 0, st>>>((S*)dst, (const S*)src, (const S*)add, (int)ctx->Vh, (F)a, (F)c);
+        TM_LAUNCH_CHECK(ctx, "twist_inv_axpy_kernel");
+        return TM_OK;
+    });
+}
+
 tm_status blas_twist_inv(tm_ctx* ctx, void* dst, const void* src, tm_prec p, double kappa, double mu,
                          int dagger, cudaStream_t st) {
     const double a = 2.0 * kappa * mu * (dagger ? -1.0 : 1.0);

@@ -29,6 +29,9 @@ tm_status blas_copy(tm_ctx* ctx, void* dst, tm_prec pd, const void* src, tm_prec
 // dst = A^-1 src  (site-local twist inverse)
 tm_status blas_twist_inv(tm_ctx* ctx, void* dst, const void* src, tm_prec p, double kappa, double mu,
                          int dagger, cudaStream_t st);
+// dst = A^-1 src + c * add
+tm_status blas_twist_inv_axpy(tm_ctx* ctx, void* dst, const void* src, const void* add, tm_prec p, double kappa,
+                              double mu, double c, cudaStream_t st);
 // ||v||^2 -> red_op
 tm_status blas_norm(tm_ctx* ctx, const void* v, tm_prec p, int red_op, cudaStream_t st);
 // full-lattice norm (2 parities)

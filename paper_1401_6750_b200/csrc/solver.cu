@@ -13,7 +13,7 @@
 // every kernel is guarded by that state.  The host only enqueues:
 //   iteration block  (GUARD_ITER)  z = Mhat^dag r ; p = z + beta p ; w = Mhat p ; x += alpha p, r -= alpha w
 //   update block     (GUARD_RU)    y += x, x = 0 ; r = bhat - Mhat y in outer precision ; resume | finish
-//   tail             (always)      s_o = A^-1 (eta_o + kappa D_oe y)
+//   tail             (always)      s_o = A^-1 eta_o + kappa [A^-1 D_oe y]   (bracket: by-product of the last update)
 // along the plan recorded by the previous solve with the same parameters, and reads the state back
 // once at the end (one host synchronisation per solve when the plan fits; otherwise it keeps
 // enqueueing [iteration, update] pairs and polls).
@@ -50,12 +50,11 @@ static tm_status job_update(tm_ctx* ctx, const SolveJob& J) {
     TM_TRY(apply_mhat(ctx, J.mo, J.y, J.tmpo, 0, J.kappa, J.mu, J.po, J.rc, RED_NONE, GUARD_RU, J.st));
     return blas_residual(ctx, J.r, J.pa, J.rs, J.ps, J.b, J.mo, J.po, RED_RU, GUARD_RU, J.st);
 }
+// s_o = A^-1 (eta_o + kappa D_oe y) = A^-1 eta_o + kappa [A^-1 D_oe y]: the bracket is the first half of Mhat y,
+// left in tmpo by the LAST reliable update that ran -- and the solve always ends on one (it is the update that
+// declares convergence or failure; y does not change after it), so the tail needs no Dslash of its own.
 static tm_status job_tail(tm_ctx* ctx, const SolveJob& J) {
-    DslashCall k;
-    memset(&k, 0, sizeof(k));
-    k.out = J.s_o; k.in = J.y; k.x = J.eta_o; k.out_parity = 1; k.kappa = J.kappa; k.mu = J.mu;
-    k.xmode = 1; k.post = 1; k.coef = J.kappa; k.red_op = RED_NONE;
-    TM_TRY(tm_dslash_launch(ctx, k, J.po, J.rc, J.st));
+    TM_TRY(blas_twist_inv_axpy(ctx, J.s_o, J.eta_o, J.tmpo, J.po, J.kappa, J.mu, J.kappa, J.st));
     TM_CUDA(ctx, cudaEventRecord(J.e1, J.st));
     return TM_OK;
 }
