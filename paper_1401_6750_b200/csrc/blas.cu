@@ -130,14 +130,19 @@ __global__ void ru_begin_kernel(Sy* __restrict__ y, Sx* __restrict__ x, int Vh, 
     const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= 3L * Vh) return;
     const int g = (int)(i / Vh), h = (int)(i % Vh);
+    // y += x ; x = 0, with both vectors possibly "zero by construction" (CgScalars::x_zero / y_zero: then they are
+    // not read, and x is not zero-filled -- RED_RU raises x_zero instead)
+    const bool xz = sc->x_zero != 0, yz = sc->y_zero != 0;
+    if (xz && !yz) return;
     typename Prec<Sx>::F a[8];
     typename Prec<Sy>::F b[8];
-    load8<Sx>(x, Vh, h, g, a);
-    load8<Sy>(y, Vh, h, g, b);
 #pragma unroll
-    for (int k = 0; k < 8; k++) { b[k] += (typename Prec<Sy>::F)a[k]; a[k] = 0; }
+    for (int k = 0; k < 8; k++) { a[k] = 0; b[k] = 0; }
+    if (!xz) load8<Sx>(x, Vh, h, g, a);
+    if (!yz) load8<Sy>(y, Vh, h, g, b);
+#pragma unroll
+    for (int k = 0; k < 8; k++) b[k] += (typename Prec<Sy>::F)a[k];
     store8<Sy>(y, Vh, h, g, b);
-    store8<Sx>(x, Vh, h, g, a);
 }
 
 tm_status blas_ru_begin(tm_ctx* ctx, void* y, tm_prec po, void* x, tm_prec pacc, cudaStream_t st) {
@@ -263,12 +268,16 @@ __global__ void __launch_bounds__(256) update_xr_kernel(SA* __restrict__ x, SA* 
     __shared__ double sm[32];
     if (guard_skip(sc, GUARD_ITER)) return;
     const FA alpha = (FA)sc->alpha;
+    const bool xz = sc->x_zero != 0;             // first update after a (re)start: x is zero by construction
     double nrm = 0.0;
     for (long i = (long)blockIdx.x * blockDim.x + threadIdx.x; i < 3L * Vh; i += (long)gridDim.x * blockDim.x) {
         const int g = (int)(i / Vh), h = (int)(i % Vh);
         FA vx[8], vr[8];
         FL vp[8], vw[8];
-        load8<SA>(x, Vh, h, g, vx);
+        if (xz) {
+#pragma unroll
+            for (int k = 0; k < 8; k++) vx[k] = 0;
+        } else load8<SA>(x, Vh, h, g, vx);
         if (r) load8<SA>(r, Vh, h, g, vr);
         else {                                       // r == NULL: the residual lives in sloppy storage only
             FL vs[8];
@@ -350,6 +359,7 @@ __global__ void scal_init_kernel(CgScalars* sc, double rho2, double delta2, int 
     CgScalars z;
     memset(&z, 0, sizeof(z));
     z.rho2 = rho2; z.delta2 = delta2; z.max_iter = max_iter;
+    z.x_zero = 1; z.y_zero = 1;
     z.slot[0] = eta2;               // ||eta||^2 when the caller knows it (else 0, filled by the norm kernel)
     *sc = z;
 }

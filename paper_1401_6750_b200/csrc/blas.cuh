@@ -27,6 +27,8 @@ struct CgScalars {
     int iters;
     int max_iter;
     int n_ru;          // reliable updates so far
+    int x_zero;        // x == 0 by construction (start of a solve / after a reliable update): x is neither read nor zero-filled
+    int y_zero;        // y == 0 by construction (no reliable update yet): y is not read
     int pause_iter[CG_MAX_PAUSES];   // iteration count at each pause (replayed by the host as a launch plan)
 };
 
@@ -71,7 +73,7 @@ __device__ __forceinline__ void apply_red_op(CgScalars* sc, int op, double s) {
     switch (op) {
         case RED_WW: sc->ww = s; sc->alpha = sc->gamma / s; break;
         case RED_RR:
-            sc->rr = s; sc->iters += 1;
+            sc->rr = s; sc->iters += 1; sc->x_zero = 0;
             if (!(s > sc->target2) || !(s > sc->ru2) || sc->iters >= sc->max_iter) sc->done = 1;
             break;
         case RED_ZZ: sc->beta = sc->gamma > 0.0 ? s / sc->gamma : 0.0; sc->gamma = s; break;
@@ -84,6 +86,7 @@ __device__ __forceinline__ void apply_red_op(CgScalars* sc, int op, double s) {
             if (sc->n_ru < CG_MAX_PAUSES) sc->pause_iter[sc->n_ru] = sc->iters;
             sc->n_ru += 1;
             sc->rr_true = s;
+            sc->x_zero = 1; sc->y_zero = 0;      // ru_begin folded x into y
             if (!(s == s)) sc->done = 3;
             else if (s <= sc->target2) sc->done = 2;
             else if (sc->iters >= sc->max_iter) sc->done = 3;

@@ -98,7 +98,8 @@ tm_status tm_solve_begin(tm_ctx* ctx, SolveJob* Jp, void* d_s, const void* d_eta
     J.y = (char*)d_s;                      // the even half of the solution is accumulated in place
     J.s_o = J.y + bo;
 
-    // ---- setup (no host synchronisation): state, ||eta||^2, bhat, y = x = 0, r = rs = bhat
+    // ---- setup (no host synchronisation): state (x and y zero by construction: CgScalars::x_zero / y_zero), ||eta||^2,
+    //      bhat, r = rs = bhat
     TM_TRY(scal_init(ctx, P->rho * P->rho, J.delta * J.delta, P->max_iter, eta_norm2 > 0 ? eta_norm2 : 0.0, st));
     if (!(eta_norm2 > 0)) TM_TRY(blas_norm_full(ctx, d_eta, po, RED_SLOT0 + 0, st));
     TM_TRY(blas_twist_inv(ctx, J.tmpo, J.eta_o, po, kappa, mu, 0, st));
@@ -109,8 +110,6 @@ tm_status tm_solve_begin(tm_ctx* ctx, SolveJob* Jp, void* d_s, const void* d_eta
         k.xmode = 1; k.coef = kappa; k.red_op = RED_NONE;
         TM_TRY(tm_dslash_launch(ctx, k, po, J.rc, st));
     }
-    TM_TRY(blas_zero(ctx, J.y, po, st));
-    TM_TRY(blas_zero(ctx, J.x, J.pa, st));
     TM_TRY(blas_residual(ctx, J.r, J.pa, J.rs, ps, J.b, nullptr, po, RED_START, GUARD_ALWAYS, st));
 
     const CgPlan& plan = ctx->plan[(int)ps];
