@@ -175,6 +175,21 @@ extern "C" tm_status tm_field_export(tm_ctx* c, void* d_canon, const void* d_int
     return tm_export_launch(c, d_canon, d_internal, prec, (cudaStream_t)stream);
 }
 
+// EXPERIMENT: two stacked parity fields per launch (source 1 at byte offset = parity bytes)
+extern "C" tm_status tm_dslash_pair(tm_ctx* c, void* d_out, const void* d_in, const void* d_x, tm_op op,
+                                    int out_parity, int dagger, double kappa, double mu, tm_prec prec, void* stream) {
+    cudaStream_t st = (cudaStream_t)stream;
+    DslashCall k;
+    memset(&k, 0, sizeof(k));
+    k.out = d_out; k.in = d_in; k.x = nullptr;
+    k.out_parity = out_parity & 1; k.dagger = dagger ? 1 : 0;
+    k.kappa = kappa; k.mu = mu; k.coef = 1.0; k.red_op = RED_NONE;
+    k.nb = 2; k.fstride = tm_parity_bytes(c, prec);
+    if (op == TM_OP_HOP_TWINV) k.post = 1;
+    if (op == TM_OP_XPAY) { k.x = d_x; k.xmode = 2; k.coef = -kappa * kappa; }
+    return tm_dslash_launch(c, k, prec, TM_R12, st);
+}
+
 extern "C" tm_status tm_dslash(tm_ctx* c, void* d_out, const void* d_in, const void* d_x, tm_op op,
                                int out_parity, int dagger, double kappa, double mu, tm_prec prec,
                                tm_recon recon, void* stream) {

@@ -100,9 +100,12 @@ __device__ __forceinline__ void apply_red_op(CgScalars* sc, int op, double s) {
 // short-lived CTAs would each hold their SM slot ~1 us longer for the fence + atomic of grid_reduce (measured:
 // +13.5 us on a 66 us launch).  reduce_finish_kernel (blas.cu), enqueued right behind, sums the partials in
 // a fixed order and applies the op.  Must be reached by all threads of the block.
-__device__ __forceinline__ void block_partial(double v, double* partials, double* sm) {
+__device__ __forceinline__ void block_partial_at(double v, double* partials, int slot, double* sm) {
     v = block_sum(v, sm);
-    if (threadIdx.x == 0) partials[blockIdx.x] = v;
+    if (threadIdx.x == 0) partials[slot] = v;
+}
+__device__ __forceinline__ void block_partial(double v, double* partials, double* sm) {
+    block_partial_at(v, partials, blockIdx.x, sm);
 }
 
 // Deterministic grid reduction: every block deposits its partial, the last one to arrive sums all

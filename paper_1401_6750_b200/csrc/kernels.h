@@ -12,6 +12,8 @@ struct DslashCall {
     int xmode, post;
     int red_op;        // RED_* applied to ||out||^2 (RED_NONE: no norm)
     int guard;         // GUARD_ALWAYS | GUARD_ITER | GUARD_RU (blas.cuh)
+    int nb;            // 0 | 1: one source; 2: a pair (source 1's fields fstride bytes behind source 0's)
+    size_t fstride;
 };
 tm_status tm_dslash_launch(tm_ctx* ctx, const DslashCall& c, tm_prec prec, tm_recon recon, cudaStream_t st);
 
