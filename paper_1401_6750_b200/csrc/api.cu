@@ -11,10 +11,10 @@ extern "C" long tm_launch_count(const tm_ctx* ctx) { return ctx ? ctx->launches 
 static bool lane_alloc(tm_ctx* c, int lane) {
     bool ok = cudaMalloc((void**)&c->d_partials, sizeof(double) * (1 << 18)) == cudaSuccess
            && cudaMalloc((void**)&c->d_counter, sizeof(unsigned int) * 4) == cudaSuccess
-           && cudaMalloc((void**)&c->d_scal, sizeof(CgScalars)) == cudaSuccess
-           && cudaMallocHost((void**)&c->h_scal, sizeof(CgScalars)) == cudaSuccess
+           && cudaMalloc((void**)&c->d_scal, 2 * sizeof(CgScalars)) == cudaSuccess
+           && cudaMallocHost((void**)&c->h_scal, 2 * sizeof(CgScalars)) == cudaSuccess
            && cudaMemset(c->d_counter, 0, sizeof(unsigned int) * 4) == cudaSuccess
-           && cudaMemset(c->d_scal, 0, sizeof(CgScalars)) == cudaSuccess;
+           && cudaMemset(c->d_scal, 0, 2 * sizeof(CgScalars)) == cudaSuccess;
     for (int i = 0; ok && i < TM_NEVENTS; i++) ok = cudaEventCreate(&c->ev[i]) == cudaSuccess;
     if (ok && lane > 0) ok = cudaStreamCreateWithFlags(&c->lane_stream, cudaStreamNonBlocking) == cudaSuccess;
     return ok;
@@ -175,19 +175,33 @@ extern "C" tm_status tm_field_export(tm_ctx* c, void* d_canon, const void* d_int
     return tm_export_launch(c, d_canon, d_internal, prec, (cudaStream_t)stream);
 }
 
-// EXPERIMENT: two stacked parity fields per launch (source 1 at byte offset = parity bytes)
+// Row f3 (multi-source Dslash): the same operator pieces as tm_dslash (HOP, HOP_TWINV, XPAY; reconstruct-12) on TWO
+// stacked parity fields per launch -- source 1's in / x / out one parity field (tm_field_bytes(prec, 0)) behind
+// source 0's.  CTAs 2k and 2k+1 work on the same 128 sites of the two sources, so the second reader of every
+// link finds it in L2 instead of HBM.  Results are bit-identical to two tm_dslash calls.
 extern "C" tm_status tm_dslash_pair(tm_ctx* c, void* d_out, const void* d_in, const void* d_x, tm_op op,
                                     int out_parity, int dagger, double kappa, double mu, tm_prec prec, void* stream) {
+    if (!c || !d_out || !d_in) return tm_fail(c, TM_EARG, "tm_dslash_pair: null argument");
+    if (d_out == d_in) return tm_fail(c, TM_EARG, "tm_dslash_pair: out must not alias in");
+    if ((int)prec < 0 || (int)prec > 3) return tm_fail(c, TM_EPREC, "tm_dslash_pair: unknown precision");
+    if (op == TM_OP_XPAY && !d_x) return tm_fail(c, TM_EARG, "tm_dslash_pair: XPAY needs x");
     cudaStream_t st = (cudaStream_t)stream;
+    TM_CUDA(c, cudaSetDevice(c->device));
     DslashCall k;
     memset(&k, 0, sizeof(k));
     k.out = d_out; k.in = d_in; k.x = nullptr;
     k.out_parity = out_parity & 1; k.dagger = dagger ? 1 : 0;
     k.kappa = kappa; k.mu = mu; k.coef = 1.0; k.red_op = RED_NONE;
-    k.nb = 2; k.fstride = tm_parity_bytes(c, prec);
-    if (op == TM_OP_HOP_TWINV) k.post = 1;
-    if (op == TM_OP_XPAY) { k.x = d_x; k.xmode = 2; k.coef = -kappa * kappa; }
-    return tm_dslash_launch(c, k, prec, TM_R12, st);
+    switch (op) {
+        case TM_OP_HOP: break;
+        case TM_OP_HOP_TWINV: k.post = 1; break;
+        case TM_OP_XPAY: k.x = d_x; k.xmode = 2; k.coef = -kappa * kappa; break;
+        default: return tm_fail(c, TM_EARG, "tm_dslash_pair: op must be HOP, HOP_TWINV or XPAY");
+    }
+    c->nb = 2;
+    const tm_status s = tm_dslash_launch(c, k, prec, TM_R12, st);
+    c->nb = 1;
+    return s;
 }
 
 extern "C" tm_status tm_dslash(tm_ctx* c, void* d_out, const void* d_in, const void* d_x, tm_op op,

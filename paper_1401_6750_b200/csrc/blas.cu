@@ -15,6 +15,13 @@ template <typename Fn> static tm_status dispatch_prec(tm_ctx* ctx, tm_prec p, Fn
 }
 #define TAGTYPE(tag) typename std::remove_pointer<decltype(tag)>::type
 
+// Paired solves (ctx->nb == 2): blockIdx.y selects the source; its vectors sit one parity vector (24 Vh elements
+// of their own type) behind source 0's, its CG state, reduction partials and counter one slot behind.
+template <typename S> __device__ __forceinline__ S* src_vec(S* p, int src, int Vh) {
+    return p ? p + (size_t)src * 24 * (size_t)Vh : p;
+}
+static inline dim3 pair_grid(const tm_ctx* ctx, unsigned gx) { return dim3(gx, (unsigned)(ctx->nb == 2 ? 2 : 1)); }
+
 static inline unsigned items_grid(const tm_ctx* ctx, int block, int nparity = 1) {
     return (unsigned)((3 * ctx->Vh * nparity + block - 1) / block);
 }
@@ -59,6 +66,7 @@ template <typename S>
 __global__ void twist_inv_kernel(S* __restrict__ dst, const S* __restrict__ src, int Vh,
                                  typename Prec<S>::F a) {
     typedef typename Prec<S>::F F;
+    dst = src_vec(dst, blockIdx.y, Vh); src = src_vec(src, blockIdx.y, Vh);
     const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= 3L * Vh) return;
     const int g = (int)(i / Vh), h = (int)(i % Vh);
@@ -82,6 +90,7 @@ template <typename S>
 __global__ void twist_inv_axpy_kernel(S* __restrict__ dst, const S* __restrict__ src, const S* __restrict__ add, int Vh,
                                       typename Prec<S>::F a, typename Prec<S>::F c) {
     typedef typename Prec<S>::F F;
+    dst = src_vec(dst, blockIdx.y, Vh); src = src_vec(src, blockIdx.y, Vh); add = src_vec(add, blockIdx.y, Vh);
     const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= 3L * Vh) return;
     const int g = (int)(i / Vh), h = (int)(i % Vh);
@@ -105,7 +114,7 @@ tm_status blas_twist_inv_axpy(tm_ctx* ctx, void* dst, const void* src, const voi
     return dispatch_prec(ctx, p, [&](auto* t) {
         typedef TAGTYPE(t) S;
         typedef typename Prec<S>::F F;
-        twist_inv_axpy_kernel<S><<<items_grid(ctx, 256), 256, 0, st>>>((S*)dst, (const S*)src, (const S*)add, (int)ctx->Vh, (F)a, (F)c);
+        twist_inv_axpy_kernel<S><<<pair_grid(ctx, items_grid(ctx, 256)), 256, 0, st>>>((S*)dst, (const S*)src, (const S*)add, (int)ctx->Vh, (F)a, (F)c);
         TM_LAUNCH_CHECK(ctx, "twist_inv_axpy_kernel");
         return TM_OK;
     });
@@ -116,7 +125,7 @@ tm_status blas_twist_inv(tm_ctx* ctx, void* dst, const void* src, tm_prec p, dou
     const double a = 2.0 * kappa * mu * (dagger ? -1.0 : 1.0);
     return dispatch_prec(ctx, p, [&](auto* t) {
         typedef TAGTYPE(t) S;
-        twist_inv_kernel<S><<<items_grid(ctx, 256), 256, 0, st>>>((S*)dst, (const S*)src, (int)ctx->Vh,
+        twist_inv_kernel<S><<<pair_grid(ctx, items_grid(ctx, 256)), 256, 0, st>>>((S*)dst, (const S*)src, (int)ctx->Vh,
                                                                (typename Prec<S>::F)a);
         TM_LAUNCH_CHECK(ctx, "twist_inv_kernel");
         return TM_OK;
@@ -126,6 +135,7 @@ tm_status blas_twist_inv(tm_ctx* ctx, void* dst, const void* src, tm_prec p, dou
 // ------------------------------------------------------------------ reliable update, part 1: y += x ; x = 0
 template <typename Sy, typename Sx>
 __global__ void ru_begin_kernel(Sy* __restrict__ y, Sx* __restrict__ x, int Vh, const CgScalars* sc) {
+    sc += blockIdx.y; y = src_vec(y, blockIdx.y, Vh); x = src_vec(x, blockIdx.y, Vh);
     if (guard_skip(sc, GUARD_RU)) return;
     const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= 3L * Vh) return;
@@ -146,7 +156,7 @@ __global__ void ru_begin_kernel(Sy* __restrict__ y, Sx* __restrict__ x, int Vh, 
 }
 
 tm_status blas_ru_begin(tm_ctx* ctx, void* y, tm_prec po, void* x, tm_prec pacc, cudaStream_t st) {
-    const unsigned grid = items_grid(ctx, 256);
+    const dim3 grid = pair_grid(ctx, items_grid(ctx, 256));
     const int Vh = (int)ctx->Vh;
     if (po == TM_F64 && pacc == TM_F64) ru_begin_kernel<double, double><<<grid, 256, 0, st>>>((double*)y, (double*)x, Vh, ctx->d_scal);
     else if (po == TM_F64 && pacc == TM_F32) ru_begin_kernel<double, float><<<grid, 256, 0, st>>>((double*)y, (float*)x, Vh, ctx->d_scal);
@@ -166,6 +176,11 @@ __global__ void __launch_bounds__(256) residual_kernel(SA* __restrict__ r, SL* _
     typedef typename Prec<SA>::F FA;
     typedef typename Prec<SL>::F FL;
     __shared__ double sm[32];
+    {
+        const int src = blockIdx.y;
+        sc += src; partials += src * TM_PSTRIDE; counter += src;
+        r = src_vec(r, src, Vh); rs = src_vec(rs, src, Vh); b = src_vec(b, src, Vh); m = src_vec(m, src, Vh);
+    }
     if (guard_skip(sc, guard)) return;
     double nrm = 0.0;
     for (long i = (long)blockIdx.x * blockDim.x + threadIdx.x; i < 3L * Vh; i += (long)gridDim.x * blockDim.x) {
@@ -201,7 +216,7 @@ static inline unsigned red_grid(const tm_ctx* ctx, long items, int block) {
 template <typename SO, typename SA, typename SL>
 static tm_status residual_launch(tm_ctx* ctx, void* r, void* rs, const void* b, const void* m, int red_op, int guard,
                                  cudaStream_t st) {
-    const unsigned grid = red_grid(ctx, 3L * ctx->Vh, 256);
+    const dim3 grid = pair_grid(ctx, red_grid(ctx, 3L * ctx->Vh, 256));
     residual_kernel<SO, SA, SL><<<grid, 256, 0, st>>>((SA*)r, (SL*)rs, (const SO*)b, (const SO*)m, (int)ctx->Vh, red_op,
                                                      guard, ctx->d_partials, ctx->d_counter, ctx->d_scal);
     TM_LAUNCH_CHECK(ctx, "residual_kernel");
@@ -266,6 +281,11 @@ __global__ void __launch_bounds__(256) update_xr_kernel(SA* __restrict__ x, SA* 
     typedef typename Prec<SA>::F FA;
     typedef typename Prec<SL>::F FL;
     __shared__ double sm[32];
+    {
+        const int src = blockIdx.y;
+        sc += src; partials += src * TM_PSTRIDE; counter += src;
+        x = src_vec(x, src, Vh); r = src_vec(r, src, Vh); p = src_vec(p, src, Vh); w = src_vec(w, src, Vh); rs = src_vec(rs, src, Vh);
+    }
     if (guard_skip(sc, GUARD_ITER)) return;
     const FA alpha = (FA)sc->alpha;
     const bool xz = sc->x_zero != 0;             // first update after a (re)start: x is zero by construction
@@ -307,7 +327,7 @@ __global__ void __launch_bounds__(256) update_xr_kernel(SA* __restrict__ x, SA* 
 
 tm_status blas_update_xr(tm_ctx* ctx, void* x, void* r, tm_prec pacc, const void* p, const void* w,
                          void* rs, tm_prec psl, cudaStream_t st) {
-    const unsigned grid = red_grid(ctx, 3L * ctx->Vh, 256);
+    const dim3 grid = pair_grid(ctx, red_grid(ctx, 3L * ctx->Vh, 256));
     const int Vh = (int)ctx->Vh;
     double* pa = ctx->d_partials; unsigned int* cn = ctx->d_counter; CgScalars* sc = ctx->d_scal;
     if (pacc == TM_F64 && psl == TM_F64)
@@ -327,6 +347,7 @@ tm_status blas_update_xr(tm_ctx* ctx, void* x, void* r, tm_prec pacc, const void
 template <typename S>
 __global__ void update_p_kernel(S* __restrict__ p, const S* __restrict__ z, int Vh, const CgScalars* sc) {
     typedef typename Prec<S>::F F;
+    sc += blockIdx.y; p = src_vec(p, blockIdx.y, Vh); z = src_vec(z, blockIdx.y, Vh);
     if (guard_skip(sc, GUARD_ITER)) return;
     const F beta = (F)sc->beta;
     const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -348,7 +369,7 @@ __global__ void update_p_kernel(S* __restrict__ p, const S* __restrict__ z, int 
 tm_status blas_update_p(tm_ctx* ctx, void* p, const void* z, tm_prec psl, cudaStream_t st) {
     return dispatch_prec(ctx, psl, [&](auto* t) {
         typedef TAGTYPE(t) S;
-        update_p_kernel<S><<<items_grid(ctx, 256), 256, 0, st>>>((S*)p, (const S*)z, (int)ctx->Vh, ctx->d_scal);
+        update_p_kernel<S><<<pair_grid(ctx, items_grid(ctx, 256)), 256, 0, st>>>((S*)p, (const S*)z, (int)ctx->Vh, ctx->d_scal);
         TM_LAUNCH_CHECK(ctx, "update_p_kernel");
         return TM_OK;
     });
@@ -361,17 +382,17 @@ __global__ void scal_init_kernel(CgScalars* sc, double rho2, double delta2, int 
     z.rho2 = rho2; z.delta2 = delta2; z.max_iter = max_iter;
     z.x_zero = 1; z.y_zero = 1;
     z.slot[0] = eta2;               // ||eta||^2 when the caller knows it (else 0, filled by the norm kernel)
-    *sc = z;
+    sc[blockIdx.x] = z;
 }
 tm_status scal_init(tm_ctx* ctx, double rho2, double delta2, int max_iter, double eta2, cudaStream_t st) {
-    scal_init_kernel<<<1, 1, 0, st>>>(ctx->d_scal, rho2, delta2, max_iter, eta2);
+    scal_init_kernel<<<ctx->nb == 2 ? 2 : 1, 1, 0, st>>>(ctx->d_scal, rho2, delta2, max_iter, eta2);
     TM_LAUNCH_CHECK(ctx, "scal_init_kernel");
     return TM_OK;
 }
 tm_status scal_get(tm_ctx* ctx, CgScalars* v, cudaStream_t st) {
-    TM_CUDA(ctx, cudaMemcpyAsync(ctx->h_scal, ctx->d_scal, sizeof(CgScalars), cudaMemcpyDeviceToHost, st));
+    TM_CUDA(ctx, cudaMemcpyAsync(ctx->h_scal, ctx->d_scal, 2 * sizeof(CgScalars), cudaMemcpyDeviceToHost, st));
     TM_CUDA(ctx, cudaStreamSynchronize(st));
-    *v = *ctx->h_scal;
+    v[0] = ctx->h_scal[0]; v[1] = ctx->h_scal[1];
     return TM_OK;
 }
 
@@ -380,6 +401,7 @@ tm_status scal_get(tm_ctx* ctx, CgScalars* v, cudaStream_t st) {
 __global__ void __launch_bounds__(1024) reduce_finish_kernel(const double* __restrict__ partials, unsigned int n,
                                                              CgScalars* sc, int op, int guard) {
     __shared__ double sm[32];
+    sc += blockIdx.x; partials += blockIdx.x * TM_PSTRIDE;      // one block per source of a paired solve
     if (guard_skip(sc, guard)) return;
     double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
     unsigned int i = threadIdx.x;
@@ -392,7 +414,7 @@ __global__ void __launch_bounds__(1024) reduce_finish_kernel(const double* __res
     if (threadIdx.x == 0) apply_red_op(sc, op, s);
 }
 tm_status tm_reduce_finish(tm_ctx* ctx, unsigned int nblocks, int op, int guard, cudaStream_t st) {
-    reduce_finish_kernel<<<1, 1024, 0, st>>>(ctx->d_partials, nblocks, ctx->d_scal, op, guard);
+    reduce_finish_kernel<<<ctx->nb == 2 ? 2 : 1, 1024, 0, st>>>(ctx->d_partials, nblocks, ctx->d_scal, op, guard);
     TM_LAUNCH_CHECK(ctx, "reduce_finish_kernel");
     return TM_OK;
 }

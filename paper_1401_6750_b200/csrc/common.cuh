@@ -76,6 +76,7 @@ struct tm_ctx {
     size_t contract_tables_bytes;
     cudaEvent_t ev[TM_NEVENTS];     // 0,1: solve; 2,3: tsm; 4: solver state download; 5: lane join
     int cur_lane;
+    int nb;                         // sources per launch of the running solve (0 | 1: one; 2: a pair, see blas.cu)
     TmLane lanes[TM_NLANES];        // parked state of the inactive lanes (the active one lives in the fields above)
     cudaStream_t lane_stream;       // stream owned by the active lane (0 for lane 0)
     int no_tma;                     // TMLOOPS_NO_TMA=1: force the generic contraction kernel (testing)

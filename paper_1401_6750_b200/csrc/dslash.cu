@@ -17,8 +17,6 @@
 #include "kernels.h"
 #include "su3.cuh"
 
-#define DSLASH_PSTRIDE (1 << 17)      // doubles between the per-block partials of source 0 and source 1
-
 template <typename F> struct DslashArgs {
     const void* in;
     const void* x;
@@ -109,9 +107,16 @@ template <typename S, int R>
 __global__ void __launch_bounds__(128) dslash_kernel(DslashArgs<typename Prec<S>::F> A) {
     typedef typename Prec<S>::F F;
     __shared__ double sm[32];
+    int bx = blockIdx.x, src = 0;
+    if (A.nb == 2) { src = bx & 1; bx >>= 1; }          // paired sources: see DslashArgs::nb
+    A.in = (const char*)A.in + src * A.fstride;
+    A.out = (char*)A.out + src * A.fstride;
+    if (A.x) A.x = (const char*)A.x + src * A.fstride;
+    A.sc += src;
+    A.partials += src * TM_PSTRIDE;
     if (guard_skip(A.sc, A.guard)) return;
     const Geom& g = A.g;
-    const int h = blockIdx.x * blockDim.x + threadIdx.x;
+    const int h = bx * blockDim.x + threadIdx.x;
     double nrm = 0.0;
     if (h < g.Vh) {
         const int xh = h % g.Xh;
@@ -192,7 +197,7 @@ __global__ void __launch_bounds__(128) dslash_kernel(DslashArgs<typename Prec<S>
             for (int i = 0; i < 24; i++) nrm += (double)acc[i] * (double)acc[i];
         }
     }
-    if (A.red_op != RED_NONE) block_partial(nrm, A.partials, sm);
+    if (A.red_op != RED_NONE) block_partial_at(nrm, A.partials, bx, sm);
 }
 
 
@@ -420,7 +425,7 @@ __global__ void __launch_bounds__(128, MINB) dslash16_kernel(DslashArgs<float> A
     A.out = (char*)A.out + src * A.fstride;
     if (A.x) A.x = (const char*)A.x + src * A.fstride;
     A.sc += src;
-    A.partials += src * DSLASH_PSTRIDE;
+    A.partials += src * TM_PSTRIDE;
     if (guard_skip(A.sc, A.guard)) return;
     const Geom& g = A.g;
     const int h = bx * blockDim.x + threadIdx.x;
@@ -547,12 +552,13 @@ static tm_status launch_t(tm_ctx* ctx, const DslashCall& c, const void* gauge, c
     A.xmode = c.xmode; A.post = c.post; A.red_op = c.red_op;
     A.partials = ctx->d_partials; A.counter = ctx->d_counter; A.sc = ctx->d_scal;
     A.guard = c.guard;
-    A.nb = 1; A.fstride = 0;
+    A.nb = ctx->nb == 2 ? 2 : 1; A.fstride = ctx->Vh * 24 * sizeof(S);
     const int block = 128;
-    const int grid = (int)((ctx->Vh + block - 1) / block);
+    const int tiles = (int)((ctx->Vh + block - 1) / block);
+    const int grid = tiles * A.nb;
     dslash_kernel<S, R><<<grid, block, 0, st>>>(A);
     TM_LAUNCH_CHECK(ctx, "dslash_kernel");
-    if (c.red_op != RED_NONE) TM_TRY(tm_reduce_finish(ctx, (unsigned)grid, c.red_op, c.guard, st));
+    if (c.red_op != RED_NONE) TM_TRY(tm_reduce_finish(ctx, (unsigned)tiles, c.red_op, c.guard, st));
     return TM_OK;
 }
 
@@ -569,7 +575,7 @@ static tm_status launch16(tm_ctx* ctx, const DslashCall& c, const void* gauge, c
     A.xmode = c.xmode; A.post = c.post; A.red_op = c.red_op;
     A.partials = ctx->d_partials; A.counter = ctx->d_counter; A.sc = ctx->d_scal;
     A.guard = c.guard;
-    A.nb = c.nb == 2 ? 2 : 1; A.fstride = c.fstride;
+    A.nb = ctx->nb == 2 ? 2 : 1; A.fstride = ctx->Vh * 24 * sizeof(S);
     const int block = 128;
     const int tiles = (int)((ctx->Vh + block - 1) / block);
     const int grid = tiles * A.nb;

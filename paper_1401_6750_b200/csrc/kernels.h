@@ -12,8 +12,6 @@ struct DslashCall {
     int xmode, post;
     int red_op;        // RED_* applied to ||out||^2 (RED_NONE: no norm)
     int guard;         // GUARD_ALWAYS | GUARD_ITER | GUARD_RU (blas.cuh)
-    int nb;            // 0 | 1: one source; 2: a pair (source 1's fields fstride bytes behind source 0's)
-    size_t fstride;
 };
 tm_status tm_dslash_launch(tm_ctx* ctx, const DslashCall& c, tm_prec prec, tm_recon recon, cudaStream_t st);
 
@@ -55,12 +53,13 @@ tm_status tm_reduce_finish(tm_ctx* ctx, unsigned int nblocks, int op, int guard,
 // reset the device state for a new solve (no host synchronisation)
 // eta2 > 0: ||eta||^2 known to the caller (Z4 noise: 12 V exactly), no norm kernel needed
 tm_status scal_init(tm_ctx* ctx, double rho2, double delta2, int max_iter, double eta2, cudaStream_t st);
-tm_status scal_get(tm_ctx* ctx, CgScalars* v, cudaStream_t st);          // download + sync
+tm_status scal_get(tm_ctx* ctx, CgScalars* v /*[2]*/, cudaStream_t st);   // download + sync
 
 // ---- solver.cu ----------------------------------------------------------------------------
 // eta, s: full-lattice internal fields of precision params->outer
 struct SolveJob {                       // one solve in flight (solver.cu: tm_solve_begin / tm_solve_end)
     tm_solve_params P;
+    int nb;                             // sources solved together (1 | 2)
     tm_prec po, ps, pa; tm_recon rc;
     double kappa, mu, delta;
     cudaStream_t st;
@@ -70,9 +69,11 @@ struct SolveJob {                       // one solve in flight (solver.cu: tm_so
     CgScalars* h_scal;
     bool tail_valid; long enq;
 };
-// eta_norm2 > 0: ||eta||^2 known exactly to the caller (skips the norm kernel); 0: computed
+// eta_norm2 > 0: ||eta||^2 known exactly to the caller (skips the norm kernel); 0: computed.
+// nb = 2: two sources solved in lockstep (every kernel launch covers both; needs eta_norm2): d_eta and d_s hold
+// [even 0][even 1][odd 0][odd 1], tm_solve_end fills info[0..1]
 tm_status tm_solve_begin(tm_ctx* ctx, SolveJob* job, void* d_s, const void* d_eta, double kappa, double mu,
-                         const tm_solve_params* params, cudaStream_t st, double eta_norm2 = 0.0);
+                         const tm_solve_params* params, cudaStream_t st, double eta_norm2 = 0.0, int nb = 1);
 tm_status tm_solve_end(tm_ctx* ctx, SolveJob* job, tm_solve_info* info);
 tm_status tm_solve_internal(tm_ctx* ctx, void* d_s, const void* d_eta, double kappa, double mu,
                             const tm_solve_params* params, tm_solve_info* info, cudaStream_t st);

@@ -59,10 +59,21 @@ static tm_status job_tail(tm_ctx* ctx, const SolveJob& J) {
     return TM_OK;
 }
 
+// every launcher reads ctx->nb; it is 2 only while a paired solve enqueues
+struct NbScope {
+    tm_ctx* c;
+    NbScope(tm_ctx* ctx, int nb) : c(ctx) { c->nb = nb; }
+    ~NbScope() { c->nb = 1; }
+};
+
 tm_status tm_solve_begin(tm_ctx* ctx, SolveJob* Jp, void* d_s, const void* d_eta, double kappa, double mu,
-                         const tm_solve_params* P, cudaStream_t st, double eta_norm2) {
+                         const tm_solve_params* P, cudaStream_t st, double eta_norm2, int nb) {
     SolveJob& J = *Jp;
     if (!P) return tm_fail(ctx, TM_EARG, "solve: null params");
+    if (nb != 1 && nb != 2) return tm_fail(ctx, TM_EARG, "solve: nb must be 1 or 2");
+    if (nb == 2 && !(eta_norm2 > 0)) return tm_fail(ctx, TM_EARG, "solve: a paired solve needs the source norm");
+    J.nb = nb;
+    NbScope scope(ctx, nb);
     const tm_prec po = P->outer, ps = P->sloppy;
     if (po != TM_F64 && po != TM_F32) return tm_fail(ctx, TM_EPREC, "solve: outer precision must be f32 or f64");
     if ((int)ps < 0 || (int)ps > 3) return tm_fail(ctx, TM_EPREC, "solve: unknown sloppy precision");
@@ -75,7 +86,9 @@ tm_status tm_solve_begin(tm_ctx* ctx, SolveJob* Jp, void* d_s, const void* d_eta
     J.rc = P->recon;
     J.delta = (P->delta > 0 && P->delta < 1) ? P->delta : 0.1;
     J.kappa = kappa; J.mu = mu; J.st = st;
-    const size_t bo = tm_parity_bytes(ctx, po), bs = tm_parity_bytes(ctx, ps), ba = tm_parity_bytes(ctx, J.pa);
+    // bytes of one parity vector per precision; a pair keeps source 1's vector right behind source 0's, and its
+    // full-lattice fields as [even 0][even 1][odd 0][odd 1]
+    const size_t bo = nb * tm_parity_bytes(ctx, po), bs = nb * tm_parity_bytes(ctx, ps), ba = nb * tm_parity_bytes(ctx, J.pa);
 
     J.e0 = ctx->ev[0]; J.e1 = ctx->ev[1];
     TM_CUDA(ctx, cudaEventRecord(J.e0, st));
@@ -129,60 +142,77 @@ tm_status tm_solve_begin(tm_ctx* ctx, SolveJob* Jp, void* d_s, const void* d_eta
     }
     J.h_scal = ctx->h_scal;
     J.e_scal = ctx->ev[4];
-    TM_CUDA(ctx, cudaMemcpyAsync(ctx->h_scal, ctx->d_scal, sizeof(CgScalars), cudaMemcpyDeviceToHost, st));
+    TM_CUDA(ctx, cudaMemcpyAsync(ctx->h_scal, ctx->d_scal, 2 * sizeof(CgScalars), cudaMemcpyDeviceToHost, st));
     TM_CUDA(ctx, cudaEventRecord(J.e_scal, st));
     return TM_OK;
 }
 
+// info: array of J.nb entries (may be NULL).  TM_ENOCONV if any source of the job missed its rho.
 tm_status tm_solve_end(tm_ctx* ctx, SolveJob* Jp, tm_solve_info* info) {
     SolveJob& J = *Jp;
     const tm_solve_params* P = &J.P;
     cudaStream_t st = J.st;
-    CgScalars sc;
+    const int nb = J.nb;
+    NbScope scope(ctx, nb);
+    CgScalars sc[2];
     TM_CUDA(ctx, cudaEventSynchronize(J.e_scal));
-    sc = *J.h_scal;
-    while (sc.done < 2) {
-        // off plan (first solve with these parameters, or this source behaves differently):
+    sc[0] = J.h_scal[0]; sc[1] = J.h_scal[1];
+    auto running = [&]() { return sc[0].done < 2 || (nb == 2 && sc[1].done < 2); };
+    while (running()) {
+        // off plan (first solve with these parameters, or a source behaves differently):
         // [iteration, update] pairs, polled every few pairs
         const int burst = 4;
         for (int k = 0; k < burst; k++) { TM_TRY(job_iteration(ctx, J)); TM_TRY(job_update(ctx, J)); J.enq++; }
         J.tail_valid = false;
-        TM_TRY(scal_get(ctx, &sc, st));
-        if (J.enq > (long)P->max_iter + 8 * (long)CG_MAX_PAUSES + 64 && sc.done < 2)
+        TM_TRY(scal_get(ctx, sc, st));
+        if (J.enq > (long)P->max_iter + 8 * (long)CG_MAX_PAUSES + 64 && running())
             return tm_fail(ctx, TM_ECUDA, "solve: device state machine did not terminate");
     }
     if (!J.tail_valid) TM_TRY(job_tail(ctx, J));
     TM_CUDA(ctx, cudaEventSynchronize(J.e1));
-    // remember where this solve paused: the launch plan of the next one
+    // remember where this solve paused: the launch plan of the next one (a pair: the union of both sources' pauses)
     CgPlan& plan = ctx->plan[(int)J.ps];
-    plan.valid = sc.n_ru <= CG_MAX_PAUSES;
+    plan.valid = sc[0].n_ru <= CG_MAX_PAUSES && (nb == 1 || sc[1].n_ru <= CG_MAX_PAUSES);
     plan.sloppy = (int)J.ps; plan.outer = (int)J.po; plan.recon = (int)J.rc; plan.max_iter = P->max_iter;
     plan.rho = P->rho; plan.delta = J.delta;
-    plan.n_pause = sc.n_ru < CG_MAX_PAUSES ? sc.n_ru : CG_MAX_PAUSES;
-    for (int k = 0; k < plan.n_pause; k++) plan.pause_iter[k] = sc.pause_iter[k];
-
+    plan.n_pause = 0;
+    {
+        int i0 = 0, i1 = 0;
+        const int n0 = sc[0].n_ru < CG_MAX_PAUSES ? sc[0].n_ru : CG_MAX_PAUSES;
+        const int n1 = nb == 2 ? (sc[1].n_ru < CG_MAX_PAUSES ? sc[1].n_ru : CG_MAX_PAUSES) : 0;
+        while ((i0 < n0 || i1 < n1) && plan.n_pause < CG_MAX_PAUSES) {
+            int v;
+            if (i1 >= n1 || (i0 < n0 && sc[0].pause_iter[i0] <= sc[1].pause_iter[i1])) v = sc[0].pause_iter[i0++];
+            else v = sc[1].pause_iter[i1++];
+            if (plan.n_pause == 0 || plan.pause_iter[plan.n_pause - 1] != v) plan.pause_iter[plan.n_pause++] = v;
+        }
+        if (i0 < n0 || i1 < n1) plan.valid = 0;
+    }
     float ms = 0;
     cudaEventElapsedTime(&ms, J.e0, J.e1);
-    const double eta2 = sc.slot[0];
-    const double resid = eta2 > 0 ? sqrt(sc.rr_true / eta2) : 0.0;
-    if (info) {
-        info->iters = sc.iters;
-        info->reliable_updates = sc.n_ru;
-        info->true_resid = resid;
-        info->ms = ms;
+    tm_status ret = TM_OK;
+    for (int b = 0; b < nb; b++) {
+        const double eta2 = sc[b].slot[0];
+        const double resid = eta2 > 0 ? sqrt(sc[b].rr_true / eta2) : 0.0;
+        if (info) {
+            info[b].iters = sc[b].iters;
+            info[b].reliable_updates = sc[b].n_ru;
+            info[b].true_resid = resid;
+            info[b].ms = ms / nb;
+        }
+        if (sc[b].done != 2) {
+            snprintf(ctx->err, sizeof(ctx->err), "solve: rho = %g not reached in %d iterations (true residual %g)",
+                     P->rho, sc[b].iters, resid);
+            ret = TM_ENOCONV;
+        }
     }
-    if (sc.done != 2) {
-        snprintf(ctx->err, sizeof(ctx->err), "solve: rho = %g not reached in %d iterations (true residual %g)",
-                 P->rho, sc.iters, resid);
-        return TM_ENOCONV;
-    }
-    return TM_OK;
+    return ret;
 }
 
 tm_status tm_solve_internal(tm_ctx* ctx, void* d_s, const void* d_eta, double kappa, double mu,
                             const tm_solve_params* P, tm_solve_info* info, cudaStream_t st) {
     SolveJob J;
-    TM_TRY(tm_solve_begin(ctx, &J, d_s, d_eta, kappa, mu, P, st));
+    TM_TRY(tm_solve_begin(ctx, &J, d_s, d_eta, kappa, mu, P, st, 0.0, 1));
     return tm_solve_end(ctx, &J, info);
 }
 
