@@ -64,9 +64,9 @@ tm_status blas_copy(tm_ctx* ctx, void* dst, tm_prec pd, const void* src, tm_prec
 // ------------------------------------------------------------------ dst = A^-1 src
 template <typename S>
 __global__ void twist_inv_kernel(S* __restrict__ dst, const S* __restrict__ src, int Vh,
-                                 typename Prec<S>::F a) {
+                                 typename Prec<S>::F a, int dst_mul, int src_mul) {
     typedef typename Prec<S>::F F;
-    dst = src_vec(dst, blockIdx.y, Vh); src = src_vec(src, blockIdx.y, Vh);
+    dst = src_vec(dst, blockIdx.y * dst_mul, Vh); src = src_vec(src, blockIdx.y * src_mul, Vh);
     const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= 3L * Vh) return;
     const int g = (int)(i / Vh), h = (int)(i % Vh);
@@ -88,9 +88,10 @@ __global__ void twist_inv_kernel(S* __restrict__ dst, const S* __restrict__ src,
 // dst = A^-1 src + c * add   (odd-site reconstruction s_o = A^-1 eta_o + kappa [A^-1 D_oe y], solver.cu)
 template <typename S>
 __global__ void twist_inv_axpy_kernel(S* __restrict__ dst, const S* __restrict__ src, const S* __restrict__ add, int Vh,
-                                      typename Prec<S>::F a, typename Prec<S>::F c) {
+                                      typename Prec<S>::F a, typename Prec<S>::F c, int dst_mul, int src_mul, int add_mul) {
     typedef typename Prec<S>::F F;
-    dst = src_vec(dst, blockIdx.y, Vh); src = src_vec(src, blockIdx.y, Vh); add = src_vec(add, blockIdx.y, Vh);
+    dst = src_vec(dst, blockIdx.y * dst_mul, Vh); src = src_vec(src, blockIdx.y * src_mul, Vh);
+    add = src_vec(add, blockIdx.y * add_mul, Vh);
     const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= 3L * Vh) return;
     const int g = (int)(i / Vh), h = (int)(i % Vh);
@@ -109,24 +110,25 @@ __global__ void twist_inv_axpy_kernel(S* __restrict__ dst, const S* __restrict__
     store8<S>(dst, Vh, h, g, v);
 }
 tm_status blas_twist_inv_axpy(tm_ctx* ctx, void* dst, const void* src, const void* add, tm_prec p, double kappa,
-                              double mu, double c, cudaStream_t st) {
+                              double mu, double c, cudaStream_t st, int dst_mul, int src_mul, int add_mul) {
     const double a = 2.0 * kappa * mu;
     return dispatch_prec(ctx, p, [&](auto* t) {
         typedef TAGTYPE(t) S;
         typedef typename Prec<S>::F F;
-        twist_inv_axpy_kernel<S><<<pair_grid(ctx, items_grid(ctx, 256)), 256, 0, st>>>((S*)dst, (const S*)src, (const S*)add, (int)ctx->Vh, (F)a, (F)c);
+        twist_inv_axpy_kernel<S><<<pair_grid(ctx, items_grid(ctx, 256)), 256, 0, st>>>((S*)dst, (const S*)src, (const S*)add, (int)ctx->Vh, (F)a, (F)c,
+                                                                                             dst_mul, src_mul, add_mul);
         TM_LAUNCH_CHECK(ctx, "twist_inv_axpy_kernel");
         return TM_OK;
     });
 }
 
 tm_status blas_twist_inv(tm_ctx* ctx, void* dst, const void* src, tm_prec p, double kappa, double mu,
-                         int dagger, cudaStream_t st) {
+                         int dagger, cudaStream_t st, int dst_mul, int src_mul) {
     const double a = 2.0 * kappa * mu * (dagger ? -1.0 : 1.0);
     return dispatch_prec(ctx, p, [&](auto* t) {
         typedef TAGTYPE(t) S;
         twist_inv_kernel<S><<<pair_grid(ctx, items_grid(ctx, 256)), 256, 0, st>>>((S*)dst, (const S*)src, (int)ctx->Vh,
-                                                               (typename Prec<S>::F)a);
+                                                               (typename Prec<S>::F)a, dst_mul, src_mul);
         TM_LAUNCH_CHECK(ctx, "twist_inv_kernel");
         return TM_OK;
     });
@@ -134,8 +136,8 @@ tm_status blas_twist_inv(tm_ctx* ctx, void* dst, const void* src, tm_prec p, dou
 
 // ------------------------------------------------------------------ reliable update, part 1: y += x ; x = 0
 template <typename Sy, typename Sx>
-__global__ void ru_begin_kernel(Sy* __restrict__ y, Sx* __restrict__ x, int Vh, const CgScalars* sc) {
-    sc += blockIdx.y; y = src_vec(y, blockIdx.y, Vh); x = src_vec(x, blockIdx.y, Vh);
+__global__ void ru_begin_kernel(Sy* __restrict__ y, Sx* __restrict__ x, int Vh, const CgScalars* sc, int y_mul) {
+    sc += blockIdx.y; y = src_vec(y, blockIdx.y * y_mul, Vh); x = src_vec(x, blockIdx.y, Vh);
     if (guard_skip(sc, GUARD_RU)) return;
     const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= 3L * Vh) return;
@@ -155,12 +157,12 @@ __global__ void ru_begin_kernel(Sy* __restrict__ y, Sx* __restrict__ x, int Vh, 
     store8<Sy>(y, Vh, h, g, b);
 }
 
-tm_status blas_ru_begin(tm_ctx* ctx, void* y, tm_prec po, void* x, tm_prec pacc, cudaStream_t st) {
+tm_status blas_ru_begin(tm_ctx* ctx, void* y, tm_prec po, void* x, tm_prec pacc, cudaStream_t st, int y_mul) {
     const dim3 grid = pair_grid(ctx, items_grid(ctx, 256));
     const int Vh = (int)ctx->Vh;
-    if (po == TM_F64 && pacc == TM_F64) ru_begin_kernel<double, double><<<grid, 256, 0, st>>>((double*)y, (double*)x, Vh, ctx->d_scal);
-    else if (po == TM_F64 && pacc == TM_F32) ru_begin_kernel<double, float><<<grid, 256, 0, st>>>((double*)y, (float*)x, Vh, ctx->d_scal);
-    else if (po == TM_F32 && pacc == TM_F32) ru_begin_kernel<float, float><<<grid, 256, 0, st>>>((float*)y, (float*)x, Vh, ctx->d_scal);
+    if (po == TM_F64 && pacc == TM_F64) ru_begin_kernel<double, double><<<grid, 256, 0, st>>>((double*)y, (double*)x, Vh, ctx->d_scal, y_mul);
+    else if (po == TM_F64 && pacc == TM_F32) ru_begin_kernel<double, float><<<grid, 256, 0, st>>>((double*)y, (float*)x, Vh, ctx->d_scal, y_mul);
+    else if (po == TM_F32 && pacc == TM_F32) ru_begin_kernel<float, float><<<grid, 256, 0, st>>>((float*)y, (float*)x, Vh, ctx->d_scal, y_mul);
     else return tm_fail(ctx, TM_EPREC, "ru_begin: unsupported precision pair");
     TM_LAUNCH_CHECK(ctx, "ru_begin_kernel");
     return TM_OK;

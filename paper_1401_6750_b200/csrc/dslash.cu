@@ -35,7 +35,8 @@ template <typename F> struct DslashArgs {
     int guard;         // GUARD_* (blas.cuh): skip unless the running solve is in the matching state
     int nb;            // sources per launch (1 | 2): CTAs 2k and 2k+1 work on the same sites of source 0 and 1,
                        // so that the second reader of every link finds it in L2
-    size_t fstride;    // bytes between the fields of the two sources (in, x, out alike)
+    size_t fstride;    // bytes of one parity vector; source 1's operands sit mul_* vectors behind source 0's
+    int mul_in, mul_x, mul_out;
 };
 
 // u (2 spins x 3 colours complex = 12 reals) = psi_up + s * B_mu psi_low
@@ -109,9 +110,9 @@ __global__ void __launch_bounds__(128) dslash_kernel(DslashArgs<typename Prec<S>
     __shared__ double sm[32];
     int bx = blockIdx.x, src = 0;
     if (A.nb == 2) { src = bx & 1; bx >>= 1; }          // paired sources: see DslashArgs::nb
-    A.in = (const char*)A.in + src * A.fstride;
-    A.out = (char*)A.out + src * A.fstride;
-    if (A.x) A.x = (const char*)A.x + src * A.fstride;
+    A.in = (const char*)A.in + src * A.mul_in * A.fstride;
+    A.out = (char*)A.out + src * A.mul_out * A.fstride;
+    if (A.x) A.x = (const char*)A.x + src * A.mul_x * A.fstride;
     A.sc += src;
     A.partials += src * TM_PSTRIDE;
     if (guard_skip(A.sc, A.guard)) return;
@@ -421,9 +422,9 @@ __global__ void __launch_bounds__(128, MINB) dslash16_kernel(DslashArgs<float> A
     __shared__ double sm[32];
     int bx = blockIdx.x, src = 0;
     if (A.nb == 2) { src = bx & 1; bx >>= 1; }
-    A.in = (const char*)A.in + src * A.fstride;
-    A.out = (char*)A.out + src * A.fstride;
-    if (A.x) A.x = (const char*)A.x + src * A.fstride;
+    A.in = (const char*)A.in + src * A.mul_in * A.fstride;
+    A.out = (char*)A.out + src * A.mul_out * A.fstride;
+    if (A.x) A.x = (const char*)A.x + src * A.mul_x * A.fstride;
     A.sc += src;
     A.partials += src * TM_PSTRIDE;
     if (guard_skip(A.sc, A.guard)) return;
@@ -553,6 +554,7 @@ static tm_status launch_t(tm_ctx* ctx, const DslashCall& c, const void* gauge, c
     A.partials = ctx->d_partials; A.counter = ctx->d_counter; A.sc = ctx->d_scal;
     A.guard = c.guard;
     A.nb = ctx->nb == 2 ? 2 : 1; A.fstride = ctx->Vh * 24 * sizeof(S);
+    A.mul_in = c.mul_in ? c.mul_in : 1; A.mul_x = c.mul_x ? c.mul_x : 1; A.mul_out = c.mul_out ? c.mul_out : 1;
     const int block = 128;
     const int tiles = (int)((ctx->Vh + block - 1) / block);
     const int grid = tiles * A.nb;
@@ -576,6 +578,7 @@ static tm_status launch16(tm_ctx* ctx, const DslashCall& c, const void* gauge, c
     A.partials = ctx->d_partials; A.counter = ctx->d_counter; A.sc = ctx->d_scal;
     A.guard = c.guard;
     A.nb = ctx->nb == 2 ? 2 : 1; A.fstride = ctx->Vh * 24 * sizeof(S);
+    A.mul_in = c.mul_in ? c.mul_in : 1; A.mul_x = c.mul_x ? c.mul_x : 1; A.mul_out = c.mul_out ? c.mul_out : 1;
     const int block = 128;
     const int tiles = (int)((ctx->Vh + block - 1) / block);
     const int grid = tiles * A.nb;

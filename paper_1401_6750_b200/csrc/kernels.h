@@ -12,6 +12,7 @@ struct DslashCall {
     int xmode, post;
     int red_op;        // RED_* applied to ||out||^2 (RED_NONE: no norm)
     int guard;         // GUARD_ALWAYS | GUARD_ITER | GUARD_RU (blas.cuh)
+    int mul_in, mul_x, mul_out;   // paired solves: source stride of each operand in parity vectors (0 = 1)
 };
 tm_status tm_dslash_launch(tm_ctx* ctx, const DslashCall& c, tm_prec prec, tm_recon recon, cudaStream_t st);
 
@@ -27,11 +28,13 @@ tm_status tm_z4_expand(tm_ctx* ctx, void* d_internal, tm_prec prec, const unsign
 tm_status blas_zero(tm_ctx* ctx, void* v, tm_prec p, cudaStream_t st);
 tm_status blas_copy(tm_ctx* ctx, void* dst, tm_prec pd, const void* src, tm_prec ps, cudaStream_t st);
 // dst = A^-1 src  (site-local twist inverse)
+// (paired solves: *_mul = distance of source 1's vector behind source 0's, in parity vectors: 1 for solver
+//  workspaces, 2 for the halves of full-lattice fields, which keep each source's [even][odd] contiguous)
 tm_status blas_twist_inv(tm_ctx* ctx, void* dst, const void* src, tm_prec p, double kappa, double mu,
-                         int dagger, cudaStream_t st);
+                         int dagger, cudaStream_t st, int dst_mul = 1, int src_mul = 1);
 // dst = A^-1 src + c * add
 tm_status blas_twist_inv_axpy(tm_ctx* ctx, void* dst, const void* src, const void* add, tm_prec p, double kappa,
-                              double mu, double c, cudaStream_t st);
+                              double mu, double c, cudaStream_t st, int dst_mul = 1, int src_mul = 1, int add_mul = 1);
 // ||v||^2 -> red_op
 tm_status blas_norm(tm_ctx* ctx, const void* v, tm_prec p, int red_op, cudaStream_t st);
 // full-lattice norm (2 parities)
@@ -43,7 +46,7 @@ tm_status blas_update_xr(tm_ctx* ctx, void* x, void* r, tm_prec pacc, const void
 //   p = z + beta p  (p = z when beta == 0: first iteration)                                  (GUARD_ITER)
 tm_status blas_update_p(tm_ctx* ctx, void* p, const void* z, tm_prec psl, cudaStream_t st);
 //   y += x ; x = 0                                                                           (GUARD_RU)
-tm_status blas_ru_begin(tm_ctx* ctx, void* y, tm_prec po, void* x, tm_prec pacc, cudaStream_t st);
+tm_status blas_ru_begin(tm_ctx* ctx, void* y, tm_prec po, void* x, tm_prec pacc, cudaStream_t st, int y_mul = 1);
 //   r = b - m (acc precision) ; rs = b - m (sloppy) ; ||b - m||^2 -> red_op (RED_START: m == NULL,
 //   GUARD_ALWAYS; RED_RU: GUARD_RU)
 tm_status blas_residual(tm_ctx* ctx, void* r, tm_prec pacc, void* rs, tm_prec psl, const void* b, const void* m,
@@ -71,7 +74,7 @@ struct SolveJob {                       // one solve in flight (solver.cu: tm_so
 };
 // eta_norm2 > 0: ||eta||^2 known exactly to the caller (skips the norm kernel); 0: computed.
 // nb = 2: two sources solved in lockstep (every kernel launch covers both; needs eta_norm2): d_eta and d_s hold
-// [even 0][even 1][odd 0][odd 1], tm_solve_end fills info[0..1]
+// [even 0][odd 0][even 1][odd 1] (two full-lattice fields back to back), tm_solve_end fills info[0..1]
 tm_status tm_solve_begin(tm_ctx* ctx, SolveJob* job, void* d_s, const void* d_eta, double kappa, double mu,
                          const tm_solve_params* params, cudaStream_t st, double eta_norm2 = 0.0, int nb = 1);
 tm_status tm_solve_end(tm_ctx* ctx, SolveJob* job, tm_solve_info* info);

@@ -21,14 +21,18 @@
 #include "kernels.h"
 
 // out = Mhat in (dagger: Mhat^dag in) on even sites; tmp: odd-parity scratch of the same precision
+// in_mul: source stride of `in` in parity vectors (2 when `in` is the even half of a full-lattice field)
 static tm_status apply_mhat(tm_ctx* ctx, void* out, const void* in, void* tmp, int dagger, double kappa,
-                            double mu, tm_prec prec, tm_recon recon, int red_op, int guard, cudaStream_t st) {
+                            double mu, tm_prec prec, tm_recon recon, int red_op, int guard, cudaStream_t st,
+                            int in_mul = 1) {
     DslashCall k;
     memset(&k, 0, sizeof(k));
     k.kappa = kappa; k.mu = mu; k.dagger = dagger; k.guard = guard;
     k.out = tmp; k.in = in; k.out_parity = 1; k.post = 1; k.coef = 1.0; k.red_op = RED_NONE;
+    k.mul_in = in_mul;
     TM_TRY(tm_dslash_launch(ctx, k, prec, recon, st));
     k.out = out; k.in = tmp; k.x = in; k.out_parity = 0; k.post = 0; k.xmode = 2; k.coef = -kappa * kappa;
+    k.mul_in = 1; k.mul_x = in_mul;
     k.red_op = red_op;
     return tm_dslash_launch(ctx, k, prec, recon, st);
 }
@@ -46,15 +50,15 @@ static tm_status job_iteration(tm_ctx* ctx, const SolveJob& J) {
     return blas_update_xr(ctx, J.x, J.r, J.pa, J.p, J.w, J.rs, J.ps, J.st);
 }
 static tm_status job_update(tm_ctx* ctx, const SolveJob& J) {
-    TM_TRY(blas_ru_begin(ctx, J.y, J.po, J.x, J.pa, J.st));
-    TM_TRY(apply_mhat(ctx, J.mo, J.y, J.tmpo, 0, J.kappa, J.mu, J.po, J.rc, RED_NONE, GUARD_RU, J.st));
+    TM_TRY(blas_ru_begin(ctx, J.y, J.po, J.x, J.pa, J.st, 2));
+    TM_TRY(apply_mhat(ctx, J.mo, J.y, J.tmpo, 0, J.kappa, J.mu, J.po, J.rc, RED_NONE, GUARD_RU, J.st, 2));
     return blas_residual(ctx, J.r, J.pa, J.rs, J.ps, J.b, J.mo, J.po, RED_RU, GUARD_RU, J.st);
 }
 // s_o = A^-1 (eta_o + kappa D_oe y) = A^-1 eta_o + kappa [A^-1 D_oe y]: the bracket is the first half of Mhat y,
 // left in tmpo by the LAST reliable update that ran -- and the solve always ends on one (it is the update that
 // declares convergence or failure; y does not change after it), so the tail needs no Dslash of its own.
 static tm_status job_tail(tm_ctx* ctx, const SolveJob& J) {
-    TM_TRY(blas_twist_inv_axpy(ctx, J.s_o, J.eta_o, J.tmpo, J.po, J.kappa, J.mu, J.kappa, J.st));
+    TM_TRY(blas_twist_inv_axpy(ctx, J.s_o, J.eta_o, J.tmpo, J.po, J.kappa, J.mu, J.kappa, J.st, 2, 2, 1));
     TM_CUDA(ctx, cudaEventRecord(J.e1, J.st));
     return TM_OK;
 }
@@ -86,9 +90,10 @@ tm_status tm_solve_begin(tm_ctx* ctx, SolveJob* Jp, void* d_s, const void* d_eta
     J.rc = P->recon;
     J.delta = (P->delta > 0 && P->delta < 1) ? P->delta : 0.1;
     J.kappa = kappa; J.mu = mu; J.st = st;
-    // bytes of one parity vector per precision; a pair keeps source 1's vector right behind source 0's, and its
-    // full-lattice fields as [even 0][even 1][odd 0][odd 1]
-    const size_t bo = nb * tm_parity_bytes(ctx, po), bs = nb * tm_parity_bytes(ctx, ps), ba = nb * tm_parity_bytes(ctx, J.pa);
+    // workspaces of a pair keep source 1's vector right behind source 0's (stride 1 parity vector); the full-lattice
+    // fields d_eta / d_s keep each source's [even][odd] contiguous (stride 2 parity vectors: the *_mul = 2 operands)
+    const size_t bo1 = tm_parity_bytes(ctx, po);
+    const size_t bo = nb * bo1, bs = nb * tm_parity_bytes(ctx, ps), ba = nb * tm_parity_bytes(ctx, J.pa);
 
     J.e0 = ctx->ev[0]; J.e1 = ctx->ev[1];
     TM_CUDA(ctx, cudaEventRecord(J.e0, st));
@@ -107,20 +112,20 @@ tm_status tm_solve_begin(tm_ctx* ctx, SolveJob* Jp, void* d_s, const void* d_eta
     TM_TRY(tm_ws(ctx, WS_OU_TMP2, bo, &J.mo));
 
     const char* eta_e = (const char*)d_eta;
-    J.eta_o = eta_e + bo;
+    J.eta_o = eta_e + bo1;
     J.y = (char*)d_s;                      // the even half of the solution is accumulated in place
-    J.s_o = J.y + bo;
+    J.s_o = J.y + bo1;
 
     // ---- setup (no host synchronisation): state (x and y zero by construction: CgScalars::x_zero / y_zero), ||eta||^2,
     //      bhat, r = rs = bhat
     TM_TRY(scal_init(ctx, P->rho * P->rho, J.delta * J.delta, P->max_iter, eta_norm2 > 0 ? eta_norm2 : 0.0, st));
     if (!(eta_norm2 > 0)) TM_TRY(blas_norm_full(ctx, d_eta, po, RED_SLOT0 + 0, st));
-    TM_TRY(blas_twist_inv(ctx, J.tmpo, J.eta_o, po, kappa, mu, 0, st));
+    TM_TRY(blas_twist_inv(ctx, J.tmpo, J.eta_o, po, kappa, mu, 0, st, 1, 2));
     {
         DslashCall k;
         memset(&k, 0, sizeof(k));
         k.out = J.b; k.in = J.tmpo; k.x = eta_e; k.out_parity = 0; k.kappa = kappa; k.mu = mu;
-        k.xmode = 1; k.coef = kappa; k.red_op = RED_NONE;
+        k.xmode = 1; k.coef = kappa; k.red_op = RED_NONE; k.mul_x = 2;
         TM_TRY(tm_dslash_launch(ctx, k, po, J.rc, st));
     }
     TM_TRY(blas_residual(ctx, J.r, J.pa, J.rs, ps, J.b, nullptr, po, RED_START, GUARD_ALWAYS, st));

@@ -9,6 +9,7 @@
 // tail and the launch gap of every kernel are covered by another source's kernels.  Nothing crosses to the
 // host per source except the solver's convergence scalars (and, in tsm_estimate_host, the packed noise).
 #include <math.h>
+#include <stdlib.h>
 #include "kernels.h"
 
 // acc0 += x ; acc1 += x (optional) ; copy = x (optional)
@@ -99,11 +100,11 @@ static tm_status convert_full(tm_ctx* ctx, void* dst, tm_prec pd, const void* sr
     return TM_OK;
 }
 
-// one (source, pass) unit of work in flight on a lane
+// one unit of work in flight on a lane: the same pass (LP | HP) of nb = 1 or 2 consecutive sources, solved together
 struct TsmJob {
-    int r, pass;
+    int r, nb, pass;
     SolveJob sj;
-    void *eta_o, *s_o;
+    void *eta_o, *s_o;          // nb full-lattice fields back to back, outer precision of the pass
     tm_prec po, ac;
     cudaStream_t st;
 };
@@ -114,7 +115,8 @@ struct TsmRun {
     size_t nr, z4_bytes; unsigned agrid;
     double ms_lp, ms_hp, worst_lp, worst_hp; long it_lp, it_hp; int noconv;
     double* acc[TM_NLANES];         // per lane: S_lp, S_lpc, S_hp, tmp (nr doubles each)
-    double* lp_keep;
+    int pair;                       // solve sources two at a time
+    double* lp_keep;                // [2][nr]: l^LP of the pair whose HP pass comes next (binary files of the correction)
 };
 
 // lane-private buffers of the active lane
@@ -126,70 +128,83 @@ static tm_status lane_buffers(TsmRun& R, int lane, cudaStream_t st) {
     return TM_OK;
 }
 
-// noise of source r in precision p into the active lane's buffer
-static tm_status job_noise(TsmRun& R, int r, tm_prec p, cudaStream_t st, void** out) {
+// noise of source r in precision p into slot b of the active lane's (two-field) buffer
+static tm_status job_noise(TsmRun& R, int r, int b, tm_prec p, cudaStream_t st, void** base) {
     tm_ctx* ctx = R.ctx;
     const unsigned char* zsrc = nullptr;
     if (R.z4) {
         if (R.z4_on_host) {
-            // staged per lane: the previous user of this lane's slot (its z4_expand) finished before that
-            // lane's solve was waited for
+            // staged per lane and slot: the previous user of the slot (a z4_expand of this lane) finished before
+            // that lane's solve was waited for
             void* slot;
-            TM_TRY(tm_ws(ctx, WS_TSM_Z4, R.z4_bytes, &slot));
+            TM_TRY(tm_ws(ctx, WS_TSM_Z4, 2 * R.z4_bytes, &slot));
+            slot = (char*)slot + (size_t)b * R.z4_bytes;
             TM_CUDA(ctx, cudaMemcpyAsync(slot, R.z4 + (size_t)r * R.z4_bytes, R.z4_bytes, cudaMemcpyHostToDevice, st));
             zsrc = (const unsigned char*)slot;
         } else zsrc = R.z4 + (size_t)r * R.z4_bytes;
     }
-    TM_TRY(tm_ws(ctx, p == TM_F32 ? WS_TSM_ETA32 : WS_TSM_ETA64, 2 * tm_parity_bytes(ctx, p), out));
-    return tm_z4_expand(ctx, *out, p, zsrc, R.P->seed, (unsigned long long)r, st);
+    const size_t fb = 2 * tm_parity_bytes(ctx, p);
+    TM_TRY(tm_ws(ctx, p == TM_F32 ? WS_TSM_ETA32 : WS_TSM_ETA64, 2 * fb, base));
+    return tm_z4_expand(ctx, (char*)*base + (size_t)b * fb, p, zsrc, R.P->seed, (unsigned long long)r, st);
 }
 
-static tm_status job_start(TsmRun& R, TsmJob& J, int r, int pass, cudaStream_t st) {
+static tm_status job_start(TsmRun& R, TsmJob& J, int r, int nb, int pass, cudaStream_t st) {
     tm_ctx* ctx = R.ctx;
     const tsm_params* P = R.P;
-    J.r = r; J.pass = pass; J.st = st;
+    J.r = r; J.nb = nb; J.pass = pass; J.st = st;
     J.po = pass ? P->hp.outer : P->lp.outer;
     J.ac = pass ? P->contract_acc_hp : P->contract_acc_lp;
-    TM_TRY(job_noise(R, r, J.po, st, &J.eta_o));
-    TM_TRY(tm_ws(ctx, J.po == TM_F32 ? WS_TSM_S32 : WS_TSM_S64, 2 * tm_parity_bytes(ctx, J.po), &J.s_o));
+    for (int b = 0; b < nb; b++) TM_TRY(job_noise(R, r + b, b, J.po, st, &J.eta_o));
+    TM_TRY(tm_ws(ctx, J.po == TM_F32 ? WS_TSM_S32 : WS_TSM_S64, 4 * tm_parity_bytes(ctx, J.po), &J.s_o));
     // Z4 noise: |eta_c| = 1 for each of the 12 V components, so ||eta||^2 = 12 V exactly (no norm kernel)
-    return tm_solve_begin(ctx, &J.sj, J.s_o, J.eta_o, P->kappa, P->mu, pass ? &P->hp : &P->lp, st, 12.0 * (double)ctx->V);
+    return tm_solve_begin(ctx, &J.sj, J.s_o, J.eta_o, P->kappa, P->mu, pass ? &P->hp : &P->lp, st, 12.0 * (double)ctx->V, nb);
 }
 
 static tm_status job_finish(TsmRun& R, TsmJob& J, int lane) {
     tm_ctx* ctx = R.ctx;
     const tsm_params* P = R.P;
     cudaStream_t st = J.st;
-    tm_solve_info si;
-    tm_status s = tm_solve_end(ctx, &J.sj, &si);
-    if (s == TM_ENOCONV) R.noconv++;
-    else if (s != TM_OK) return s;
-    if (J.pass) { R.ms_hp += si.ms; R.it_hp += si.iters; R.worst_hp = fmax(R.worst_hp, si.true_resid); }
-    else        { R.ms_lp += si.ms; R.it_lp += si.iters; R.worst_lp = fmax(R.worst_lp, si.true_resid); }
-    void *s_c = J.s_o, *eta_c = J.eta_o;
-    if (J.ac != J.po) {
-        TM_TRY(tm_ws(ctx, J.ac == TM_F32 ? WS_TSM_S32 : WS_TSM_S64, 2 * tm_parity_bytes(ctx, J.ac), &s_c));
-        TM_TRY(convert_full(ctx, s_c, J.ac, J.s_o, J.po, st));
-        TM_TRY(job_noise(R, J.r, J.ac, st, &eta_c));
-    }
+    tm_solve_info si[2];
+    tm_status s = tm_solve_end(ctx, &J.sj, si);
+    if (s != TM_OK && s != TM_ENOCONV) return s;
     double* A = R.acc[lane];
     const size_t nr = R.nr;
     double *S_lp = A, *S_lpc = A + nr, *S_hp = A + 2 * nr, *tmp = A + 3 * nr;
-    TM_TRY(tm_contract_internal(ctx, tmp, s_c, eta_c, P->kappa, P->mu, P->h_momenta, P->nmom, J.ac, st));
-    const int do_hp = J.r < P->n_hp;
-    double* copy = R.d_per_source ? (double*)R.d_per_source + (size_t)(J.pass ? P->n_lp + J.r : J.r) * nr : nullptr;
-    if (J.pass) tsm_accumulate_kernel<<<R.agrid, 256, 0, st>>>(S_hp, nullptr, copy, tmp, nr);
-    else        tsm_accumulate_kernel<<<R.agrid, 256, 0, st>>>(S_lp, do_hp ? S_lpc : nullptr, copy, tmp, nr);
-    TM_LAUNCH_CHECK(ctx, "tsm_accumulate_kernel");
-    if (!J.pass && R.d_files_lp) {
-        binary_add_kernel<<<R.agrid, 256, 0, st>>>((double*)R.d_files_lp + (size_t)binary_file_of(J.r) * nr, tmp, nullptr, nr);
-        TM_LAUNCH_CHECK(ctx, "binary_add_kernel");
-    }
-    if (R.lp_keep && do_hp) {
-        if (!J.pass) TM_CUDA(ctx, cudaMemcpyAsync(R.lp_keep, tmp, nr * sizeof(double), cudaMemcpyDeviceToDevice, st));
-        else {
-            binary_add_kernel<<<R.agrid, 256, 0, st>>>((double*)R.d_files_corr + (size_t)binary_file_of(J.r) * nr, tmp, R.lp_keep, nr);
+    for (int b = 0; b < J.nb; b++) {
+        const int r = J.r + b;
+        if (J.pass) { R.ms_hp += si[b].ms; R.it_hp += si[b].iters; R.worst_hp = fmax(R.worst_hp, si[b].true_resid); }
+        else        { R.ms_lp += si[b].ms; R.it_lp += si[b].iters; R.worst_lp = fmax(R.worst_lp, si[b].true_resid); }
+        const tm_solve_params* sp = J.pass ? &P->hp : &P->lp;
+        if (!(si[b].true_resid <= sp->rho * (1.0 + 1e-12))) R.noconv++;
+        const size_t fbo = 2 * tm_parity_bytes(ctx, J.po);
+        void *s_c = (char*)J.s_o + b * fbo, *eta_c = (char*)J.eta_o + b * fbo;
+        if (J.ac != J.po) {
+            const size_t fba = 2 * tm_parity_bytes(ctx, J.ac);
+            void* sbuf;
+            TM_TRY(tm_ws(ctx, J.ac == TM_F32 ? WS_TSM_S32 : WS_TSM_S64, 2 * fba, &sbuf));
+            TM_TRY(convert_full(ctx, sbuf, J.ac, s_c, J.po, st));
+            s_c = sbuf;
+            void* ebase;
+            TM_TRY(job_noise(R, r, 0, J.ac, st, &ebase));
+            eta_c = ebase;
+        }
+        TM_TRY(tm_contract_internal(ctx, tmp, s_c, eta_c, P->kappa, P->mu, P->h_momenta, P->nmom, J.ac, st));
+        const int do_hp = r < P->n_hp;
+        double* copy = R.d_per_source ? (double*)R.d_per_source + (size_t)(J.pass ? P->n_lp + r : r) * nr : nullptr;
+        if (J.pass) tsm_accumulate_kernel<<<R.agrid, 256, 0, st>>>(S_hp, nullptr, copy, tmp, nr);
+        else        tsm_accumulate_kernel<<<R.agrid, 256, 0, st>>>(S_lp, do_hp ? S_lpc : nullptr, copy, tmp, nr);
+        TM_LAUNCH_CHECK(ctx, "tsm_accumulate_kernel");
+        if (!J.pass && R.d_files_lp) {
+            binary_add_kernel<<<R.agrid, 256, 0, st>>>((double*)R.d_files_lp + (size_t)binary_file_of(r) * nr, tmp, nullptr, nr);
             TM_LAUNCH_CHECK(ctx, "binary_add_kernel");
+        }
+        if (R.lp_keep && do_hp) {
+            double* keep = R.lp_keep + (size_t)b * nr;
+            if (!J.pass) TM_CUDA(ctx, cudaMemcpyAsync(keep, tmp, nr * sizeof(double), cudaMemcpyDeviceToDevice, st));
+            else {
+                binary_add_kernel<<<R.agrid, 256, 0, st>>>((double*)R.d_files_corr + (size_t)binary_file_of(r) * nr, tmp, keep, nr);
+                TM_LAUNCH_CHECK(ctx, "binary_add_kernel");
+            }
         }
     }
     return TM_OK;
@@ -221,17 +236,28 @@ static tm_status tsm_pipeline(TsmRun& R, int NL, cudaStream_t st, void* d_out) {
         if (l) TM_CUDA(ctx, cudaStreamWaitEvent(lst[l], fork, 0));
         TM_TRY(lane_buffers(R, l, lst[l]));
     }
-    const int njobs = P->n_lp + P->n_hp;
+    // job list: sources in pairs (r, r+1); each pair's LP pass is followed by its HP pass when r < n_hp
+    // (an odd source at the end of either range is solved alone)
     TsmJob jobs[TM_NLANES];
-    int jr = 0, jpass = 0;                          // next job to start: r = 0: LP, HP; r = 1: LP, HP; ...
-    for (int j = 0; j < njobs + NL; j++) {
+    bool busy[TM_NLANES] = {false};
+    int jr = 0, jpass = 0;
+    bool more = true;
+    for (int j = 0;; j++) {
         const int l = j % NL;
         TM_TRY(tm_lane_use(ctx, l));
-        if (j >= NL) TM_TRY(job_finish(R, jobs[l], l));
-        if (j < njobs) {
-            TM_TRY(job_start(R, jobs[l], jr, jpass, lst[l]));
-            if (!jpass && jr < P->n_hp) jpass = 1; else { jpass = 0; jr++; }
+        if (busy[l]) { TM_TRY(job_finish(R, jobs[l], l)); busy[l] = false; }
+        if (more) {
+            const int lim = jpass ? P->n_hp : P->n_lp;
+            const int nb = (R.pair && jr + 1 < lim) ? 2 : 1;
+            TM_TRY(job_start(R, jobs[l], jr, nb, jpass, lst[l]));
+            busy[l] = true;
+            if (!jpass && jr < P->n_hp) jpass = 1;
+            else { jpass = 0; jr += 2 - (R.pair ? 0 : 1); }
+            more = jr < P->n_lp;
         }
+        bool any = more;
+        for (int k = 0; k < NL; k++) any = any || busy[k];
+        if (!any) break;
     }
     // join
     cudaEvent_t joined[TM_NLANES];
@@ -277,12 +303,13 @@ static tm_status tsm_core(tm_ctx* ctx, void* d_out, void* d_per_source, const ts
     R.nr = 2 * (size_t)160 * P->nmom * ctx->X[3];                // doubles per per-source array
     R.z4_bytes = 3 * ctx->V;
     R.agrid = (unsigned)((R.nr + 255) / 256);
+    { const char* e = getenv("TMLOOPS_NO_PAIRS"); R.pair = !(e && e[0] == '1'); }
     // the binary-storage files are shared accumulators: one lane keeps their additions ordered
     const int NL = (d_files_lp || d_files_corr || P->n_lp + P->n_hp < 2) ? 1 : TM_NLANES;
     if (d_files_lp) TM_CUDA(ctx, cudaMemsetAsync(d_files_lp, 0, (size_t)loop_binary_nfiles(P->n_lp) * R.nr * sizeof(double), st));
     if (d_files_corr && P->n_hp) {
         TM_CUDA(ctx, cudaMemsetAsync(d_files_corr, 0, (size_t)loop_binary_nfiles(P->n_hp) * R.nr * sizeof(double), st));
-        TM_TRY(tm_ws(ctx, WS_TSM_KEEP, R.nr * sizeof(double), (void**)&R.lp_keep));
+        TM_TRY(tm_ws(ctx, WS_TSM_KEEP, 2 * R.nr * sizeof(double), (void**)&R.lp_keep));
     }
     cudaEvent_t e0 = ctx->ev[2], e1 = ctx->ev[3];
     TM_CUDA(ctx, cudaEventRecord(e0, st));
