@@ -93,3 +93,23 @@ def test_tsm_edge_cases(setup):
         with pytest.raises(t.TmError) as e:
             ctx.tsm_estimate(1, 0, k, mu, mom, bad, HP, seed=1)
         assert e.value.status == t.TM_ENOCONV
+
+
+def test_tsm_pairs_equal_single_source_solves(setup, monkeypatch):
+    """Sources are solved two per launch by default; every per-source array must be bit-identical to the
+    one-source-per-launch path (TMLOOPS_NO_PAIRS=1), for even and odd N_LP / N_HP."""
+    t = tm()
+    dims, U, mom = setup
+    k, mu = C1["kappa"], C1["mu"]
+    with t.TmContext(dims, -1) as ctx:
+        ctx.tm_load_gauge(U)
+        for n_lp, n_hp in ((5, 3), (4, 2), (2, 1)):
+            monkeypatch.delenv("TMLOOPS_NO_PAIRS", raising=False)
+            out_p, ps_p, info_p = ctx.tsm_estimate(n_lp, n_hp, k, mu, mom, LP, HP, t.TM_F32, t.TM_F64, seed=3, per_source=True)
+            monkeypatch.setenv("TMLOOPS_NO_PAIRS", "1")
+            out_s, ps_s, info_s = ctx.tsm_estimate(n_lp, n_hp, k, mu, mom, LP, HP, t.TM_F32, t.TM_F64, seed=3, per_source=True)
+            monkeypatch.delenv("TMLOOPS_NO_PAIRS", raising=False)
+            assert np.array_equal(to_np(ps_p), to_np(ps_s)), (n_lp, n_hp)
+            assert info_p["iters_lp"] == info_s["iters_lp"] and info_p["iters_hp"] == info_s["iters_hp"]
+            assert info_p["launches"] < info_s["launches"]
+            assert rel_l2(to_np(out_p), to_np(out_s)) <= 1e-13        # lanes sum the sources in another order
