@@ -9,12 +9,12 @@ extern "C" long tm_launch_count(const tm_ctx* ctx) { return ctx ? ctx->launches 
 
 // allocate the private resources of a lane into the context's active fields
 static bool lane_alloc(tm_ctx* c, int lane) {
-    bool ok = cudaMalloc((void**)&c->d_partials, sizeof(double) * (1 << 18)) == cudaSuccess
+    bool ok = cudaMalloc((void**)&c->d_partials, sizeof(double) * TM_MAXNB * TM_PSTRIDE) == cudaSuccess
            && cudaMalloc((void**)&c->d_counter, sizeof(unsigned int) * 4) == cudaSuccess
-           && cudaMalloc((void**)&c->d_scal, 2 * sizeof(CgScalars)) == cudaSuccess
-           && cudaMallocHost((void**)&c->h_scal, 2 * sizeof(CgScalars)) == cudaSuccess
+           && cudaMalloc((void**)&c->d_scal, TM_MAXNB * sizeof(CgScalars)) == cudaSuccess
+           && cudaMallocHost((void**)&c->h_scal, TM_MAXNB * sizeof(CgScalars)) == cudaSuccess
            && cudaMemset(c->d_counter, 0, sizeof(unsigned int) * 4) == cudaSuccess
-           && cudaMemset(c->d_scal, 0, 2 * sizeof(CgScalars)) == cudaSuccess;
+           && cudaMemset(c->d_scal, 0, TM_MAXNB * sizeof(CgScalars)) == cudaSuccess;
     for (int i = 0; ok && i < TM_NEVENTS; i++) ok = cudaEventCreate(&c->ev[i]) == cudaSuccess;
     if (ok && lane > 0) ok = cudaStreamCreateWithFlags(&c->lane_stream, cudaStreamNonBlocking) == cudaSuccess;
     return ok;

@@ -15,12 +15,12 @@ template <typename Fn> static tm_status dispatch_prec(tm_ctx* ctx, tm_prec p, Fn
 }
 #define TAGTYPE(tag) typename std::remove_pointer<decltype(tag)>::type
 
-// Paired solves (ctx->nb == 2): blockIdx.y selects the source; its vectors sit one parity vector (24 Vh elements
-// of their own type) behind source 0's, its CG state, reduction partials and counter one slot behind.
+// Grouped solves (ctx->nb = 2 | 4): blockIdx.y selects the source; consecutive sources' vectors sit one parity vector
+// (24 Vh elements of their own type) apart, their CG states, reduction partials and counters one slot apart.
 template <typename S> __device__ __forceinline__ S* src_vec(S* p, int src, int Vh) {
     return p ? p + (size_t)src * 24 * (size_t)Vh : p;
 }
-static inline dim3 pair_grid(const tm_ctx* ctx, unsigned gx) { return dim3(gx, (unsigned)(ctx->nb == 2 ? 2 : 1)); }
+static inline dim3 pair_grid(const tm_ctx* ctx, unsigned gx) { return dim3(gx, (unsigned)(ctx->nb > 1 ? ctx->nb : 1)); }
 
 static inline unsigned items_grid(const tm_ctx* ctx, int block, int nparity = 1) {
     return (unsigned)((3 * ctx->Vh * nparity + block - 1) / block);
@@ -387,14 +387,14 @@ __global__ void scal_init_kernel(CgScalars* sc, double rho2, double delta2, int 
     sc[blockIdx.x] = z;
 }
 tm_status scal_init(tm_ctx* ctx, double rho2, double delta2, int max_iter, double eta2, cudaStream_t st) {
-    scal_init_kernel<<<ctx->nb == 2 ? 2 : 1, 1, 0, st>>>(ctx->d_scal, rho2, delta2, max_iter, eta2);
+    scal_init_kernel<<<ctx->nb > 1 ? ctx->nb : 1, 1, 0, st>>>(ctx->d_scal, rho2, delta2, max_iter, eta2);
     TM_LAUNCH_CHECK(ctx, "scal_init_kernel");
     return TM_OK;
 }
 tm_status scal_get(tm_ctx* ctx, CgScalars* v, cudaStream_t st) {
-    TM_CUDA(ctx, cudaMemcpyAsync(ctx->h_scal, ctx->d_scal, 2 * sizeof(CgScalars), cudaMemcpyDeviceToHost, st));
+    TM_CUDA(ctx, cudaMemcpyAsync(ctx->h_scal, ctx->d_scal, TM_MAXNB * sizeof(CgScalars), cudaMemcpyDeviceToHost, st));
     TM_CUDA(ctx, cudaStreamSynchronize(st));
-    v[0] = ctx->h_scal[0]; v[1] = ctx->h_scal[1];
+    for (int b = 0; b < TM_MAXNB; b++) v[b] = ctx->h_scal[b];
     return TM_OK;
 }
 
@@ -416,7 +416,7 @@ __global__ void __launch_bounds__(1024) reduce_finish_kernel(const double* __res
     if (threadIdx.x == 0) apply_red_op(sc, op, s);
 }
 tm_status tm_reduce_finish(tm_ctx* ctx, unsigned int nblocks, int op, int guard, cudaStream_t st) {
-    reduce_finish_kernel<<<ctx->nb == 2 ? 2 : 1, 1024, 0, st>>>(ctx->d_partials, nblocks, ctx->d_scal, op, guard);
+    reduce_finish_kernel<<<ctx->nb > 1 ? ctx->nb : 1, 1024, 0, st>>>(ctx->d_partials, nblocks, ctx->d_scal, op, guard);
     TM_LAUNCH_CHECK(ctx, "reduce_finish_kernel");
     return TM_OK;
 }

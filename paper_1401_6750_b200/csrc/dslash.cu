@@ -109,7 +109,7 @@ __global__ void __launch_bounds__(128) dslash_kernel(DslashArgs<typename Prec<S>
     typedef typename Prec<S>::F F;
     __shared__ double sm[32];
     int bx = blockIdx.x, src = 0;
-    if (A.nb == 2) { src = bx & 1; bx >>= 1; }          // paired sources: see DslashArgs::nb
+    if (A.nb > 1) { src = bx & (A.nb - 1); bx >>= (31 - __clz(A.nb)); }   // grouped sources (nb = 2 | 4): see DslashArgs::nb
     A.in = (const char*)A.in + src * A.mul_in * A.fstride;
     A.out = (char*)A.out + src * A.mul_out * A.fstride;
     if (A.x) A.x = (const char*)A.x + src * A.mul_x * A.fstride;
@@ -421,7 +421,7 @@ template <typename S, int DAGGER, int PIPE, int MINB>
 __global__ void __launch_bounds__(128, MINB) dslash16_kernel(DslashArgs<float> A) {
     __shared__ double sm[32];
     int bx = blockIdx.x, src = 0;
-    if (A.nb == 2) { src = bx & 1; bx >>= 1; }
+    if (A.nb > 1) { src = bx & (A.nb - 1); bx >>= (31 - __clz(A.nb)); }
     A.in = (const char*)A.in + src * A.mul_in * A.fstride;
     A.out = (char*)A.out + src * A.mul_out * A.fstride;
     if (A.x) A.x = (const char*)A.x + src * A.mul_x * A.fstride;
@@ -553,7 +553,7 @@ static tm_status launch_t(tm_ctx* ctx, const DslashCall& c, const void* gauge, c
     A.xmode = c.xmode; A.post = c.post; A.red_op = c.red_op;
     A.partials = ctx->d_partials; A.counter = ctx->d_counter; A.sc = ctx->d_scal;
     A.guard = c.guard;
-    A.nb = ctx->nb == 2 ? 2 : 1; A.fstride = ctx->Vh * 24 * sizeof(S);
+    A.nb = ctx->nb > 1 ? ctx->nb : 1; A.fstride = ctx->Vh * 24 * sizeof(S);
     A.mul_in = c.mul_in ? c.mul_in : 1; A.mul_x = c.mul_x ? c.mul_x : 1; A.mul_out = c.mul_out ? c.mul_out : 1;
     const int block = 128;
     const int tiles = (int)((ctx->Vh + block - 1) / block);
@@ -577,7 +577,7 @@ static tm_status launch16(tm_ctx* ctx, const DslashCall& c, const void* gauge, c
     A.xmode = c.xmode; A.post = c.post; A.red_op = c.red_op;
     A.partials = ctx->d_partials; A.counter = ctx->d_counter; A.sc = ctx->d_scal;
     A.guard = c.guard;
-    A.nb = ctx->nb == 2 ? 2 : 1; A.fstride = ctx->Vh * 24 * sizeof(S);
+    A.nb = ctx->nb > 1 ? ctx->nb : 1; A.fstride = ctx->Vh * 24 * sizeof(S);
     A.mul_in = c.mul_in ? c.mul_in : 1; A.mul_x = c.mul_x ? c.mul_x : 1; A.mul_out = c.mul_out ? c.mul_out : 1;
     const int block = 128;
     const int tiles = (int)((ctx->Vh + block - 1) / block);

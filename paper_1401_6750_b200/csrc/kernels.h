@@ -56,13 +56,13 @@ tm_status tm_reduce_finish(tm_ctx* ctx, unsigned int nblocks, int op, int guard,
 // reset the device state for a new solve (no host synchronisation)
 // eta2 > 0: ||eta||^2 known to the caller (Z4 noise: 12 V exactly), no norm kernel needed
 tm_status scal_init(tm_ctx* ctx, double rho2, double delta2, int max_iter, double eta2, cudaStream_t st);
-tm_status scal_get(tm_ctx* ctx, CgScalars* v /*[2]*/, cudaStream_t st);   // download + sync
+tm_status scal_get(tm_ctx* ctx, CgScalars* v /*[TM_MAXNB]*/, cudaStream_t st);   // download + sync
 
 // ---- solver.cu ----------------------------------------------------------------------------
 // eta, s: full-lattice internal fields of precision params->outer
 struct SolveJob {                       // one solve in flight (solver.cu: tm_solve_begin / tm_solve_end)
     tm_solve_params P;
-    int nb;                             // sources solved together (1 | 2)
+    int nb;                             // sources solved together (1 | 2 | 4)
     tm_prec po, ps, pa; tm_recon rc;
     double kappa, mu, delta;
     cudaStream_t st;
@@ -73,8 +73,8 @@ struct SolveJob {                       // one solve in flight (solver.cu: tm_so
     bool tail_valid; long enq;
 };
 // eta_norm2 > 0: ||eta||^2 known exactly to the caller (skips the norm kernel); 0: computed.
-// nb = 2: two sources solved in lockstep (every kernel launch covers both; needs eta_norm2): d_eta and d_s hold
-// [even 0][odd 0][even 1][odd 1] (two full-lattice fields back to back), tm_solve_end fills info[0..1]
+// nb = 2 | 4: that many sources solved in lockstep (every kernel launch covers all of them; needs eta_norm2): d_eta
+// and d_s hold nb full-lattice fields back to back, tm_solve_end fills info[0..nb-1]
 tm_status tm_solve_begin(tm_ctx* ctx, SolveJob* job, void* d_s, const void* d_eta, double kappa, double mu,
                          const tm_solve_params* params, cudaStream_t st, double eta_norm2 = 0.0, int nb = 1);
 tm_status tm_solve_end(tm_ctx* ctx, SolveJob* job, tm_solve_info* info);

@@ -74,8 +74,8 @@ tm_status tm_solve_begin(tm_ctx* ctx, SolveJob* Jp, void* d_s, const void* d_eta
                          const tm_solve_params* P, cudaStream_t st, double eta_norm2, int nb) {
     SolveJob& J = *Jp;
     if (!P) return tm_fail(ctx, TM_EARG, "solve: null params");
-    if (nb != 1 && nb != 2) return tm_fail(ctx, TM_EARG, "solve: nb must be 1 or 2");
-    if (nb == 2 && !(eta_norm2 > 0)) return tm_fail(ctx, TM_EARG, "solve: a paired solve needs the source norm");
+    if (nb != 1 && nb != 2 && nb != 4) return tm_fail(ctx, TM_EARG, "solve: nb must be 1, 2 or 4");
+    if (nb > 1 && !(eta_norm2 > 0)) return tm_fail(ctx, TM_EARG, "solve: a grouped solve needs the source norm");
     J.nb = nb;
     NbScope scope(ctx, nb);
     const tm_prec po = P->outer, ps = P->sloppy;
@@ -147,7 +147,7 @@ tm_status tm_solve_begin(tm_ctx* ctx, SolveJob* Jp, void* d_s, const void* d_eta
     }
     J.h_scal = ctx->h_scal;
     J.e_scal = ctx->ev[4];
-    TM_CUDA(ctx, cudaMemcpyAsync(ctx->h_scal, ctx->d_scal, 2 * sizeof(CgScalars), cudaMemcpyDeviceToHost, st));
+    TM_CUDA(ctx, cudaMemcpyAsync(ctx->h_scal, ctx->d_scal, TM_MAXNB * sizeof(CgScalars), cudaMemcpyDeviceToHost, st));
     TM_CUDA(ctx, cudaEventRecord(J.e_scal, st));
     return TM_OK;
 }
@@ -159,10 +159,14 @@ tm_status tm_solve_end(tm_ctx* ctx, SolveJob* Jp, tm_solve_info* info) {
     cudaStream_t st = J.st;
     const int nb = J.nb;
     NbScope scope(ctx, nb);
-    CgScalars sc[2];
+    CgScalars sc[TM_MAXNB];
     TM_CUDA(ctx, cudaEventSynchronize(J.e_scal));
-    sc[0] = J.h_scal[0]; sc[1] = J.h_scal[1];
-    auto running = [&]() { return sc[0].done < 2 || (nb == 2 && sc[1].done < 2); };
+    for (int b = 0; b < TM_MAXNB; b++) sc[b] = J.h_scal[b];
+    auto running = [&]() {
+        for (int b = 0; b < nb; b++)
+            if (sc[b].done < 2) return true;
+        return false;
+    };
     while (running()) {
         // off plan (first solve with these parameters, or a source behaves differently):
         // [iteration, update] pairs, polled every few pairs
@@ -175,23 +179,27 @@ tm_status tm_solve_end(tm_ctx* ctx, SolveJob* Jp, tm_solve_info* info) {
     }
     if (!J.tail_valid) TM_TRY(job_tail(ctx, J));
     TM_CUDA(ctx, cudaEventSynchronize(J.e1));
-    // remember where this solve paused: the launch plan of the next one (a pair: the union of both sources' pauses)
+    // remember where this solve paused: the launch plan of the next one (a group: the union of its sources' pauses)
     CgPlan& plan = ctx->plan[(int)J.ps];
-    plan.valid = sc[0].n_ru <= CG_MAX_PAUSES && (nb == 1 || sc[1].n_ru <= CG_MAX_PAUSES);
+    plan.valid = 1;
     plan.sloppy = (int)J.ps; plan.outer = (int)J.po; plan.recon = (int)J.rc; plan.max_iter = P->max_iter;
     plan.rho = P->rho; plan.delta = J.delta;
     plan.n_pause = 0;
     {
-        int i0 = 0, i1 = 0;
-        const int n0 = sc[0].n_ru < CG_MAX_PAUSES ? sc[0].n_ru : CG_MAX_PAUSES;
-        const int n1 = nb == 2 ? (sc[1].n_ru < CG_MAX_PAUSES ? sc[1].n_ru : CG_MAX_PAUSES) : 0;
-        while ((i0 < n0 || i1 < n1) && plan.n_pause < CG_MAX_PAUSES) {
-            int v;
-            if (i1 >= n1 || (i0 < n0 && sc[0].pause_iter[i0] <= sc[1].pause_iter[i1])) v = sc[0].pause_iter[i0++];
-            else v = sc[1].pause_iter[i1++];
-            if (plan.n_pause == 0 || plan.pause_iter[plan.n_pause - 1] != v) plan.pause_iter[plan.n_pause++] = v;
+        int idx[TM_MAXNB] = {0};
+        for (;;) {
+            int best = -1, v = 0;
+            for (int b = 0; b < nb; b++) {
+                if (sc[b].n_ru > CG_MAX_PAUSES) plan.valid = 0;
+                const int n = sc[b].n_ru < CG_MAX_PAUSES ? sc[b].n_ru : CG_MAX_PAUSES;
+                if (idx[b] < n && (best < 0 || sc[b].pause_iter[idx[b]] < v)) { best = b; v = sc[b].pause_iter[idx[b]]; }
+            }
+            if (best < 0) break;
+            idx[best]++;
+            if (plan.n_pause && plan.pause_iter[plan.n_pause - 1] == v) continue;
+            if (plan.n_pause == CG_MAX_PAUSES) { plan.valid = 0; break; }
+            plan.pause_iter[plan.n_pause++] = v;
         }
-        if (i0 < n0 || i1 < n1) plan.valid = 0;
     }
     float ms = 0;
     cudaEventElapsedTime(&ms, J.e0, J.e1);

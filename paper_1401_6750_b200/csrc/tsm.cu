@@ -9,6 +9,7 @@
 // tail and the launch gap of every kernel are covered by another source's kernels.  Nothing crosses to the
 // host per source except the solver's convergence scalars (and, in tsm_estimate_host, the packed noise).
 #include <math.h>
+#include <vector>
 #include <stdlib.h>
 #include "kernels.h"
 
@@ -100,7 +101,7 @@ static tm_status convert_full(tm_ctx* ctx, void* dst, tm_prec pd, const void* sr
     return TM_OK;
 }
 
-// one unit of work in flight on a lane: the same pass (LP | HP) of nb = 1 or 2 consecutive sources, solved together
+// one unit of work in flight on a lane: the same pass (LP | HP) of nb = 1, 2 or 4 consecutive sources, solved together
 struct TsmJob {
     int r, nb, pass;
     SolveJob sj;
@@ -115,8 +116,8 @@ struct TsmRun {
     size_t nr, z4_bytes; unsigned agrid;
     double ms_lp, ms_hp, worst_lp, worst_hp; long it_lp, it_hp; int noconv;
     double* acc[TM_NLANES];         // per lane: S_lp, S_lpc, S_hp, tmp (nr doubles each)
-    int pair;                       // solve sources two at a time
-    double* lp_keep;                // [2][nr]: l^LP of the pair whose HP pass comes next (binary files of the correction)
+    int group;                      // sources per solve (1 | 2 | 4; TMLOOPS_GROUP, default 4)
+    double* lp_keep;                // [TM_MAXNB][nr]: l^LP of the pair whose HP pass comes next (binary files of the correction)
 };
 
 // lane-private buffers of the active lane
@@ -128,7 +129,7 @@ static tm_status lane_buffers(TsmRun& R, int lane, cudaStream_t st) {
     return TM_OK;
 }
 
-// noise of source r in precision p into slot b of the active lane's (two-field) buffer
+// noise of source r in precision p into slot b of the active lane's (TM_MAXNB-field) buffer
 static tm_status job_noise(TsmRun& R, int r, int b, tm_prec p, cudaStream_t st, void** base) {
     tm_ctx* ctx = R.ctx;
     const unsigned char* zsrc = nullptr;
@@ -137,14 +138,14 @@ static tm_status job_noise(TsmRun& R, int r, int b, tm_prec p, cudaStream_t st, 
             // staged per lane and slot: the previous user of the slot (a z4_expand of this lane) finished before
             // that lane's solve was waited for
             void* slot;
-            TM_TRY(tm_ws(ctx, WS_TSM_Z4, 2 * R.z4_bytes, &slot));
+            TM_TRY(tm_ws(ctx, WS_TSM_Z4, TM_MAXNB * R.z4_bytes, &slot));
             slot = (char*)slot + (size_t)b * R.z4_bytes;
             TM_CUDA(ctx, cudaMemcpyAsync(slot, R.z4 + (size_t)r * R.z4_bytes, R.z4_bytes, cudaMemcpyHostToDevice, st));
             zsrc = (const unsigned char*)slot;
         } else zsrc = R.z4 + (size_t)r * R.z4_bytes;
     }
     const size_t fb = 2 * tm_parity_bytes(ctx, p);
-    TM_TRY(tm_ws(ctx, p == TM_F32 ? WS_TSM_ETA32 : WS_TSM_ETA64, 2 * fb, base));
+    TM_TRY(tm_ws(ctx, p == TM_F32 ? WS_TSM_ETA32 : WS_TSM_ETA64, TM_MAXNB * fb, base));
     return tm_z4_expand(ctx, (char*)*base + (size_t)b * fb, p, zsrc, R.P->seed, (unsigned long long)r, st);
 }
 
@@ -155,7 +156,7 @@ static tm_status job_start(TsmRun& R, TsmJob& J, int r, int nb, int pass, cudaSt
     J.po = pass ? P->hp.outer : P->lp.outer;
     J.ac = pass ? P->contract_acc_hp : P->contract_acc_lp;
     for (int b = 0; b < nb; b++) TM_TRY(job_noise(R, r + b, b, J.po, st, &J.eta_o));
-    TM_TRY(tm_ws(ctx, J.po == TM_F32 ? WS_TSM_S32 : WS_TSM_S64, 4 * tm_parity_bytes(ctx, J.po), &J.s_o));
+    TM_TRY(tm_ws(ctx, J.po == TM_F32 ? WS_TSM_S32 : WS_TSM_S64, TM_MAXNB * 2 * tm_parity_bytes(ctx, J.po), &J.s_o));
     // Z4 noise: |eta_c| = 1 for each of the 12 V components, so ||eta||^2 = 12 V exactly (no norm kernel)
     return tm_solve_begin(ctx, &J.sj, J.s_o, J.eta_o, P->kappa, P->mu, pass ? &P->hp : &P->lp, st, 12.0 * (double)ctx->V, nb);
 }
@@ -164,7 +165,7 @@ static tm_status job_finish(TsmRun& R, TsmJob& J, int lane) {
     tm_ctx* ctx = R.ctx;
     const tsm_params* P = R.P;
     cudaStream_t st = J.st;
-    tm_solve_info si[2];
+    tm_solve_info si[TM_MAXNB];
     tm_status s = tm_solve_end(ctx, &J.sj, si);
     if (s != TM_OK && s != TM_ENOCONV) return s;
     double* A = R.acc[lane];
@@ -181,7 +182,7 @@ static tm_status job_finish(TsmRun& R, TsmJob& J, int lane) {
         if (J.ac != J.po) {
             const size_t fba = 2 * tm_parity_bytes(ctx, J.ac);
             void* sbuf;
-            TM_TRY(tm_ws(ctx, J.ac == TM_F32 ? WS_TSM_S32 : WS_TSM_S64, 2 * fba, &sbuf));
+            TM_TRY(tm_ws(ctx, J.ac == TM_F32 ? WS_TSM_S32 : WS_TSM_S64, TM_MAXNB * fba, &sbuf));
             TM_TRY(convert_full(ctx, sbuf, J.ac, s_c, J.po, st));
             s_c = sbuf;
             void* ebase;
@@ -199,7 +200,7 @@ static tm_status job_finish(TsmRun& R, TsmJob& J, int lane) {
             TM_LAUNCH_CHECK(ctx, "binary_add_kernel");
         }
         if (R.lp_keep && do_hp) {
-            double* keep = R.lp_keep + (size_t)b * nr;
+            double* keep = R.lp_keep + (size_t)(r % TM_MAXNB) * nr;
             if (!J.pass) TM_CUDA(ctx, cudaMemcpyAsync(keep, tmp, nr * sizeof(double), cudaMemcpyDeviceToDevice, st));
             else {
                 binary_add_kernel<<<R.agrid, 256, 0, st>>>((double*)R.d_files_corr + (size_t)binary_file_of(r) * nr, tmp, keep, nr);
@@ -236,28 +237,31 @@ static tm_status tsm_pipeline(TsmRun& R, int NL, cudaStream_t st, void* d_out) {
         if (l) TM_CUDA(ctx, cudaStreamWaitEvent(lst[l], fork, 0));
         TM_TRY(lane_buffers(R, l, lst[l]));
     }
-    // job list: sources in pairs (r, r+1); each pair's LP pass is followed by its HP pass when r < n_hp
-    // (an odd source at the end of either range is solved alone)
+    // job list: sources in groups of R.group; a group's LP pass (split into solves of 4, 2 or 1 sources) is followed
+    // by the HP pass of those of its sources that have one (r < n_hp)
+    struct JobSpec { int r, nb, pass; };
+    std::vector<JobSpec> list;
+    for (int g = 0; g < P->n_lp; g += R.group)
+        for (int pass = 0; pass < 2; pass++) {
+            const int lim = pass ? P->n_hp : P->n_lp;
+            int r = g, m = lim - g < R.group ? lim - g : R.group;
+            while (m > 0) {
+                const int nb = m >= 4 ? 4 : m >= 2 ? 2 : 1;
+                list.push_back({r, nb, pass});
+                r += nb; m -= nb;
+            }
+        }
     TsmJob jobs[TM_NLANES];
     bool busy[TM_NLANES] = {false};
-    int jr = 0, jpass = 0;
-    bool more = true;
-    for (int j = 0;; j++) {
+    const int njobs = (int)list.size();
+    for (int j = 0; j < njobs + NL; j++) {
         const int l = j % NL;
         TM_TRY(tm_lane_use(ctx, l));
         if (busy[l]) { TM_TRY(job_finish(R, jobs[l], l)); busy[l] = false; }
-        if (more) {
-            const int lim = jpass ? P->n_hp : P->n_lp;
-            const int nb = (R.pair && jr + 1 < lim) ? 2 : 1;
-            TM_TRY(job_start(R, jobs[l], jr, nb, jpass, lst[l]));
+        if (j < njobs) {
+            TM_TRY(job_start(R, jobs[l], list[j].r, list[j].nb, list[j].pass, lst[l]));
             busy[l] = true;
-            if (!jpass && jr < P->n_hp) jpass = 1;
-            else { jpass = 0; jr += 2 - (R.pair ? 0 : 1); }
-            more = jr < P->n_lp;
         }
-        bool any = more;
-        for (int k = 0; k < NL; k++) any = any || busy[k];
-        if (!any) break;
     }
     // join
     cudaEvent_t joined[TM_NLANES];
@@ -303,13 +307,17 @@ static tm_status tsm_core(tm_ctx* ctx, void* d_out, void* d_per_source, const ts
     R.nr = 2 * (size_t)160 * P->nmom * ctx->X[3];                // doubles per per-source array
     R.z4_bytes = 3 * ctx->V;
     R.agrid = (unsigned)((R.nr + 255) / 256);
-    { const char* e = getenv("TMLOOPS_NO_PAIRS"); R.pair = !(e && e[0] == '1'); }
+    {
+        const char* e = getenv("TMLOOPS_GROUP");      // tuning / testing knob: sources per solve
+        const int gsz = e ? atoi(e) : TM_MAXNB;
+        R.group = gsz >= 4 ? 4 : gsz >= 2 ? 2 : 1;
+    }
     // the binary-storage files are shared accumulators: one lane keeps their additions ordered
     const int NL = (d_files_lp || d_files_corr || P->n_lp + P->n_hp < 2) ? 1 : TM_NLANES;
     if (d_files_lp) TM_CUDA(ctx, cudaMemsetAsync(d_files_lp, 0, (size_t)loop_binary_nfiles(P->n_lp) * R.nr * sizeof(double), st));
     if (d_files_corr && P->n_hp) {
         TM_CUDA(ctx, cudaMemsetAsync(d_files_corr, 0, (size_t)loop_binary_nfiles(P->n_hp) * R.nr * sizeof(double), st));
-        TM_TRY(tm_ws(ctx, WS_TSM_KEEP, 2 * R.nr * sizeof(double), (void**)&R.lp_keep));
+        TM_TRY(tm_ws(ctx, WS_TSM_KEEP, TM_MAXNB * R.nr * sizeof(double), (void**)&R.lp_keep));
     }
     cudaEvent_t e0 = ctx->ev[2], e1 = ctx->ev[3];
     TM_CUDA(ctx, cudaEventRecord(e0, st));

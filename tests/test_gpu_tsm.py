@@ -95,20 +95,22 @@ def test_tsm_edge_cases(setup):
         assert e.value.status == t.TM_ENOCONV
 
 
-def test_tsm_pairs_equal_single_source_solves(setup, monkeypatch):
-    """Sources are solved two per launch by default; every per-source array must be bit-identical to the
-    one-source-per-launch path (TMLOOPS_NO_PAIRS=1), for even and odd N_LP / N_HP."""
+def test_tsm_grouped_solves_equal_single_source_solves(setup, monkeypatch):
+    """Sources are solved four (two, one at the ragged end) per launch by default; every per-source array must be
+    bit-identical to the one-source-per-launch path (TMLOOPS_GROUP=1), for ragged N_LP / N_HP."""
     t = tm()
     dims, U, mom = setup
     k, mu = C1["kappa"], C1["mu"]
     with t.TmContext(dims, -1) as ctx:
         ctx.tm_load_gauge(U)
-        for n_lp, n_hp in ((5, 3), (4, 2), (2, 1)):
-            monkeypatch.delenv("TMLOOPS_NO_PAIRS", raising=False)
+        for n_lp, n_hp, group in ((7, 3, None), (9, 6, None), (4, 4, None), (5, 3, "2"), (2, 1, None)):
+            monkeypatch.delenv("TMLOOPS_GROUP", raising=False)
+            if group:
+                monkeypatch.setenv("TMLOOPS_GROUP", group)
             out_p, ps_p, info_p = ctx.tsm_estimate(n_lp, n_hp, k, mu, mom, LP, HP, t.TM_F32, t.TM_F64, seed=3, per_source=True)
-            monkeypatch.setenv("TMLOOPS_NO_PAIRS", "1")
+            monkeypatch.setenv("TMLOOPS_GROUP", "1")
             out_s, ps_s, info_s = ctx.tsm_estimate(n_lp, n_hp, k, mu, mom, LP, HP, t.TM_F32, t.TM_F64, seed=3, per_source=True)
-            monkeypatch.delenv("TMLOOPS_NO_PAIRS", raising=False)
+            monkeypatch.delenv("TMLOOPS_GROUP", raising=False)
             assert np.array_equal(to_np(ps_p), to_np(ps_s)), (n_lp, n_hp)
             assert info_p["iters_lp"] == info_s["iters_lp"] and info_p["iters_hp"] == info_s["iters_hp"]
             assert info_p["launches"] < info_s["launches"]
