@@ -79,12 +79,13 @@ tm_status tm_dslash(tm_ctx* ctx, void* d_out, const void* d_in, const void* d_x,
                     tm_recon recon, void* stream);
 
 /* Row f3 of SURVEY.md sec 8 (multi-source Dslash; the N_LP ~ 1e2-1e3 sources are independent): the
- * operator pieces HOP, HOP_TWINV, XPAY of tm_dslash (reconstruct-12) applied to TWO parity fields in one launch.
- * d_out, d_in, d_x: two internal parity fields back to back (source 1 at byte offset tm_field_bytes(prec, 0)).
- * CTAs 2k and 2k+1 work on the same sites of the two sources, so every link crosses HBM once per pair (the second
- * reader finds it in L2).  Results are bit-identical to two tm_dslash calls.  Asynchronous on stream. */
-tm_status tm_dslash_pair(tm_ctx* ctx, void* d_out, const void* d_in, const void* d_x, tm_op op,
-                         int out_parity, int dagger, double kappa, double mu, tm_prec prec, void* stream);
+ * operator pieces HOP, HOP_TWINV, XPAY of tm_dslash (reconstruct-12) applied to nb = 1, 2, 4 or 8 parity fields in
+ * one launch.  d_out, d_in, d_x: nb internal parity fields back to back (source b at byte offset
+ * b * tm_field_bytes(prec, 0)).  CTAs nb*k .. nb*k + nb-1 work on the same sites of the nb sources, so every link
+ * crosses HBM once per group (the later readers find it in L2).  Results are bit-identical to nb tm_dslash calls.
+ * tsm_estimate solves its sources in such groups (8 by default).  Asynchronous on stream. */
+tm_status tm_dslash_multi(tm_ctx* ctx, void* d_out, const void* d_in, const void* d_x, int nb, tm_op op,
+                          int out_parity, int dagger, double kappa, double mu, tm_prec prec, void* stream);
 
 /* eq. 2.1: even-odd preconditioned CG on Mhat^dag Mhat (CGLS recurrences, x0 = 0) in `sloppy`
  * storage with reliable updates in `outer` precision (TM_F32 or TM_F64, >= sloppy).

@@ -30,7 +30,7 @@ PREC_BYTES = {TM_F64: 8, TM_F32: 4, TM_F16: 2, TM_BF16: 2}
 
 EXPORTS = [
     "tm_create", "tm_destroy", "tm_last_error", "tm_load_gauge", "tm_field_bytes",
-    "tm_field_import", "tm_field_export", "tm_dslash", "tm_dslash_pair", "tm_cg_solve", "loop_contract_project",
+    "tm_field_import", "tm_field_export", "tm_dslash", "tm_dslash_multi", "tm_cg_solve", "loop_contract_project",
     "tsm_estimate", "tsm_estimate_host", "tm_launch_count",
     "loop_binary_nfiles", "loop_binary_accumulate", "loop_binary_recover", "tsm_estimate_binary",
 ]
@@ -94,7 +94,7 @@ def load_library():
     L.tm_field_import.argtypes = [vp, vp, vp, ci, vp]
     L.tm_field_export.argtypes = [vp, vp, vp, ci, vp]
     L.tm_dslash.argtypes = [vp, vp, vp, vp, ci, ci, ci, cd, cd, ci, ci, vp]
-    L.tm_dslash_pair.argtypes = [vp, vp, vp, vp, ci, ci, ci, cd, cd, ci, vp]
+    L.tm_dslash_multi.argtypes = [vp, vp, vp, vp, ci, ci, ci, ci, cd, cd, ci, vp]
     L.tm_cg_solve.argtypes = [vp, vp, vp, cd, cd, ctypes.POINTER(tm_solve_params),
                               ctypes.POINTER(tm_solve_info), vp]
     L.loop_contract_project.argtypes = [vp, vp, vp, vp, cd, cd, ctypes.POINTER(ci), ci, ci, vp]
@@ -229,11 +229,11 @@ class TmContext:
                                        int(prec), int(recon), _stream()))
         return out
 
-    def tm_dslash_pair(self, out, inp, x, op, out_parity, dagger, kappa, mu, prec):
-        """Two stacked internal parity fields (source 1 one parity field behind source 0) in one launch."""
-        self._check(self.lib.tm_dslash_pair(self.h, out.data_ptr(), inp.data_ptr(),
-                                            x.data_ptr() if x is not None else None, int(op), int(out_parity),
-                                            int(bool(dagger)), float(kappa), float(mu), int(prec), _stream()))
+    def tm_dslash_multi(self, out, inp, x, nb, op, out_parity, dagger, kappa, mu, prec):
+        """nb (1, 2, 4, 8) stacked internal parity fields (source b at b parity fields behind source 0) in one launch."""
+        self._check(self.lib.tm_dslash_multi(self.h, out.data_ptr(), inp.data_ptr(),
+                                             x.data_ptr() if x is not None else None, int(nb), int(op), int(out_parity),
+                                             int(bool(dagger)), float(kappa), float(mu), int(prec), _stream()))
         return out
 
     def apply_M(self, psi, kappa, mu, prec=TM_F64, recon=TM_R18, dagger=False):

@@ -10,10 +10,10 @@ extern "C" long tm_launch_count(const tm_ctx* ctx) { return ctx ? ctx->launches 
 // allocate the private resources of a lane into the context's active fields
 static bool lane_alloc(tm_ctx* c, int lane) {
     bool ok = cudaMalloc((void**)&c->d_partials, sizeof(double) * TM_MAXNB * TM_PSTRIDE) == cudaSuccess
-           && cudaMalloc((void**)&c->d_counter, sizeof(unsigned int) * 4) == cudaSuccess
+           && cudaMalloc((void**)&c->d_counter, sizeof(unsigned int) * TM_MAXNB) == cudaSuccess
            && cudaMalloc((void**)&c->d_scal, TM_MAXNB * sizeof(CgScalars)) == cudaSuccess
            && cudaMallocHost((void**)&c->h_scal, TM_MAXNB * sizeof(CgScalars)) == cudaSuccess
-           && cudaMemset(c->d_counter, 0, sizeof(unsigned int) * 4) == cudaSuccess
+           && cudaMemset(c->d_counter, 0, sizeof(unsigned int) * TM_MAXNB) == cudaSuccess
            && cudaMemset(c->d_scal, 0, TM_MAXNB * sizeof(CgScalars)) == cudaSuccess;
     for (int i = 0; ok && i < TM_NEVENTS; i++) ok = cudaEventCreate(&c->ev[i]) == cudaSuccess;
     if (ok && lane > 0) ok = cudaStreamCreateWithFlags(&c->lane_stream, cudaStreamNonBlocking) == cudaSuccess;
@@ -175,16 +175,17 @@ extern "C" tm_status tm_field_export(tm_ctx* c, void* d_canon, const void* d_int
     return tm_export_launch(c, d_canon, d_internal, prec, (cudaStream_t)stream);
 }
 
-// Row f3 (multi-source Dslash): the same operator pieces as tm_dslash (HOP, HOP_TWINV, XPAY; reconstruct-12) on TWO
-// stacked parity fields per launch -- source 1's in / x / out one parity field (tm_field_bytes(prec, 0)) behind
-// source 0's.  CTAs 2k and 2k+1 work on the same 128 sites of the two sources, so the second reader of every
-// link finds it in L2 instead of HBM.  Results are bit-identical to two tm_dslash calls.
-extern "C" tm_status tm_dslash_pair(tm_ctx* c, void* d_out, const void* d_in, const void* d_x, tm_op op,
-                                    int out_parity, int dagger, double kappa, double mu, tm_prec prec, void* stream) {
-    if (!c || !d_out || !d_in) return tm_fail(c, TM_EARG, "tm_dslash_pair: null argument");
-    if (d_out == d_in) return tm_fail(c, TM_EARG, "tm_dslash_pair: out must not alias in");
-    if ((int)prec < 0 || (int)prec > 3) return tm_fail(c, TM_EPREC, "tm_dslash_pair: unknown precision");
-    if (op == TM_OP_XPAY && !d_x) return tm_fail(c, TM_EARG, "tm_dslash_pair: XPAY needs x");
+// Row f3 (multi-source Dslash): the same operator pieces as tm_dslash (HOP, HOP_TWINV, XPAY; reconstruct-12) on nb
+// stacked parity fields per launch -- source b's in / x / out sit b parity fields (tm_field_bytes(prec, 0)) behind
+// source 0's.  CTAs nb*k .. nb*k + nb-1 work on the same 128 sites of the nb sources, so the later readers of every
+// link find it in L2 instead of HBM.  Results are bit-identical to nb tm_dslash calls.
+extern "C" tm_status tm_dslash_multi(tm_ctx* c, void* d_out, const void* d_in, const void* d_x, int nb, tm_op op,
+                                     int out_parity, int dagger, double kappa, double mu, tm_prec prec, void* stream) {
+    if (!c || !d_out || !d_in) return tm_fail(c, TM_EARG, "tm_dslash_multi: null argument");
+    if (d_out == d_in) return tm_fail(c, TM_EARG, "tm_dslash_multi: out must not alias in");
+    if ((int)prec < 0 || (int)prec > 3) return tm_fail(c, TM_EPREC, "tm_dslash_multi: unknown precision");
+    if (nb < 1 || nb > TM_MAXNB || (nb & (nb - 1))) return tm_fail(c, TM_EARG, "tm_dslash_multi: nb must be 1, 2, 4 or 8");
+    if (op == TM_OP_XPAY && !d_x) return tm_fail(c, TM_EARG, "tm_dslash_multi: XPAY needs x");
     cudaStream_t st = (cudaStream_t)stream;
     TM_CUDA(c, cudaSetDevice(c->device));
     DslashCall k;
@@ -196,9 +197,9 @@ extern "C" tm_status tm_dslash_pair(tm_ctx* c, void* d_out, const void* d_in, co
         case TM_OP_HOP: break;
         case TM_OP_HOP_TWINV: k.post = 1; break;
         case TM_OP_XPAY: k.x = d_x; k.xmode = 2; k.coef = -kappa * kappa; break;
-        default: return tm_fail(c, TM_EARG, "tm_dslash_pair: op must be HOP, HOP_TWINV or XPAY");
+        default: return tm_fail(c, TM_EARG, "tm_dslash_multi: op must be HOP, HOP_TWINV or XPAY");
     }
-    c->nb = 2;
+    c->nb = nb;
     const tm_status s = tm_dslash_launch(c, k, prec, TM_R12, st);
     c->nb = 1;
     return s;

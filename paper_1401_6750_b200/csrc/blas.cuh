@@ -32,7 +32,7 @@ struct CgScalars {
     int pause_iter[CG_MAX_PAUSES];   // iteration count at each pause (replayed by the host as a launch plan)
 };
 
-#define TM_MAXNB 4                // sources solved together at most (every kernel launch covers all of them)
+#define TM_MAXNB 8                // sources solved together at most (every kernel launch covers all of them)
 #define TM_PSTRIDE (1 << 18)     // doubles between the reduction partials of consecutive sources of a grouped solve
 
 enum { GUARD_ALWAYS = 0, GUARD_ITER = 1, GUARD_RU = 2 };     // run iff guard == 0 || done == guard - 1

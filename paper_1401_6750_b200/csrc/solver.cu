@@ -74,7 +74,7 @@ tm_status tm_solve_begin(tm_ctx* ctx, SolveJob* Jp, void* d_s, const void* d_eta
                          const tm_solve_params* P, cudaStream_t st, double eta_norm2, int nb) {
     SolveJob& J = *Jp;
     if (!P) return tm_fail(ctx, TM_EARG, "solve: null params");
-    if (nb != 1 && nb != 2 && nb != 4) return tm_fail(ctx, TM_EARG, "solve: nb must be 1, 2 or 4");
+    if (nb < 1 || nb > TM_MAXNB || (nb & (nb - 1))) return tm_fail(ctx, TM_EARG, "solve: nb must be a power of two <= TM_MAXNB");
     if (nb > 1 && !(eta_norm2 > 0)) return tm_fail(ctx, TM_EARG, "solve: a grouped solve needs the source norm");
     J.nb = nb;
     NbScope scope(ctx, nb);

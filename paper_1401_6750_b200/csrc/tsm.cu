@@ -101,7 +101,7 @@ static tm_status convert_full(tm_ctx* ctx, void* dst, tm_prec pd, const void* sr
     return TM_OK;
 }
 
-// one unit of work in flight on a lane: the same pass (LP | HP) of nb = 1, 2 or 4 consecutive sources, solved together
+// one unit of work in flight on a lane: the same pass (LP | HP) of nb = 1, 2, 4 or 8 consecutive sources, solved together
 struct TsmJob {
     int r, nb, pass;
     SolveJob sj;
@@ -110,13 +110,17 @@ struct TsmJob {
     cudaStream_t st;
 };
 
+#ifndef TM_GROUP_DEFAULT
+#define TM_GROUP_DEFAULT 8
+#endif
+
 struct TsmRun {
     tm_ctx* ctx; const tsm_params* P; void* d_per_source; void* d_files_lp; void* d_files_corr;
     const unsigned char* z4; int z4_on_host;
     size_t nr, z4_bytes; unsigned agrid;
     double ms_lp, ms_hp, worst_lp, worst_hp; long it_lp, it_hp; int noconv;
     double* acc[TM_NLANES];         // per lane: S_lp, S_lpc, S_hp, tmp (nr doubles each)
-    int group;                      // sources per solve (1 | 2 | 4; TMLOOPS_GROUP, default 4)
+    int group;                      // sources per solve (1 | 2 | 4 | 8; TMLOOPS_GROUP, default TM_GROUP_DEFAULT)
     double* lp_keep;                // [TM_MAXNB][nr]: l^LP of the pair whose HP pass comes next (binary files of the correction)
 };
 
@@ -246,7 +250,8 @@ static tm_status tsm_pipeline(TsmRun& R, int NL, cudaStream_t st, void* d_out) {
             const int lim = pass ? P->n_hp : P->n_lp;
             int r = g, m = lim - g < R.group ? lim - g : R.group;
             while (m > 0) {
-                const int nb = m >= 4 ? 4 : m >= 2 ? 2 : 1;
+                int nb = 1;
+                while (2 * nb <= m && 2 * nb <= TM_MAXNB) nb *= 2;
                 list.push_back({r, nb, pass});
                 r += nb; m -= nb;
             }
@@ -309,8 +314,9 @@ static tm_status tsm_core(tm_ctx* ctx, void* d_out, void* d_per_source, const ts
     R.agrid = (unsigned)((R.nr + 255) / 256);
     {
         const char* e = getenv("TMLOOPS_GROUP");      // tuning / testing knob: sources per solve
-        const int gsz = e ? atoi(e) : TM_MAXNB;
-        R.group = gsz >= 4 ? 4 : gsz >= 2 ? 2 : 1;
+        const int gsz = e ? atoi(e) : TM_GROUP_DEFAULT;
+        R.group = 1;
+        while (2 * R.group <= gsz && 2 * R.group <= TM_MAXNB) R.group *= 2;
     }
     // the binary-storage files are shared accumulators: one lane keeps their additions ordered
     const int NL = (d_files_lp || d_files_corr || P->n_lp + P->n_hp < 2) ? 1 : TM_NLANES;

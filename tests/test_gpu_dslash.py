@@ -129,33 +129,33 @@ def test_import_export_roundtrip_and_errors():
 
 
 @pytest.mark.parametrize("prec", ["f64", "f32", "f16", "bf16"])
-def test_dslash_pair_equals_two_single_launches(prec):
-    """Row f3: two sources per launch (links shared through L2) -- bit-identical to two tm_dslash calls."""
+@pytest.mark.parametrize("nb", [2, 4, 8])
+def test_dslash_multi_equals_single_launches(prec, nb):
+    """Row f3: nb sources per launch (links shared through L2) -- bit-identical to nb tm_dslash calls."""
     import torch
     t = tm()
-    dims = (8, 8, 8, 16)
+    dims = (8, 8, 8, 16) if nb < 8 else (6, 4, 6, 10)
     k, mu = 0.1565, 0.004
     U = inputs.gauge_field(dims, 0.3, 3)
     with t.TmContext(dims, -1) as ctx:
         ctx.tm_load_gauge(U)
         P = t.PREC[prec]
         pb = ctx.tm_field_bytes(P, False)
-        fields = []
-        for seed in (1, 2, 3, 4):
-            f = ctx.tm_field_import(inputs.random_spinor(dims, seed), P)
-            fields.append(f[:pb])
-        inp = torch.cat(fields[:2])
-        x = torch.cat(fields[2:])
+        fields = [ctx.tm_field_import(inputs.random_spinor(dims, seed), P) for seed in range(1, nb + 1)]
+        inp = torch.cat([f[:pb] for f in fields])          # even halves as inputs
+        x = torch.cat([f[pb:] for f in fields])            # odd halves as the x operand
         for op in (t.TM_OP_HOP, t.TM_OP_HOP_TWINV, t.TM_OP_XPAY):
             for par in (0, 1):
                 for dag in (False, True):
                     out = torch.empty_like(inp)
-                    ctx.tm_dslash_pair(out, inp, x, op, par, dag, k, mu, P)
-                    for b in range(2):
+                    ctx.tm_dslash_multi(out, inp, x, nb, op, par, dag, k, mu, P)
+                    for b in range(nb):
                         ref = torch.empty(pb, dtype=torch.uint8, device=out.device)
                         ctx.tm_dslash(ref, inp[b * pb:(b + 1) * pb], x[b * pb:(b + 1) * pb], op, par, dag, k, mu, P, 12)
-                        assert bool((out[b * pb:(b + 1) * pb] == ref).all()), (prec, op, par, dag, b)
+                        assert bool((out[b * pb:(b + 1) * pb] == ref).all()), (prec, nb, op, par, dag, b)
         with pytest.raises(t.TmError):
-            ctx.tm_dslash_pair(inp, inp, x, t.TM_OP_HOP, 0, False, k, mu, P)        # out aliases in
+            ctx.tm_dslash_multi(inp, inp, x, nb, t.TM_OP_HOP, 0, False, k, mu, P)        # out aliases in
         with pytest.raises(t.TmError):
-            ctx.tm_dslash_pair(torch.empty_like(inp), inp, None, t.TM_OP_XPAY, 0, False, k, mu, P)
+            ctx.tm_dslash_multi(torch.empty_like(inp), inp, None, nb, t.TM_OP_XPAY, 0, False, k, mu, P)
+        with pytest.raises(t.TmError):
+            ctx.tm_dslash_multi(torch.empty_like(inp), inp, x, 3, t.TM_OP_HOP, 0, False, k, mu, P)

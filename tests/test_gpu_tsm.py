@@ -96,14 +96,14 @@ def test_tsm_edge_cases(setup):
 
 
 def test_tsm_grouped_solves_equal_single_source_solves(setup, monkeypatch):
-    """Sources are solved four (two, one at the ragged end) per launch by default; every per-source array must be
+    """Sources are solved eight (four, two, one at the ragged end) per launch by default; every per-source array must be
     bit-identical to the one-source-per-launch path (TMLOOPS_GROUP=1), for ragged N_LP / N_HP."""
     t = tm()
     dims, U, mom = setup
     k, mu = C1["kappa"], C1["mu"]
     with t.TmContext(dims, -1) as ctx:
         ctx.tm_load_gauge(U)
-        for n_lp, n_hp, group in ((7, 3, None), (9, 6, None), (4, 4, None), (5, 3, "2"), (2, 1, None)):
+        for n_lp, n_hp, group in ((7, 3, None), (19, 11, None), (9, 6, "4"), (5, 3, "2"), (2, 1, None)):
             monkeypatch.delenv("TMLOOPS_GROUP", raising=False)
             if group:
                 monkeypatch.setenv("TMLOOPS_GROUP", group)
