@@ -45,11 +45,11 @@ def peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
-def ncu_traffic(prec):
+def ncu_traffic(prec, suffix=""):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
     `ncu --set full` summary (text) of the same kernel, or None when no capture of it is committed."""
     import re
-    p = os.path.join(ROOT, "profiles", "r01_dslash16_%s.md" % prec)
+    p = os.path.join(ROOT, "profiles", "r01_dslash16_%s%s.md" % (prec, suffix))
     if not os.path.exists(p):
         return None, None
     tot, scale = 0.0, {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
@@ -220,6 +220,32 @@ def time_dslash(ctx, tmod, torch, prec, recon, kappa, mu, napp, op_name="XPAY"):
     return e0.elapsed_time(e1) / napp
 
 
+def time_dslash_multi(ctx, tmod, torch, prec, nb, kappa, mu, napp):
+    """Average CUDA-event time of one nb-source parity-Dslash launch (XPAY, reconstruct-12), as tsm_estimate launches it."""
+    P = tmod.PREC[prec]
+    pb = ctx.tm_field_bytes(P, False)
+    tdt = {"f64": torch.float64, "f32": torch.float32, "f16": torch.float16, "bf16": torch.bfloat16}[prec]
+    nbuf = 3
+    ins = [torch.empty(nb * pb, dtype=torch.uint8, device=ctx.tdev) for _ in range(nbuf)]
+    outs = [torch.empty(nb * pb, dtype=torch.uint8, device=ctx.tdev) for _ in range(nbuf)]
+    xs = torch.empty(nb * pb, dtype=torch.uint8, device=ctx.tdev)
+    g = torch.Generator(device=ctx.tdev)
+    g.manual_seed(4321)
+    for b in ins + [xs]:
+        v = b.view(tdt)
+        v.copy_((torch.rand(v.shape, generator=g, device=ctx.tdev, dtype=torch.float32) - 0.5).to(tdt))
+    for i in range(4):
+        ctx.tm_dslash_multi(outs[i % nbuf], ins[i % nbuf], xs, nb, tmod.TM_OP_XPAY, 0, False, kappa, mu, P)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for i in range(napp):
+        ctx.tm_dslash_multi(outs[i % nbuf], ins[i % nbuf], xs, nb, tmod.TM_OP_XPAY, 0, False, kappa, mu, P)
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / napp
+
+
 def dslash_bytes_per_site(prec, recon, xpay):
     b = {"f64": 8, "f32": 4, "f16": 2, "bf16": 2}[prec]
     return (48 + 8 * recon + (24 if xpay else 0)) * b     # SURVEY.md sec 8d: read 1 spinor, 8 links, write 1 (+ x)
@@ -344,6 +370,20 @@ def run_b200(args, cfg):
                 "algorithmic_bytes_per_launch": dslash_bytes_per_site(LP["sloppy"], 12, True) * Vh,
                 "how": "CUDA events around %d back-to-back launches on the current stream, 4 rotating field pairs" % napp}
     roofline["traffic"], roofline["traffic_source"] = ncu_traffic(LP["sloppy"])
+    # the same kernel as tsm_estimate launches it: GROUP sources per launch, links read from HBM once per group
+    # (later readers hit L2).  Two accountings: the bytes such a launch must move (spinors per source, links once),
+    # and the single-source equivalent (SURVEY.md sec 8d bytes per site x sites x sources).
+    GROUP = 8
+    t_g = time_dslash_multi(ctx, tmod, torch, LP["sloppy"], GROUP, kappa, mu, 60)
+    b16 = 2
+    must_move = (GROUP * (48 + 24) + 8 * 12) * b16 * Vh
+    roofline["grouped"] = {
+        "sources_per_launch": GROUP, "us_per_launch": t_g * 1e3, "us_per_source": t_g * 1e3 / GROUP,
+        "hbm_bytes_per_launch": must_move, "achieved_GBps": must_move / (t_g * 1e-3) / 1e9,
+        "frac_of_peak": must_move / (t_g * 1e-3) / 1e9 / peak,
+        "single_source_equivalent_GBps": GROUP * dslash_bytes_per_site(LP["sloppy"], 12, True) * Vh / (t_g * 1e-3) / 1e9,
+        "traffic": ncu_traffic(LP["sloppy"], "_group8")[0],
+        "note": "not HBM-bound any more: limited by instruction issue and board power (DESIGN.md sec 6)"}
 
     it_lp = np.mean([i["iters_lp"] for i in infos])
     it_hp = np.mean([i["iters_hp"] for i in infos])

@@ -24,6 +24,7 @@ def main():
     ap.add_argument("--dims", type=int, nargs=4, default=[32, 32, 32, 64])
     ap.add_argument("--napp", type=int, default=6)
     ap.add_argument("--op", default="XPAY")
+    ap.add_argument("--nb", type=int, default=1, help="dslash: sources per launch (tm_dslash_multi)")
     ap.add_argument("--eps", type=float, default=0.2)
     ap.add_argument("--kappa", type=float, default=0.161231)
     ap.add_argument("--mu", type=float, default=0.004)
@@ -41,25 +42,34 @@ def main():
     if a.what == "dslash":
         tdt = {"f64": torch.float64, "f32": torch.float32, "f16": torch.float16, "bf16": torch.bfloat16}[a.prec]
         nb = 3
-        ins = [ctx.empty_field(P, False) for _ in range(nb)]
-        outs = [ctx.empty_field(P, False) for _ in range(nb)]
-        xs = ctx.empty_field(P, False)
+        pb = ctx.tm_field_bytes(P, False)
+        ins = [torch.empty(a.nb * pb, dtype=torch.uint8, device=dev) for _ in range(nb)]
+        outs = [torch.empty(a.nb * pb, dtype=torch.uint8, device=dev) for _ in range(nb)]
+        xs = torch.empty(a.nb * pb, dtype=torch.uint8, device=dev)
         for b in ins + [xs]:
             v = b.view(tdt)
             v.copy_((torch.rand(v.shape, device=dev, dtype=torch.float32) - 0.5).to(tdt))
         op = getattr(tmod, "TM_OP_" + a.op)
+
+        def launch(i):
+            if a.nb == 1:
+                ctx.tm_dslash(outs[i % nb], ins[i % nb], xs, op, 0, False, a.kappa, a.mu, P, a.recon)
+            else:
+                ctx.tm_dslash_multi(outs[i % nb], ins[i % nb], xs, a.nb, op, 0, False, a.kappa, a.mu, P)
         for i in range(3):
-            ctx.tm_dslash(outs[i % nb], ins[i % nb], xs, op, 0, False, a.kappa, a.mu, P, a.recon)
+            launch(i)
         torch.cuda.synchronize()
         e0.record()
         for i in range(a.napp):
-            ctx.tm_dslash(outs[i % nb], ins[i % nb], xs, op, 0, False, a.kappa, a.mu, P, a.recon)
+            launch(i)
         e1.record()
         torch.cuda.synchronize()
         V = inputs.volume(dims)
         us = e0.elapsed_time(e1) * 1e3 / a.napp
-        nbytes = (48 + 8 * a.recon + (24 if a.op == "XPAY" else 0)) * tmod.PREC_BYTES[P] * (V // 2)
-        print("dslash %s r%d %s: %.1f us/launch, %.0f GB/s algorithmic" % (a.prec, a.recon, a.op, us, nbytes / us / 1e3))
+        xb = 24 if a.op == "XPAY" else 0
+        nbytes = (a.nb * (48 + xb) + 8 * a.recon) * tmod.PREC_BYTES[P] * (V // 2)
+        print("dslash %s r%d %s, %d source(s) per launch: %.1f us/launch, %.0f GB/s (spinors per source, links once per launch)"
+              % (a.prec, a.recon, a.op, a.nb, us, nbytes / us / 1e3))
     elif a.what == "sweep":
         # BASELINE.json configs[4] (bandwidth sweep): standalone parity Dslash (XPAY epilogue) and one CG iteration
         # (4 Dslash + fused BLAS-1) per storage precision / reconstruct; a.napp applications each
