@@ -387,7 +387,9 @@ def run_b200(args, cfg):
 
     it_lp = np.mean([i["iters_lp"] for i in infos])
     it_hp = np.mean([i["iters_hp"] for i in infos])
+    free_b, total_b = torch.cuda.mem_get_info()
     extras = {
+        "hbm_in_use_gb": (total_b - free_b) / 1e9,     # gauge copies + 2 lanes x 8 sources of solver workspaces + noise
         "dslash": ds,
         "lp_iters_per_source": it_lp / n_lp, "hp_iters_per_source": it_hp / max(1, n_hp),
         "lp_cg_iters_per_sec": it_lp / (np.mean([i["ms_lp_solve"] for i in infos]) * 1e-3),
