@@ -313,8 +313,23 @@ static tm_status tsm_core(tm_ctx* ctx, void* d_out, void* d_per_source, const ts
     R.z4_bytes = 3 * ctx->V;
     R.agrid = (unsigned)((R.nr + 255) / 256);
     {
-        const char* e = getenv("TMLOOPS_GROUP");      // tuning / testing knob: sources per solve
-        const int gsz = e ? atoi(e) : TM_GROUP_DEFAULT;
+        // sources per solve: TM_GROUP_DEFAULT, reduced until the lanes' workspaces (noise + solution in outer precision,
+        // 5 sloppy vectors, x and r, 3 outer-precision vectors per source; the HP pass is the larger one) stay below
+        // 45 % of the device memory, so that a large lattice degrades to smaller groups instead of running out of
+        // memory (48^3x96: groups of 2).  TMLOOPS_GROUP overrides (tuning / tests).
+        auto per_source = [&](const tm_solve_params& sp) {
+            const double bo = (double)tm_parity_bytes(ctx, sp.outer), bs = (double)tm_parity_bytes(ctx, sp.sloppy);
+            const double ba = (double)tm_parity_bytes(ctx, sp.sloppy == TM_F64 ? TM_F64 : TM_F32);
+            return 7.0 * bo + 5.0 * bs + 2.0 * ba;
+        };
+        double need = per_source(P->lp);
+        if (P->n_hp && per_source(P->hp) > need) need = per_source(P->hp);
+        size_t free_b = 0, total_b = 0;
+        TM_CUDA(ctx, cudaMemGetInfo(&free_b, &total_b));
+        int gsz = TM_GROUP_DEFAULT;
+        while (gsz > 1 && (double)gsz * TM_NLANES * need > 0.45 * (double)total_b) gsz /= 2;
+        const char* e = getenv("TMLOOPS_GROUP");
+        if (e) gsz = atoi(e);
         R.group = 1;
         while (2 * R.group <= gsz && 2 * R.group <= TM_MAXNB) R.group *= 2;
     }

@@ -93,6 +93,9 @@ def test_tsm_edge_cases(setup):
         with pytest.raises(t.TmError) as e:
             ctx.tsm_estimate(1, 0, k, mu, mom, bad, HP, seed=1)
         assert e.value.status == t.TM_ENOCONV
+        with pytest.raises(t.TmError) as e:                          # the same inside a group of sources
+            ctx.tsm_estimate(3, 2, k, mu, mom, bad, HP, seed=1)
+        assert e.value.status == t.TM_ENOCONV
 
 
 def test_tsm_grouped_solves_equal_single_source_solves(setup, monkeypatch):
