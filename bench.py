@@ -364,7 +364,7 @@ def run_b200(args, cfg):
         ds[prec + "_r%d" % recon] = {"us": t_ms * 1e3, "GBps": nbytes / (t_ms * 1e-3) / 1e9,
                                      "GFLOPs": (1320 + 96) * Vh / (t_ms * 1e-3) / 1e9}
     dom = ds[LP["sloppy"] + "_r12"]
-    roofline = {"bound": "hbm", "kernel": "dslash_kernel<%s,12> XPAY (Mhat second half)" % LP["sloppy"],
+    roofline = {"bound": "hbm", "kernel": "dslash16_kernel<%s> reconstruct-12 XPAY (second half of Mhat), one source per launch" % LP["sloppy"],
                 "achieved": dom["GBps"], "peak": peak, "unit": "GB/s", "frac": dom["GBps"] / peak,
                 "traffic": None, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": dslash_bytes_per_site(LP["sloppy"], 12, True) * Vh,
