@@ -186,3 +186,9 @@ def binary_recover(files, counts, N: int):
     st = lib().orc_binary_recover(out.ctypes.data_as(ctypes.c_void_p), p_f, counts.ctypes.data_as(ctypes.c_void_p),
                                   ctypes.c_int(f.shape[0]), ctypes.c_int(N), ctypes.c_long(ln))
     return out if st == 0 else None
+
+
+def loops_project_explicit(s, U, kappa, mu, momenta, tb=-1, t0=0, t1=None) -> np.ndarray:
+    """Variant of reading 5: the generalised one-end trick with D_W applied explicitly,
+    l[1] = s^dag g5 X g5 D_W s with g5 D_W s = g5 (M s) - 2 i kappa mu s, i.e. the loops of (s, eta := M s)."""
+    return loops_project(s, apply_M(s, U, kappa, mu, tb), U, kappa, mu, momenta, tb, t0, t1)

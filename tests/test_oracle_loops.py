@@ -222,3 +222,36 @@ def test_binary_storage_fig2(orc):
     assert np.allclose(files.sum(axis=0) / 13, ps[:13].mean(axis=0), atol=1e-14)      # nothing is lost
     # O(log2 N) files
     assert [orc.binary_nfiles(n) for n in (1, 2, 3, 4, 7, 8, 500, 1023)] == [1, 2, 2, 3, 3, 4, 9, 10]
+
+
+def test_explicit_dw_variant(orc):
+    """Row f3 / reading 5: with D_W applied explicitly the f = 1 loops differ from the eta-based ones by the
+    bilinears of gamma5 (eta - M s); they coincide when M s = eta."""
+    dims = (4, 2, 2, 4)
+    k, mu = 0.156, 0.01
+    U = inputs.gauge_field(dims, 0.3, 11)
+    s = inputs.random_spinor(dims, 12)
+    eta = inputs.random_spinor(dims, 13)
+    mom = inputs.momentum_list(1)
+    a = orc.loops_project(s, eta, U, k, mu, mom, -1)
+    b = orc.loops_project_explicit(s, U, k, mu, mom, -1)
+    assert np.allclose(a[0], b[0], atol=1e-13)                      # f = 0 does not see eta
+    # ultra-local f = 1 difference = sum_x e^{ipx} s^dag g5 Gamma_n g5 (eta - M s), written out with numpy
+    r = eta - orc.apply_M(s, U, k, mu, -1)
+    g5 = orc.gamma(4)
+    lx, ly, lz, lt = dims
+    for n in (0, 3, 9, 15):
+        X = g5 @ orc.Gamma(n) @ g5
+        site = np.einsum("tzyxac,ab,tzyxbc->tzyx", s.conj(), X, r)
+        for kk, (px, py, pz) in enumerate(mom):
+            ph = np.exp(2j * np.pi * (px * np.arange(lx)[None, None, :] / lx + py * np.arange(ly)[None, :, None] / ly
+                                      + pz * np.arange(lz)[:, None, None] / lz))
+            ref = (site * ph[None]).sum(axis=(1, 2, 3))
+            assert np.allclose(a[1, n, kk] - b[1, n, kk], ref, atol=1e-12), (n, kk)
+    # a true solution: both variants agree
+    eta = inputs.z4_source(dims, 5, 0)
+    s_sol, _, tr, st = orc.solve(eta, U, k, mu, 1e-13)
+    assert st == 0
+    a = orc.loops_project(s_sol, eta, U, k, mu, mom, -1)
+    b = orc.loops_project_explicit(s_sol, U, k, mu, mom, -1)
+    assert np.linalg.norm(a - b) <= 1e-10 * np.linalg.norm(a)
