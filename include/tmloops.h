@@ -110,6 +110,13 @@ tm_status loop_contract_project(tm_ctx* ctx, void* d_out, const void* d_s, const
                                 double kappa, double mu, const int* h_momenta, int nmom,
                                 tm_prec acc, void* stream);
 
+/* Row f3 variant (reading 5): the same 160 projected insertions with the generalised one-end trick's
+ * D_W applied EXPLICITLY: g = g5 D_W s = g5 (M s) - 2 i kappa mu s instead of g5 eta - 2 i kappa mu s, i.e. the loops
+ * of (s, eta := M s); it differs from loop_contract_project by the bilinears of g5 (eta - M s) and costs one extra
+ * full operator application (in precision acc, reconstruct-12 for TM_F32, -18 for TM_F64). */
+tm_status loop_contract_project_explicit(tm_ctx* ctx, void* d_out, const void* d_s, double kappa, double mu,
+                                         const int* h_momenta, int nmom, tm_prec acc, void* stream);
+
 /* sec 2.1: L_TSM = (1/N_LP) sum_{r<N_LP} l_r^LP + (1/N_HP) sum_{r<N_HP} (l_r^HP - l_r^LP);
  * the HP sources are the first n_hp of the LP sources.  Z4 noise eta_r[c] = i^k, c = (site*4+spin)*3+col:
  * d_z4 != NULL: packed exponents, byte j of source r holds k[4j+m] in bits 2m..2m+1,

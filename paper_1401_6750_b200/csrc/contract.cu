@@ -504,3 +504,26 @@ extern "C" tm_status loop_contract_project(tm_ctx* ctx, void* d_out, const void*
     TM_TRY(tm_import_launch(ctx, ei, d_eta, acc, st));
     return tm_contract_internal(ctx, d_out, si, ei, kappa, mu, h_momenta, nmom, acc, st);
 }
+
+extern "C" tm_status loop_contract_project_explicit(tm_ctx* ctx, void* d_out, const void* d_s, double kappa, double mu,
+                                                    const int* h_momenta, int nmom, tm_prec acc, void* stream) {
+    if (!ctx || !d_out || !d_s) return tm_fail(ctx, TM_EARG, "loop_contract_project_explicit: null argument");
+    if (acc != TM_F64 && acc != TM_F32) return tm_fail(ctx, TM_EPREC, "loop_contract_project_explicit: acc must be f32 or f64");
+    cudaStream_t st = (cudaStream_t)stream;
+    TM_CUDA(ctx, cudaSetDevice(ctx->device));
+    const size_t pb = tm_parity_bytes(ctx, acc);
+    void *si, *ms;
+    TM_TRY(tm_ws(ctx, WS_CT_S, 2 * pb, &si));
+    TM_TRY(tm_ws(ctx, WS_CT_ETA, 2 * pb, &ms));
+    TM_TRY(tm_import_launch(ctx, si, d_s, acc, st));
+    // ms = M s: out_p = A s_p - kappa D_pq s_q for both parities
+    const tm_recon rc = acc == TM_F64 ? TM_R18 : TM_R12;
+    for (int p = 0; p < 2; p++) {
+        DslashCall k;
+        memset(&k, 0, sizeof(k));
+        k.out = (char*)ms + p * pb; k.in = (const char*)si + (1 - p) * pb; k.x = (const char*)si + p * pb;
+        k.out_parity = p; k.xmode = 2; k.coef = -kappa; k.kappa = kappa; k.mu = mu; k.red_op = RED_NONE;
+        TM_TRY(tm_dslash_launch(ctx, k, acc, rc, st));
+    }
+    return tm_contract_internal(ctx, d_out, si, ms, kappa, mu, h_momenta, nmom, acc, st);
+}

@@ -100,3 +100,22 @@ def test_contract_of_a_solution(orc):
     check_blocks(got, ref, 1e-12)
     # gamma5 insertion at p = 0 summed over t is ||s||^2 (oracle pin (ii), now on the GPU result)
     assert abs(got[0, 15, 0, :].sum() - np.vdot(to_np(s), to_np(s))) <= 1e-10 * np.vdot(to_np(s), to_np(s)).real
+
+
+@pytest.mark.parametrize("acc", ["f64", "f32"])
+def test_contract_explicit_dw_variant(orc, acc):
+    """Row f3 variant: D_W applied explicitly (loops of (s, M s)) vs the oracle's composition."""
+    t = tm()
+    dims = (8, 8, 8, 4)
+    U, s, _ = case(dims, 0.25, 9)
+    k, mu = 0.1563, 0.0055
+    mom = inputs.momentum_list(4)
+    ref = orc.loops_project_explicit(s, U, k, mu, mom, -1)
+    with t.TmContext(dims, -1) as ctx:
+        ctx.tm_load_gauge(U)
+        got = to_np(ctx.loop_contract_project_explicit(s, k, mu, mom, t.PREC[acc]))
+        check_blocks(got, ref, TOL[acc] * (3 if acc == "f32" else 1))      # one more fp32 operator application
+        # and it differs from the eta-based loops unless M s = eta
+        eta = inputs.z4_source(dims, 1, 0)
+        other = to_np(ctx.loop_contract_project(s, eta, k, mu, mom, t.PREC[acc]))
+        assert rel_l2(other[1], got[1]) > 1e-2 and rel_l2(other[0], got[0]) <= 10 * TOL[acc]
