@@ -29,6 +29,8 @@ struct CgScalars {
     int n_ru;          // reliable updates so far
     int x_zero;        // x == 0 by construction (start of a solve / after a reliable update): x is neither read nor zero-filled
     int y_zero;        // y == 0 by construction (no reliable update yet): y is not read
+    int iters_at_ru;   // iteration count at the last reliable update (a reliable update is forced every 100 iterations)
+    int stall;         // consecutive reliable updates that did not halve the true residual while far from the target
     int pause_iter[CG_MAX_PAUSES];   // iteration count at each pause (replayed by the host as a launch plan)
 };
 
@@ -77,7 +79,8 @@ __device__ __forceinline__ void apply_red_op(CgScalars* sc, int op, double s) {
         case RED_WW: sc->ww = s; sc->alpha = sc->gamma / s; break;
         case RED_RR:
             sc->rr = s; sc->iters += 1; sc->x_zero = 0;
-            if (!(s > sc->target2) || !(s > sc->ru2) || sc->iters >= sc->max_iter) sc->done = 1;
+            if (!(s > sc->target2) || !(s > sc->ru2) || sc->iters >= sc->max_iter || sc->iters - sc->iters_at_ru >= 100)
+                sc->done = 1;
             break;
         case RED_ZZ: sc->beta = sc->gamma > 0.0 ? s / sc->gamma : 0.0; sc->gamma = s; break;
         case RED_START:
@@ -87,12 +90,17 @@ __device__ __forceinline__ void apply_red_op(CgScalars* sc, int op, double s) {
             break;
         case RED_RU:
             if (sc->n_ru < CG_MAX_PAUSES) sc->pause_iter[sc->n_ru] = sc->iters;
+            // stagnation: the iterated residual fell by delta (or met the target) but the TRUE residual did not even
+            // halve, twice in a row, while still more than 2x above the target -> the sloppy precision's floor is
+            // reached (e.g. pure fp32 asked for 1e-8); give up instead of iterating to max_iter
+            if (sc->n_ru > 0 && s > 0.25 * sc->rr_true && s > 4.0 * sc->target2) sc->stall += 1; else sc->stall = 0;
             sc->n_ru += 1;
             sc->rr_true = s;
+            sc->iters_at_ru = sc->iters;
             sc->x_zero = 1; sc->y_zero = 0;      // ru_begin folded x into y
             if (!(s == s)) sc->done = 3;
             else if (s <= sc->target2) sc->done = 2;
-            else if (sc->iters >= sc->max_iter) sc->done = 3;
+            else if (sc->iters >= sc->max_iter || sc->stall >= 2) sc->done = 3;
             else { sc->rr = s; sc->ru2 = sc->delta2 * s; sc->done = 0; }
             break;
         default: if (op >= RED_SLOT0) sc->slot[op - RED_SLOT0] = s; break;
