@@ -68,6 +68,7 @@ def test_c2_dslash_all_precisions_and_fp32_solve(orc):
         print("c2 fp32/fp32:", info, true)
         assert true <= 5e-7 and abs(info["true_resid"] - true) <= 2e-7, (true, info)
         assert info["status"] == t.TM_ENOCONV or true <= 1e-8
+        assert info["iters"] < 1000, info          # stagnation is detected, the solver does not run to max_iter
         s, info = ctx.tm_cg_solve(eta, c["kappa"], c["mu"], "f32", "f64", 12, 1e-8, 5000)
         true = orc.true_residual(to_np(s), to_np(eta), U_h, c["kappa"], c["mu"], -1)
         assert true <= 1e-8 and abs(info["true_resid"] - true) <= 5e-10, (true, info)
