@@ -16,6 +16,7 @@
 //   (1 + s g_mu) psi = (u, s B^dag u),  u = psi_up + s B psi_low.
 #include "kernels.h"
 #include "su3.cuh"
+#include "contract.cuh"      // P2<float>: packed complex-pair arithmetic (FFMA2 / FADD2)
 
 template <typename F> struct DslashArgs {
     const void* in;
@@ -539,6 +540,230 @@ __global__ void __launch_bounds__(128, MINB) dslash16_kernel(DslashArgs<float> A
     if (A.red_op != RED_NONE) block_partial_at(nrm, A.partials, bx, sm);
 }
 
+// =====================================================================================================
+// fp32 storage, reconstruct-12, packed arithmetic: one complex number per 64-bit register pair, Blackwell FFMA2 /
+// FADD2 (fma.rn.f32x2 with a broadcast real scalar: one issue slot per complex-times-real FMA).  Same mathematics
+// and data layout as dslash_kernel<float, 12>; ~20 % fewer instructions per site (the grouped launches of this
+// kernel are bound by instruction issue and board power, not by HBM).
+typedef P2<float>::T c2;     // (re, im)
+
+template <int MU, int FWD, int DAGGER>
+__device__ __forceinline__ void hop32(const float* in, const float* gauge, size_t Vh, int par_out, size_t h_out,
+                                      size_t h_nb, float bsign, bool wrap, c2* acc) {
+    constexpr float SGN = (float)((FWD ? -1 : 1) * (DAGGER ? -1 : 1));      // forward: (1 - g), backward: (1 + g)
+    c2 p[12];
+    {
+        const float4* f = reinterpret_cast<const float4*>(in) + h_nb;
+#pragma unroll
+        for (int k = 0; k < 6; k++) {
+            const float4 q = __ldg(f + (size_t)k * Vh);
+            p[2 * k] = P2<float>::make(q.x, q.y);
+            p[2 * k + 1] = P2<float>::make(q.z, q.w);
+        }
+    }
+    float U[18];
+    {
+        const size_t hl = FWD ? h_out : h_nb;
+        const int pl = FWD ? par_out : 1 - par_out;
+        const float4* g = reinterpret_cast<const float4*>(gauge) + ((size_t)(pl * 4 + MU) * 3 * Vh + hl);
+#pragma unroll
+        for (int k = 0; k < 3; k++) {
+            const float4 q = __ldcs(g + (size_t)k * Vh);
+            U[4 * k] = q.x; U[4 * k + 1] = q.y; U[4 * k + 2] = q.z; U[4 * k + 3] = q.w;
+        }
+#pragma unroll
+        for (int c = 0; c < 3; c++) {          // row 2 = conj(row0 x row1)
+            const int i = (c + 1) % 3, j = (c + 2) % 3;
+            const float ar = U[2 * i], ai = U[2 * i + 1], br = U[6 + 2 * j], bi = U[6 + 2 * j + 1];
+            const float cr = U[2 * j], ci = U[2 * j + 1], dr = U[6 + 2 * i], di = U[6 + 2 * i + 1];
+            float re = ar * br; re -= ai * bi; re -= cr * dr; re += ci * di;
+            float im = ar * bi; im += ai * br; im -= cr * di; im -= ci * dr;
+            U[12 + 2 * c] = re;
+            U[12 + 2 * c + 1] = -im;
+        }
+    }
+    // half-spinor u = psi_up + s B_mu psi_low (B_x = -i s_x, B_y = -i s_y, B_z = -i s_z, B_t = 1)
+    c2 u[6];
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        const c2 p0 = p[c], p1 = p[3 + c], p2 = p[6 + c], p3 = p[9 + c];
+        if (MU == 0) {          // (-i psi3, -i psi2)
+            u[c] = P2<float>::fma_s(-SGN, times_i<float>(p3), p0);
+            u[3 + c] = P2<float>::fma_s(-SGN, times_i<float>(p2), p1);
+        } else if (MU == 1) {   // (-psi3, psi2)
+            u[c] = P2<float>::fma_s(-SGN, p3, p0);
+            u[3 + c] = P2<float>::fma_s(SGN, p2, p1);
+        } else if (MU == 2) {   // (-i psi2, i psi3)
+            u[c] = P2<float>::fma_s(-SGN, times_i<float>(p2), p0);
+            u[3 + c] = P2<float>::fma_s(SGN, times_i<float>(p3), p1);
+        } else {                // (psi2, psi3)
+            u[c] = P2<float>::fma_s(SGN, p2, p0);
+            u[3 + c] = P2<float>::fma_s(SGN, p3, p1);
+        }
+    }
+    if (MU == 3 && wrap) {
+#pragma unroll
+        for (int i = 0; i < 6; i++) u[i] = P2<float>::mul_s(bsign, u[i]);
+    }
+    // v = U u (forward) or U^dag u (backward): (ur + i ui) x = ur x + ui (i x), accumulators updated round-robin
+    c2 v[6];
+#pragma unroll
+    for (int i = 0; i < 6; i++) v[i] = P2<float>::make(0.f, 0.f);
+#pragma unroll
+    for (int b = 0; b < 3; b++) {
+        const c2 ib0 = times_i<float>(u[b]), ib1 = times_i<float>(u[3 + b]);
+        float ur[3], ui[3];
+#pragma unroll
+        for (int a = 0; a < 3; a++) {
+            ur[a] = FWD ? U[(a * 3 + b) * 2] : U[(b * 3 + a) * 2];
+            ui[a] = FWD ? U[(a * 3 + b) * 2 + 1] : -U[(b * 3 + a) * 2 + 1];
+        }
+#pragma unroll
+        for (int a = 0; a < 3; a++) {
+            v[a] = P2<float>::fma_s(ur[a], u[b], v[a]);
+            v[3 + a] = P2<float>::fma_s(ur[a], u[3 + b], v[3 + a]);
+        }
+#pragma unroll
+        for (int a = 0; a < 3; a++) {
+            v[a] = P2<float>::fma_s(ui[a], ib0, v[a]);
+            v[3 + a] = P2<float>::fma_s(ui[a], ib1, v[3 + a]);
+        }
+    }
+    // acc_up += v ; acc_low += s B_mu^dag v
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        const c2 v0 = v[c], v1 = v[3 + c];
+        acc[c] = P2<float>::add(acc[c], v0);
+        acc[3 + c] = P2<float>::add(acc[3 + c], v1);
+        if (MU == 0) {          // (i v1, i v0)
+            acc[6 + c] = P2<float>::fma_s(SGN, times_i<float>(v1), acc[6 + c]);
+            acc[9 + c] = P2<float>::fma_s(SGN, times_i<float>(v0), acc[9 + c]);
+        } else if (MU == 1) {   // (v1, -v0)
+            acc[6 + c] = P2<float>::fma_s(SGN, v1, acc[6 + c]);
+            acc[9 + c] = P2<float>::fma_s(-SGN, v0, acc[9 + c]);
+        } else if (MU == 2) {   // (i v0, -i v1)
+            acc[6 + c] = P2<float>::fma_s(SGN, times_i<float>(v0), acc[6 + c]);
+            acc[9 + c] = P2<float>::fma_s(-SGN, times_i<float>(v1), acc[9 + c]);
+        } else {                // (v0, v1)
+            acc[6 + c] = P2<float>::fma_s(SGN, v0, acc[6 + c]);
+            acc[9 + c] = P2<float>::fma_s(SGN, v1, acc[9 + c]);
+        }
+    }
+}
+
+template <int DAGGER>
+__global__ void __launch_bounds__(128, 4) dslash32_kernel(DslashArgs<float> A) {
+    __shared__ double sm[32];
+    int bx = blockIdx.x, src = 0;
+    if (A.nb > 1) { src = bx & (A.nb - 1); bx >>= (31 - __clz(A.nb)); }   // grouped sources: see DslashArgs::nb
+    A.in = (const char*)A.in + src * A.mul_in * A.fstride;
+    A.out = (char*)A.out + src * A.mul_out * A.fstride;
+    if (A.x) A.x = (const char*)A.x + src * A.mul_x * A.fstride;
+    A.sc += src;
+    A.partials += src * TM_PSTRIDE;
+    if (guard_skip(A.sc, A.guard)) return;
+    const Geom& g = A.g;
+    const int h = bx * blockDim.x + threadIdx.x;
+    double nrm = 0.0;
+    if (h < g.Vh) {
+        const int xh = h % g.Xh;
+        int q = h / g.Xh;
+        const int y = q % g.X1; q /= g.X1;
+        const int z = q % g.X2;
+        const int t = q / g.X2;
+        const int odd = (y + z + t + A.parity) & 1;
+        const float* in = (const float*)A.in;
+        const float* gauge = (const float*)A.gauge;
+        const size_t Vh = g.Vh;
+        c2 acc[12];
+#pragma unroll
+        for (int i = 0; i < 12; i++) acc[i] = P2<float>::make(0.f, 0.f);
+        const int row = h - xh;
+        const int xp = row + (odd ? (xh + 1 == g.Xh ? 0 : xh + 1) : xh);
+        const int xm = row + (odd ? xh : (xh == 0 ? g.Xh - 1 : xh - 1));
+        const int yp = (y + 1 == g.X1) ? h - (g.X1 - 1) * g.s1 : h + g.s1;
+        const int ym = (y == 0) ? h + (g.X1 - 1) * g.s1 : h - g.s1;
+        const int zp = (z + 1 == g.X2) ? h - (g.X2 - 1) * g.s2 : h + g.s2;
+        const int zm = (z == 0) ? h + (g.X2 - 1) * g.s2 : h - g.s2;
+        const bool wp = (t + 1 == g.X3), wm = (t == 0);
+        const int tp = wp ? h - (g.X3 - 1) * g.s3 : h + g.s3;
+        const int tm = wm ? h + (g.X3 - 1) * g.s3 : h - g.s3;
+        const int par = A.parity;
+        hop32<0, 1, DAGGER>(in, gauge, Vh, par, h, xp, 1.f, false, acc);
+        hop32<0, 0, DAGGER>(in, gauge, Vh, par, h, xm, 1.f, false, acc);
+        hop32<1, 1, DAGGER>(in, gauge, Vh, par, h, yp, 1.f, false, acc);
+        hop32<1, 0, DAGGER>(in, gauge, Vh, par, h, ym, 1.f, false, acc);
+        hop32<2, 1, DAGGER>(in, gauge, Vh, par, h, zp, 1.f, false, acc);
+        hop32<2, 0, DAGGER>(in, gauge, Vh, par, h, zm, 1.f, false, acc);
+        hop32<3, 1, DAGGER>(in, gauge, Vh, par, h, tp, A.tb, wp, acc);
+        hop32<3, 0, DAGGER>(in, gauge, Vh, par, h, tm, A.tb, wm, acc);
+        // epilogue: res = c acc (+ x | + A x, A = 1 + i a g5), optional A^-1 = (1 - i a g5)/(1 + a^2), store, norm
+        const float cf = A.c, a = A.a;
+        if (A.xmode) {
+            const float4* xf = reinterpret_cast<const float4*>(A.x) + h;
+#pragma unroll
+            for (int k = 0; k < 6; k++) {
+                const float4 q4 = __ldg(xf + (size_t)k * Vh);
+                const c2 xa = P2<float>::make(q4.x, q4.y), xb = P2<float>::make(q4.z, q4.w);
+                c2 ra = P2<float>::fma_s(cf, acc[2 * k], xa), rb = P2<float>::fma_s(cf, acc[2 * k + 1], xb);
+                if (A.xmode == 2) {             // + i a x on the upper spins (pairs 0..5), - i a x on the lower ones
+                    const float sa = k < 3 ? a : -a;
+                    ra = P2<float>::fma_s(sa, times_i<float>(xa), ra);
+                    rb = P2<float>::fma_s(sa, times_i<float>(xb), rb);
+                }
+                acc[2 * k] = ra; acc[2 * k + 1] = rb;
+            }
+        } else {
+#pragma unroll
+            for (int i = 0; i < 12; i++) acc[i] = P2<float>::mul_s(cf, acc[i]);
+        }
+        if (A.post) {
+            const float n = 1.f / (1.f + a * a);
+#pragma unroll
+            for (int i = 0; i < 12; i++) {
+                const float sa = i < 6 ? -a : a;            // (1 - i a) on the upper spins, (1 + i a) on the lower ones
+                acc[i] = P2<float>::mul_s(n, P2<float>::fma_s(sa, times_i<float>(acc[i]), acc[i]));
+            }
+        }
+        float4* of = reinterpret_cast<float4*>(A.out) + h;
+        float n2 = 0.f;
+#pragma unroll
+        for (int k = 0; k < 6; k++) {
+            float4 o;
+            P2<float>::get(acc[2 * k], o.x, o.y);
+            P2<float>::get(acc[2 * k + 1], o.z, o.w);
+            of[(size_t)k * Vh] = o;
+            n2 = fmaf(o.x, o.x, n2); n2 = fmaf(o.y, o.y, n2); n2 = fmaf(o.z, o.z, n2); n2 = fmaf(o.w, o.w, n2);
+        }
+        nrm = (double)n2;
+    }
+    if (A.red_op != RED_NONE) block_partial_at(nrm, A.partials, bx, sm);
+}
+
+static tm_status launch32(tm_ctx* ctx, const DslashCall& c, const void* gauge, cudaStream_t st) {
+    DslashArgs<float> A;
+    A.in = c.in; A.x = c.x; A.out = c.out; A.gauge = gauge;
+    A.g = tm_geom(ctx);
+    A.parity = c.out_parity;
+    A.dsign = c.dagger ? -1.f : 1.f;
+    A.tb = (float)ctx->tb;
+    A.a = (float)(2.0 * c.kappa * c.mu * (c.dagger ? -1.0 : 1.0));
+    A.c = (float)c.coef;
+    A.xmode = c.xmode; A.post = c.post; A.red_op = c.red_op;
+    A.partials = ctx->d_partials; A.counter = ctx->d_counter; A.sc = ctx->d_scal;
+    A.guard = c.guard;
+    A.nb = ctx->nb > 1 ? ctx->nb : 1; A.fstride = ctx->Vh * 24 * sizeof(float);
+    A.mul_in = c.mul_in ? c.mul_in : 1; A.mul_x = c.mul_x ? c.mul_x : 1; A.mul_out = c.mul_out ? c.mul_out : 1;
+    const int block = 128;
+    const int tiles = (int)((ctx->Vh + block - 1) / block);
+    const int grid = tiles * A.nb;
+    if (c.dagger) dslash32_kernel<1><<<grid, block, 0, st>>>(A);
+    else          dslash32_kernel<0><<<grid, block, 0, st>>>(A);
+    TM_LAUNCH_CHECK(ctx, "dslash32_kernel");
+    if (c.red_op != RED_NONE) TM_TRY(tm_reduce_finish(ctx, (unsigned)tiles, c.red_op, c.guard, st));
+    return TM_OK;
+}
+
 template <typename S, int R>
 static tm_status launch_t(tm_ctx* ctx, const DslashCall& c, const void* gauge, cudaStream_t st) {
     typedef typename Prec<S>::F F;
@@ -597,7 +822,7 @@ tm_status tm_dslash_launch(tm_ctx* ctx, const DslashCall& c, tm_prec prec, tm_re
     const bool r12 = (recon == TM_R12);
     switch (prec) {
         case TM_F64:  return r12 ? launch_t<double, 12>(ctx, c, gauge, st) : launch_t<double, 18>(ctx, c, gauge, st);
-        case TM_F32:  return r12 ? launch_t<float, 12>(ctx, c, gauge, st) : launch_t<float, 18>(ctx, c, gauge, st);
+        case TM_F32:  return r12 ? launch32(ctx, c, gauge, st) : launch_t<float, 18>(ctx, c, gauge, st);
         case TM_F16:  return r12 ? launch16<__half>(ctx, c, gauge, st) : launch_t<__half, 18>(ctx, c, gauge, st);
         case TM_BF16: return r12 ? launch16<__nv_bfloat16>(ctx, c, gauge, st)
                                  : launch_t<__nv_bfloat16, 18>(ctx, c, gauge, st);
