@@ -90,3 +90,27 @@ def test_contract_c4_sampled_timeslices(orc, c4, acc, tol):
             for name, sl in (("local", slice(0, 16)), ("deriv", slice(16, 80))):
                 e = rel_l2(got[f, sl, :, ts], ref[f, sl])
                 assert e <= tol, (acc, ts, f, name, e)
+
+
+def test_tsm_c4_grouped_launches(orc, c4, monkeypatch):
+    """The launch configuration bench.py times: sources solved 8 per launch on two lanes.  Per-source arrays must be
+    bit-identical to the one-source-per-launch path, and a grouped solution must pass the oracle's residual check."""
+    t, ctx, U_h, eta = c4
+    mom = inputs.momentum_list(9)
+    n_lp, n_hp = 16, 8
+    monkeypatch.delenv("TMLOOPS_GROUP", raising=False)
+    out_g, ps_g, info_g = ctx.tsm_estimate(n_lp, n_hp, C4["kappa"], C4["mu"], mom, LP, HP, t.TM_F32, t.TM_F64,
+                                           seed=C4["src_seed"], per_source=True)
+    monkeypatch.setenv("TMLOOPS_GROUP", "1")
+    out_1, ps_1, info_1 = ctx.tsm_estimate(n_lp, n_hp, C4["kappa"], C4["mu"], mom, LP, HP, t.TM_F32, t.TM_F64,
+                                           seed=C4["src_seed"], per_source=True)
+    monkeypatch.delenv("TMLOOPS_GROUP", raising=False)
+    assert bool((ps_g == ps_1).all())
+    assert info_g["launches"] * 4 < info_1["launches"]
+    assert info_g["worst_resid_lp"] <= LP["rho"] and info_g["worst_resid_hp"] <= HP["rho"]
+    assert rel_l2(to_np(out_g), to_np(out_1)) <= 1e-13
+    # source 0 of the run is the fixture's eta (same seed, stream 0): its LP loops = loops of a single LP solve
+    s, _ = ctx.tm_cg_solve(eta, C4["kappa"], C4["mu"], **LP)
+    assert orc.true_residual(to_np(s), to_np(eta), U_h, C4["kappa"], C4["mu"], -1) <= LP["rho"]
+    single = ctx.loop_contract_project(s, eta, C4["kappa"], C4["mu"], mom, t.TM_F32)
+    assert rel_l2(to_np(ps_g[0]), to_np(single)) <= 1e-5
