@@ -64,7 +64,8 @@ extern "C" tm_status tm_create(tm_ctx** out, const int dims[4], int t_boundary, 
         return TM_EARG;
     }
     const size_t V = (size_t)dims[0] * dims[1] * dims[2] * dims[3];
-    if (V / 2 > 0x3fffffffULL) { snprintf(g_last_error, sizeof(g_last_error), "tm_create: lattice too large"); return TM_EDIM; }
+    // one reduction partial per 128-site Dslash CTA must fit a source's slot of the partials buffer (TM_PSTRIDE)
+    if (V / 2 > (size_t)128 * TM_PSTRIDE) { snprintf(g_last_error, sizeof(g_last_error), "tm_create: lattice too large (more than %zu sites)", (size_t)256 * TM_PSTRIDE); return TM_EDIM; }
     int ndev = 0;
     cudaError_t e = cudaGetDeviceCount(&ndev);
     if (e != cudaSuccess || ndev <= 0 || device < 0 || device >= ndev) {

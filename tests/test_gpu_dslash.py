@@ -126,6 +126,9 @@ def test_import_export_roundtrip_and_errors():
         t.TmContext((3, 4, 4, 4))
     with pytest.raises(t.TmError):
         t.TmContext((4, 4, 4, 4), t_boundary=0)
+    with pytest.raises(t.TmError) as e:                       # maximum size: rejected before anything is allocated
+        t.TmContext((128, 128, 128, 256))
+    assert e.value.status == t.TM_EDIM
 
 
 @pytest.mark.parametrize("prec", ["f64", "f32", "f16", "bf16"])
