@@ -192,3 +192,21 @@ def loops_project_explicit(s, U, kappa, mu, momenta, tb=-1, t0=0, t1=None) -> np
     """Variant of reading 5: the generalised one-end trick with D_W applied explicitly,
     l[1] = s^dag g5 X g5 D_W s with g5 D_W s = g5 (M s) - 2 i kappa mu s, i.e. the loops of (s, eta := M s)."""
     return loops_project(s, apply_M(s, U, kappa, mu, tb), U, kappa, mu, momenta, tb, t0, t1)
+
+
+def loops_project_sym(s, eta, U, kappa, mu, momenta, tb=-1, t0=0, t1=None) -> np.ndarray:
+    """Variant of reading 4 (row f3): one-derivative insertions with the symmetrised derivative
+    1/2 [s^dag g5 G (D psi) - (D s)^dag g5 G psi]; ultra-local entries as in loops_project."""
+    s, p_s = _c(s)
+    eta, p_eta = _c(eta)
+    U, p_U = _c(U)
+    T = s.shape[0]
+    if t1 is None:
+        t1 = T
+    mom = np.ascontiguousarray(momenta, dtype=np.int32).reshape(-1, 3)
+    out = np.zeros((2, 80, len(mom), T), dtype=np.complex128)
+    lib().orc_loops_project_sym(out.ctypes.data_as(ctypes.c_void_p), p_s, p_eta, p_U,
+                                _dims(dims_of(s)), ctypes.c_int(tb), ctypes.c_double(kappa),
+                                ctypes.c_double(mu), mom.ctypes.data_as(ctypes.c_void_p),
+                                ctypes.c_int(len(mom)), ctypes.c_int(t0), ctypes.c_int(t1))
+    return out

@@ -336,6 +336,27 @@ static void loops_at_site(cplx out[160], const cplx *s, const cplx *g, const cpl
     }
 }
 
+/* Variant of reading 4: the left-right symmetrised derivative,
+ *   out[f*80 + 16+16m+n] = 1/2 [ s^dag g5 Gamma_n (D_m psi) - (D_m s)^dag g5 Gamma_n psi ],  psi = s (f = 0) | g (f = 1);
+ * the ultra-local entries are those of loops_at_site.  Written from the definition: D_m applied to s as well. */
+static void loops_at_site_sym(cplx out[160], const cplx *s, const cplx *g, const cplx *U,
+                              const int *dims, int tb, long x, cplx g5G[16][4][4])
+{
+    const cplx *fam[2] = { s, g };
+    for (int f = 0; f < 2; f++) {
+        for (int n = 0; n < 16; n++)
+            out[f * 80 + n] = bilinear(s + x * 12, g5G[n], fam[f] + x * 12);
+        for (int m = 0; m < 4; m++) {
+            cplx dpsi[12], ds[12];
+            cov_deriv_site(dpsi, fam[f], U, dims, tb, x, m);
+            cov_deriv_site(ds, s, U, dims, tb, x, m);
+            for (int n = 0; n < 16; n++)
+                out[f * 80 + 16 + 16 * m + n] = 0.5 * (bilinear(s + x * 12, g5G[n], dpsi)
+                                                       - bilinear(ds, g5G[n], fam[f] + x * 12));
+        }
+    }
+}
+
 static void make_g5G(cplx g5G[16][4][4])
 {
     cplx g5[4][4];
@@ -365,9 +386,9 @@ void orc_loops_sites(cplx *out, const cplx *s, const cplx *eta, const cplx *U, c
  *   out[((f*80+i)*nmom + k)*T + t] = sum_{x,y,z} exp(+2 pi i (px x/Lx + py y/Ly + pz z/Lz)) l_{f,i}(x,y,z,t)
  * by the direct sum.  momenta: int [nmom][3] = (px,py,pz).  Entries of out for
  * other t are left untouched. */
-void orc_loops_project(cplx *out, const cplx *s, const cplx *eta, const cplx *U, const int *dims,
-                       int tb, double kappa, double mu, const int *momenta, int nmom,
-                       int t0, int t1)
+static void loops_project_impl(cplx *out, const cplx *s, const cplx *eta, const cplx *U, const int *dims,
+                               int tb, double kappa, double mu, const int *momenta, int nmom,
+                               int t0, int t1, int sym)
 {
     const int Lx = dims[0], Ly = dims[1], Lz = dims[2], T = dims[3];
     const long V = (long)Lx * Ly * Lz * T, V3 = (long)Lx * Ly * Lz;
@@ -378,7 +399,10 @@ void orc_loops_project(cplx *out, const cplx *s, const cplx *eta, const cplx *U,
     make_g(g, s, eta, V, kappa, mu);
     for (int t = t0; t < t1; t++) {
 #pragma omp parallel for schedule(static)
-        for (long k = 0; k < V3; k++) loops_at_site(l + k * 160, s, g, U, dims, tb, (long)t * V3 + k, g5G);
+        for (long k = 0; k < V3; k++) {
+            if (sym) loops_at_site_sym(l + k * 160, s, g, U, dims, tb, (long)t * V3 + k, g5G);
+            else     loops_at_site(l + k * 160, s, g, U, dims, tb, (long)t * V3 + k, g5G);
+        }
 #pragma omp parallel for schedule(dynamic, 1)
         for (int q = 0; q < nmom; q++) {
             cplx acc[160];
@@ -397,6 +421,21 @@ void orc_loops_project(cplx *out, const cplx *s, const cplx *eta, const cplx *U,
         }
     }
     free(g); free(l);
+}
+
+void orc_loops_project(cplx *out, const cplx *s, const cplx *eta, const cplx *U, const int *dims,
+                       int tb, double kappa, double mu, const int *momenta, int nmom,
+                       int t0, int t1)
+{
+    loops_project_impl(out, s, eta, U, dims, tb, kappa, mu, momenta, nmom, t0, t1, 0);
+}
+
+/* same with the symmetrised derivative (loops_at_site_sym) */
+void orc_loops_project_sym(cplx *out, const cplx *s, const cplx *eta, const cplx *U, const int *dims,
+                           int tb, double kappa, double mu, const int *momenta, int nmom,
+                           int t0, int t1)
+{
+    loops_project_impl(out, s, eta, U, dims, tb, kappa, mu, momenta, nmom, t0, t1, 1);
 }
 
 /* sec 2.1 + reading 14:

@@ -255,3 +255,46 @@ def test_explicit_dw_variant(orc):
     a = orc.loops_project(s_sol, eta, U, k, mu, mom, -1)
     b = orc.loops_project_explicit(s_sol, U, k, mu, mom, -1)
     assert np.linalg.norm(a - b) <= 1e-10 * np.linalg.norm(a)
+
+
+def test_symmetrised_derivative_variant(orc):
+    """Row f3 / reading 4: D<-> = (D-> - D<-)/2.  Pins: summation by parts (D_mu is anti-Hermitian, so at p = 0 the
+    symmetrised and the right-acting loops coincide); for f = 0 and Hermitian g5 Gamma_n the symmetrised insertion
+    is i Im of the right-acting one at every site, hence its p = 0 projection is purely imaginary; gauge invariance."""
+    dims = (4, 2, 2, 4)
+    k, mu = 0.156, 0.01
+    U = inputs.gauge_field(dims, 0.3, 21)
+    s = inputs.random_spinor(dims, 22)
+    eta = inputs.random_spinor(dims, 23)
+    mom = inputs.momentum_list(1)
+    a = orc.loops_project(s, eta, U, k, mu, mom, -1)
+    b = orc.loops_project_sym(s, eta, U, k, mu, mom, -1)
+    assert np.allclose(a[:, :16], b[:, :16], atol=1e-13)                      # ultra-local entries untouched
+    # p = 0 (first momentum of the list), summed over t: D anti-Hermitian => sum_x (D s)^dag X psi = - sum_x s^dag X D psi
+    assert tuple(mom[0]) == (0, 0, 0)
+    assert np.allclose(a[:, 16:, 0].sum(axis=-1), b[:, 16:, 0].sum(axis=-1), atol=1e-11)
+    assert np.abs(a[:, 16:] - b[:, 16:]).max() > 1e-3                          # but they differ mode by mode
+    # f = 0, Hermitian g5 Gamma_n (n in {0, 7, 11, 13, 14, 15}): l_sym(x) = i Im l(x); at p = 0 per timeslice: purely imaginary
+    for n in (0, 7, 11, 13, 14, 15):
+        M = orc.gamma(4) @ orc.Gamma(n)
+        assert np.allclose(M, M.conj().T)
+        for m in range(4):
+            i = 16 + 16 * m + n
+            assert np.allclose(b[0, i, 0].real, 0, atol=1e-11)
+            assert np.allclose(b[0, i, 0].imag, a[0, i, 0].imag, atol=1e-11)
+    # gauge invariance under a random g(x) applied to (U, s, eta)
+    rng = np.random.default_rng(5)
+    lt, lz, ly, lx = s.shape[:4]
+    h = rng.normal(size=(lt, lz, ly, lx, 3, 3)) + 1j * rng.normal(size=(lt, lz, ly, lx, 3, 3))
+    q, _ = np.linalg.qr(h)
+    q = q / np.linalg.det(q)[..., None, None] ** (1 / 3)
+    Ug = np.empty_like(U)
+    shifts = [(3, -1), (2, -1), (1, -1), (0, -1)]                              # x+mu for mu = x, y, z, t
+    for m in range(4):
+        ax, sh = shifts[m]
+        Ug[..., m, :, :] = q @ U[..., m, :, :] @ np.roll(q, sh, axis=ax).conj().swapaxes(-1, -2)
+    sg = np.einsum("...ab,...sb->...sa", q, s)
+    eg = np.einsum("...ab,...sb->...sa", q, eta)
+    # antiperiodic time boundary is a property of the fields, not of g(x): g is periodic, so the loops are invariant
+    c = orc.loops_project_sym(sg, eg, Ug, k, mu, mom, -1)
+    assert np.linalg.norm(c - b) <= 1e-11 * np.linalg.norm(b)
