@@ -117,6 +117,14 @@ tm_status loop_contract_project(tm_ctx* ctx, void* d_out, const void* d_s, const
 tm_status loop_contract_project_explicit(tm_ctx* ctx, void* d_out, const void* d_s, double kappa, double mu,
                                          const int* h_momenta, int nmom, tm_prec acc, void* stream);
 
+/* Row f3 variant (reading 4): the same output with the left-right SYMMETRISED derivative in the 128
+ * one-derivative insertions, l[f][16+16m+n] = 1/2 [ s^dag g5 G_n (D_m psi) - (D_m s)^dag g5 G_n psi ] (psi = s | g);
+ * ultra-local entries as in loop_contract_project.  Obtained from the same primitive with the arguments swapped
+ * (two contraction passes + a small assembly kernel); h_momenta must contain -p for every p (TM_EARG otherwise). */
+tm_status loop_contract_project_sym(tm_ctx* ctx, void* d_out, const void* d_s, const void* d_eta,
+                                    double kappa, double mu, const int* h_momenta, int nmom,
+                                    tm_prec acc, void* stream);
+
 /* sec 2.1: L_TSM = (1/N_LP) sum_{r<N_LP} l_r^LP + (1/N_HP) sum_{r<N_HP} (l_r^HP - l_r^LP);
  * the HP sources are the first n_hp of the LP sources.  Z4 noise eta_r[c] = i^k, c = (site*4+spin)*3+col:
  * d_z4 != NULL: packed exponents, byte j of source r holds k[4j+m] in bits 2m..2m+1,

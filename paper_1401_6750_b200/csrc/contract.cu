@@ -527,3 +527,106 @@ extern "C" tm_status loop_contract_project_explicit(tm_ctx* ctx, void* d_out, co
     }
     return tm_contract_internal(ctx, d_out, si, ms, kappa, mu, h_momenta, nmom, acc, st);
 }
+
+// ------------------------------------------------------------------ row f3 variant: symmetrised derivative
+// l_sym[f][16+16m+n] = 1/2 [ s^dag g5 G_n (D_m psi) - (D_m s)^dag g5 G_n psi ],  psi = s | g.
+// The second term is a relabeling of the same primitive: with (g5 G_n)^dag = eta_n g5 G_n and g5 G_n g5 = eps_n G_n,
+//   (D s)^dag g5 G_n s = eta_n conj( s^dag g5 G_n D s )                                  -> A[0] of prim(s, eta)
+//   (D s)^dag g5 G_n g = eta_n conj( eps_n (B[1] + 2 i kappa mu B[0]) + 2 i kappa mu A[0] ),  B = prim(eta, s)
+// site by site, i.e. after projection the same expressions with p -> -p inside the conj (the momentum list must be
+// closed under p -> -p).  Two contraction passes + this assembly; the ultra-local entries are A's.
+__global__ void sym_assemble_kernel(double2* __restrict__ out, const double2* __restrict__ A, const double2* __restrict__ B,
+                                    const int* __restrict__ negidx, unsigned eta_neg, unsigned eps_neg, double twokmu,
+                                    int nmom, int T) {
+    const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const size_t per_f = (size_t)80 * nmom * T;
+    if (idx >= 2 * per_f) return;
+    const int f = (int)(idx / per_f);
+    size_t r = idx % per_f;
+    const int i = (int)(r / ((size_t)nmom * T));
+    r %= (size_t)nmom * T;
+    const int k = (int)(r / T), t = (int)(r % T);
+    if (i < 16) { out[idx] = A[idx]; return; }
+    const int n = (i - 16) & 15;
+    const double es = (eta_neg >> n) & 1u ? -1.0 : 1.0, ps = (eps_neg >> n) & 1u ? -1.0 : 1.0;
+    const size_t at_neg = ((size_t)i * nmom + negidx[k]) * T + t;         // entry (f = 0, i, -p_k, t)
+    const double2 a0n = A[at_neg];
+    double2 y;                                                              // the bracket of the second term at -p
+    if (f == 0) y = a0n;
+    else {
+        const double2 b0 = B[at_neg], b1 = B[per_f + at_neg];
+        y.x = ps * (b1.x - twokmu * b0.y) - twokmu * a0n.y;
+        y.y = ps * (b1.y + twokmu * b0.x) + twokmu * a0n.x;
+    }
+    const double2 a = A[idx];
+    out[idx] = make_double2(0.5 * (a.x - es * y.x), 0.5 * (a.y + es * y.y));
+}
+
+extern "C" tm_status loop_contract_project_sym(tm_ctx* ctx, void* d_out, const void* d_s, const void* d_eta,
+                                               double kappa, double mu, const int* h_momenta, int nmom,
+                                               tm_prec acc, void* stream) {
+    if (!ctx || !d_out || !d_s || !d_eta) return tm_fail(ctx, TM_EARG, "loop_contract_project_sym: null argument");
+    if (acc != TM_F64 && acc != TM_F32) return tm_fail(ctx, TM_EPREC, "loop_contract_project_sym: acc must be f32 or f64");
+    if (!h_momenta || nmom < 1) return tm_fail(ctx, TM_EARG, "loop_contract_project_sym: need at least one momentum");
+    std::vector<int> neg(nmom, -1);
+    for (int k = 0; k < nmom; k++)
+        for (int j = 0; j < nmom; j++)
+            if (h_momenta[3 * j] == -h_momenta[3 * k] && h_momenta[3 * j + 1] == -h_momenta[3 * k + 1]
+                && h_momenta[3 * j + 2] == -h_momenta[3 * k + 2]) { neg[k] = j; break; }
+    for (int k = 0; k < nmom; k++)
+        if (neg[k] < 0) return tm_fail(ctx, TM_EARG, "loop_contract_project_sym: the momentum list must contain -p for every p");
+    // signs of the Gamma algebra, multiplied out here (independent of the oracle)
+    unsigned eta_neg = 0, eps_neg = 0;
+    {
+        const cd I(0, 1);
+        cd sig[4][2][2] = {{{0, 1}, {1, 0}}, {{0, -I}, {I, 0}}, {{1, 0}, {0, -1}}, {{1, 0}, {0, 1}}};
+        cd gam[4][4][4], g5[4][4];
+        memset(gam, 0, sizeof(gam));
+        for (int m = 0; m < 4; m++)
+            for (int i = 0; i < 2; i++)
+                for (int j = 0; j < 2; j++) {
+                    const cd Bm = (m < 3) ? -I * sig[m][i][j] : sig[3][i][j];
+                    gam[m][i][2 + j] = Bm;
+                    gam[m][2 + j][i] = std::conj(Bm);
+                }
+        memset(g5, 0, sizeof(g5));
+        for (int i = 0; i < 4; i++) g5[i][i] = 1;
+        for (int m = 0; m < 4; m++) mat4mul(g5, g5, gam[m]);
+        for (int n = 0; n < 16; n++) {
+            cd G[4][4], M[4][4], W[4][4];
+            memset(G, 0, sizeof(G));
+            for (int i = 0; i < 4; i++) G[i][i] = 1;
+            for (int m = 0; m < 4; m++)
+                if ((n >> m) & 1) mat4mul(G, G, gam[m]);
+            mat4mul(M, g5, G);                       // g5 Gamma_n
+            mat4mul(W, M, g5);                       // g5 Gamma_n g5
+            // M^dag = eta M and W = eps G: read the sign off a nonzero entry
+            for (int a = 0; a < 4; a++)
+                for (int b = 0; b < 4; b++) {
+                    if (std::abs(M[a][b]) > 0.5 && std::abs(std::conj(M[b][a]) + M[a][b]) < 1e-12) eta_neg |= 1u << n;
+                    if (std::abs(G[a][b]) > 0.5 && std::abs(W[a][b] + G[a][b]) < 1e-12) eps_neg |= 1u << n;
+                }
+        }
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    TM_CUDA(ctx, cudaSetDevice(ctx->device));
+    const size_t pb = tm_parity_bytes(ctx, acc);
+    const size_t nout = (size_t)160 * nmom * ctx->X[3];
+    void *si, *ei, *A, *B, *dneg;
+    TM_TRY(tm_ws(ctx, WS_CT_S, 2 * pb, &si));
+    TM_TRY(tm_ws(ctx, WS_CT_ETA, 2 * pb, &ei));
+    TM_TRY(tm_ws(ctx, WS_API_A, nout * 16, &A));
+    TM_TRY(tm_ws(ctx, WS_API_B, nout * 16, &B));
+    TM_TRY(tm_ws(ctx, WS_API_C, (size_t)nmom * sizeof(int), &dneg));
+    TM_CUDA(ctx, cudaMemcpyAsync(dneg, neg.data(), (size_t)nmom * sizeof(int), cudaMemcpyHostToDevice, st));
+    TM_CUDA(ctx, cudaStreamSynchronize(st));         // neg is a local host vector
+    TM_TRY(tm_import_launch(ctx, si, d_s, acc, st));
+    TM_TRY(tm_import_launch(ctx, ei, d_eta, acc, st));
+    TM_TRY(tm_contract_internal(ctx, A, si, ei, kappa, mu, h_momenta, nmom, acc, st));
+    TM_TRY(tm_contract_internal(ctx, B, ei, si, kappa, mu, h_momenta, nmom, acc, st));
+    sym_assemble_kernel<<<(unsigned)((nout + 255) / 256), 256, 0, st>>>((double2*)d_out, (const double2*)A, (const double2*)B,
+                                                                       (const int*)dneg, eta_neg, eps_neg, 2.0 * kappa * mu,
+                                                                       nmom, ctx->X[3]);
+    TM_LAUNCH_CHECK(ctx, "sym_assemble_kernel");
+    return TM_OK;
+}

@@ -119,3 +119,22 @@ def test_contract_explicit_dw_variant(orc, acc):
         eta = inputs.z4_source(dims, 1, 0)
         other = to_np(ctx.loop_contract_project(s, eta, k, mu, mom, t.PREC[acc]))
         assert rel_l2(other[1], got[1]) > 1e-2 and rel_l2(other[0], got[0]) <= 10 * TOL[acc]
+
+
+@pytest.mark.parametrize("acc", ["f64", "f32"])
+@pytest.mark.parametrize("tb", [-1, 1])
+def test_contract_symmetrised_derivative_variant(orc, acc, tb):
+    """Row f3 variant: symmetrised derivative, assembled from two passes of the same primitive, vs the oracle's
+    direct definition (D applied to s as well)."""
+    t = tm()
+    dims = (8, 4, 6, 4)
+    U, s, eta = case(dims, 0.25, 17)
+    k, mu = 0.1563, 0.0055
+    mom = inputs.momentum_list(4)
+    ref = orc.loops_project_sym(s, eta, U, k, mu, mom, tb)
+    with t.TmContext(dims, tb) as ctx:
+        ctx.tm_load_gauge(U)
+        got = to_np(ctx.loop_contract_project_sym(s, eta, k, mu, mom, t.PREC[acc]))
+        check_blocks(got, ref, TOL[acc] * (4 if acc == "f32" else 50))     # differences of two O(1) passes
+        with pytest.raises(t.TmError):                                      # not closed under p -> -p
+            ctx.loop_contract_project_sym(s, eta, k, mu, np.array([[1, 0, 0]], dtype=np.int32), t.PREC[acc])
