@@ -110,6 +110,13 @@ tm_status loop_contract_project(tm_ctx* ctx, void* d_out, const void* d_s, const
                                 double kappa, double mu, const int* h_momenta, int nmom,
                                 tm_prec acc, void* stream);
 
+/* PAPER.md:88 ("GPU kernels to contract a single time slice or a whole vector", for time-dilution): the same call
+ * restricted to ONE timeslice t0 -- 1/T of the work.  d_out keeps the shape [2][80][nmom][T]: column t0 is
+ * computed, every other column is set to zero. */
+tm_status loop_contract_project_timeslice(tm_ctx* ctx, void* d_out, const void* d_s, const void* d_eta,
+                                          double kappa, double mu, const int* h_momenta, int nmom, int t0,
+                                          tm_prec acc, void* stream);
+
 /* Row f3 variant (reading 5): the same 160 projected insertions with the generalised one-end trick's
  * D_W applied EXPLICITLY: g = g5 D_W s = g5 (M s) - 2 i kappa mu s instead of g5 eta - 2 i kappa mu s, i.e. the loops
  * of (s, eta := M s); it differs from loop_contract_project by the bilinears of g5 (eta - M s) and costs one extra

@@ -31,7 +31,7 @@ PREC_BYTES = {TM_F64: 8, TM_F32: 4, TM_F16: 2, TM_BF16: 2}
 EXPORTS = [
     "tm_create", "tm_destroy", "tm_last_error", "tm_load_gauge", "tm_field_bytes",
     "tm_field_import", "tm_field_export", "tm_dslash", "tm_dslash_multi", "tm_cg_solve", "loop_contract_project",
-    "loop_contract_project_explicit", "loop_contract_project_sym",
+    "loop_contract_project_explicit", "loop_contract_project_sym", "loop_contract_project_timeslice",
     "tsm_estimate", "tsm_estimate_host", "tm_launch_count",
     "loop_binary_nfiles", "loop_binary_accumulate", "loop_binary_recover", "tsm_estimate_binary",
 ]
@@ -99,6 +99,7 @@ def load_library():
     L.tm_cg_solve.argtypes = [vp, vp, vp, cd, cd, ctypes.POINTER(tm_solve_params),
                               ctypes.POINTER(tm_solve_info), vp]
     L.loop_contract_project.argtypes = [vp, vp, vp, vp, cd, cd, ctypes.POINTER(ci), ci, ci, vp]
+    L.loop_contract_project_timeslice.argtypes = [vp, vp, vp, vp, cd, cd, ctypes.POINTER(ci), ci, ci, ci, vp]
     L.loop_contract_project_sym.argtypes = [vp, vp, vp, vp, cd, cd, ctypes.POINTER(ci), ci, ci, vp]
     L.loop_contract_project_explicit.argtypes = [vp, vp, vp, cd, cd, ctypes.POINTER(ci), ci, ci, vp]
     L.tsm_estimate.argtypes = [vp, vp, vp, ctypes.POINTER(tsm_params), ctypes.POINTER(tsm_info), vp]
@@ -272,6 +273,18 @@ class TmContext:
         self._check(self.lib.loop_contract_project(
             self.h, out.data_ptr(), s.data_ptr(), eta.data_ptr(), float(kappa), float(mu),
             mom.ctypes.data_as(ctypes.POINTER(ctypes.c_int)), len(mom), int(acc), _stream()))
+        return out
+
+    def loop_contract_project_timeslice(self, s, eta, kappa, mu, momenta, t0, acc=TM_F64):
+        """Single-timeslice contraction: column t0 of the [2,80,nmom,T] output, zeros elsewhere."""
+        torch = _torch()
+        s = self._dev(s, torch.complex128)
+        eta = self._dev(eta, torch.complex128)
+        mom = np.ascontiguousarray(momenta, dtype=np.int32).reshape(-1, 3)
+        out = torch.empty((2, 80, len(mom), self.T), dtype=torch.complex128, device=self.tdev)
+        self._check(self.lib.loop_contract_project_timeslice(
+            self.h, out.data_ptr(), s.data_ptr(), eta.data_ptr(), float(kappa), float(mu),
+            mom.ctypes.data_as(ctypes.POINTER(ctypes.c_int)), len(mom), int(t0), int(acc), _stream()))
         return out
 
     def loop_contract_project_sym(self, s, eta, kappa, mu, momenta, acc=TM_F64):

@@ -43,7 +43,7 @@ __global__ void __launch_bounds__((NP + CT_NC) * 32, 1) contract_xy_kernel(Contr
     F* swx = reinterpret_cast<F*>(buf + (size_t)NS * CT_NCC * CT_BSC);   // [Lx][8]
     F* swy = swx + (size_t)A.g.X0 * 8;                           // [Ly][8]
     const Geom& g = A.g;
-    const int zt = blockIdx.x;
+    const int zt = blockIdx.x + A.t_first * g.X2;
     const int z = zt % g.X2, t = zt / g.X2;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     for (int i = threadIdx.x; i < g.X0 * 8; i += NTHREADS) swx[i] = ((const F*)A.wx)[i];
@@ -206,13 +206,14 @@ struct AssembleArgs {
     const short* qidx;         // [4][4][4]: index of Qcc, Qcs, Qsc, Qss for (m,n), -1 if absent
     const double* wz;          // [Lz][8]
     int nmom, T, Lz, NQ;
+    int t_first;               // first timeslice handled (blockIdx.y = 0)
     double twokmu;             // 2 kappa mu
 };
 
 // z-stage: every x/y partial sum is read exactly once and reduced against the 7 real z-weights
 template <typename F>
 __global__ void __launch_bounds__(CT_THREADS) contract_zsum_kernel(AssembleArgs A) {
-    const int q = blockIdx.x, t = blockIdx.y, jr = threadIdx.x;
+    const int q = blockIdx.x, t = blockIdx.y + A.t_first, jr = threadIdx.x;
     const F* qb = (const F*)A.qbuf + ((size_t)t * A.Lz * A.NQ + q) * CT_THREADS + jr;
     double acc[7];
 #pragma unroll
@@ -233,7 +234,7 @@ __global__ void __launch_bounds__(CT_THREADS) contract_zsum_kernel(AssembleArgs 
 // site-independent Gamma change of basis
 __global__ void __launch_bounds__(CT_THREADS) contract_assemble_kernel(AssembleArgs A) {
     __shared__ double zre[CT_THREADS], zim[CT_THREADS];
-    const int k = blockIdx.x, t = blockIdx.y;
+    const int k = blockIdx.x, t = blockIdx.y + A.t_first;
     const int jr = threadIdx.x;
     const int px = A.mom[3 * k], py = A.mom[3 * k + 1], pz = A.mom[3 * k + 2];
     const int m = abs(px), n = abs(py), l = abs(pz);
@@ -391,12 +392,12 @@ template <> struct XyConfig<float>  { static constexpr int NP = 8, NS = 3; };
 template <> struct XyConfig<double> { static constexpr int NP = 4, NS = 2; };
 
 template <typename S, int R>
-static tm_status launch_xy(tm_ctx* ctx, const ContractArgs& A, int prune, cudaStream_t st) {
+static tm_status launch_xy(tm_ctx* ctx, const ContractArgs& A, int prune, int nt, cudaStream_t st) {
     constexpr int NP = XyConfig<S>::NP, NS = XyConfig<S>::NS;
     constexpr int NT = (NP + CT_NC) * 32;
     const size_t smem = (size_t)NS * CT_NCC * CT_BSC * 2 * sizeof(S) + (size_t)(ctx->X[0] + ctx->X[1]) * 8 * sizeof(S);
     if (smem > 227 * 1024) return tm_fail(ctx, TM_EDIM, "contract: Lx + Ly too large for the shared-memory weight tables");
-    const unsigned grid = (unsigned)(ctx->X[2] * ctx->X[3]);
+    const unsigned grid = (unsigned)(ctx->X[2] * nt);
     if (prune) {
         TM_CUDA(ctx, cudaFuncSetAttribute(contract_xy_kernel<S, R, 1, NP, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         contract_xy_kernel<S, R, 1, NP, NS><<<grid, NT, smem, st>>>(A);
@@ -409,7 +410,10 @@ static tm_status launch_xy(tm_ctx* ctx, const ContractArgs& A, int prune, cudaSt
 }
 
 tm_status tm_contract_internal(tm_ctx* ctx, void* d_out, const void* d_s, const void* d_eta, double kappa,
-                               double mu, const int* h_momenta, int nmom, tm_prec acc, cudaStream_t st) {
+                               double mu, const int* h_momenta, int nmom, tm_prec acc, cudaStream_t st,
+                               int t_first, int nt) {
+    if (nt <= 0) { t_first = 0; nt = ctx->X[3]; }                 // default: every timeslice
+    if (t_first < 0 || t_first + nt > ctx->X[3]) return tm_fail(ctx, TM_EARG, "contract: timeslice range outside the lattice");
     if (acc != TM_F64 && acc != TM_F32) return tm_fail(ctx, TM_EPREC, "contract: acc must be f32 or f64");
     if (!h_momenta || nmom < 1) return tm_fail(ctx, TM_EARG, "contract: need at least one momentum");
     int prune = 1;
@@ -468,9 +472,10 @@ tm_status tm_contract_internal(tm_ctx* ctx, void* d_out, const void* d_s, const 
     A.wy = tb + (acc == TM_F64 ? L.off_wy64 : L.off_wy32);
     A.g = tm_geom(ctx);
     A.tb = (double)ctx->tb;
-    if (acc == TM_F64) TM_TRY((launch_xy<double, 18>(ctx, A, prune, st)));
-    else if (!ctx->no_tma && tm_contract_tma_usable(ctx)) TM_TRY(tm_contract_xy_tma(ctx, qbuf, d_s, d_eta, gauge, A.wx, A.wy, prune, st));
-    else TM_TRY((launch_xy<float, 12>(ctx, A, prune, st)));
+    A.t_first = t_first;
+    if (acc == TM_F64) TM_TRY((launch_xy<double, 18>(ctx, A, prune, nt, st)));
+    else if (!ctx->no_tma && tm_contract_tma_usable(ctx)) TM_TRY(tm_contract_xy_tma(ctx, qbuf, d_s, d_eta, gauge, A.wx, A.wy, prune, t_first, nt, st));
+    else TM_TRY((launch_xy<float, 12>(ctx, A, prune, nt, st)));
 
     AssembleArgs B;
     B.qbuf = qbuf; B.out = d_out;
@@ -478,13 +483,13 @@ tm_status tm_contract_internal(tm_ctx* ctx, void* d_out, const void* d_s, const 
     B.mom = (const int*)(tb + L.off_mom);
     B.qidx = (const short*)(tb + L.off_qidx);
     B.wz = (const double*)(tb + L.off_wz);
-    B.nmom = nmom; B.T = ctx->X[3]; B.Lz = ctx->X[2]; B.NQ = nq;
+    B.nmom = nmom; B.T = ctx->X[3]; B.Lz = ctx->X[2]; B.NQ = nq; B.t_first = t_first;
     B.twokmu = 2.0 * kappa * mu;
-    dim3 zgrid((unsigned)nq, (unsigned)ctx->X[3]);
+    dim3 zgrid((unsigned)nq, (unsigned)nt);
     if (acc == TM_F64) contract_zsum_kernel<double><<<zgrid, CT_THREADS, 0, st>>>(B);
     else contract_zsum_kernel<float><<<zgrid, CT_THREADS, 0, st>>>(B);
     TM_LAUNCH_CHECK(ctx, "contract_zsum_kernel");
-    dim3 grid((unsigned)nmom, (unsigned)ctx->X[3]);
+    dim3 grid((unsigned)nmom, (unsigned)nt);
     contract_assemble_kernel<<<grid, CT_THREADS, 0, st>>>(B);
     TM_LAUNCH_CHECK(ctx, "contract_assemble_kernel");
     return TM_OK;
@@ -629,4 +634,25 @@ extern "C" tm_status loop_contract_project_sym(tm_ctx* ctx, void* d_out, const v
                                                                        nmom, ctx->X[3]);
     TM_LAUNCH_CHECK(ctx, "sym_assemble_kernel");
     return TM_OK;
+}
+
+// A12 of SURVEY.md sec 2 ("GPU kernels to contract a single time slice or a whole vector"): the same 160
+// projected insertions for ONE timeslice t0 (what a time-diluted source needs); 1/T of the work of the whole-vector
+// call.  d_out keeps the [2][80][nmom][T] shape: column t0 is computed, every other column is zero.
+extern "C" tm_status loop_contract_project_timeslice(tm_ctx* ctx, void* d_out, const void* d_s, const void* d_eta,
+                                                     double kappa, double mu, const int* h_momenta, int nmom, int t0,
+                                                     tm_prec acc, void* stream) {
+    if (!ctx || !d_out || !d_s || !d_eta) return tm_fail(ctx, TM_EARG, "loop_contract_project_timeslice: null argument");
+    if (acc != TM_F64 && acc != TM_F32) return tm_fail(ctx, TM_EPREC, "loop_contract_project_timeslice: acc must be f32 or f64");
+    if (t0 < 0 || t0 >= ctx->X[3]) return tm_fail(ctx, TM_EARG, "loop_contract_project_timeslice: t0 outside the lattice");
+    if (nmom < 1) return tm_fail(ctx, TM_EARG, "loop_contract_project_timeslice: need at least one momentum");
+    cudaStream_t st = (cudaStream_t)stream;
+    TM_CUDA(ctx, cudaSetDevice(ctx->device));
+    void *si, *ei;
+    TM_TRY(tm_ws(ctx, WS_CT_S, 2 * tm_parity_bytes(ctx, acc), &si));
+    TM_TRY(tm_ws(ctx, WS_CT_ETA, 2 * tm_parity_bytes(ctx, acc), &ei));
+    TM_TRY(tm_import_launch(ctx, si, d_s, acc, st));
+    TM_TRY(tm_import_launch(ctx, ei, d_eta, acc, st));
+    TM_CUDA(ctx, cudaMemsetAsync(d_out, 0, (size_t)160 * nmom * ctx->X[3] * 16, st));
+    return tm_contract_internal(ctx, d_out, si, ei, kappa, mu, h_momenta, nmom, acc, st, t0, 1);
 }

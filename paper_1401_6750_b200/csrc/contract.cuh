@@ -21,6 +21,7 @@ struct ContractArgs {
     const void* wy;        // [Ly][8]
     Geom g;
     double tb;
+    int t_first;           // first timeslice of the launch (grid = Lz x number of timeslices)
 };
 
 // ---- pair arithmetic: one complex number (re, im) per pair.  fp32 pairs live in one 64-bit register

@@ -33,6 +33,7 @@ struct TmaContractArgs {
     const float* wy;       // [Ly][8]
     Geom g;
     float tb;
+    int t_first;           // first timeslice of the launch
 };
 
 // shared-memory plan (bytes), every TMA destination 128-byte aligned
@@ -267,7 +268,7 @@ contract_xy_tma_kernel(const __grid_constant__ CUtensorMap tm_s, const __grid_co
     sh.swy = reinterpret_cast<float*>(smem_raw + P.off_wy);
     sh.bar_full = smem_u32(smem_raw + P.off_bar);
     sh.bar_empty = sh.bar_full + 8 * TX_NSI;
-    const int zt = blockIdx.x;
+    const int zt = blockIdx.x + A.t_first * g.X2;
     const int z = zt % g.X2, t = zt / g.X2;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int Xh = g.Xh;
@@ -436,7 +437,7 @@ bool tm_contract_tma_usable(const tm_ctx* ctx) {
 
 // s, eta: fp32 full-lattice internal fields; gauge: fp32 reconstruct-12 internal copy; wx, wy: float tables
 tm_status tm_contract_xy_tma(tm_ctx* ctx, void* qbuf, const void* d_s, const void* d_eta, const void* gauge,
-                             const void* wx, const void* wy, int prune, cudaStream_t st) {
+                             const void* wx, const void* wy, int prune, int t_first, int nt, cudaStream_t st) {
     const int Xh = ctx->Xh;
     const cuuint64_t Vh = ctx->Vh;
     CUtensorMap ms, me, mgf, mgb;
@@ -459,8 +460,9 @@ tm_status tm_contract_xy_tma(tm_ctx* ctx, void* qbuf, const void* d_s, const voi
     A.qbuf = qbuf; A.wx = (const float*)wx; A.wy = (const float*)wy;
     A.g = tm_geom(ctx);
     A.tb = (float)ctx->tb;
+    A.t_first = t_first;
     const TxPlan P = tx_plan(ctx->X[0], ctx->X[1]);
-    const unsigned grid = (unsigned)(ctx->X[2] * ctx->X[3]);
+    const unsigned grid = (unsigned)(ctx->X[2] * nt);
     if (prune) {
         TM_CUDA(ctx, cudaFuncSetAttribute(contract_xy_tma_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, P.total));
         contract_xy_tma_kernel<1><<<grid, TX_NTHREADS, P.total, st>>>(ms, me, mgf, mgb, A);

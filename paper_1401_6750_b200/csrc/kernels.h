@@ -85,10 +85,10 @@ tm_status tm_solve_internal(tm_ctx* ctx, void* d_s, const void* d_eta, double ka
 // s, eta: full-lattice internal fields of precision acc (TM_F32 | TM_F64); out: complex128 [2][80][nmom][T]
 tm_status tm_contract_internal(tm_ctx* ctx, void* d_out, const void* d_s, const void* d_eta,
                                double kappa, double mu, const int* h_momenta, int nmom, tm_prec acc,
-                               cudaStream_t st);
+                               cudaStream_t st, int t_first = 0, int nt = 0 /* 0: all timeslices */);
 // contract_tma.cu: TMA-staged fast path of the site + x/y-DFT stage (fp32, Lx <= 32)
 bool tm_contract_tma_usable(const tm_ctx* ctx);
 tm_status tm_contract_xy_tma(tm_ctx* ctx, void* qbuf, const void* d_s, const void* d_eta, const void* gauge,
-                             const void* wx, const void* wy, int prune, cudaStream_t st);
+                             const void* wx, const void* wy, int prune, int t_first, int nt, cudaStream_t st);
 // acc += x on complex128 arrays of n complex numbers
 tm_status tm_accumulate(tm_ctx* ctx, void* d_acc, const void* d_x, size_t n, cudaStream_t st);

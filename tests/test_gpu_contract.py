@@ -138,3 +138,27 @@ def test_contract_symmetrised_derivative_variant(orc, acc, tb):
         check_blocks(got, ref, TOL[acc] * (4 if acc == "f32" else 50))     # differences of two O(1) passes
         with pytest.raises(t.TmError):                                      # not closed under p -> -p
             ctx.loop_contract_project_sym(s, eta, k, mu, np.array([[1, 0, 0]], dtype=np.int32), t.PREC[acc])
+
+
+@pytest.mark.parametrize("acc", ["f64", "f32"])
+def test_contract_single_timeslice(orc, acc):
+    """the single-timeslice contraction (time-dilution) = column t0 of the whole-vector call, zeros
+    elsewhere; checked against the oracle restricted to that timeslice, at the time boundary and inside."""
+    t = tm()
+    dims = (8, 8, 8, 6)
+    U, s, eta = case(dims, 0.25, 27)
+    k, mu = 0.1563, 0.0055
+    mom = inputs.momentum_list(2)
+    with t.TmContext(dims, -1) as ctx:
+        ctx.tm_load_gauge(U)
+        full = to_np(ctx.loop_contract_project(s, eta, k, mu, mom, t.PREC[acc]))
+        for t0 in (0, 3, 5):
+            ref = orc.loops_project(s, eta, U, k, mu, mom, -1, t0, t0 + 1)
+            got = to_np(ctx.loop_contract_project_timeslice(s, eta, k, mu, mom, t0, t.PREC[acc]))
+            check_blocks(got, ref, TOL[acc])
+            assert np.array_equal(got[..., t0], full[..., t0])
+            mask = np.ones(dims[3], dtype=bool)
+            mask[t0] = False
+            assert not got[..., mask].any()
+        with pytest.raises(t.TmError):
+            ctx.loop_contract_project_timeslice(s, eta, k, mu, mom, dims[3], t.PREC[acc])
