@@ -30,6 +30,9 @@
  * throws or aborts across the ABI; text of the last error via tm_last_error.  There is NO CPU
  * fallback: without a CUDA device tm_create fails with TM_ECUDA.
  * Calls are stream-ordered; those that fill an *_info struct synchronise the stream at the end.
+ * One stream at a time per context: state the context builds lazily (reduced-precision gauge copies, contraction
+ * tables, workspaces) is ordered on the stream of the call that built it, so a caller that moves a context to another
+ * stream must order the two streams itself (event or synchronisation).  A context is not thread-safe.
  */
 #ifndef TMLOOPS_H
 #define TMLOOPS_H
@@ -59,6 +62,16 @@ typedef enum { TM_OP_HOP = 0, TM_OP_HOP_TWINV = 1, TM_OP_XPAY = 2, TM_OP_M_FULL 
 tm_status tm_create(tm_ctx** ctx, const int dims[4], int t_boundary, int device);
 tm_status tm_destroy(tm_ctx* ctx);
 const char* tm_last_error(const tm_ctx* ctx);
+
+/* Context options (no environment variables, no global state: everything lives in the opaque context).
+ *   TM_OPT_GROUP          sources solved per launch by tsm_estimate*: 0 = automatic (8, halved until the workspaces
+ *                         fit the device memory), or 1 | 2 | 4 | 8
+ *   TM_OPT_CONTRACT_PATH  site + x/y-DFT stage of the contraction: 0 = automatic (fastest usable), 1 = generic kernel
+ *                         (read-only-cache loads; any Lx, fp64), 2 = TMA-staged fp32 kernel with the DFT on the fp32 pipe,
+ *                         3 = TMA-staged fp32 kernel with the DFT on the tensor cores (tcgen05, split-fp32 operands)
+ * TM_EARG for an unknown option or value. */
+typedef enum { TM_OPT_GROUP = 0, TM_OPT_CONTRACT_PATH = 1 } tm_option;
+tm_status tm_set_option(tm_ctx* ctx, tm_option opt, int value);
 
 /* d_U: device, canonical complex128 [V][4][3][3].  Copied into the context (fp64 master);
  * previously built reduced-precision copies are dropped. */
@@ -138,9 +151,16 @@ tm_status loop_contract_project_sym(tm_ctx* ctx, void* d_out, const void* d_s, c
  *               layout [n_lp][3V] bytes (device);
  * d_z4 == NULL: generated on the device from `seed` with the counter hash of DESIGN.md
  *               (k = h(seed, r, c) & 3). */
+/* Sharding by source (the sources are independent): local source j = 0..n_lp-1 of a call
+ * is the GLOBAL source r = src_first + j * src_stride (src_stride 0 is read as 1), which names its noise stream
+ * h(seed, r, .); d_z4 is indexed by the local j.  Rank k of W ranks takes src_first = k, src_stride = W, so the first
+ * N_HP global sources -- the ones that also get an HP solve -- are spread evenly: n_hp = ceil((N_HP - k) / W).
+ * d_solutions: optional (NULL ok) device complex128 [n_lp + n_hp][V][4][3], receives every solution s_r in canonical
+ * layout (LP first, then HP) so that a checker can evaluate residuals and loops of the run's own solutions. */
 typedef struct { int n_lp, n_hp; tm_solve_params lp, hp; double kappa, mu;
                  const int* h_momenta; int nmom; tm_prec contract_acc_lp, contract_acc_hp;
-                 const unsigned char* d_z4; unsigned long long seed; } tsm_params;
+                 const unsigned char* d_z4; unsigned long long seed;
+                 int src_first, src_stride; void* d_solutions; } tsm_params;
 typedef struct { double ms_total, ms_lp_solve, ms_hp_solve, ms_contract; long iters_lp, iters_hp;
                  double worst_resid_lp, worst_resid_hp; int launches; } tsm_info;
 /* d_out: device complex128 [2][80][nmom][T]; d_per_source: optional (NULL ok) device complex128
@@ -148,6 +168,15 @@ typedef struct { double ms_total, ms_lp_solve, ms_hp_solve, ms_contract; long it
  * TM_ENOCONV if any solve missed its rho (outputs still filled). */
 tm_status tsm_estimate(tm_ctx* ctx, void* d_out, void* d_per_source, const tsm_params* params,
                        tsm_info* info, void* stream);
+/* The same loop, stopped before the division: d_sums = complex128 [3][2][80][nmom][T] receives the raw accumulators
+ * S_LP = sum_r l_r^LP (all n_lp local sources), S_LPc = sum_{r<n_hp} l_r^LP, S_HP = sum_{r<n_hp} l_r^HP.  With sources
+ * sharded over ranks (src_first / src_stride above) the only exchange of a multi-GPU run is one all-reduce (sum) of
+ * these three arrays, followed by tsm_combine_sums on every rank:
+ *   d_out = S_LP / n_lp_total + (S_HP - S_LPc) / n_hp_total      (n_hp_total = 0: the second term is dropped). */
+tm_status tsm_partial_sums(tm_ctx* ctx, void* d_sums, void* d_per_source, const tsm_params* params,
+                           tsm_info* info, void* stream);
+tm_status tsm_combine_sums(tm_ctx* ctx, void* d_out, const void* d_sums, int n_lp_total, int n_hp_total,
+                           int nmom, void* stream);
 /* Same with HOST buffers: h_z4 (pinned or pageable host memory, may be NULL -> seed) is copied
  * to the device source by source and h_out is copied back, all inside the call. */
 tm_status tsm_estimate_host(tm_ctx* ctx, void* h_out, const unsigned char* h_z4,
@@ -162,8 +191,10 @@ tm_status tsm_estimate_host(tm_ctx* ctx, void* h_out, const unsigned char* h_z4,
  *                           Fig. 2: N = 13 = 1101b -> the files holding 8, 4 and 1 sources).
  * d_files: device complex128 [nfiles][len], zeroed by the caller before the first source; d_loop, d_out:
  * device complex128 [len]; len = number of complex entries of one per-source array (160 * nmom * T).
- * n_stored = number of sources accumulated so far: recover returns TM_EARG when N needs a file that is
- * missing or not yet complete.  Asynchronous on stream. */
+ * n_stored = number of sources accumulated so far.  Recoverable N: any N whose binary digits name COMPLETE files, and
+ * N = n_stored itself (the sum of every file, the partially filled last one included, divided by n_stored) -- so a run
+ * of 500 + 20 sources can always recover its own full estimate; recover returns TM_EARG for any other N.
+ * Asynchronous on stream. */
 int loop_binary_nfiles(int n_sources);
 tm_status loop_binary_accumulate(tm_ctx* ctx, void* d_files, const void* d_loop, int r, size_t len, void* stream);
 tm_status loop_binary_recover(tm_ctx* ctx, void* d_out, const void* d_files, int n_stored, int N, size_t len,
@@ -175,6 +206,12 @@ tm_status loop_binary_recover(tm_ctx* ctx, void* d_out, const void* d_files, int
  *   recover(files_lp, N_LP') + recover(files_corr, N_HP').  Both are zeroed inside the call. */
 tm_status tsm_estimate_binary(tm_ctx* ctx, void* d_out, void* d_files_lp, void* d_files_corr,
                               const tsm_params* params, tsm_info* info, void* stream);
+
+/* Measured fp32 FMA peak of the device in TFLOP/s (2 flop per FMA lane): the ALU roofline denominator of the contraction
+ * kernel (measure it, do not quote it).  mode 0: scalar FFMA, mode 1: packed FFMA2 (the instruction
+ * the contraction and the fp32 Dslash issue); iters rounds of 16 independent FMAs per thread, best of 3 launches.
+ * Synchronises the stream. */
+tm_status tm_fma_peak(tm_ctx* ctx, int mode, int iters, double* tflops, void* stream);
 
 /* number of kernels launched by this context so far (bench.py's gpu_launches) */
 long tm_launch_count(const tm_ctx* ctx);

@@ -475,11 +475,24 @@ void orc_binary_store(cplx *files, int *counts, const cplx *per_source, int n, l
 
 /* "Reconstruction is straightforward, taking into account the base-2 structure": the estimator from N
  * sources is the sum of the files whose weight 2^k is a binary digit of N, divided by N (Fig. 2:
- * N = 13 = 1101b -> the files with 1, 4 and 8 sources).  Returns 0, or -1 when a needed file does not
- * exist or is incomplete (counts[k] != 2^k). */
+ * N = 13 = 1101b -> the files with 1, 4 and 8 sources).  "With this storage method one can recover the
+ * data for any number of sources": the one N the digits rule cannot serve while the last
+ * file is still filling is the number of sources stored so far, n = sum_k counts[k]; for N = n the
+ * estimator is the sum of EVERY file, the partial one included, divided by n (reading 21).
+ * Returns 0, or -1 when N is neither n nor made of complete files (counts[k] == 2^k). */
 int orc_binary_recover(cplx *out, const cplx *files, const int *counts, int nfiles, int N, long len)
 {
     if (N < 1) return -1;
+    long n = 0;
+    for (int k = 0; k < nfiles; k++) n += counts[k];
+    if (N == n) {                                        /* everything stored so far */
+        for (long j = 0; j < len; j++) {
+            out[j] = 0;
+            for (int k = 0; k < nfiles; k++) out[j] += files[(long)k * len + j];
+            out[j] /= N;
+        }
+        return 0;
+    }
     for (int k = 0; (1L << k) <= N; k++)
         if ((N >> k) & 1)
             if (k >= nfiles || counts[k] != (1 << k)) return -1;

@@ -19,12 +19,13 @@ import numpy as np
 from . import inputs  # noqa: F401  (seeded input generators; no method arithmetic)
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.environ.get("TMLOOPS_LIB") or os.path.join(_HERE, "libtmloops.so")
+LIB_PATH = os.path.join(_HERE, "libtmloops.so")
 
 TM_OK, TM_EARG, TM_EDIM, TM_EPREC, TM_ECUDA, TM_ENOCONV, TM_EALLOC = range(7)
 TM_F64, TM_F32, TM_F16, TM_BF16 = range(4)
 TM_R18, TM_R12 = 18, 12
 TM_OP_HOP, TM_OP_HOP_TWINV, TM_OP_XPAY, TM_OP_M_FULL, TM_OP_MHAT = range(5)
+TM_OPT_GROUP, TM_OPT_CONTRACT_PATH = range(2)
 PREC = {"f64": TM_F64, "f32": TM_F32, "f16": TM_F16, "bf16": TM_BF16}
 PREC_BYTES = {TM_F64: 8, TM_F32: 4, TM_F16: 2, TM_BF16: 2}
 
@@ -32,7 +33,8 @@ EXPORTS = [
     "tm_create", "tm_destroy", "tm_last_error", "tm_load_gauge", "tm_field_bytes",
     "tm_field_import", "tm_field_export", "tm_dslash", "tm_dslash_multi", "tm_cg_solve", "loop_contract_project",
     "loop_contract_project_explicit", "loop_contract_project_sym", "loop_contract_project_timeslice",
-    "tsm_estimate", "tsm_estimate_host", "tm_launch_count",
+    "tsm_estimate", "tsm_estimate_host", "tm_launch_count", "tm_set_option", "tsm_partial_sums", "tsm_combine_sums",
+    "tm_fma_peak",
     "loop_binary_nfiles", "loop_binary_accumulate", "loop_binary_recover", "tsm_estimate_binary",
 ]
 
@@ -59,7 +61,8 @@ class tsm_params(ctypes.Structure):
                 ("kappa", ctypes.c_double), ("mu", ctypes.c_double),
                 ("h_momenta", ctypes.POINTER(ctypes.c_int)), ("nmom", ctypes.c_int),
                 ("contract_acc_lp", ctypes.c_int), ("contract_acc_hp", ctypes.c_int),
-                ("d_z4", ctypes.c_void_p), ("seed", ctypes.c_ulonglong)]
+                ("d_z4", ctypes.c_void_p), ("seed", ctypes.c_ulonglong),
+                ("src_first", ctypes.c_int), ("src_stride", ctypes.c_int), ("d_solutions", ctypes.c_void_p)]
 
 
 class tsm_info(ctypes.Structure):
@@ -110,6 +113,10 @@ def load_library():
     L.loop_binary_recover.argtypes = [vp, vp, vp, ci, ci, ctypes.c_size_t, vp]
     L.tsm_estimate_binary.argtypes = [vp, vp, vp, vp, ctypes.POINTER(tsm_params), ctypes.POINTER(tsm_info), vp]
     L.tm_launch_count.argtypes = [vp]
+    L.tm_set_option.argtypes = [vp, ci, ci]
+    L.tsm_partial_sums.argtypes = [vp, vp, vp, ctypes.POINTER(tsm_params), ctypes.POINTER(tsm_info), vp]
+    L.tsm_combine_sums.argtypes = [vp, vp, vp, ci, ci, ci, vp]
+    L.tm_fma_peak.argtypes = [vp, ci, ci, ctypes.POINTER(cd), vp]
     L.tm_launch_count.restype = ctypes.c_long
     _lib = L
     return L
@@ -187,6 +194,16 @@ class TmContext:
     # ------------------------------------------------------------------ fields
     def launch_count(self) -> int:
         return int(self.lib.tm_launch_count(self.h))
+
+    def tm_set_option(self, opt: int, value: int):
+        """TM_OPT_GROUP (0 = automatic | 1 | 2 | 4 | 8) or TM_OPT_CONTRACT_PATH (0 = automatic | 1 | 2 | 3); see tmloops.h."""
+        self._check(self.lib.tm_set_option(self.h, int(opt), int(value)))
+
+    def tm_fma_peak(self, mode: int = 1, iters: int = 4096) -> float:
+        """Measured fp32 FMA peak in TFLOP/s (mode 0: FFMA, 1: FFMA2)."""
+        v = ctypes.c_double(0.0)
+        self._check(self.lib.tm_fma_peak(self.h, int(mode), int(iters), ctypes.byref(v), _stream()))
+        return float(v.value)
 
     def tm_load_gauge(self, U):
         """U: complex128 [T,Lz,Ly,Lx,4,3,3] (numpy or torch)."""
@@ -311,7 +328,8 @@ class TmContext:
         return out
 
     # ------------------------------------------------------------------ TSM
-    def _tsm_params(self, n_lp, n_hp, kappa, mu, momenta, lp, hp, acc_lp, acc_hp, d_z4, seed):
+    def _tsm_params(self, n_lp, n_hp, kappa, mu, momenta, lp, hp, acc_lp, acc_hp, d_z4, seed,
+                    src_first=0, src_stride=1, d_solutions=None):
         mom = np.ascontiguousarray(momenta, dtype=np.int32).reshape(-1, 3)
         P = tsm_params()
         P.n_lp, P.n_hp = int(n_lp), int(n_hp)
@@ -323,6 +341,8 @@ class TmContext:
         P.contract_acc_lp, P.contract_acc_hp = int(acc_lp), int(acc_hp)
         P.d_z4 = d_z4
         P.seed = int(seed)
+        P.src_first, P.src_stride = int(src_first), int(src_stride)
+        P.d_solutions = d_solutions
         return P, mom
 
     @staticmethod
@@ -333,27 +353,50 @@ class TmContext:
                     launches=info.launches, status=st)
 
     def tsm_estimate(self, n_lp, n_hp, kappa, mu, momenta, lp, hp, acc_lp=TM_F32, acc_hp=TM_F64,
-                     z4=None, seed=0, per_source=False, raise_on_noconv=True):
+                     z4=None, seed=0, per_source=False, raise_on_noconv=True, solutions=False,
+                     src_first=0, src_stride=1, partial_sums=False):
         """sec 2.1: TSM estimate, complex128 [2,80,nmom,T] (device-resident inputs).
 
         z4: optional uint8 cuda tensor [n_lp, 3V] of packed Z4 exponents (None: generated on the
-        device from ``seed``).  lp / hp: dicts(sloppy, outer, recon, rho, max_iter, delta)."""
+        device from ``seed``).  lp / hp: dicts(sloppy, outer, recon, rho, max_iter, delta).
+        solutions=True: info["solutions"] = complex128 [n_lp + n_hp, T,Lz,Ly,Lx,4,3], the run's own solutions.
+        src_first / src_stride: local source j is global source src_first + j * src_stride (sharding by source).
+        partial_sums=True: the first return value is the raw accumulators [3,2,80,nmom,T] (tsm_partial_sums)."""
         torch = _torch()
         d_z4 = None
         if z4 is not None:
             z4 = self._dev(z4, torch.uint8)
             assert z4.numel() == n_lp * 3 * self.V
             d_z4 = z4.data_ptr()
-        P, mom = self._tsm_params(n_lp, n_hp, kappa, mu, momenta, lp, hp, acc_lp, acc_hp, d_z4, seed)
-        out = torch.empty((2, 80, len(mom), self.T), dtype=torch.complex128, device=self.tdev)
+        sol = None
+        if solutions:
+            lx, ly, lz, lt = self.dims
+            sol = torch.empty((n_lp + n_hp, lt, lz, ly, lx, 4, 3), dtype=torch.complex128, device=self.tdev)
+        P, mom = self._tsm_params(n_lp, n_hp, kappa, mu, momenta, lp, hp, acc_lp, acc_hp, d_z4, seed,
+                                  src_first, src_stride, sol.data_ptr() if sol is not None else None)
+        shape = (2, 80, len(mom), self.T)
+        out = torch.empty(((3,) + shape) if partial_sums else shape, dtype=torch.complex128, device=self.tdev)
         ps = None
         if per_source:
-            ps = torch.empty((n_lp + n_hp, 2, 80, len(mom), self.T), dtype=torch.complex128, device=self.tdev)
+            ps = torch.empty((n_lp + n_hp,) + shape, dtype=torch.complex128, device=self.tdev)
         info = tsm_info()
-        st = self.lib.tsm_estimate(self.h, out.data_ptr(), ps.data_ptr() if ps is not None else None,
-                                   ctypes.byref(P), ctypes.byref(info), _stream())
+        fn = self.lib.tsm_partial_sums if partial_sums else self.lib.tsm_estimate
+        st = fn(self.h, out.data_ptr(), ps.data_ptr() if ps is not None else None,
+                ctypes.byref(P), ctypes.byref(info), _stream())
         self._check(st, allow=() if raise_on_noconv else (TM_ENOCONV,))
-        return out, ps, self._tsm_info(info, st)
+        d = self._tsm_info(info, st)
+        if sol is not None:
+            d["solutions"] = sol
+        return out, ps, d
+
+    def tsm_combine_sums(self, sums, n_lp_total, n_hp_total):
+        """out = S_LP / n_lp_total + (S_HP - S_LPc) / n_hp_total from the (all-reduced) raw accumulators [3,2,80,nmom,T]."""
+        torch = _torch()
+        assert sums.dtype == torch.complex128 and sums.is_contiguous() and sums.shape[0] == 3
+        out = torch.empty(tuple(sums.shape[1:]), dtype=torch.complex128, device=self.tdev)
+        self._check(self.lib.tsm_combine_sums(self.h, out.data_ptr(), sums.data_ptr(), int(n_lp_total), int(n_hp_total),
+                                              int(sums.shape[3]), _stream()))
+        return out
 
     # ------------------------------------------------------------------ binary storage (sec 2.1.1, Fig. 2)
     def loop_binary_nfiles(self, n_sources: int) -> int:

@@ -83,7 +83,6 @@ extern "C" tm_status tm_create(tm_ctx** out, const int dims[4], int t_boundary, 
     c->V = V; c->Vh = V / 2;
     c->tb = t_boundary;
     c->device = device;
-    { const char* e = getenv("TMLOOPS_NO_TMA"); c->no_tma = (e && e[0] == '1'); }
     cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
     bool ok = lane_alloc(c, 0);
     if (!ok) {
@@ -93,6 +92,22 @@ extern "C" tm_status tm_create(tm_ctx** out, const int dims[4], int t_boundary, 
     }
     *out = c;
     return TM_OK;
+}
+
+extern "C" tm_status tm_set_option(tm_ctx* c, tm_option opt, int value) {
+    if (!c) return TM_EARG;
+    switch (opt) {
+        case TM_OPT_GROUP:
+            if (value != 0 && value != 1 && value != 2 && value != 4 && value != 8)
+                return tm_fail(c, TM_EARG, "tm_set_option: TM_OPT_GROUP must be 0 (automatic), 1, 2, 4 or 8");
+            c->opt_group = value;
+            return TM_OK;
+        case TM_OPT_CONTRACT_PATH:
+            if (value < 0 || value > 3) return tm_fail(c, TM_EARG, "tm_set_option: TM_OPT_CONTRACT_PATH must be 0..3");
+            c->opt_contract = value;
+            return TM_OK;
+    }
+    return tm_fail(c, TM_EARG, "tm_set_option: unknown option");
 }
 
 static void drop_gauge_copies(tm_ctx* c) {

@@ -24,6 +24,7 @@ struct CgScalars;   // blas.cuh
 // waiting for the device (every kernel is guarded by the device-side state, so a wrong plan costs
 // only no-op launches or an extra host round trip, never a different result).
 #define CG_MAX_PAUSES 48
+#define TM_NPLANS 6
 struct CgPlan {
     int valid;
     int sloppy, outer, recon, max_iter;
@@ -66,7 +67,8 @@ struct tm_ctx {
     unsigned int* d_counter;        // last-block-done counter
     CgScalars* d_scal;              // device scalars of the running solve
     CgScalars* h_scal;              // pinned mirror
-    CgPlan plan[4];                 // per sloppy precision
+    CgPlan plan[TM_NPLANS];         // launch plans keyed by the full parameter tuple (LP and HP keep their own), round-robin eviction
+    int plan_next;
     // generic workspace pool (freed in tm_destroy): named slots grown on demand
     void* scratch[TM_MAX_SCRATCH];
     size_t scratch_bytes[TM_MAX_SCRATCH];
@@ -79,7 +81,8 @@ struct tm_ctx {
     int nb;                         // sources per launch of the running solve (0 | 1: one; 2: a pair, see blas.cu)
     TmLane lanes[TM_NLANES];        // parked state of the inactive lanes (the active one lives in the fields above)
     cudaStream_t lane_stream;       // stream owned by the active lane (0 for lane 0)
-    int no_tma;                     // TMLOOPS_NO_TMA=1: force the generic contraction kernel (testing)
+    int opt_group;                  // TM_OPT_GROUP: 0 = automatic | 1 | 2 | 4 | 8 sources per solve
+    int opt_contract;               // TM_OPT_CONTRACT_PATH: 0 = automatic | 1 generic | 2 TMA + fp32-pipe DFT | 3 TMA + tensor-core DFT
 };
 
 static inline tm_status tm_fail(tm_ctx* c, tm_status s, const char* msg) {

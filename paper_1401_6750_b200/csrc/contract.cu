@@ -474,7 +474,7 @@ tm_status tm_contract_internal(tm_ctx* ctx, void* d_out, const void* d_s, const 
     A.tb = (double)ctx->tb;
     A.t_first = t_first;
     if (acc == TM_F64) TM_TRY((launch_xy<double, 18>(ctx, A, prune, nt, st)));
-    else if (!ctx->no_tma && tm_contract_tma_usable(ctx)) TM_TRY(tm_contract_xy_tma(ctx, qbuf, d_s, d_eta, gauge, A.wx, A.wy, prune, t_first, nt, st));
+    else if (ctx->opt_contract != 1 && tm_contract_tma_usable(ctx)) TM_TRY(tm_contract_xy_tma(ctx, qbuf, d_s, d_eta, gauge, A.wx, A.wy, prune, t_first, nt, st));
     else TM_TRY((launch_xy<float, 12>(ctx, A, prune, nt, st)));
 
     AssembleArgs B;

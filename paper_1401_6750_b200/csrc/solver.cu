@@ -63,6 +63,27 @@ static tm_status job_tail(tm_ctx* ctx, const SolveJob& J) {
     return TM_OK;
 }
 
+// Launch plans are keyed by the whole parameter tuple, so LP and HP solves that share a sloppy precision (or two
+// parameter sets used alternately) keep their own plan instead of evicting each other's on every pass.
+static bool plan_matches(const CgPlan& p, const SolveJob& J) {
+    return p.valid && p.sloppy == (int)J.ps && p.outer == (int)J.po && p.recon == (int)J.rc
+        && p.max_iter == J.P.max_iter && p.rho == J.P.rho && p.delta == J.delta;
+}
+static CgPlan* find_plan(tm_ctx* ctx, const SolveJob& J) {
+    for (int i = 0; i < TM_NPLANS; i++)
+        if (plan_matches(ctx->plan[i], J)) return &ctx->plan[i];
+    return nullptr;
+}
+static CgPlan* plan_slot(tm_ctx* ctx, const SolveJob& J) {
+    CgPlan* p = find_plan(ctx, J);
+    if (p) return p;
+    for (int i = 0; i < TM_NPLANS; i++)
+        if (!ctx->plan[i].valid) return &ctx->plan[i];
+    p = &ctx->plan[ctx->plan_next];
+    ctx->plan_next = (ctx->plan_next + 1) % TM_NPLANS;
+    return p;
+}
+
 // every launcher reads ctx->nb; it is 2 only while a paired solve enqueues
 struct NbScope {
     tm_ctx* c;
@@ -130,9 +151,11 @@ tm_status tm_solve_begin(tm_ctx* ctx, SolveJob* Jp, void* d_s, const void* d_eta
     }
     TM_TRY(blas_residual(ctx, J.r, J.pa, J.rs, ps, J.b, nullptr, po, RED_START, GUARD_ALWAYS, st));
 
-    const CgPlan& plan = ctx->plan[(int)ps];
-    const bool have_plan = plan.valid && plan.sloppy == (int)ps && plan.outer == (int)po && plan.recon == (int)J.rc
-                        && plan.max_iter == P->max_iter && plan.rho == P->rho && plan.delta == J.delta;
+    const CgPlan* planp = find_plan(ctx, J);
+    const bool have_plan = planp != nullptr;
+    CgPlan plan_copy;
+    if (have_plan) plan_copy = *planp;
+    const CgPlan& plan = plan_copy;
     J.tail_valid = false;
     J.enq = 0;                                      // iteration blocks enqueued so far
     if (have_plan) {
@@ -167,20 +190,31 @@ tm_status tm_solve_end(tm_ctx* ctx, SolveJob* Jp, tm_solve_info* info) {
             if (sc[b].done < 2) return true;
         return false;
     };
+    // progress of the device state machine: every [iteration, update] pair advances a running source by one iteration
+    // (state 0) or one reliable update (state 1), whatever the host had enqueued speculatively before
+    auto progress = [&]() {
+        long p = 0;
+        for (int b = 0; b < nb; b++) p += (long)sc[b].iters + (long)sc[b].n_ru + (sc[b].done >= 2 ? 1 : 0);
+        return p;
+    };
+    int stuck = 0;
     while (running()) {
         // off plan (first solve with these parameters, or a source behaves differently):
         // [iteration, update] pairs, polled every few pairs
         const int burst = 4;
+        const long before = progress();
         for (int k = 0; k < burst; k++) { TM_TRY(job_iteration(ctx, J)); TM_TRY(job_update(ctx, J)); J.enq++; }
         J.tail_valid = false;
         TM_TRY(scal_get(ctx, sc, st));
-        if (J.enq > (long)P->max_iter + 8 * (long)CG_MAX_PAUSES + 64 && running())
-            return tm_fail(ctx, TM_ECUDA, "solve: device state machine did not terminate");
+        // failsafe on the DEVICE's own counters (not on the number of blocks enqueued, many of which the guards turn
+        // into no-ops): only a state machine that did not move at all over several polls is broken
+        stuck = (running() && progress() == before) ? stuck + 1 : 0;
+        if (stuck >= 3) return tm_fail(ctx, TM_ECUDA, "solve: device state machine did not advance");
     }
     if (!J.tail_valid) TM_TRY(job_tail(ctx, J));
     TM_CUDA(ctx, cudaEventSynchronize(J.e1));
     // remember where this solve paused: the launch plan of the next one (a group: the union of its sources' pauses)
-    CgPlan& plan = ctx->plan[(int)J.ps];
+    CgPlan& plan = *plan_slot(ctx, J);
     plan.valid = 1;
     plan.sloppy = (int)J.ps; plan.outer = (int)J.po; plan.recon = (int)J.rc; plan.max_iter = P->max_iter;
     plan.rho = P->rho; plan.delta = J.delta;

@@ -25,15 +25,24 @@ __global__ void tsm_accumulate_kernel(double* __restrict__ acc0, double* __restr
 }
 
 // out = S_LP / n_lp + (S_HP - S_LPc) / n_hp, the three sums taken over the lanes in lane order
+// (raw != 0: out[3][n] = the three sums themselves, for the all-reduce of a multi-GPU run: SURVEY.md sec 8e)
 struct TsmLaneAcc { int n; const double* acc[TM_NLANES]; };
-__global__ void tsm_combine_kernel(double* __restrict__ out, TsmLaneAcc L, double inv_lp, double inv_hp, size_t n) {
+__global__ void tsm_combine_kernel(double* __restrict__ out, TsmLaneAcc L, double inv_lp, double inv_hp, size_t n, int raw) {
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     double slp = 0.0, slpc = 0.0, shp = 0.0;
     for (int l = 0; l < L.n; l++) {
         slp += L.acc[l][i]; slpc += L.acc[l][n + i]; shp += L.acc[l][2 * n + i];
     }
-    out[i] = slp * inv_lp + (shp - slpc) * inv_hp;
+    if (raw) { out[i] = slp; out[n + i] = slpc; out[2 * n + i] = shp; }
+    else out[i] = slp * inv_lp + (shp - slpc) * inv_hp;
+}
+// out = S_LP / n_lp + (S_HP - S_LPc) / n_hp from the raw sums [3][n] (after the all-reduce over ranks)
+__global__ void tsm_combine_sums_kernel(double* __restrict__ out, const double* __restrict__ sums, double inv_lp,
+                                        double inv_hp, size_t n) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    out[i] = sums[i] * inv_lp + (sums[2 * n + i] - sums[n + i]) * inv_hp;
 }
 
 // binary storage (sec 2.1.1): file += x  |  file += x - y
@@ -81,14 +90,19 @@ extern "C" tm_status loop_binary_recover(tm_ctx* ctx, void* d_out, const void* d
                                          size_t len, void* stream) {
     if (!ctx || !d_out || !d_files || len == 0) return tm_fail(ctx, TM_EARG, "loop_binary_recover: bad argument");
     if (N < 1 || N > n_stored) return tm_fail(ctx, TM_EARG, "loop_binary_recover: need 1 <= N <= n_stored");
-    // file k is complete when all of its 2^k sources are in: 2^(k+1) - 1 <= n_stored
-    for (int k = 0; (1L << k) <= N; k++)
-        if (((N >> k) & 1) && ((1L << (k + 1)) - 1) > n_stored)
-            return tm_fail(ctx, TM_EARG, "loop_binary_recover: N needs a file that is not complete yet");
+    // "one can recover the data for any number of sources": N = n_stored is the sum of EVERY file, the
+    // partially filled last one included; any other N must be made of complete files (file k is complete when all of
+    // its 2^k sources are in: 2^(k+1) - 1 <= n_stored), named by its binary digits
+    unsigned mask = (unsigned)N;
+    if (N == n_stored) mask = (1u << loop_binary_nfiles(n_stored)) - 1u;
+    else
+        for (int k = 0; (1L << k) <= N; k++)
+            if (((N >> k) & 1) && ((1L << (k + 1)) - 1) > n_stored)
+                return tm_fail(ctx, TM_EARG, "loop_binary_recover: N needs a file that is not complete yet");
     TM_CUDA(ctx, cudaSetDevice(ctx->device));
     const size_t nr = 2 * len;
     binary_recover_kernel<<<(unsigned)((nr + 255) / 256), 256, 0, (cudaStream_t)stream>>>(
-        (double*)d_out, (const double*)d_files, (unsigned)N, 1.0 / N, nr);
+        (double*)d_out, (const double*)d_files, mask, 1.0 / N, nr);
     TM_LAUNCH_CHECK(ctx, "binary_recover_kernel");
     return TM_OK;
 }
@@ -116,11 +130,12 @@ struct TsmJob {
 
 struct TsmRun {
     tm_ctx* ctx; const tsm_params* P; void* d_per_source; void* d_files_lp; void* d_files_corr;
-    const unsigned char* z4; int z4_on_host;
+    const unsigned char* z4; int z4_on_host; int raw_sums;
+    long src_first, src_stride;       // local source j is global source src_first + j * src_stride (its noise stream)
     size_t nr, z4_bytes; unsigned agrid;
     double ms_lp, ms_hp, worst_lp, worst_hp; long it_lp, it_hp; int noconv;
     double* acc[TM_NLANES];         // per lane: S_lp, S_lpc, S_hp, tmp (nr doubles each)
-    int group;                      // sources per solve (1 | 2 | 4 | 8; TMLOOPS_GROUP, default TM_GROUP_DEFAULT)
+    int group;                      // sources per solve (1 | 2 | 4 | 8; TM_OPT_GROUP, default TM_GROUP_DEFAULT)
     double* lp_keep;                // [TM_MAXNB][nr]: l^LP of the pair whose HP pass comes next (binary files of the correction)
 };
 
@@ -150,7 +165,8 @@ static tm_status job_noise(TsmRun& R, int r, int b, tm_prec p, cudaStream_t st, 
     }
     const size_t fb = 2 * tm_parity_bytes(ctx, p);
     TM_TRY(tm_ws(ctx, p == TM_F32 ? WS_TSM_ETA32 : WS_TSM_ETA64, TM_MAXNB * fb, base));
-    return tm_z4_expand(ctx, (char*)*base + (size_t)b * fb, p, zsrc, R.P->seed, (unsigned long long)r, st);
+    return tm_z4_expand(ctx, (char*)*base + (size_t)b * fb, p, zsrc, R.P->seed,
+                        (unsigned long long)(R.src_first + (long)r * R.src_stride), st);
 }
 
 static tm_status job_start(TsmRun& R, TsmJob& J, int r, int nb, int pass, cudaStream_t st) {
@@ -183,6 +199,9 @@ static tm_status job_finish(TsmRun& R, TsmJob& J, int lane) {
         if (!(si[b].true_resid <= sp->rho * (1.0 + 1e-12))) R.noconv++;
         const size_t fbo = 2 * tm_parity_bytes(ctx, J.po);
         void *s_c = (char*)J.s_o + b * fbo, *eta_c = (char*)J.eta_o + b * fbo;
+        if (P->d_solutions)      // the run's own solution of this (source, pass), canonical layout, for the checker
+            TM_TRY(tm_export_launch(ctx, (char*)P->d_solutions + (size_t)(J.pass ? P->n_lp + r : r) * ctx->V * 12 * 16,
+                                    s_c, J.po, st));
         if (J.ac != J.po) {
             const size_t fba = 2 * tm_parity_bytes(ctx, J.ac);
             void* sbuf;
@@ -280,14 +299,14 @@ static tm_status tsm_pipeline(TsmRun& R, int NL, cudaStream_t st, void* d_out) {
     TsmLaneAcc LA;
     LA.n = NL;
     for (int l = 0; l < TM_NLANES; l++) LA.acc[l] = l < NL ? R.acc[l] : nullptr;
-    tsm_combine_kernel<<<R.agrid, 256, 0, st>>>((double*)d_out, LA, 1.0 / P->n_lp, P->n_hp ? 1.0 / P->n_hp : 0.0, R.nr);
+    tsm_combine_kernel<<<R.agrid, 256, 0, st>>>((double*)d_out, LA, 1.0 / P->n_lp, P->n_hp ? 1.0 / P->n_hp : 0.0, R.nr, R.raw_sums);
     TM_LAUNCH_CHECK(ctx, "tsm_combine_kernel");
     return TM_OK;
 }
 
 static tm_status tsm_core(tm_ctx* ctx, void* d_out, void* d_per_source, const tsm_params* P, tsm_info* info,
                           const unsigned char* z4, int z4_on_host, cudaStream_t st,
-                          void* d_files_lp = nullptr, void* d_files_corr = nullptr) {
+                          void* d_files_lp = nullptr, void* d_files_corr = nullptr, int raw_sums = 0) {
     if (!P || !d_out) return tm_fail(ctx, TM_EARG, "tsm_estimate: null argument");
     if (P->n_lp < 1 || P->n_hp < 0 || P->n_hp > P->n_lp)
         return tm_fail(ctx, TM_EARG, "tsm_estimate: need 1 <= n_lp and 0 <= n_hp <= n_lp");
@@ -308,7 +327,9 @@ static tm_status tsm_core(tm_ctx* ctx, void* d_out, void* d_per_source, const ts
     TsmRun R;
     memset(&R, 0, sizeof(R));
     R.ctx = ctx; R.P = P; R.d_per_source = d_per_source; R.d_files_lp = d_files_lp; R.d_files_corr = d_files_corr;
-    R.z4 = z4; R.z4_on_host = z4_on_host;
+    R.z4 = z4; R.z4_on_host = z4_on_host; R.raw_sums = raw_sums;
+    R.src_first = P->src_first; R.src_stride = P->src_stride > 0 ? P->src_stride : 1;
+    if (P->src_first < 0 || P->src_stride < 0) return tm_fail(ctx, TM_EARG, "tsm_estimate: src_first and src_stride must be >= 0");
     R.nr = 2 * (size_t)160 * P->nmom * ctx->X[3];                // doubles per per-source array
     R.z4_bytes = 3 * ctx->V;
     R.agrid = (unsigned)((R.nr + 255) / 256);
@@ -316,7 +337,7 @@ static tm_status tsm_core(tm_ctx* ctx, void* d_out, void* d_per_source, const ts
         // sources per solve: TM_GROUP_DEFAULT, reduced until the lanes' workspaces (noise + solution in outer precision,
         // 5 sloppy vectors, x and r, 3 outer-precision vectors per source; the HP pass is the larger one) stay below
         // 45 % of the device memory, so that a large lattice degrades to smaller groups instead of running out of
-        // memory (48^3x96: groups of 2).  TMLOOPS_GROUP overrides (tuning / tests).
+        // memory (48^3x96: groups of 4).  tm_set_option(TM_OPT_GROUP) overrides (tuning / tests).
         auto per_source = [&](const tm_solve_params& sp) {
             const double bo = (double)tm_parity_bytes(ctx, sp.outer), bs = (double)tm_parity_bytes(ctx, sp.sloppy);
             const double ba = (double)tm_parity_bytes(ctx, sp.sloppy == TM_F64 ? TM_F64 : TM_F32);
@@ -328,8 +349,7 @@ static tm_status tsm_core(tm_ctx* ctx, void* d_out, void* d_per_source, const ts
         TM_CUDA(ctx, cudaMemGetInfo(&free_b, &total_b));
         int gsz = TM_GROUP_DEFAULT;
         while (gsz > 1 && (double)gsz * TM_NLANES * need > 0.45 * (double)total_b) gsz /= 2;
-        const char* e = getenv("TMLOOPS_GROUP");
-        if (e) gsz = atoi(e);
+        if (ctx->opt_group) gsz = ctx->opt_group;          // tm_set_option(TM_OPT_GROUP)
         R.group = 1;
         while (2 * R.group <= gsz && 2 * R.group <= TM_MAXNB) R.group *= 2;
     }
@@ -378,6 +398,25 @@ extern "C" tm_status tsm_estimate(tm_ctx* ctx, void* d_out, void* d_per_source, 
                                   tsm_info* info, void* stream) {
     if (!ctx) return TM_EARG;
     return tsm_core(ctx, d_out, d_per_source, P, info, P ? P->d_z4 : nullptr, 0, (cudaStream_t)stream);
+}
+
+extern "C" tm_status tsm_partial_sums(tm_ctx* ctx, void* d_sums, void* d_per_source, const tsm_params* P,
+                                      tsm_info* info, void* stream) {
+    if (!ctx) return TM_EARG;
+    return tsm_core(ctx, d_sums, d_per_source, P, info, P ? P->d_z4 : nullptr, 0, (cudaStream_t)stream, nullptr, nullptr, 1);
+}
+
+extern "C" tm_status tsm_combine_sums(tm_ctx* ctx, void* d_out, const void* d_sums, int n_lp_total, int n_hp_total,
+                                      int nmom, void* stream) {
+    if (!ctx) return TM_EARG;
+    if (!d_out || !d_sums || n_lp_total < 1 || n_hp_total < 0 || nmom < 1)
+        return tm_fail(ctx, TM_EARG, "tsm_combine_sums: bad argument");
+    TM_CUDA(ctx, cudaSetDevice(ctx->device));
+    const size_t nr = 2 * (size_t)160 * nmom * ctx->X[3];
+    tsm_combine_sums_kernel<<<(unsigned)((nr + 255) / 256), 256, 0, (cudaStream_t)stream>>>(
+        (double*)d_out, (const double*)d_sums, 1.0 / n_lp_total, n_hp_total ? 1.0 / n_hp_total : 0.0, nr);
+    TM_LAUNCH_CHECK(ctx, "tsm_combine_sums_kernel");
+    return TM_OK;
 }
 
 extern "C" tm_status tsm_estimate_binary(tm_ctx* ctx, void* d_out, void* d_files_lp, void* d_files_corr,

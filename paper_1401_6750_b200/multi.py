@@ -1,9 +1,12 @@
 """Multi-GPU scale-out of the TSM loop: by source.
 
-Sources are independent, so every rank holds a full gauge replica, runs
-``tsm_estimate`` on its own block of sources and the only exchange is one all-reduce of the
-momentum-space estimate (160 * nmom * T complex128; 20 MB at 32^3x64) at the end.  No data-path
-collective exists inside the solver or the contraction.
+Sources are independent, so every rank holds a full gauge replica and runs the TSM loop on its own
+share of ONE (N_LP, N_HP) workload: rank k of W takes the global sources r = k, k + W, k + 2W, ... (``shard``), which
+spreads the first N_HP sources -- the ones that also get a high-precision solve -- evenly over the ranks.  The only
+exchange is one all-reduce (sum) of the three raw momentum-space accumulators S_LP, S_LPc, S_HP
+(3 x 160 * nmom * T complex128; 3 x 20 MB at 32^3x64) at the end; the division by N_LP and N_HP is done once, in the
+library (``tsm_combine_sums``).  No collective exists inside the solver or the contraction, so there is nothing to
+fuse with a compute kernel.  This module holds no TSM arithmetic: index bookkeeping and the collective only.
 """
 from __future__ import annotations
 
@@ -11,27 +14,38 @@ import torch
 import torch.distributed as dist
 
 
-def rank_seed(seed: int, rank: int) -> int:
-    """Noise seed of a rank: disjoint counter-hash streams per rank."""
-    return int(seed) + 1000003 * int(rank)
+def shard(n_lp_total: int, n_hp_total: int, rank: int, world: int):
+    """(n_lp_local, n_hp_local, src_first, src_stride) of rank `rank` of `world`: round-robin by global source index."""
+    if not (0 <= rank < world):
+        raise ValueError("shard: need 0 <= rank < world")
+    if n_hp_total > n_lp_total:
+        raise ValueError("shard: need n_hp_total <= n_lp_total")
+    n_lp = len(range(rank, n_lp_total, world))
+    n_hp = len(range(rank, n_hp_total, world))
+    return n_lp, n_hp, rank, world
 
 
-def combine_over_ranks(local_estimate: torch.Tensor, n_lp_local: int, n_hp_local: int, group=None) -> torch.Tensor:
-    """Global TSM estimate from per-rank estimates.
+def allreduce_sums(sums: torch.Tensor, group=None) -> torch.Tensor:
+    """In-place all-reduce (sum) of the raw accumulators [3, 2, 80, nmom, T] complex128 over the ranks."""
+    if dist.is_initialized() and dist.get_world_size(group) > 1:
+        buf = torch.view_as_real(sums)          # complex all-reduce through the real view (nccl and gloo alike)
+        dist.all_reduce(buf, op=dist.ReduceOp.SUM, group=group)
+    return sums
 
-    L = sum_ranks (n_lp_r / N_LP) L_r, valid when every rank has the same N_HP/N_LP ratio (then
-    the LP mean and the correction mean are both weighted by n_lp_r / N_LP); checked here."""
-    if not dist.is_initialized() or dist.get_world_size(group) == 1:
-        return local_estimate
-    counts = torch.tensor([float(n_lp_local), float(n_hp_local)], dtype=torch.float64, device=local_estimate.device)
-    allc = [torch.empty_like(counts) for _ in range(dist.get_world_size(group))]
-    dist.all_gather(allc, counts, group=group)
-    n_lp = sum(float(c[0]) for c in allc)
-    n_hp = sum(float(c[1]) for c in allc)
-    for c in allc:
-        if abs(float(c[1]) * n_lp - float(c[0]) * n_hp) > 1e-9 * max(1.0, n_lp * n_hp):
-            raise ValueError("combine_over_ranks: ranks must share the same N_HP / N_LP ratio")
-    # complex all-reduce through the real view (works for nccl and gloo alike)
-    buf = torch.view_as_real(local_estimate * (n_lp_local / n_lp)).contiguous()
-    dist.all_reduce(buf, op=dist.ReduceOp.SUM, group=group)
-    return torch.view_as_complex(buf)
+
+def tsm_estimate_sharded(ctx, n_lp_total, n_hp_total, kappa, mu, momenta, lp, hp, acc_lp, acc_hp, seed=0, z4=None,
+                         group=None, **kw):
+    """One (N_LP, N_HP) TSM workload split over the ranks of the process group: returns (estimate, info).
+
+    z4 (optional): this rank's packed noise, [n_lp_local, 3V], local source j = global source rank + j * world."""
+    rank = dist.get_rank(group) if dist.is_initialized() else 0
+    world = dist.get_world_size(group) if dist.is_initialized() else 1
+    n_lp, n_hp, first, stride = shard(n_lp_total, n_hp_total, rank, world)
+    shape = (3, 2, 80, len(momenta), ctx.T)
+    if n_lp > 0:
+        sums, _, info = ctx.tsm_estimate(n_lp, n_hp, kappa, mu, momenta, lp, hp, acc_lp, acc_hp, z4=z4, seed=seed,
+                                         src_first=first, src_stride=stride, partial_sums=True, **kw)
+    else:                                       # more ranks than sources: this rank contributes zeros
+        sums, info = torch.zeros(shape, dtype=torch.complex128, device=ctx.tdev), {}
+    allreduce_sums(sums, group)
+    return ctx.tsm_combine_sums(sums, n_lp_total, n_hp_total), info

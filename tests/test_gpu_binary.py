@@ -38,6 +38,39 @@ def test_accumulate_and_recover_vs_oracle(orc):
         assert rel_l2(to_np(ctx.loop_binary_recover(files, n, 13)), ps[sel].mean(axis=0)) <= 1e-15
         with pytest.raises(t.TmError):
             ctx.loop_binary_recover(files, n, 16)
+        # the headline run's counts: 500 sources and 20 corrections leave a partially filled last file; N = n_stored
+        # recovers everything stored ("for any number of sources"), the complete prefix still works
+        for n_big in (500, 20):
+            big = rng.normal(size=(n_big, 2, 5)) + 1j * rng.normal(size=(n_big, 2, 5))
+            d_big = torch.from_numpy(big).cuda()
+            files = torch.zeros((ctx.loop_binary_nfiles(n_big), 2, 5), dtype=torch.complex128, device="cuda")
+            for r in range(n_big):
+                ctx.loop_binary_accumulate(files, d_big[r], r)
+            ref_files, counts = orc.binary_store(big)
+            assert np.array_equal(to_np(files), ref_files)
+            full = 2 ** (len(counts) - 1) - 1
+            for N in (n_big, full, 1):
+                assert rel_l2(to_np(ctx.loop_binary_recover(files, n_big, N)), orc.binary_recover(ref_files, counts, N)) <= 1e-15
+            assert rel_l2(to_np(ctx.loop_binary_recover(files, n_big, n_big)), big.mean(axis=0)) <= 1e-14
+            with pytest.raises(t.TmError):
+                ctx.loop_binary_recover(files, n_big, n_big - 1 if (n_big - 1) > full else full + 1)
+
+
+def test_tsm_binary_partial_last_file(orc):
+    """A run whose counts are not 2^K - 1 (like 500 + 20) recovers its own full estimate from the files."""
+    t = tm()
+    dims, k, mu = C1["dims"], C1["kappa"], C1["mu"]
+    U = inputs.gauge_field(dims, C1["eps"], C1["seed"])
+    mom = inputs.momentum_list(1)
+    n_lp, n_hp = 6, 2
+    with t.TmContext(dims, -1) as ctx:
+        ctx.tm_load_gauge(U)
+        out, ps, _ = ctx.tsm_estimate(n_lp, n_hp, k, mu, mom, LP, HP, t.TM_F32, t.TM_F64, seed=9, per_source=True)
+        out2, f_lp, f_co, _ = ctx.tsm_estimate_binary(n_lp, n_hp, k, mu, mom, LP, HP, t.TM_F32, t.TM_F64, seed=9)
+        ps = to_np(ps)
+        rec = to_np(ctx.loop_binary_recover(f_lp, n_lp, n_lp)) + to_np(ctx.loop_binary_recover(f_co, n_hp, n_hp))
+        assert rel_l2(rec, to_np(out2)) <= 1e-13 and rel_l2(rec, to_np(out)) <= 1e-13
+        assert rel_l2(rec, orc.tsm_combine(ps[:n_lp], ps[n_lp:])) <= 1e-12
 
 
 def test_tsm_with_binary_files(orc):

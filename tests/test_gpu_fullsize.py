@@ -92,19 +92,19 @@ def test_contract_c4_sampled_timeslices(orc, c4, acc, tol):
                 assert e <= tol, (acc, ts, f, name, e)
 
 
-def test_tsm_c4_grouped_launches(orc, c4, monkeypatch):
+def test_tsm_c4_grouped_launches(orc, c4):
     """The launch configuration bench.py times: sources solved 8 per launch on two lanes.  Per-source arrays must be
     bit-identical to the one-source-per-launch path, and a grouped solution must pass the oracle's residual check."""
     t, ctx, U_h, eta = c4
     mom = inputs.momentum_list(9)
     n_lp, n_hp = 16, 8
-    monkeypatch.delenv("TMLOOPS_GROUP", raising=False)
+    ctx.tm_set_option(t.TM_OPT_GROUP, 0)
     out_g, ps_g, info_g = ctx.tsm_estimate(n_lp, n_hp, C4["kappa"], C4["mu"], mom, LP, HP, t.TM_F32, t.TM_F64,
                                            seed=C4["src_seed"], per_source=True)
-    monkeypatch.setenv("TMLOOPS_GROUP", "1")
+    ctx.tm_set_option(t.TM_OPT_GROUP, 1)
     out_1, ps_1, info_1 = ctx.tsm_estimate(n_lp, n_hp, C4["kappa"], C4["mu"], mom, LP, HP, t.TM_F32, t.TM_F64,
                                            seed=C4["src_seed"], per_source=True)
-    monkeypatch.delenv("TMLOOPS_GROUP", raising=False)
+    ctx.tm_set_option(t.TM_OPT_GROUP, 0)
     assert bool((ps_g == ps_1).all())
     assert info_g["launches"] * 4 < info_1["launches"]
     assert info_g["worst_resid_lp"] <= LP["rho"] and info_g["worst_resid_hp"] <= HP["rho"]
@@ -114,3 +114,28 @@ def test_tsm_c4_grouped_launches(orc, c4, monkeypatch):
     assert orc.true_residual(to_np(s), to_np(eta), U_h, C4["kappa"], C4["mu"], -1) <= LP["rho"]
     single = ctx.loop_contract_project(s, eta, C4["kappa"], C4["mu"], mom, t.TM_F32)
     assert rel_l2(to_np(ps_g[0]), to_np(single)) <= 1e-5
+
+
+def test_tsm_c4_run_solutions_inside_a_group(orc, c4):
+    """SURVEY.md sec 8 c.3 (1), (2) on the bench's launch configuration: the run's OWN solutions of sources inside a
+    group of 8 (not source 0), checked by the oracle -- true residual against that source's noise, and the oracle's
+    loops of the GPU's s on sampled timeslices against the run's per-source array (1e-5 fp32 / 1e-12 fp64)."""
+    from paper_1401_6750_b200 import inputs_torch
+    t, ctx, U_h, eta = c4
+    mom = inputs.momentum_list(9)
+    n_lp, n_hp = 8, 4
+    _, ps, info = ctx.tsm_estimate(n_lp, n_hp, C4["kappa"], C4["mu"], mom, LP, HP, t.TM_F32, t.TM_F64,
+                                   seed=C4["src_seed"], per_source=True, solutions=True)
+    sol = info["solutions"]
+    for j, ts in ((3, 17), (6, 63), (n_lp + 2, 0)):
+        r, rho, tol = (j, LP["rho"], 1e-5) if j < n_lp else (j - n_lp, HP["rho"], 1e-12)
+        eta_r = to_np(inputs_torch.z4_source(C4["dims"], C4["src_seed"], r, sol.device))
+        s_h = to_np(sol[j])
+        true = orc.true_residual(s_h, eta_r, U_h, C4["kappa"], C4["mu"], -1)
+        assert true <= rho, (j, true)
+        ref = orc.loops_project(s_h, eta_r, U_h, C4["kappa"], C4["mu"], mom, -1, ts, ts + 1)[..., ts]
+        got = to_np(ps[j])
+        for f in (0, 1):
+            for sl in (slice(0, 16), slice(16, 80)):
+                e = rel_l2(got[f, sl, :, ts], ref[f, sl])
+                assert e <= tol, (j, ts, f, sl, e)

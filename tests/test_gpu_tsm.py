@@ -98,23 +98,94 @@ def test_tsm_edge_cases(setup):
         assert e.value.status == t.TM_ENOCONV
 
 
-def test_tsm_grouped_solves_equal_single_source_solves(setup, monkeypatch):
+def test_tsm_grouped_solves_equal_single_source_solves(setup):
     """Sources are solved eight (four, two, one at the ragged end) per launch by default; every per-source array must be
-    bit-identical to the one-source-per-launch path (TMLOOPS_GROUP=1), for ragged N_LP / N_HP."""
+    bit-identical to the one-source-per-launch path (tm_set_option(TM_OPT_GROUP, 1)), for ragged N_LP / N_HP."""
     t = tm()
     dims, U, mom = setup
     k, mu = C1["kappa"], C1["mu"]
     with t.TmContext(dims, -1) as ctx:
         ctx.tm_load_gauge(U)
-        for n_lp, n_hp, group in ((7, 3, None), (19, 11, None), (9, 6, "4"), (5, 3, "2"), (2, 1, None)):
-            monkeypatch.delenv("TMLOOPS_GROUP", raising=False)
-            if group:
-                monkeypatch.setenv("TMLOOPS_GROUP", group)
+        with pytest.raises(t.TmError):
+            ctx.tm_set_option(t.TM_OPT_GROUP, 3)
+        with pytest.raises(t.TmError):
+            ctx.tm_set_option(7, 0)
+        for n_lp, n_hp, group in ((7, 3, 0), (19, 11, 0), (9, 6, 4), (5, 3, 2), (2, 1, 0)):
+            ctx.tm_set_option(t.TM_OPT_GROUP, group)
             out_p, ps_p, info_p = ctx.tsm_estimate(n_lp, n_hp, k, mu, mom, LP, HP, t.TM_F32, t.TM_F64, seed=3, per_source=True)
-            monkeypatch.setenv("TMLOOPS_GROUP", "1")
+            ctx.tm_set_option(t.TM_OPT_GROUP, 1)
             out_s, ps_s, info_s = ctx.tsm_estimate(n_lp, n_hp, k, mu, mom, LP, HP, t.TM_F32, t.TM_F64, seed=3, per_source=True)
-            monkeypatch.delenv("TMLOOPS_GROUP", raising=False)
+            ctx.tm_set_option(t.TM_OPT_GROUP, 0)
             assert np.array_equal(to_np(ps_p), to_np(ps_s)), (n_lp, n_hp)
             assert info_p["iters_lp"] == info_s["iters_lp"] and info_p["iters_hp"] == info_s["iters_hp"]
             assert info_p["launches"] < info_s["launches"]
             assert rel_l2(to_np(out_p), to_np(out_s)) <= 1e-13        # lanes sum the sources in another order
+
+
+def test_tsm_run_solutions_checked_by_oracle(orc, setup):
+    """SURVEY.md sec 8 c.3 steps (1), (2) done ON the run: tsm_estimate hands back its own solutions (d_solutions) and
+    the oracle evaluates, for EVERY source of a group of 8 plus a ragged tail (and both passes), the true residual
+    against that source's own noise and the loops of the GPU's own s -- a mis-paired (s, eta) inside a group fails
+    both.  Contractions of a given s: 1e-5 (fp32 accumulate, LP) / 1e-12 (fp64, HP) per block."""
+    t = tm()
+    dims, U, mom = setup
+    k, mu = C1["kappa"], C1["mu"]
+    n_lp, n_hp = 11, 3
+    with t.TmContext(dims, -1) as ctx:
+        ctx.tm_load_gauge(U)
+        out, ps, info = ctx.tsm_estimate(n_lp, n_hp, k, mu, mom, LP, HP, t.TM_F32, t.TM_F64, seed=C1["src_seed"],
+                                         per_source=True, solutions=True)
+        ps, sol = to_np(ps), to_np(info["solutions"])
+        out_plain, ps_plain, _ = ctx.tsm_estimate(n_lp, n_hp, k, mu, mom, LP, HP, t.TM_F32, t.TM_F64,
+                                                  seed=C1["src_seed"], per_source=True)
+        assert np.array_equal(to_np(ps_plain), ps) and np.array_equal(to_np(out_plain), to_np(out))
+    worst = 0.0
+    for j in range(n_lp + n_hp):
+        r, rho, tol = (j, LP["rho"], 1e-5) if j < n_lp else (j - n_lp, HP["rho"], 1e-12)
+        eta = inputs.z4_source(dims, C1["src_seed"], r)
+        true = orc.true_residual(sol[j], eta, U, k, mu, -1)
+        assert true <= rho, (j, true)
+        worst = max(worst, true) if j < n_lp else worst
+        ref = orc.loops_project(sol[j], eta, U, k, mu, mom, -1)
+        for f in (0, 1):
+            for sl in (slice(0, 16), slice(16, 80)):
+                assert rel_l2(ps[j][f, sl], ref[f, sl]) <= tol, (j, f, sl)
+    assert abs(worst - info["worst_resid_lp"]) <= 0.05 * LP["rho"]
+
+
+def test_tsm_sharded_partial_sums(orc, setup):
+    """SURVEY.md sec 8e on one device: the (N_LP, N_HP) workload split round-robin over W 'ranks' (src_first = k,
+    src_stride = W), each returning the raw accumulators S_LP, S_LPc, S_HP; their sum, combined by tsm_combine_sums,
+    equals the single-call estimate, and every shard's per-source arrays are those of the global sources it names."""
+    import torch
+    t = tm()
+    from paper_1401_6750_b200 import multi
+    dims, U, mom = setup
+    k, mu = C1["kappa"], C1["mu"]
+    n_lp, n_hp = 9, 3
+    with t.TmContext(dims, -1) as ctx:
+        ctx.tm_load_gauge(U)
+        out, ps, _ = ctx.tsm_estimate(n_lp, n_hp, k, mu, mom, LP, HP, t.TM_F32, t.TM_F64, seed=5, per_source=True)
+        ps = to_np(ps)
+        for W in (2, 4):
+            total = torch.zeros((3,) + tuple(out.shape), dtype=torch.complex128, device="cuda")
+            for rank in range(W):
+                nl, nh, first, stride = multi.shard(n_lp, n_hp, rank, W)
+                sums, ps_r, _ = ctx.tsm_estimate(nl, nh, k, mu, mom, LP, HP, t.TM_F32, t.TM_F64, seed=5, per_source=True,
+                                                 src_first=first, src_stride=stride, partial_sums=True)
+                ps_r, sums_h = to_np(ps_r), to_np(sums)
+                glob = list(range(rank, n_lp, W))
+                for j, r in enumerate(glob):
+                    assert np.array_equal(ps_r[j], ps[r]), (W, rank, j)
+                for j, r in enumerate(list(range(rank, n_hp, W))):
+                    assert np.array_equal(ps_r[nl + j], ps[n_lp + r]), (W, rank, j)
+                assert rel_l2(sums_h[0], ps_r[:nl].sum(axis=0)) <= 1e-14
+                if nh:
+                    assert rel_l2(sums_h[1], ps_r[:nh].sum(axis=0)) <= 1e-14
+                    assert rel_l2(sums_h[2], ps_r[nl:].sum(axis=0)) <= 1e-14
+                else:
+                    assert not sums_h[1].any() and not sums_h[2].any()
+                total += sums
+            got = to_np(ctx.tsm_combine_sums(total, n_lp, n_hp))
+            assert rel_l2(got, orc.tsm_combine(ps[:n_lp], ps[n_lp:])) <= 1e-12
+            assert rel_l2(got, to_np(out)) <= 1e-13

@@ -214,12 +214,23 @@ def test_binary_storage_fig2(orc):
         assert len(sel) == N
         assert np.allclose(orc.binary_recover(files, counts, N), ps[sel].mean(axis=0), atol=1e-14)
     assert np.allclose(orc.binary_recover(files, counts, 15), ps.mean(axis=0), atol=1e-14)
-    # an incomplete last file (13 sources generated) cannot serve N = 8..15, the complete ones still serve N <= 7
+    # an incomplete last file (13 sources generated) cannot serve N = 8..12, 14, 15; the complete ones still serve
+    # N <= 7, and N = 13 = everything stored so far is the sum of every file, the partial one included
+    # ("one can recover the data for any number of sources"): nothing is lost
     files, counts = orc.binary_store(ps[:13])
     assert list(counts) == [1, 2, 4, 6]
-    assert orc.binary_recover(files, counts, 13) is None and orc.binary_recover(files, counts, 16) is None
+    for N in (8, 9, 12, 14, 15, 16):
+        assert orc.binary_recover(files, counts, N) is None
     assert np.allclose(orc.binary_recover(files, counts, 7), ps[:7].mean(axis=0), atol=1e-14)
-    assert np.allclose(files.sum(axis=0) / 13, ps[:13].mean(axis=0), atol=1e-14)      # nothing is lost
+    assert np.allclose(orc.binary_recover(files, counts, 13), ps[:13].mean(axis=0), atol=1e-14)
+    # the headline run: 500 LP sources and 20 corrections are recoverable in full, brute force on the plain means
+    for n in (500, 20):
+        big = rng.normal(size=(n, 3)) + 1j * rng.normal(size=(n, 3))
+        files, counts = orc.binary_store(big)
+        assert int(counts.sum()) == n and counts[-1] != 2 ** (len(counts) - 1)
+        assert np.allclose(orc.binary_recover(files, counts, n), big.mean(axis=0), atol=1e-13)
+        full = 2 ** (len(counts) - 1) - 1                # the largest complete prefix (255 | 15)
+        assert np.allclose(orc.binary_recover(files, counts, full), big[:full].mean(axis=0), atol=1e-13)
     # O(log2 N) files
     assert [orc.binary_nfiles(n) for n in (1, 2, 3, 4, 7, 8, 500, 1023)] == [1, 2, 2, 3, 3, 4, 9, 10]
 
