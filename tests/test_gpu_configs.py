@@ -56,8 +56,9 @@ def test_c2_dslash_all_precisions_and_fp32_solve(orc):
                 ctx.tm_dslash(fout, fin, None, t.TM_OP_M_FULL, 0, False, c["kappa"], c["mu"], P, recon)
                 first = fout.clone()
                 assert rel_l2(to_np(ctx.tm_field_export(fout, P)), ref) <= TOL[prec], (prec, recon)
-                # "repeated applications": same input, same launch, same bits (no race, no stale state)
-                for _ in range(50):
+                # BASELINE.json configs[1]: "1000 repeated Dslash applications": same input, same launch, same bits
+                # (no race, no stale state)
+                for _ in range(1000):
                     ctx.tm_dslash(fout, fin, None, t.TM_OP_M_FULL, 0, False, c["kappa"], c["mu"], P, recon)
                 assert bool((fout == first).all()), (prec, recon)
         eta = inputs_torch.z4_source(c["dims"], c["src_seed"], 0, dev)

@@ -114,7 +114,7 @@ def test_contract_explicit_dw_variant(orc, acc):
     with t.TmContext(dims, -1) as ctx:
         ctx.tm_load_gauge(U)
         got = to_np(ctx.loop_contract_project_explicit(s, k, mu, mom, t.PREC[acc]))
-        check_blocks(got, ref, TOL[acc] * (3 if acc == "f32" else 1))      # one more fp32 operator application
+        check_blocks(got, ref, TOL[acc])       # north_star tolerance, no carve-out (measured: 9e-16 / 1.2e-7)
         # and it differs from the eta-based loops unless M s = eta
         eta = inputs.z4_source(dims, 1, 0)
         other = to_np(ctx.loop_contract_project(s, eta, k, mu, mom, t.PREC[acc]))
@@ -135,7 +135,7 @@ def test_contract_symmetrised_derivative_variant(orc, acc, tb):
     with t.TmContext(dims, tb) as ctx:
         ctx.tm_load_gauge(U)
         got = to_np(ctx.loop_contract_project_sym(s, eta, k, mu, mom, t.PREC[acc]))
-        check_blocks(got, ref, TOL[acc] * (4 if acc == "f32" else 50))     # differences of two O(1) passes
+        check_blocks(got, ref, TOL[acc])       # north_star tolerance, no carve-out (measured: 6e-16 / 1e-7)
         with pytest.raises(t.TmError):                                      # not closed under p -> -p
             ctx.loop_contract_project_sym(s, eta, k, mu, np.array([[1, 0, 0]], dtype=np.int32), t.PREC[acc])
 

@@ -56,7 +56,7 @@ def _oracle_D(orc, psi, U, tb, dagger):
     return psi - orc.apply_M(psi, U, 1.0, 0.0, tb, dagger)
 
 
-@pytest.mark.parametrize("prec", ["f64", "f32", "bf16"])
+@pytest.mark.parametrize("prec", ["f64", "f32", "f16", "bf16"])
 @pytest.mark.parametrize("dagger", [False, True])
 def test_parity_ops(orc, prec, dagger):
     """HOP, HOP_TWINV, XPAY and MHAT on one parity vs compositions of the oracle's full operator."""

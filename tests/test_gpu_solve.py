@@ -46,8 +46,9 @@ def test_solve_c1(orc, c1, sloppy, outer, recon, rho):
     assert info["iters"] > 0
     # reported residual is honest (outer-precision evaluation of the same quantity)
     assert abs(info["true_resid"] - true) <= 0.05 * rho + 1e-6 * (outer == "f32")
-    # sigma_max/sigma_min(M) ~ 20 on these fields: error <= cond * residual
-    assert rel_l2(s, s_ref) <= 40 * rho
+    # error <= cond(M) * residual with sigma_max/sigma_min(M) ~ 20 on these fields ("<~ 20 rho";
+    # measured 2.3 - 3.2 rho)
+    assert rel_l2(s, s_ref) <= 20 * rho
 
 
 def test_solve_medium_mixed(orc):

@@ -268,6 +268,38 @@ def test_explicit_dw_variant(orc):
     assert np.linalg.norm(a - b) <= 1e-10 * np.linalg.norm(a)
 
 
+def test_symmetrised_derivative_explicit_bilinears(orc, small_case):
+    """orc_loops_project_sym from its definition, written out with numpy and the oracle-independent dense D_m
+    (dense_ref.dense_cov_deriv) acting on BOTH s and psi: for every timeslice, momentum, family f, direction m and all
+    16 Gamma_n,   l_sym = sum_x e^{+ip.x} 1/2 [ s^dag g5 G_n (D_m psi) - (D_m s)^dag g5 G_n psi ](x),  psi = s | g.
+    A wrong sign of the second term, a missing 1/2, a conjugation slip or a family mix-up fails this."""
+    dims, k, mu, tb, U, eta, s = small_case
+    lx, ly, lz, lt = dims
+    V = int(np.prod(dims))
+    mom = inputs.momentum_list(2)
+    got = orc.loops_project_sym(s, eta, U, k, mu, mom, tb)
+    sf = s.reshape(V, 4, 3)
+    g = np.einsum("ab,xbc->xac", dr.GAMMA5, eta.reshape(V, 4, 3)) - 2j * k * mu * sf
+    fam = [sf, g]
+    zz, yy, xx = np.meshgrid(np.arange(lz), np.arange(ly), np.arange(lx), indexing="ij")
+    phases = [np.exp(2j * np.pi * (px * xx / lx + py * yy / ly + pz * zz / lz)) for px, py, pz in mom]
+    for m in range(4):
+        D = dr.dense_cov_deriv(U, dims, m, tb)
+        Ds = (D @ sf.ravel()).reshape(V, 4, 3)
+        for f in range(2):
+            Dpsi = (D @ fam[f].ravel()).reshape(V, 4, 3)
+            for n in range(16):
+                X = dr.GAMMA5 @ dr.big_gamma(n)
+                site = 0.5 * (np.einsum("xac,ab,xbc->x", sf.conj(), X, Dpsi)
+                              - np.einsum("xac,ab,xbc->x", Ds.conj(), X, fam[f]))
+                site = site.reshape(lt, lz, ly, lx)
+                for kk, ph in enumerate(phases):
+                    want = (site * ph[None]).sum(axis=(1, 2, 3))
+                    assert np.allclose(got[f, 16 + 16 * m + n, kk], want, atol=1e-12), (m, f, n, kk)
+    # the ultra-local entries are the plain ones
+    assert np.allclose(got[:, :16], orc.loops_project(s, eta, U, k, mu, mom, tb)[:, :16], atol=1e-13)
+
+
 def test_symmetrised_derivative_variant(orc):
     """Row f3 / reading 4: D<-> = (D-> - D<-)/2.  Pins: summation by parts (D_mu is anti-Hermitian, so at p = 0 the
     symmetrised and the right-acting loops coincide); for f = 0 and Hermitian g5 Gamma_n the symmetrised insertion
