@@ -73,9 +73,12 @@ const char* tm_last_error(const tm_ctx* ctx);
 typedef enum { TM_OPT_GROUP = 0, TM_OPT_CONTRACT_PATH = 1 } tm_option;
 tm_status tm_set_option(tm_ctx* ctx, tm_option opt, int value);
 
-/* d_U: device, canonical complex128 [V][4][3][3].  Copied into the context (fp64 master);
- * previously built reduced-precision copies are dropped. */
+/* d_U: device, canonical complex128 [V][4][3][3].  Copied into the context (fp64 master) asynchronously on stream;
+ * previously built reduced-precision copies are marked stale and repacked on their next use.
+ * tm_load_gauge_host: the same from HOST memory (pinned for a truly asynchronous copy); the buffer must stay valid
+ * until the stream has passed the call. */
 tm_status tm_load_gauge(tm_ctx* ctx, const void* d_U, void* stream);
+tm_status tm_load_gauge_host(tm_ctx* ctx, const void* h_U, void* stream);
 
 /* bytes of an internal field of the given storage precision (full_lattice: 0 = one parity). */
 size_t tm_field_bytes(const tm_ctx* ctx, tm_prec prec, int full_lattice);
@@ -122,6 +125,13 @@ tm_status tm_cg_solve(tm_ctx* ctx, void* d_s, const void* d_eta, double kappa, d
 tm_status loop_contract_project(tm_ctx* ctx, void* d_out, const void* d_s, const void* d_eta,
                                 double kappa, double mu, const int* h_momenta, int nmom,
                                 tm_prec acc, void* stream);
+
+/* The same call on fields that are already in the internal layout of precision acc (full-lattice fields made by
+ * tm_field_import: what the TSM loop hands to the contraction after a solve) -- no canonical -> internal conversion
+ * inside, so it times and profiles as the loop runs it.  d_s_int, d_eta_int: tm_field_bytes(acc, 1) bytes each. */
+tm_status loop_contract_project_fields(tm_ctx* ctx, void* d_out, const void* d_s_int, const void* d_eta_int,
+                                       double kappa, double mu, const int* h_momenta, int nmom,
+                                       tm_prec acc, void* stream);
 
 /* PAPER.md:88 ("GPU kernels to contract a single time slice or a whole vector", for time-dilution): the same call
  * restricted to ONE timeslice t0 -- 1/T of the work.  d_out keeps the shape [2][80][nmom][T]: column t0 is
@@ -177,10 +187,16 @@ tm_status tsm_partial_sums(tm_ctx* ctx, void* d_sums, void* d_per_source, const 
                            tsm_info* info, void* stream);
 tm_status tsm_combine_sums(tm_ctx* ctx, void* d_out, const void* d_sums, int n_lp_total, int n_hp_total,
                            int nmom, void* stream);
-/* Same with HOST buffers: h_z4 (pinned or pageable host memory, may be NULL -> seed) is copied
- * to the device source by source and h_out is copied back, all inside the call. */
+/* Same with HOST buffers (PAPER.md:104-106 names source generation and transfers as the bottlenecks of the paper's own
+ * code; Fig. 4 / PAPER.md:115 is the all-on-GPU scheme): h_z4 (pinned or pageable host memory, [n_lp][3V] bytes, may be
+ * NULL -> seed) is uploaded by a copy stream in group-sized chunks that run ahead of the solves (the whole packed noise
+ * stays resident on the device when it fits a quarter of the free memory, else it is staged source by source), and
+ * h_out (complex128 [2][80][nmom][T]) is copied back, all inside the call, which returns after the copy back.
+ * tsm_partial_sums_host: the same for the raw accumulators, h_sums = complex128 [3][2][80][nmom][T]. */
 tm_status tsm_estimate_host(tm_ctx* ctx, void* h_out, const unsigned char* h_z4,
                             const tsm_params* params, tsm_info* info, void* stream);
+tm_status tsm_partial_sums_host(tm_ctx* ctx, void* h_sums, const unsigned char* h_z4,
+                                const tsm_params* params, tsm_info* info, void* stream);
 
 /* sec 2.1.1 (Fig. 2): binary storage of partial sums, on the device, in momentum space.
  * File k = 0, 1, 2, ... (the paper's File.2^k) holds the SUM of the per-source arrays of the 2^k sources

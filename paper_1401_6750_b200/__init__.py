@@ -33,7 +33,8 @@ EXPORTS = [
     "tm_create", "tm_destroy", "tm_last_error", "tm_load_gauge", "tm_field_bytes",
     "tm_field_import", "tm_field_export", "tm_dslash", "tm_dslash_multi", "tm_cg_solve", "loop_contract_project",
     "loop_contract_project_explicit", "loop_contract_project_sym", "loop_contract_project_timeslice",
-    "tsm_estimate", "tsm_estimate_host", "tm_launch_count", "tm_set_option", "tsm_partial_sums", "tsm_combine_sums",
+    "loop_contract_project_fields",
+    "tsm_estimate", "tsm_estimate_host", "tsm_partial_sums_host", "tm_load_gauge_host", "tm_launch_count", "tm_set_option", "tsm_partial_sums", "tsm_combine_sums",
     "tm_fma_peak",
     "loop_binary_nfiles", "loop_binary_accumulate", "loop_binary_recover", "tsm_estimate_binary",
 ]
@@ -93,6 +94,7 @@ def load_library():
     L.tm_last_error.argtypes = [vp]
     L.tm_last_error.restype = ctypes.c_char_p
     L.tm_load_gauge.argtypes = [vp, vp, vp]
+    L.tm_load_gauge_host.argtypes = [vp, vp, vp]
     L.tm_field_bytes.argtypes = [vp, ci, ci]
     L.tm_field_bytes.restype = ctypes.c_size_t
     L.tm_field_import.argtypes = [vp, vp, vp, ci, vp]
@@ -102,11 +104,13 @@ def load_library():
     L.tm_cg_solve.argtypes = [vp, vp, vp, cd, cd, ctypes.POINTER(tm_solve_params),
                               ctypes.POINTER(tm_solve_info), vp]
     L.loop_contract_project.argtypes = [vp, vp, vp, vp, cd, cd, ctypes.POINTER(ci), ci, ci, vp]
+    L.loop_contract_project_fields.argtypes = [vp, vp, vp, vp, cd, cd, ctypes.POINTER(ci), ci, ci, vp]
     L.loop_contract_project_timeslice.argtypes = [vp, vp, vp, vp, cd, cd, ctypes.POINTER(ci), ci, ci, ci, vp]
     L.loop_contract_project_sym.argtypes = [vp, vp, vp, vp, cd, cd, ctypes.POINTER(ci), ci, ci, vp]
     L.loop_contract_project_explicit.argtypes = [vp, vp, vp, cd, cd, ctypes.POINTER(ci), ci, ci, vp]
     L.tsm_estimate.argtypes = [vp, vp, vp, ctypes.POINTER(tsm_params), ctypes.POINTER(tsm_info), vp]
     L.tsm_estimate_host.argtypes = [vp, vp, vp, ctypes.POINTER(tsm_params), ctypes.POINTER(tsm_info), vp]
+    L.tsm_partial_sums_host.argtypes = [vp, vp, vp, ctypes.POINTER(tsm_params), ctypes.POINTER(tsm_info), vp]
     L.loop_binary_nfiles.argtypes = [ci]
     L.loop_binary_nfiles.restype = ci
     L.loop_binary_accumulate.argtypes = [vp, vp, vp, ci, ctypes.c_size_t, vp]
@@ -210,8 +214,15 @@ class TmContext:
         torch = _torch()
         U = self._dev(U, torch.complex128)
         assert U.numel() == self.V * 36
-        self._check(self.lib.tm_load_gauge(self.h, U.data_ptr(), _stream()))
-        torch.cuda.current_stream().synchronize()
+        self._check(self.lib.tm_load_gauge(self.h, U.data_ptr(), _stream()))     # stream-ordered, like U's own lifetime
+
+    def tm_load_gauge_host(self, U_host):
+        """U_host: CPU complex128 tensor [T,Lz,Ly,Lx,4,3,3] (pinned: asynchronous upload straight into the context's master).
+        The caller keeps it alive and unchanged until the stream has passed the copy."""
+        torch = _torch()
+        assert U_host.device.type == "cpu" and U_host.dtype == torch.complex128 and U_host.is_contiguous()
+        assert U_host.numel() == self.V * 36
+        self._check(self.lib.tm_load_gauge_host(self.h, U_host.data_ptr(), _stream()))
 
     def tm_field_bytes(self, prec, full_lattice=True) -> int:
         return int(self.lib.tm_field_bytes(self.h, int(prec), 1 if full_lattice else 0))
@@ -289,6 +300,17 @@ class TmContext:
         out = torch.empty((2, 80, len(mom), self.T), dtype=torch.complex128, device=self.tdev)
         self._check(self.lib.loop_contract_project(
             self.h, out.data_ptr(), s.data_ptr(), eta.data_ptr(), float(kappa), float(mu),
+            mom.ctypes.data_as(ctypes.POINTER(ctypes.c_int)), len(mom), int(acc), _stream()))
+        return out
+
+    def loop_contract_project_fields(self, s_int, eta_int, kappa, mu, momenta, acc=TM_F32, out=None):
+        """loop_contract_project on internal-layout fields (tm_field_import(.., acc)): no layout conversion inside."""
+        torch = _torch()
+        mom = np.ascontiguousarray(momenta, dtype=np.int32).reshape(-1, 3)
+        if out is None:
+            out = torch.empty((2, 80, len(mom), self.T), dtype=torch.complex128, device=self.tdev)
+        self._check(self.lib.loop_contract_project_fields(
+            self.h, out.data_ptr(), s_int.data_ptr(), eta_int.data_ptr(), float(kappa), float(mu),
             mom.ctypes.data_as(ctypes.POINTER(ctypes.c_int)), len(mom), int(acc), _stream()))
         return out
 
@@ -435,9 +457,11 @@ class TmContext:
         return out, f_lp, (f_co if n_hp else None), self._tsm_info(info, st)
 
     def tsm_estimate_host(self, n_lp, n_hp, kappa, mu, momenta, lp, hp, acc_lp=TM_F32, acc_hp=TM_F64,
-                          z4_host=None, seed=0, out_host=None, raise_on_noconv=True):
-        """Same through HOST buffers: z4_host (numpy/torch CPU uint8 [n_lp,3V], pinned or not) is
-        uploaded source by source and the result is copied back inside the call."""
+                          z4_host=None, seed=0, out_host=None, raise_on_noconv=True,
+                          src_first=0, src_stride=1, partial_sums=False):
+        """Same through HOST buffers: z4_host (numpy/torch CPU uint8 [n_lp,3V], pinned or not) is uploaded by a copy
+        stream running ahead of the solves and the result (partial_sums: the raw accumulators [3,2,80,nmom,T]) is
+        copied back inside the call."""
         torch = _torch()
         h_z4 = None
         if z4_host is not None:
@@ -446,11 +470,15 @@ class TmContext:
             assert z4_host.device.type == "cpu" and z4_host.dtype == torch.uint8 and z4_host.is_contiguous()
             assert z4_host.numel() == n_lp * 3 * self.V
             h_z4 = z4_host.data_ptr()
-        P, mom = self._tsm_params(n_lp, n_hp, kappa, mu, momenta, lp, hp, acc_lp, acc_hp, None, seed)
+        P, mom = self._tsm_params(n_lp, n_hp, kappa, mu, momenta, lp, hp, acc_lp, acc_hp, None, seed, src_first, src_stride)
+        shape = (2, 80, len(mom), self.T)
+        if partial_sums:
+            shape = (3,) + shape
         if out_host is None:
-            out_host = torch.empty((2, 80, len(mom), self.T), dtype=torch.complex128).pin_memory()
+            out_host = torch.empty(shape, dtype=torch.complex128).pin_memory()
+        assert out_host.device.type == "cpu" and out_host.dtype == torch.complex128 and tuple(out_host.shape) == shape
         info = tsm_info()
-        st = self.lib.tsm_estimate_host(self.h, out_host.data_ptr(), h_z4, ctypes.byref(P),
-                                        ctypes.byref(info), _stream())
+        fn = self.lib.tsm_partial_sums_host if partial_sums else self.lib.tsm_estimate_host
+        st = fn(self.h, out_host.data_ptr(), h_z4, ctypes.byref(P), ctypes.byref(info), _stream())
         self._check(st, allow=() if raise_on_noconv else (TM_ENOCONV,))
         return out_host, self._tsm_info(info, st)

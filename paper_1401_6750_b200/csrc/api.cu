@@ -113,7 +113,7 @@ extern "C" tm_status tm_set_option(tm_ctx* c, tm_option opt, int value) {
 static void drop_gauge_copies(tm_ctx* c) {
     for (int p = 0; p < 4; p++)
         for (int r = 0; r < 2; r++)
-            if (c->gauge[p][r]) { cudaFree(c->gauge[p][r]); c->gauge[p][r] = nullptr; }
+            if (c->gauge[p][r]) { cudaFree(c->gauge[p][r]); c->gauge[p][r] = nullptr; c->gauge_valid[p][r] = 0; }
 }
 
 extern "C" tm_status tm_destroy(tm_ctx* c) {
@@ -122,6 +122,7 @@ extern "C" tm_status tm_destroy(tm_ctx* c) {
     cudaDeviceSynchronize();
     drop_gauge_copies(c);
     if (c->d_Ucanon) cudaFree(c->d_Ucanon);
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     lane_park(c, &c->lanes[c->cur_lane]);
     for (int l = 0; l < TM_NLANES; l++) {
         TmLane* L = &c->lanes[l];
@@ -159,19 +160,28 @@ tm_status tm_ws(tm_ctx* c, int slot, size_t bytes, void** out) {
     return TM_OK;
 }
 
-extern "C" tm_status tm_load_gauge(tm_ctx* c, const void* d_U, void* stream) {
-    if (!c || !d_U) return tm_fail(c, TM_EARG, "tm_load_gauge: null argument");
-    cudaStream_t st = (cudaStream_t)stream;
+// A new master: the reduced-precision copies keep their allocations and are marked stale (repacked from the master on
+// their next use, on the stream of that use), so loading a gauge field costs one copy and no synchronisation.
+static tm_status load_gauge_impl(tm_ctx* c, const void* U, cudaMemcpyKind kind, cudaStream_t st) {
     TM_CUDA(c, cudaSetDevice(c->device));
     const size_t bytes = c->V * 4 * 9 * 16;
     if (!c->d_Ucanon) {
         cudaError_t e = cudaMalloc(&c->d_Ucanon, bytes);
         if (e != cudaSuccess) { cudaGetLastError(); c->d_Ucanon = nullptr; return tm_fail(c, TM_EALLOC, "tm_load_gauge: out of device memory"); }
     }
-    TM_CUDA(c, cudaStreamSynchronize(st));
-    drop_gauge_copies(c);
-    TM_CUDA(c, cudaMemcpyAsync(c->d_Ucanon, d_U, bytes, cudaMemcpyDeviceToDevice, st));
+    memset(c->gauge_valid, 0, sizeof(c->gauge_valid));
+    TM_CUDA(c, cudaMemcpyAsync(c->d_Ucanon, U, bytes, kind, st));
     return TM_OK;
+}
+
+extern "C" tm_status tm_load_gauge(tm_ctx* c, const void* d_U, void* stream) {
+    if (!c || !d_U) return tm_fail(c, TM_EARG, "tm_load_gauge: null argument");
+    return load_gauge_impl(c, d_U, cudaMemcpyDeviceToDevice, (cudaStream_t)stream);
+}
+
+extern "C" tm_status tm_load_gauge_host(tm_ctx* c, const void* h_U, void* stream) {
+    if (!c || !h_U) return tm_fail(c, TM_EARG, "tm_load_gauge_host: null argument");
+    return load_gauge_impl(c, h_U, cudaMemcpyHostToDevice, (cudaStream_t)stream);
 }
 
 extern "C" size_t tm_field_bytes(const tm_ctx* c, tm_prec prec, int full_lattice) {

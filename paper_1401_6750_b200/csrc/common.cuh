@@ -62,6 +62,8 @@ struct tm_ctx {
     long launches;
     void* d_Ucanon;                 // fp64 master, canonical [V][4][3][3] complex128
     void* gauge[4][2];              // [prec][recon==12] internal copies, built lazily
+    int gauge_valid[4][2];          // 0: allocated but stale (a new master was loaded) -> repacked on next use
+    cudaStream_t copy_stream;       // host -> device prefetch of the packed noise (tsm_estimate_host), created on first use
     // reduction scratch
     double* d_partials;             // per-block partial sums
     unsigned int* d_counter;        // last-block-done counter

@@ -510,6 +510,15 @@ extern "C" tm_status loop_contract_project(tm_ctx* ctx, void* d_out, const void*
     return tm_contract_internal(ctx, d_out, si, ei, kappa, mu, h_momenta, nmom, acc, st);
 }
 
+extern "C" tm_status loop_contract_project_fields(tm_ctx* ctx, void* d_out, const void* d_s_int, const void* d_eta_int,
+                                                  double kappa, double mu, const int* h_momenta, int nmom,
+                                                  tm_prec acc, void* stream) {
+    if (!ctx || !d_out || !d_s_int || !d_eta_int) return tm_fail(ctx, TM_EARG, "loop_contract_project_fields: null argument");
+    if (acc != TM_F64 && acc != TM_F32) return tm_fail(ctx, TM_EPREC, "loop_contract_project_fields: acc must be f32 or f64");
+    TM_CUDA(ctx, cudaSetDevice(ctx->device));
+    return tm_contract_internal(ctx, d_out, d_s_int, d_eta_int, kappa, mu, h_momenta, nmom, acc, (cudaStream_t)stream);
+}
+
 extern "C" tm_status loop_contract_project_explicit(tm_ctx* ctx, void* d_out, const void* d_s, double kappa, double mu,
                                                     const int* h_momenta, int nmom, tm_prec acc, void* stream) {
     if (!ctx || !d_out || !d_s) return tm_fail(ctx, TM_EARG, "loop_contract_project_explicit: null argument");

@@ -50,7 +50,7 @@ tm_status tm_get_gauge(tm_ctx* ctx, tm_prec prec, tm_recon recon, cudaStream_t s
     if ((int)prec < 0 || (int)prec > 3) return tm_fail(ctx, TM_EPREC, "unknown precision");
     const int r = (recon == TM_R12) ? 1 : 0;
     void** slot = &ctx->gauge[prec][r];
-    if (!*slot) {
+    if (!*slot || !ctx->gauge_valid[prec][r]) {
         tm_status s = TM_OK;
         switch (prec) {
             case TM_F64:  s = r ? gauge_pack_t<double, 12>(ctx, slot, st) : gauge_pack_t<double, 18>(ctx, slot, st); break;
@@ -59,6 +59,7 @@ tm_status tm_get_gauge(tm_ctx* ctx, tm_prec prec, tm_recon recon, cudaStream_t s
             case TM_BF16: s = r ? gauge_pack_t<__nv_bfloat16, 12>(ctx, slot, st) : gauge_pack_t<__nv_bfloat16, 18>(ctx, slot, st); break;
         }
         TM_TRY(s);
+        ctx->gauge_valid[prec][r] = 1;
     }
     *out = *slot;
     return TM_OK;

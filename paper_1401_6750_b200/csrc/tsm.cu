@@ -137,6 +137,10 @@ struct TsmRun {
     double* acc[TM_NLANES];         // per lane: S_lp, S_lpc, S_hp, tmp (nr doubles each)
     int group;                      // sources per solve (1 | 2 | 4 | 8; TM_OPT_GROUP, default TM_GROUP_DEFAULT)
     double* lp_keep;                // [TM_MAXNB][nr]: l^LP of the pair whose HP pass comes next (binary files of the correction)
+    // host noise (tsm_estimate_host): the whole packed noise of the run is prefetched into one device buffer on the
+    // context's copy stream, one chunk (= one group of sources) and one event at a time, while earlier groups solve
+    unsigned char* z4_all;          // device [n_lp][3V] (NULL: per-source staging on the lane's own stream)
+    std::vector<cudaEvent_t>* z4_ev;    // event of chunk k = sources [k * group, (k + 1) * group)
 };
 
 // lane-private buffers of the active lane
@@ -153,7 +157,10 @@ static tm_status job_noise(TsmRun& R, int r, int b, tm_prec p, cudaStream_t st, 
     tm_ctx* ctx = R.ctx;
     const unsigned char* zsrc = nullptr;
     if (R.z4) {
-        if (R.z4_on_host) {
+        if (R.z4_on_host && R.z4_all) {
+            TM_CUDA(ctx, cudaStreamWaitEvent(st, (*R.z4_ev)[r / R.group], 0));
+            zsrc = R.z4_all + (size_t)r * R.z4_bytes;
+        } else if (R.z4_on_host) {
             // staged per lane and slot: the previous user of the slot (a z4_expand of this lane) finished before
             // that lane's solve was waited for
             void* slot;
@@ -362,7 +369,37 @@ static tm_status tsm_core(tm_ctx* ctx, void* d_out, void* d_per_source, const ts
     }
     cudaEvent_t e0 = ctx->ev[2], e1 = ctx->ev[3];
     TM_CUDA(ctx, cudaEventRecord(e0, st));
+    std::vector<cudaEvent_t> z4_events;
+    if (z4 && z4_on_host) {
+        // 180 GB of HBM: the packed noise of a whole run (3V bytes per source: 3.1 GB for 500 sources at 32^3x64) stays
+        // resident.  It is uploaded on the copy stream in group-sized chunks behind the caller's stream (e0), each chunk
+        // with its own event, so only the first group's copy is exposed; the lanes wait per chunk (job_noise).  A run whose
+        // noise would take more than a quarter of the free memory keeps the per-source staging on the lane's stream.
+        size_t free_b = 0, total_b = 0;
+        TM_CUDA(ctx, cudaMemGetInfo(&free_b, &total_b));
+        const size_t all = (size_t)P->n_lp * R.z4_bytes;
+        void* buf = nullptr;
+        if (all <= free_b / 4 + ctx->scratch_bytes[WS_TSM_Z4] && tm_ws(ctx, WS_TSM_Z4, all, &buf) == TM_OK) {
+            if (!ctx->copy_stream) TM_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
+            TM_CUDA(ctx, cudaStreamWaitEvent(ctx->copy_stream, e0, 0));
+            R.z4_all = (unsigned char*)buf;
+            R.z4_ev = &z4_events;
+            for (int r0 = 0; r0 < P->n_lp; r0 += R.group) {
+                const int n = P->n_lp - r0 < R.group ? P->n_lp - r0 : R.group;
+                TM_CUDA(ctx, cudaMemcpyAsync(R.z4_all + (size_t)r0 * R.z4_bytes, z4 + (size_t)r0 * R.z4_bytes,
+                                             (size_t)n * R.z4_bytes, cudaMemcpyHostToDevice, ctx->copy_stream));
+                cudaEvent_t ev;
+                TM_CUDA(ctx, cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
+                z4_events.push_back(ev);
+                TM_CUDA(ctx, cudaEventRecord(ev, ctx->copy_stream));
+            }
+        } else cudaGetLastError();
+    }
     tm_status s = tsm_pipeline(R, NL, st, d_out);
+    if (!z4_events.empty()) {
+        if (s != TM_OK) cudaStreamSynchronize(ctx->copy_stream);
+        for (cudaEvent_t ev : z4_events) cudaEventDestroy(ev);     // deferred by the runtime until the event has completed
+    }
     if (s != TM_OK) {
         // leave no lane running behind the caller's back
         for (int l = 1; l < NL; l++)
@@ -425,18 +462,29 @@ extern "C" tm_status tsm_estimate_binary(tm_ctx* ctx, void* d_out, void* d_files
     return tsm_core(ctx, d_out, nullptr, P, info, P ? P->d_z4 : nullptr, 0, (cudaStream_t)stream, d_files_lp, d_files_corr);
 }
 
-extern "C" tm_status tsm_estimate_host(tm_ctx* ctx, void* h_out, const unsigned char* h_z4, const tsm_params* P,
-                                       tsm_info* info, void* stream) {
-    if (!ctx) return TM_EARG;
+static tm_status tsm_host(tm_ctx* ctx, void* h_out, const unsigned char* h_z4, const tsm_params* P, tsm_info* info,
+                          cudaStream_t st, int raw_sums) {
     if (!h_out || !P) return tm_fail(ctx, TM_EARG, "tsm_estimate_host: null argument");
-    cudaStream_t st = (cudaStream_t)stream;
+    if (P->nmom < 1) return tm_fail(ctx, TM_EARG, "tsm_estimate_host: need at least one momentum");
     TM_CUDA(ctx, cudaSetDevice(ctx->device));
-    const size_t bytes = (size_t)160 * P->nmom * ctx->X[3] * 16;
+    const size_t bytes = (size_t)(raw_sums ? 3 : 1) * 160 * P->nmom * ctx->X[3] * 16;
     void* d_out;
     TM_TRY(tm_ws(ctx, WS_API_B, bytes, &d_out));
-    tm_status s = tsm_core(ctx, d_out, nullptr, P, info, h_z4, 1, st);
+    tm_status s = tsm_core(ctx, d_out, nullptr, P, info, h_z4, 1, st, nullptr, nullptr, raw_sums);
     if (s != TM_OK && s != TM_ENOCONV) return s;
     TM_CUDA(ctx, cudaMemcpyAsync(h_out, d_out, bytes, cudaMemcpyDeviceToHost, st));
     TM_CUDA(ctx, cudaStreamSynchronize(st));
     return s;
+}
+
+extern "C" tm_status tsm_estimate_host(tm_ctx* ctx, void* h_out, const unsigned char* h_z4, const tsm_params* P,
+                                       tsm_info* info, void* stream) {
+    if (!ctx) return TM_EARG;
+    return tsm_host(ctx, h_out, h_z4, P, info, (cudaStream_t)stream, 0);
+}
+
+extern "C" tm_status tsm_partial_sums_host(tm_ctx* ctx, void* h_sums, const unsigned char* h_z4, const tsm_params* P,
+                                           tsm_info* info, void* stream) {
+    if (!ctx) return TM_EARG;
+    return tsm_host(ctx, h_sums, h_z4, P, info, (cudaStream_t)stream, 1);
 }

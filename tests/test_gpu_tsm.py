@@ -56,6 +56,12 @@ def test_tsm_decomposition(orc, setup):
         # host-buffer entry point == device entry point
         out3, _ = ctx.tsm_estimate_host(n_lp, n_hp, k, mu, mom, LP, HP, t.TM_F32, t.TM_F64, z4_host=z4)
         assert np.array_equal(out3.numpy(), out)
+        # gauge field uploaded from pinned host memory (stale copies repacked) + raw accumulators through the host entry
+        import torch
+        ctx.tm_load_gauge_host(torch.from_numpy(np.ascontiguousarray(U)).pin_memory())
+        sums, _ = ctx.tsm_estimate_host(n_lp, n_hp, k, mu, mom, LP, HP, t.TM_F32, t.TM_F64, z4_host=z4, partial_sums=True)
+        out4 = ctx.tsm_combine_sums(sums.to(ctx.tdev), n_lp, n_hp)
+        assert rel_l2(to_np(out4), out) <= 1e-14
 
 
 def test_tsm_identity_nlp_equals_nhp(orc, setup):
