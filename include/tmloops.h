@@ -198,6 +198,26 @@ tm_status tsm_estimate_host(tm_ctx* ctx, void* h_out, const unsigned char* h_z4,
 tm_status tsm_partial_sums_host(tm_ctx* ctx, void* h_sums, const unsigned char* h_z4,
                                 const tsm_params* params, tsm_info* info, void* stream);
 
+/* Row f4 of SURVEY.md sec 8 -- time dilution ("we also worked with time-dilution [6], so there are GPU
+ * kernels to contract a single time slice or a whole vector"; it combines with the TSM; reading 22).
+ *
+ * loop_plain_project_timeslice: the plain bilinears of a pair (a, b) on timeslice t0 (t0 = -1: on every timeslice),
+ *   d_out[(i*nmom + k)*T + t] = sum_{x,y,z} exp(+2 pi i p_k.x / L) a(x,t)^dag X_i b(x,t),
+ *   X_n = G_n (n < 16), X_{16+16m+n} = G_n D_m (D_m acting on b);  columns t != t0 are set to zero.
+ * d_a, d_b: device canonical complex128 spinors; d_out: device complex128 [80][nmom][T].
+ *
+ * tsm_estimate_time_diluted: the TSM estimator of the time-diluted plain loops.  For every noise vector r and every
+ * timeslice t0: eta_r^(t0) = eta_r restricted to t0, M s = eta_r^(t0) (LP for all r, HP as well for r < n_hp; the T
+ * diluted sources of a noise vector are solved 8 per launch), l_r[i][k][t0] = the bilinear above of (eta_r^(t0), s) on
+ * timeslice t0 -- T solves and T single-timeslice contractions per noise vector and pass -- then
+ *   d_out = (1/n_lp) sum_r l_r^LP + (1/n_hp) sum_{r<n_hp} (l_r^HP - l_r^LP)          complex128 [80][nmom][T].
+ * d_per_source: optional (NULL ok) [n_lp + n_hp][80][nmom][T].  params as for tsm_estimate (d_solutions is not used);
+ * TM_ENOCONV if any solve missed its rho (outputs still filled).  Synchronises the stream at the end. */
+tm_status loop_plain_project_timeslice(tm_ctx* ctx, void* d_out, const void* d_a, const void* d_b,
+                                       const int* h_momenta, int nmom, int t0, tm_prec acc, void* stream);
+tm_status tsm_estimate_time_diluted(tm_ctx* ctx, void* d_out, void* d_per_source, const tsm_params* params,
+                                    tsm_info* info, void* stream);
+
 /* sec 2.1.1 (Fig. 2): binary storage of partial sums, on the device, in momentum space.
  * File k = 0, 1, 2, ... (the paper's File.2^k) holds the SUM of the per-source arrays of the 2^k sources
  * r = 2^k - 1 ... 2^(k+1) - 2, so n sources need loop_binary_nfiles(n) = ceil(log2(n + 1)) arrays instead of n.

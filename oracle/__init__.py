@@ -210,3 +210,46 @@ def loops_project_sym(s, eta, U, kappa, mu, momenta, tb=-1, t0=0, t1=None) -> np
                                 ctypes.c_double(mu), mom.ctypes.data_as(ctypes.c_void_p),
                                 ctypes.c_int(len(mom)), ctypes.c_int(t0), ctypes.c_int(t1))
     return out
+
+
+# ---------------------------------------------------------------------------- time dilution (row f4)
+def time_dilute(eta, t0: int) -> np.ndarray:
+    """eta^(t0): the noise vector restricted to timeslice t0 (reading 22)."""
+    eta, p_eta = _c(eta)
+    out = np.empty_like(eta)
+    lib().orc_time_dilute(out.ctypes.data_as(ctypes.c_void_p), p_eta, _dims(dims_of(eta)), ctypes.c_int(t0))
+    return out
+
+
+def plain_loops_project(a, b, U, momenta, tb=-1, t0=0, t1=None) -> np.ndarray:
+    """Plain bilinears sum_x e^{ipx} a^dag X_i b per timeslice, [80, nmom, T]; X_n = Gamma_n, X_{16+16m+n} = Gamma_n D_m
+    (D_m on b); timeslices outside [t0, t1) are zero."""
+    a, p_a = _c(a)
+    b, p_b = _c(b)
+    U, p_U = _c(U)
+    T = a.shape[0]
+    if t1 is None:
+        t1 = T
+    mom = np.ascontiguousarray(momenta, dtype=np.int32).reshape(-1, 3)
+    out = np.zeros((80, len(mom), T), dtype=np.complex128)
+    lib().orc_plain_loops_project(out.ctypes.data_as(ctypes.c_void_p), p_a, p_b, p_U, _dims(dims_of(a)),
+                                  ctypes.c_int(tb), mom.ctypes.data_as(ctypes.c_void_p), ctypes.c_int(len(mom)),
+                                  ctypes.c_int(t0), ctypes.c_int(t1))
+    return out
+
+
+def loops_time_diluted(eta, U, kappa, mu, rho, momenta, tb=-1, max_iter=10000):
+    """Time-diluted plain loops of ONE noise vector (reading 22), step by step: for every t0, restrict eta to the
+    timeslice, solve M s = eta^(t0), contract that single timeslice.  Returns ([80, nmom, T], worst true residual)."""
+    T = eta.shape[0]
+    mom = np.ascontiguousarray(momenta, dtype=np.int32).reshape(-1, 3)
+    out = np.zeros((80, len(mom), T), dtype=np.complex128)
+    worst = 0.0
+    for t0 in range(T):
+        e = time_dilute(eta, t0)
+        s, _, tr, st = solve(e, U, kappa, mu, rho, tb, max_iter)
+        if st != 0:
+            raise RuntimeError("oracle solve did not converge")
+        worst = max(worst, tr)
+        out[:, :, t0] = plain_loops_project(e, s, U, mom, tb, t0, t0 + 1)[:, :, t0]
+    return out, worst

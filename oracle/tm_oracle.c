@@ -23,13 +23,17 @@
  *                                                                   -> orc_cov_deriv
  *   sec 2.2/2.3 PAPER.md:88,94-100  "array with a time-slice index", Fourier
  *                               transform, cut in p^2               -> orc_loops_project
+ *   sec 2.2  PAPER.md:88, 92    time-dilution: sources on one timeslice, "contract a single
+ *                               time slice"                         -> orc_time_dilute, orc_plain_loops_project
  *
  * Pins (tests/test_oracle_*.py, all -m "not gpu"): gamma algebra; gamma5-
  * hermiticity; free-field plane waves vs the momentum-space closed form;
  * gauge covariance / invariance; dense assembly + LU on 2^4; full-dilution
  * loops vs traces of dense inverses; summation by parts; numpy.fft cross-check
  * of the projection; TSM identity; Fig. 2's 13-source example of the binary
- * storage.  No function here is "parity unpinned".
+ * storage; time dilution: exact spin-colour-site dilution of one timeslice vs the
+ * trace of the dense inverse, dense-D_m einsum, linearity in t0.  No function here
+ * is "parity unpinned".
  *
  * Conventions (readings 1-7,15,16): dims = {Lx,Ly,Lz,T}; site index
  * ((t*Lz+z)*Ly+y)*Lx+x; directions mu = 0,1,2,3 = x,y,z,t; spinor
@@ -436,6 +440,65 @@ void orc_loops_project_sym(cplx *out, const cplx *s, const cplx *eta, const cplx
                            int t0, int t1)
 {
     loops_project_impl(out, s, eta, U, dims, tb, kappa, mu, momenta, nmom, t0, t1, 1);
+}
+
+/* ------------------------------------------------------- time dilution (row f4) */
+/* PAPER.md:88 "we also worked with time-dilution [6], so there are GPU kernels to contract a single time slice or a
+ * whole vector" + DESIGN.md reading 22.  A time-diluted source eta^(t0) is the noise vector restricted to timeslice t0
+ * (zero elsewhere); with M s^(t0) = eta^(t0) the plain stochastic estimator of the loop on that timeslice is
+ *     l[i][k][t0] = sum_{x in t0} exp(+2 pi i p_k.x/L)  eta^(t0)(x)^dag  X_i  s^(t0)(x),
+ *     X_n = Gamma_n (n < 16),   X_{16+16m+n} = Gamma_n D_m   (D_m acting on s: reading 4)
+ * (E[eta eta^dag] = 1 on the timeslice, so E[l] = sum_x e^{ipx} tr[X_i M^-1(x,x)]; the noise of the other T-1
+ * timeslices never enters: that is the variance reduction).  The function below is the bilinear itself for any pair
+ * (a, b) and timeslices t0 <= t < t1, by the direct sum:
+ *     out[(i*nmom + k)*T + t] = sum_{x,y,z} exp(+2 pi i p_k.x/L) a(x,t)^dag X_i b(x,t);
+ * entries of out for other t are left untouched. */
+void orc_plain_loops_project(cplx *out, const cplx *a, const cplx *b, const cplx *U, const int *dims,
+                             int tb, const int *momenta, int nmom, int t0, int t1)
+{
+    const int Lx = dims[0], Ly = dims[1], Lz = dims[2], T = dims[3];
+    const long V3 = (long)Lx * Ly * Lz;
+    cplx *l = malloc(V3 * 80 * sizeof(cplx));
+    cplx G[16][4][4];
+    for (int n = 0; n < 16; n++) Gamma_mat(n, G[n]);
+    for (int t = t0; t < t1; t++) {
+#pragma omp parallel for schedule(static)
+        for (long k = 0; k < V3; k++) {
+            const long x = (long)t * V3 + k;
+            cplx *o = l + k * 80;
+            for (int n = 0; n < 16; n++) o[n] = bilinear(a + x * 12, G[n], b + x * 12);
+            for (int m = 0; m < 4; m++) {
+                cplx d[12];
+                cov_deriv_site(d, b, U, dims, tb, x, m);
+                for (int n = 0; n < 16; n++) o[16 + 16 * m + n] = bilinear(a + x * 12, G[n], d);
+            }
+        }
+#pragma omp parallel for schedule(dynamic, 1)
+        for (int q = 0; q < nmom; q++) {
+            cplx acc[80];
+            memset(acc, 0, sizeof(acc));
+            for (int z = 0; z < Lz; z++)
+                for (int y = 0; y < Ly; y++)
+                    for (int x = 0; x < Lx; x++) {
+                        const double ph = 2.0 * M_PI * ((double)momenta[q * 3 + 0] * x / Lx
+                                                        + (double)momenta[q * 3 + 1] * y / Ly
+                                                        + (double)momenta[q * 3 + 2] * z / Lz);
+                        const cplx e = cos(ph) + I * sin(ph);
+                        const cplx *lx = l + (((long)z * Ly + y) * Lx + x) * 80;
+                        for (int j = 0; j < 80; j++) acc[j] += e * lx[j];
+                    }
+            for (int j = 0; j < 80; j++) out[((long)j * nmom + q) * T + t] = acc[j];
+        }
+    }
+    free(l);
+}
+
+/* eta^(t0): the noise vector restricted to timeslice t0 (PAPER.md:88 time-dilution; reading 22) */
+void orc_time_dilute(cplx *out, const cplx *eta, const int *dims, int t0)
+{
+    const long V3 = (long)dims[0] * dims[1] * dims[2], V = V3 * dims[3];
+    for (long j = 0; j < V * 12; j++) out[j] = 0;
+    for (long j = 0; j < V3 * 12; j++) out[(long)t0 * V3 * 12 + j] = eta[(long)t0 * V3 * 12 + j];
 }
 
 /* sec 2.1 + reading 14:

@@ -34,7 +34,8 @@ EXPORTS = [
     "tm_field_import", "tm_field_export", "tm_dslash", "tm_dslash_multi", "tm_cg_solve", "loop_contract_project",
     "loop_contract_project_explicit", "loop_contract_project_sym", "loop_contract_project_timeslice",
     "loop_contract_project_fields",
-    "tsm_estimate", "tsm_estimate_host", "tsm_partial_sums_host", "tm_load_gauge_host", "tm_launch_count", "tm_set_option", "tsm_partial_sums", "tsm_combine_sums",
+    "tsm_estimate", "tsm_estimate_host", "tsm_partial_sums_host", "tm_load_gauge_host",
+    "loop_plain_project_timeslice", "tsm_estimate_time_diluted", "tm_launch_count", "tm_set_option", "tsm_partial_sums", "tsm_combine_sums",
     "tm_fma_peak",
     "loop_binary_nfiles", "loop_binary_accumulate", "loop_binary_recover", "tsm_estimate_binary",
 ]
@@ -110,6 +111,8 @@ def load_library():
     L.loop_contract_project_explicit.argtypes = [vp, vp, vp, cd, cd, ctypes.POINTER(ci), ci, ci, vp]
     L.tsm_estimate.argtypes = [vp, vp, vp, ctypes.POINTER(tsm_params), ctypes.POINTER(tsm_info), vp]
     L.tsm_estimate_host.argtypes = [vp, vp, vp, ctypes.POINTER(tsm_params), ctypes.POINTER(tsm_info), vp]
+    L.loop_plain_project_timeslice.argtypes = [vp, vp, vp, vp, ctypes.POINTER(ci), ci, ci, ci, vp]
+    L.tsm_estimate_time_diluted.argtypes = [vp, vp, vp, ctypes.POINTER(tsm_params), ctypes.POINTER(tsm_info), vp]
     L.tsm_partial_sums_host.argtypes = [vp, vp, vp, ctypes.POINTER(tsm_params), ctypes.POINTER(tsm_info), vp]
     L.loop_binary_nfiles.argtypes = [ci]
     L.loop_binary_nfiles.restype = ci
@@ -410,6 +413,38 @@ class TmContext:
         if sol is not None:
             d["solutions"] = sol
         return out, ps, d
+
+    # ------------------------------------------------------------------ time dilution (row f4)
+    def loop_plain_project_timeslice(self, a, b, momenta, t0=-1, acc=TM_F64):
+        """Plain bilinears a^dag X_i b on timeslice t0 (-1: every timeslice), complex128 [80, nmom, T]."""
+        torch = _torch()
+        a = self._dev(a, torch.complex128)
+        b = self._dev(b, torch.complex128)
+        mom = np.ascontiguousarray(momenta, dtype=np.int32).reshape(-1, 3)
+        out = torch.empty((80, len(mom), self.T), dtype=torch.complex128, device=self.tdev)
+        self._check(self.lib.loop_plain_project_timeslice(
+            self.h, out.data_ptr(), a.data_ptr(), b.data_ptr(),
+            mom.ctypes.data_as(ctypes.POINTER(ctypes.c_int)), len(mom), int(t0), int(acc), _stream()))
+        return out
+
+    def tsm_estimate_time_diluted(self, n_lp, n_hp, kappa, mu, momenta, lp, hp, acc_lp=TM_F32, acc_hp=TM_F64,
+                                  z4=None, seed=0, per_source=False, raise_on_noconv=True, src_first=0, src_stride=1):
+        """TSM estimate of the time-diluted plain loops: (out [80,nmom,T], per_source | None, info)."""
+        torch = _torch()
+        d_z4 = None
+        if z4 is not None:
+            z4 = self._dev(z4, torch.uint8)
+            assert z4.numel() == n_lp * 3 * self.V
+            d_z4 = z4.data_ptr()
+        P, mom = self._tsm_params(n_lp, n_hp, kappa, mu, momenta, lp, hp, acc_lp, acc_hp, d_z4, seed, src_first, src_stride)
+        shape = (80, len(mom), self.T)
+        out = torch.empty(shape, dtype=torch.complex128, device=self.tdev)
+        ps = torch.empty((n_lp + n_hp,) + shape, dtype=torch.complex128, device=self.tdev) if per_source else None
+        info = tsm_info()
+        st = self.lib.tsm_estimate_time_diluted(self.h, out.data_ptr(), ps.data_ptr() if ps is not None else None,
+                                                ctypes.byref(P), ctypes.byref(info), _stream())
+        self._check(st, allow=() if raise_on_noconv else (TM_ENOCONV,))
+        return out, ps, self._tsm_info(info, st)
 
     def tsm_combine_sums(self, sums, n_lp_total, n_hp_total):
         """out = S_LP / n_lp_total + (S_HP - S_LPc) / n_hp_total from the (all-reduced) raw accumulators [3,2,80,nmom,T]."""

@@ -19,9 +19,10 @@ tm_status tm_dslash_launch(tm_ctx* ctx, const DslashCall& c, tm_prec prec, tm_re
 // ---- layout.cu ----------------------------------------------------------------------------
 tm_status tm_import_launch(tm_ctx* ctx, void* d_internal, const void* d_canon, tm_prec prec, cudaStream_t st);
 tm_status tm_export_launch(tm_ctx* ctx, void* d_canon, const void* d_internal, tm_prec prec, cudaStream_t st);
-// Z4 noise into a full-lattice internal field: packed exponents (d_z4 != NULL) or counter hash
+// Z4 noise into a full-lattice internal field: packed exponents (d_z4 != NULL) or counter hash;
+// t_only >= 0: restricted to that timeslice (time dilution), zero elsewhere
 tm_status tm_z4_expand(tm_ctx* ctx, void* d_internal, tm_prec prec, const unsigned char* d_z4,
-                       unsigned long long seed, unsigned long long r, cudaStream_t st);
+                       unsigned long long seed, unsigned long long r, cudaStream_t st, int t_only = -1);
 
 // ---- blas.cu ------------------------------------------------------------------------------
 // parity-vector operations (n = 24*Vh reals each); all asynchronous on st

@@ -2,12 +2,13 @@
 // (SURVEY.md sec 8b "Boundary", "Input recipe".)
 #include "kernels.h"
 
-__device__ __forceinline__ void site_coords(const Geom& g, int par, int h, int& lex) {
+__device__ __forceinline__ int site_coords(const Geom& g, int par, int h, int& lex) {     // returns t
     int q = h / g.Xh;
     const int y = q % g.X1; q /= g.X1;
     const int z = q % g.X2;
     const int t = q / g.X2;
     lex = 2 * h + ((y + z + t + par) & 1);
+    return t;
 }
 
 template <typename S, int R>
@@ -134,15 +135,23 @@ __host__ __device__ __forceinline__ unsigned long long mix64(unsigned long long 
     return z;
 }
 
+// t_only >= 0: time dilution -- the noise restricted to timeslice t_only, zero elsewhere
 template <typename S>
 __global__ void z4_expand_kernel(S* __restrict__ f, const unsigned char* __restrict__ packed,
-                                 unsigned long long base, Geom g) {
+                                 unsigned long long base, Geom g, int t_only) {
     typedef typename Prec<S>::F F;
     const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= 2L * g.Vh) return;
     const int par = (int)(idx / g.Vh), h = (int)(idx % g.Vh);
     int lex;
-    site_coords(g, par, h, lex);
+    const int t = site_coords(g, par, h, lex);
+    if (t_only >= 0 && t != t_only) {
+        F v[24];
+#pragma unroll
+        for (int i = 0; i < 24; i++) v[i] = F(0);
+        store_spinor<S>(f + (size_t)par * g.Vh * 24, g.Vh, h, v);
+        return;
+    }
     unsigned int bits = 0;     // 12 exponents, 2 bits each
     if (packed) {
         const unsigned char* p = packed + (size_t)lex * 3;
@@ -163,14 +172,14 @@ __global__ void z4_expand_kernel(S* __restrict__ f, const unsigned char* __restr
 }
 
 tm_status tm_z4_expand(tm_ctx* ctx, void* d_int, tm_prec prec, const unsigned char* d_z4,
-                       unsigned long long seed, unsigned long long r, cudaStream_t st) {
+                       unsigned long long seed, unsigned long long r, cudaStream_t st, int t_only) {
     const unsigned long long base = mix64(seed * 0x9E3779B97F4A7C15ULL + r);
     const long n = 2L * ctx->Vh;
     const unsigned grid = (unsigned)((n + 127) / 128);
     const Geom g = tm_geom(ctx);
     switch (prec) {
-        case TM_F64: z4_expand_kernel<double><<<grid, 128, 0, st>>>((double*)d_int, d_z4, base, g); break;
-        case TM_F32: z4_expand_kernel<float><<<grid, 128, 0, st>>>((float*)d_int, d_z4, base, g); break;
+        case TM_F64: z4_expand_kernel<double><<<grid, 128, 0, st>>>((double*)d_int, d_z4, base, g, t_only); break;
+        case TM_F32: z4_expand_kernel<float><<<grid, 128, 0, st>>>((float*)d_int, d_z4, base, g, t_only); break;
         default: return tm_fail(ctx, TM_EPREC, "z4 expand: precision must be f32 or f64");
     }
     TM_LAUNCH_CHECK(ctx, "z4_expand_kernel");
