@@ -400,8 +400,9 @@ def profile_mode(args, cfg):
         print("dslash %s r%d XPAY, %d source(s) per launch: %.1f us/launch, %.0f GB/s (spinors per source, links once per launch)"
               % (args.prec, args.recon, nb, ms * 1e3, nbytes / ms / 1e6))
     elif args.what == "contract":
+        ctx.tm_set_option(tmod.TM_OPT_CONTRACT_PATH, args.contract_path)
         ms = time_contract(ctx, tmod, torch, inputs_torch, cfg, args.prec, args.napp)
-        print("contract %s: %.3f ms/call (xy + zsum + assemble, internal-layout inputs)" % (args.prec, ms))
+        print("contract %s path %d: %.3f ms/call (xy + zsum + assemble, internal-layout inputs)" % (args.prec, args.contract_path, ms))
     elif args.what in ("solve", "blas"):
         eta = inputs_torch.z4_source(dims, cfg["src_seed"], 0, dev)
         P = LP if args.prec in ("f16", "bf16") else HP
@@ -446,6 +447,7 @@ def run_b200(args, cfg):
         z4_dev[j] = inputs_torch.z4_packed(dims, seed, first + j * stride, dev)
     ctx = tmod.TmContext(dims, -1, local)
     ctx.tm_load_gauge(U)
+    ctx.tm_set_option(tmod.TM_OPT_CONTRACT_PATH, args.contract_path)
 
     def step():
         return multi.tsm_estimate_sharded(ctx, n_lp_job, n_hp_job, kappa, mu, mom, LP, HP, tmod.TM_F32, tmod.TM_F64,
@@ -638,6 +640,8 @@ def main():
                     help="N > 1: shard the one (N_LP, N_HP) workload over the ranks (strong) or run N times the workload (weak)")
     ap.add_argument("--what", default="step", choices=["step", "dslash", "dslash_group", "contract", "blas", "solve"],
                     help="step: the bench line; otherwise run one kernel family a few times (ncu captures)")
+    ap.add_argument("--contract-path", type=int, default=0, choices=[0, 1, 2, 3],
+                    help="TM_OPT_CONTRACT_PATH of the fp32 contraction (0 = automatic, see include/tmloops.h)")
     ap.add_argument("--prec", default="f16", help="--what != step: storage precision (contract: f32 | f64)")
     ap.add_argument("--recon", type=int, default=12)
     ap.add_argument("--napp", type=int, default=6)

@@ -68,7 +68,10 @@ const char* tm_last_error(const tm_ctx* ctx);
  *                         fit the device memory), or 1 | 2 | 4 | 8
  *   TM_OPT_CONTRACT_PATH  site + x/y-DFT stage of the contraction: 0 = automatic (fastest usable), 1 = generic kernel
  *                         (read-only-cache loads; any Lx, fp64), 2 = TMA-staged fp32 kernel with the DFT on the fp32 pipe,
- *                         3 = TMA-staged fp32 kernel with the DFT on the tensor cores (tcgen05, split-fp32 operands)
+ *                         3 = TMA-staged fp32 kernel with the x-stage of the DFT on the tensor cores (tf32 MMAs on
+ *                         split-fp32 operands, hi*hi + lo*hi + hi*lo: same 1e-5 bound) and a forward-only s-family
+ *                         derivative (whole-vector calls; never the automatic choice: measured slower than 2);
+ *                         2 and 3 need Lx <= 32 and fall back to 1 otherwise
  * TM_EARG for an unknown option or value. */
 typedef enum { TM_OPT_GROUP = 0, TM_OPT_CONTRACT_PATH = 1 } tm_option;
 tm_status tm_set_option(tm_ctx* ctx, tm_option opt, int value);

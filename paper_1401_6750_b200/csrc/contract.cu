@@ -208,6 +208,9 @@ struct AssembleArgs {
     int nmom, T, Lz, NQ;
     int t_first;               // first timeslice handled (blockIdx.y = 0)
     double twokmu;             // 2 kappa mu
+    int half0;                 // s-family derivative slots hold only the forward half F_mu (contract_mma.cu); every
+                               // timeslice must have been summed
+    int L[3];                  // Lx, Ly, Lz
 };
 
 // z-stage: every x/y partial sum is read exactly once and reduced against the 7 real z-weights
@@ -234,36 +237,47 @@ __global__ void __launch_bounds__(CT_THREADS) contract_zsum_kernel(AssembleArgs 
 // site-independent Gamma change of basis
 __global__ void __launch_bounds__(CT_THREADS) contract_assemble_kernel(AssembleArgs A) {
     __shared__ double zre[CT_THREADS], zim[CT_THREADS];
+    __shared__ double zre_tm[32], zim_tm[32];               // half0: the t-derivative slot of the s family at t - 1
     const int k = blockIdx.x, t = blockIdx.y + A.t_first;
     const int jr = threadIdx.x;
     const int px = A.mom[3 * k], py = A.mom[3 * k + 1], pz = A.mom[3 * k + 2];
     const int m = abs(px), n = abs(py), l = abs(pz);
     const double sx = px < 0 ? -1.0 : 1.0, sy = py < 0 ? -1.0 : 1.0, sz = pz < 0 ? -1.0 : 1.0;
     const short* qi = A.qidx + (m * 4 + n) * 4;
-    const double* zb = A.zbuf + (size_t)t * A.NQ * 7 * CT_THREADS + jr;
-    // X[c] = sum_z cos(2 pi l z / L) Q_X(z), X[s] = sum_z sin(...) Q_X(z) for X in cc, cs, sc, ss
-    double C[4], S[4];
+    // Z(tq) = sum over the timeslice of exp(+i p.x) times real component jr
+    auto Zof = [&](int tq, double& re, double& im) {
+        const double* zb = A.zbuf + (size_t)tq * A.NQ * 7 * CT_THREADS + jr;
+        // X[c] = sum_z cos(2 pi l z / L) Q_X(z), X[s] = sum_z sin(...) Q_X(z) for X in cc, cs, sc, ss
+        double C[4], S[4];
 #pragma unroll
-    for (int x = 0; x < 4; x++) {
-        const int iq = qi[x];
-        C[x] = 0.0; S[x] = 0.0;
-        if (iq >= 0) {
-            const double* e = zb + (size_t)iq * 7 * CT_THREADS;
-            C[x] = l ? e[(size_t)(2 * l - 1) * CT_THREADS] : e[0];
-            S[x] = l ? e[(size_t)(2 * l) * CT_THREADS] : 0.0;
+        for (int x = 0; x < 4; x++) {
+            const int iq = qi[x];
+            C[x] = 0.0; S[x] = 0.0;
+            if (iq >= 0) {
+                const double* e = zb + (size_t)iq * 7 * CT_THREADS;
+                C[x] = l ? e[(size_t)(2 * l - 1) * CT_THREADS] : e[0];
+                S[x] = l ? e[(size_t)(2 * l) * CT_THREADS] : 0.0;
+            }
         }
-    }
-    // (cos mx + i sx sin mx)(cos ny + i sy sin ny)(cos lz + i sz sin lz)
-    const double wrC = C[0] - sx * sy * C[3], wiC = sx * C[2] + sy * C[1];
-    const double wrS = S[0] - sx * sy * S[3], wiS = sx * S[2] + sy * S[1];
-    zre[jr] = wrC - sz * wiS;
-    zim[jr] = wiC + sz * wrS;
+        // (cos mx + i sx sin mx)(cos ny + i sy sin ny)(cos lz + i sz sin lz)
+        const double wrC = C[0] - sx * sy * C[3], wiC = sx * C[2] + sy * C[1];
+        const double wrS = S[0] - sx * sy * S[3], wiS = sx * S[2] + sy * S[1];
+        re = wrC - sz * wiS;
+        im = wiC + sz * wrS;
+    };
+    Zof(t, zre[jr], zim[jr]);
+    if (A.half0 && jr >= 4 * 32 && jr < 5 * 32) Zof(t == 0 ? A.T - 1 : t - 1, zre_tm[jr - 4 * 32], zim_tm[jr - 4 * 32]);
     __syncthreads();
     if (jr < 160) {
         const int f = jr / 80, i = jr % 80;
         const int nG = i < 16 ? i : (i - 16) & 15;
         const int d = i < 16 ? 0 : 1 + ((i - 16) >> 4);
         const double scale = d ? 0.5 : 1.0;
+        // half0: C~[a][b](p,t) = F~[a][b](p,t) - e^{i p_mu} conj(F~[b][a](-p,t')), and for real fields Z(-p) = conj(Z(p))
+        double phr = 1.0, phi = 0.0;
+        if (A.half0 && d >= 1 && d <= 3) sincospi(2.0 * (double)A.mom[3 * k + d - 1] / (double)A.L[d - 1], &phi, &phr);
+        const double* br_ = (d == 4) ? zre_tm - 4 * 32 : zre;
+        const double* bi_ = (d == 4) ? zim_tm - 4 * 32 : zim;
         double l0r = 0, l0i = 0, l1r = 0, l1i = 0;
 #pragma unroll
         for (int a = 0; a < 4; a++) {
@@ -271,7 +285,13 @@ __global__ void __launch_bounds__(CT_THREADS) contract_assemble_kernel(AssembleA
             const double pr = c_gamma.phre[nG][a], pi = c_gamma.phim[nG][a];
             {   // s family: raw complex value = (Z[re comp]) + i (Z[im comp]) with each Z complex
                 const int j = (d * 32) + (a * 4 + bcol) * 2;
-                const double rr = zre[j] - zim[j + 1], ri = zim[j] + zre[j + 1];
+                double rr = zre[j] - zim[j + 1], ri = zim[j] + zre[j + 1];
+                if (A.half0 && d) {
+                    const int jt = (d * 32) + (bcol * 4 + a) * 2;            // transposed component
+                    const double cr = br_[jt] + bi_[jt + 1], ci = bi_[jt] - br_[jt + 1];   // conj(F~[b][a](-p))
+                    rr -= phr * cr - phi * ci;
+                    ri -= phr * ci + phi * cr;
+                }
                 l0r += pr * rr - pi * ri;
                 l0i += pr * ri + pi * rr;
             }
@@ -371,7 +391,7 @@ static ContractTables table_layout(const tm_ctx* c, int nmom) {
     return L;
 }
 
-static void build_qidx(short* qidx, int prune, int* nq) {
+void tm_contract_qidx(short* qidx, int prune, int* nq) {
     int q = 0;
     for (int m = 0; m < 4; m++)
         for (int n = 0; n < 4; n++) {
@@ -435,7 +455,7 @@ tm_status tm_contract_internal(tm_ctx* ctx, void* d_out, const void* d_s, const 
         fill_weights((double*)(host.data() + L.off_wz), ctx->X[2]);
         memcpy(host.data() + L.off_mom, h_momenta, (size_t)nmom * 12);
         int nq;
-        build_qidx((short*)(host.data() + L.off_qidx), prune, &nq);
+        tm_contract_qidx((short*)(host.data() + L.off_qidx), prune, &nq);
     }
     static_assert(sizeof(int) == 4, "int momenta");
     if (!ctx->h_contract_tables || ctx->contract_tables_bytes != L.total
@@ -473,8 +493,15 @@ tm_status tm_contract_internal(tm_ctx* ctx, void* d_out, const void* d_s, const 
     A.g = tm_geom(ctx);
     A.tb = (double)ctx->tb;
     A.t_first = t_first;
+    // the forward-only s family of contract_mma.cu needs timeslice t - 1 in the assembly: whole-vector launches only
+    // (measured at c4, profiles/r02_contract_paths.md: 0.98 ms against 0.93 ms for contract_tma.cu although it issues
+    // 40 % fewer FFMA2 -- both are bound by shared-memory operand traffic + fp32 pipe time, which add up -- so it is
+    // not the automatic choice)
+    const bool half0 = acc == TM_F32 && nt == ctx->X[3] && ctx->opt_contract == 3 && tm_contract_mma_usable(ctx);
     if (acc == TM_F64) TM_TRY((launch_xy<double, 18>(ctx, A, prune, nt, st)));
-    else if (ctx->opt_contract != 1 && tm_contract_tma_usable(ctx)) TM_TRY(tm_contract_xy_tma(ctx, qbuf, d_s, d_eta, gauge, A.wx, A.wy, prune, t_first, nt, st));
+    else if (half0) TM_TRY(tm_contract_xy_mma(ctx, qbuf, d_s, d_eta, gauge, A.wx, A.wy, prune, t_first, nt, st));
+    else if (ctx->opt_contract != 1 && tm_contract_tma_usable(ctx))
+        TM_TRY(tm_contract_xy_tma(ctx, qbuf, d_s, d_eta, gauge, A.wx, A.wy, prune, t_first, nt, st));
     else TM_TRY((launch_xy<float, 12>(ctx, A, prune, nt, st)));
 
     AssembleArgs B;
@@ -485,6 +512,8 @@ tm_status tm_contract_internal(tm_ctx* ctx, void* d_out, const void* d_s, const 
     B.wz = (const double*)(tb + L.off_wz);
     B.nmom = nmom; B.T = ctx->X[3]; B.Lz = ctx->X[2]; B.NQ = nq; B.t_first = t_first;
     B.twokmu = 2.0 * kappa * mu;
+    B.half0 = half0 ? 1 : 0;
+    B.L[0] = ctx->X[0]; B.L[1] = ctx->X[1]; B.L[2] = ctx->X[2];
     dim3 zgrid((unsigned)nq, (unsigned)nt);
     if (acc == TM_F64) contract_zsum_kernel<double><<<zgrid, CT_THREADS, 0, st>>>(B);
     else contract_zsum_kernel<float><<<zgrid, CT_THREADS, 0, st>>>(B);

@@ -91,5 +91,10 @@ tm_status tm_contract_internal(tm_ctx* ctx, void* d_out, const void* d_s, const 
 bool tm_contract_tma_usable(const tm_ctx* ctx);
 tm_status tm_contract_xy_tma(tm_ctx* ctx, void* qbuf, const void* d_s, const void* d_eta, const void* gauge,
                              const void* wx, const void* wy, int prune, int t_first, int nt, cudaStream_t st);
+// contract_mma.cu: the same with the x-stage DFT on the tensor cores (mma.sync tf32, split-fp32 operands)
+bool tm_contract_mma_usable(const tm_ctx* ctx);
+tm_status tm_contract_xy_mma(tm_ctx* ctx, void* qbuf, const void* d_s, const void* d_eta, const void* gauge,
+                             const void* wx, const void* wy, int prune, int t_first, int nt, cudaStream_t st);
+void tm_contract_qidx(short* qidx, int prune, int* nq);   // contract.cu: layout of the x/y partial sums Q
 // acc += x on complex128 arrays of n complex numbers
 tm_status tm_accumulate(tm_ctx* ctx, void* d_acc, const void* d_x, size_t n, cudaStream_t st);

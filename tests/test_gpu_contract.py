@@ -156,9 +156,36 @@ def test_contract_single_timeslice(orc, acc):
             ref = orc.loops_project(s, eta, U, k, mu, mom, -1, t0, t0 + 1)
             got = to_np(ctx.loop_contract_project_timeslice(s, eta, k, mu, mom, t0, t.PREC[acc]))
             check_blocks(got, ref, TOL[acc])
-            assert np.array_equal(got[..., t0], full[..., t0])
+            assert np.array_equal(got[..., t0], full[..., t0])      # same kernel, launched on one timeslice
             mask = np.ones(dims[3], dtype=bool)
             mask[t0] = False
             assert not got[..., mask].any()
         with pytest.raises(t.TmError):
             ctx.loop_contract_project_timeslice(s, eta, k, mu, mom, dims[3], t.PREC[acc])
+
+
+@pytest.mark.parametrize("path", [1, 2, 3])
+@pytest.mark.parametrize("dims,tb", [
+    ((4, 4, 4, 8), -1),      # c1 shape: 28 idle lanes per row
+    ((6, 4, 6, 10), 1),      # unequal extents, Xh = 3
+    ((16, 6, 4, 4), -1),     # half-filled rows
+    ((32, 8, 2, 4), -1),     # full rows (the c4 row shape), both time boundaries inside the launch
+    ((24, 4, 4, 2), 1),      # c3 row shape
+])
+def test_contract_fp32_paths(orc, path, dims, tb):
+    """The three implementations of the fp32 site + x/y-DFT stage (TM_OPT_CONTRACT_PATH: generic kernel, TMA-staged with
+    the DFT on the fp32 pipe, TMA-staged with the DFT on the tensor cores as split-fp32 tf32 MMAs) each against the
+    oracle at the north_star bound, for the pruned (p^2 <= 9) and the unpruned accumulator sets."""
+    t = tm()
+    U, s, eta = case(dims, 0.25, 31)
+    k, mu = 0.1563, 0.0055
+    unpruned = np.array([[3, 3, 3], [-3, 3, -2], [2, -3, 1], [0, 0, 0], [-1, -2, -3], [3, -1, 0], [1, 3, 0], [-3, -3, 0]],
+                        dtype=np.int32)
+    with t.TmContext(dims, tb) as ctx:
+        ctx.tm_load_gauge(U)
+        ctx.tm_set_option(t.TM_OPT_CONTRACT_PATH, path)
+        for mom in (inputs.momentum_list(9), unpruned):
+            ref = orc.loops_project(s, eta, U, k, mu, mom, tb)
+            got = to_np(ctx.loop_contract_project(s, eta, k, mu, mom, t.TM_F32))
+            check_blocks(got, ref, TOL["f32"])
+        ctx.tm_set_option(t.TM_OPT_CONTRACT_PATH, 0)
