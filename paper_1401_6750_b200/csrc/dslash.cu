@@ -204,17 +204,17 @@ __global__ void __launch_bounds__(128) dslash_kernel(DslashArgs<typename Prec<S>
 
 
 // =====================================================================================================
-// 16-bit storage path (fp16 / bf16), reconstruct-12.  Blackwell's mixed-precision FMA
+// 16-bit storage path (fp16 / bf16), reconstruct-12 and -18.  Blackwell's mixed-precision FMA
 // (PTX fma.rn.f32.f16 / .bf16 -> SASS FHFMA with .H0/.H1 operand selects) multiplies two 16-bit
 // operands straight out of the packed registers and accumulates in fp32, so neither the links nor
 // the neighbour spinors are ever unpacked: one 32-bit register = one complex number (re, im).
 //   project     packed half2 arithmetic on the loaded spinor (result rounded to storage precision)
-//   row 2       conj(row0 x row1) by FHFMA in fp32, packed back to 16 bit
+//   row 2       reconstruct-12: conj(row0 x row1) by FHFMA in fp32, packed back to 16 bit; reconstruct-18: loaded
 //   SU(3) * u   FHFMA, fp32 accumulate
 //   reconstruct   fp32, packed FADD2 / FFMA2 on (re, im) register pairs where the pairing allows
 //   epilogue / norm   fp32 (as in the generic kernel)
 //   links       the 8 links of a site are copied by cp.async into thread-private shared-memory slots at kernel
-//               start (24 KB per CTA; no barrier: a thread reads only what it copied), so 2/3 of the kernel's
+//               start (24 KB per CTA, 36 KB for reconstruct-18; no barrier: a thread reads only what it copied), so 2/3 of the kernel's
 //               bytes are in flight without holding registers; spinors are register loads one hop ahead
 template <typename S> struct Pk;
 template <> struct Pk<__half> {
@@ -281,16 +281,25 @@ __device__ __forceinline__ void project16(const unsigned* p, unsigned* u) {
 
 // stage_link16: the link of one hop copied into the thread's private shared-memory slots with cp.async (no
 // registers held while the copy is in flight); slot k * 128 of the thread's column, k = 0..2
-template <int MU, int FWD, typename S>
-__device__ __forceinline__ void stage_link16(const S* gauge, size_t Vh, int par_out, size_t h_out, size_t h_nb, uint2* slot) {
+// Link storage of the 16-bit copies (common.cuh GaugeLayout): reconstruct-12 = 3 chunks of 8 bytes (two complex
+// numbers each), reconstruct-18 = 9 chunks of 4 bytes (one complex number each); LinkSlot<R>::T is one chunk.
+template <int R> struct LinkSlot;
+template <> struct LinkSlot<12> { typedef uint2 T; static constexpr int NCH = 3; };
+template <> struct LinkSlot<18> { typedef unsigned T; static constexpr int NCH = 9; };
+
+template <int MU, int FWD, typename S, int R>
+__device__ __forceinline__ void stage_link16(const S* gauge, size_t Vh, int par_out, size_t h_out, size_t h_nb,
+                                             typename LinkSlot<R>::T* slot) {
+    typedef typename LinkSlot<R>::T C;
+    constexpr int NCH = LinkSlot<R>::NCH;
     const size_t hl = FWD ? h_out : h_nb;
     const int pl = FWD ? par_out : 1 - par_out;
-    const unsigned gi = (unsigned)(pl * 4 + MU) * 3u * (unsigned)Vh + (unsigned)hl;
-    const uint2* g = reinterpret_cast<const uint2*>(gauge);
+    const unsigned gi = (unsigned)(pl * 4 + MU) * (unsigned)NCH * (unsigned)Vh + (unsigned)hl;
+    const C* g = reinterpret_cast<const C*>(gauge);
 #pragma unroll
-    for (int k = 0; k < 3; k++) {
+    for (int k = 0; k < NCH; k++) {
         const unsigned dst = (unsigned)__cvta_generic_to_shared(slot + k * 128);
-        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(g + (gi + (unsigned)k * (unsigned)Vh)) : "memory");
+        asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" ::"r"(dst), "l"(g + (gi + (unsigned)k * (unsigned)Vh)), "n"(sizeof(C)) : "memory");
     }
     asm volatile("cp.async.commit_group;" ::: "memory");
 }
@@ -308,8 +317,12 @@ __device__ __forceinline__ void read_link16(const uint2* slot, unsigned* U) {
 #pragma unroll
     for (int k = 0; k < 3; k++) { const uint2 q = slot[k * 128]; U[2 * k] = q.x; U[2 * k + 1] = q.y; }
 }
+__device__ __forceinline__ void read_link16(const unsigned* slot, unsigned* U) {
+#pragma unroll
+    for (int k = 0; k < 9; k++) U[k] = slot[k * 128];
+}
 
-template <int MU, int FWD, typename S>
+template <int MU, int FWD, typename S, int R>
 __device__ __forceinline__ void load16(const S* in, const S* gauge, size_t Vh, int par_out, size_t h_out, size_t h_nb,
                                        unsigned* p, unsigned* U) {
     const uint4* f = reinterpret_cast<const uint4*>(in) + h_nb;
@@ -320,13 +333,19 @@ __device__ __forceinline__ void load16(const S* in, const S* gauge, size_t Vh, i
     }
     const size_t hl = FWD ? h_out : h_nb;
     const int pl = FWD ? par_out : 1 - par_out;
-    // 32-bit element index (8 * 3 * Vh < 2^31 for every supported lattice): one IMAD.WIDE per load
-    const unsigned gi = (unsigned)(pl * 4 + MU) * 3u * (unsigned)Vh + (unsigned)hl;
-    const uint2* g = reinterpret_cast<const uint2*>(gauge);
+    // 32-bit element index (8 * 9 * Vh < 2^31 for every supported lattice): one IMAD.WIDE per load
+    const unsigned gi = (unsigned)(pl * 4 + MU) * (unsigned)LinkSlot<R>::NCH * (unsigned)Vh + (unsigned)hl;
+    if (R == 12) {
+        const uint2* g = reinterpret_cast<const uint2*>(gauge);
 #pragma unroll
-    for (int k = 0; k < 3; k++) {
-        const uint2 q = __ldcs(g + (gi + (unsigned)k * (unsigned)Vh));
-        U[2 * k] = q.x; U[2 * k + 1] = q.y;
+        for (int k = 0; k < 3; k++) {
+            const uint2 q = __ldcs(g + (gi + (unsigned)k * (unsigned)Vh));
+            U[2 * k] = q.x; U[2 * k + 1] = q.y;
+        }
+    } else {
+        const unsigned* g = reinterpret_cast<const unsigned*>(gauge);
+#pragma unroll
+        for (int k = 0; k < 9; k++) U[k] = __ldcs(g + (gi + (unsigned)k * (unsigned)Vh));
     }
 }
 
@@ -371,13 +390,13 @@ __device__ __forceinline__ void reconstruct16(const float* v, float* acc) {
     }
 }
 
-template <int MU, int FWD, int DAGGER, typename S>
+template <int MU, int FWD, int DAGGER, typename S, int R>
 __device__ __forceinline__ void compute16(const unsigned* p, const unsigned* Uin, float bsign, bool wrap, float* acc) {
     typedef typename Pk<S>::V2 V2;
     constexpr int SGN = (FWD ? -1 : 1) * (DAGGER ? -1 : 1);       // forward: (1 - g), backward: (1 + g)
     unsigned U[9], u[6];
 #pragma unroll
-    for (int i = 0; i < 6; i++) U[i] = Uin[i];
+    for (int i = 0; i < R / 2; i++) U[i] = Uin[i];
     project16<MU, SGN, S>(p, u);
     if (MU == 3 && wrap) {
         const V2 b2 = Pk<S>::make(bsign, bsign);
@@ -386,7 +405,7 @@ __device__ __forceinline__ void compute16(const unsigned* p, const unsigned* Uin
     }
     // row 2 = conj(row0 x row1) = conj(a_i b_j - a_j b_i): one FHFMA chain per real (negation is an operand modifier)
 #pragma unroll
-    for (int c = 0; c < 3; c++) {
+    for (int c = 0; c < (R == 12 ? 3 : 0); c++) {
         const int i = (c + 1) % 3, j = (c + 2) % 3;
         float re = 0.f, nim = 0.f;
         re  = Pk<S>::template fma<0, 0, 0>(U[i], U[3 + j], re);
@@ -418,7 +437,7 @@ __device__ __forceinline__ void compute16(const unsigned* p, const unsigned* Uin
     reconstruct16<MU, SGN>(v, acc);
 }
 
-template <typename S, int DAGGER, int PIPE, int MINB>
+template <typename S, int DAGGER, int PIPE, int MINB, int R>
 __global__ void __launch_bounds__(128, MINB) dslash16_kernel(DslashArgs<float> A) {
     __shared__ double sm[32];
     int bx = blockIdx.x, src = 0;
@@ -456,46 +475,47 @@ __global__ void __launch_bounds__(128, MINB) dslash16_kernel(DslashArgs<float> A
         const int tp = wp ? h - (g.X3 - 1) * g.s3 : h + g.s3;
         const int tm = wm ? h + (g.X3 - 1) * g.s3 : h - g.s3;
         const int par = A.parity;
-        unsigned pa[12], ua[6];
+        unsigned pa[12], ua[R / 2];
+        constexpr int LS = LinkSlot<R>::NCH * 128;             // slots of one hop
         if (PIPE == 2) {
             // links: all 8 hops staged by cp.async up front (thread-private slots, no barrier needed);
             // spinors: register loads one hop ahead
-            __shared__ uint2 smg[24 * 128];
-            uint2* sl = smg + threadIdx.x;
-            stage_link16<0, 1, S>(gauge, Vh, par, h, xp, sl + 0 * 384);
-            stage_link16<0, 0, S>(gauge, Vh, par, h, xm, sl + 1 * 384);
-            stage_link16<1, 1, S>(gauge, Vh, par, h, yp, sl + 2 * 384);
-            stage_link16<1, 0, S>(gauge, Vh, par, h, ym, sl + 3 * 384);
-            stage_link16<2, 1, S>(gauge, Vh, par, h, zp, sl + 4 * 384);
-            stage_link16<2, 0, S>(gauge, Vh, par, h, zm, sl + 5 * 384);
-            stage_link16<3, 1, S>(gauge, Vh, par, h, tp, sl + 6 * 384);
-            stage_link16<3, 0, S>(gauge, Vh, par, h, tm, sl + 7 * 384);
+            __shared__ typename LinkSlot<R>::T smg[8 * LS];
+            typename LinkSlot<R>::T* sl = smg + threadIdx.x;
+            stage_link16<0, 1, S, R>(gauge, Vh, par, h, xp, sl + 0 * LS);
+            stage_link16<0, 0, S, R>(gauge, Vh, par, h, xm, sl + 1 * LS);
+            stage_link16<1, 1, S, R>(gauge, Vh, par, h, yp, sl + 2 * LS);
+            stage_link16<1, 0, S, R>(gauge, Vh, par, h, ym, sl + 3 * LS);
+            stage_link16<2, 1, S, R>(gauge, Vh, par, h, zp, sl + 4 * LS);
+            stage_link16<2, 0, S, R>(gauge, Vh, par, h, zm, sl + 5 * LS);
+            stage_link16<3, 1, S, R>(gauge, Vh, par, h, tp, sl + 6 * LS);
+            stage_link16<3, 0, S, R>(gauge, Vh, par, h, tm, sl + 7 * LS);
             unsigned pb[12];
             load_spinor16<S>(in, Vh, xp, pa);
             load_spinor16<S>(in, Vh, xm, pb);
-            cp_wait<7>(); read_link16(sl + 0 * 384, ua); compute16<0, 1, DAGGER, S>(pa, ua, 1.f, false, acc);
+            cp_wait<7>(); read_link16(sl + 0 * LS, ua); compute16<0, 1, DAGGER, S, R>(pa, ua, 1.f, false, acc);
             load_spinor16<S>(in, Vh, yp, pa);
-            cp_wait<6>(); read_link16(sl + 1 * 384, ua); compute16<0, 0, DAGGER, S>(pb, ua, 1.f, false, acc);
+            cp_wait<6>(); read_link16(sl + 1 * LS, ua); compute16<0, 0, DAGGER, S, R>(pb, ua, 1.f, false, acc);
             load_spinor16<S>(in, Vh, ym, pb);
-            cp_wait<5>(); read_link16(sl + 2 * 384, ua); compute16<1, 1, DAGGER, S>(pa, ua, 1.f, false, acc);
+            cp_wait<5>(); read_link16(sl + 2 * LS, ua); compute16<1, 1, DAGGER, S, R>(pa, ua, 1.f, false, acc);
             load_spinor16<S>(in, Vh, zp, pa);
-            cp_wait<4>(); read_link16(sl + 3 * 384, ua); compute16<1, 0, DAGGER, S>(pb, ua, 1.f, false, acc);
+            cp_wait<4>(); read_link16(sl + 3 * LS, ua); compute16<1, 0, DAGGER, S, R>(pb, ua, 1.f, false, acc);
             load_spinor16<S>(in, Vh, zm, pb);
-            cp_wait<3>(); read_link16(sl + 4 * 384, ua); compute16<2, 1, DAGGER, S>(pa, ua, 1.f, false, acc);
+            cp_wait<3>(); read_link16(sl + 4 * LS, ua); compute16<2, 1, DAGGER, S, R>(pa, ua, 1.f, false, acc);
             load_spinor16<S>(in, Vh, tp, pa);
-            cp_wait<2>(); read_link16(sl + 5 * 384, ua); compute16<2, 0, DAGGER, S>(pb, ua, 1.f, false, acc);
+            cp_wait<2>(); read_link16(sl + 5 * LS, ua); compute16<2, 0, DAGGER, S, R>(pb, ua, 1.f, false, acc);
             load_spinor16<S>(in, Vh, tm, pb);
-            cp_wait<1>(); read_link16(sl + 6 * 384, ua); compute16<3, 1, DAGGER, S>(pa, ua, A.tb, wp, acc);
-            cp_wait<0>(); read_link16(sl + 7 * 384, ua); compute16<3, 0, DAGGER, S>(pb, ua, A.tb, wm, acc);
+            cp_wait<1>(); read_link16(sl + 6 * LS, ua); compute16<3, 1, DAGGER, S, R>(pa, ua, A.tb, wp, acc);
+            cp_wait<0>(); read_link16(sl + 7 * LS, ua); compute16<3, 0, DAGGER, S, R>(pb, ua, A.tb, wm, acc);
         } else {
-            load16<0, 1, S>(in, gauge, Vh, par, h, xp, pa, ua); compute16<0, 1, DAGGER, S>(pa, ua, 1.f, false, acc);
-            load16<0, 0, S>(in, gauge, Vh, par, h, xm, pa, ua); compute16<0, 0, DAGGER, S>(pa, ua, 1.f, false, acc);
-            load16<1, 1, S>(in, gauge, Vh, par, h, yp, pa, ua); compute16<1, 1, DAGGER, S>(pa, ua, 1.f, false, acc);
-            load16<1, 0, S>(in, gauge, Vh, par, h, ym, pa, ua); compute16<1, 0, DAGGER, S>(pa, ua, 1.f, false, acc);
-            load16<2, 1, S>(in, gauge, Vh, par, h, zp, pa, ua); compute16<2, 1, DAGGER, S>(pa, ua, 1.f, false, acc);
-            load16<2, 0, S>(in, gauge, Vh, par, h, zm, pa, ua); compute16<2, 0, DAGGER, S>(pa, ua, 1.f, false, acc);
-            load16<3, 1, S>(in, gauge, Vh, par, h, tp, pa, ua); compute16<3, 1, DAGGER, S>(pa, ua, A.tb, wp, acc);
-            load16<3, 0, S>(in, gauge, Vh, par, h, tm, pa, ua); compute16<3, 0, DAGGER, S>(pa, ua, A.tb, wm, acc);
+            load16<0, 1, S, R>(in, gauge, Vh, par, h, xp, pa, ua); compute16<0, 1, DAGGER, S, R>(pa, ua, 1.f, false, acc);
+            load16<0, 0, S, R>(in, gauge, Vh, par, h, xm, pa, ua); compute16<0, 0, DAGGER, S, R>(pa, ua, 1.f, false, acc);
+            load16<1, 1, S, R>(in, gauge, Vh, par, h, yp, pa, ua); compute16<1, 1, DAGGER, S, R>(pa, ua, 1.f, false, acc);
+            load16<1, 0, S, R>(in, gauge, Vh, par, h, ym, pa, ua); compute16<1, 0, DAGGER, S, R>(pa, ua, 1.f, false, acc);
+            load16<2, 1, S, R>(in, gauge, Vh, par, h, zp, pa, ua); compute16<2, 1, DAGGER, S, R>(pa, ua, 1.f, false, acc);
+            load16<2, 0, S, R>(in, gauge, Vh, par, h, zm, pa, ua); compute16<2, 0, DAGGER, S, R>(pa, ua, 1.f, false, acc);
+            load16<3, 1, S, R>(in, gauge, Vh, par, h, tp, pa, ua); compute16<3, 1, DAGGER, S, R>(pa, ua, A.tb, wp, acc);
+            load16<3, 0, S, R>(in, gauge, Vh, par, h, tm, pa, ua); compute16<3, 0, DAGGER, S, R>(pa, ua, A.tb, wm, acc);
         }
         // epilogue: res = c * acc (+ x | + A x), optional A^-1, store, optional norm
         const float cf = A.c, a = A.a;
@@ -789,7 +809,7 @@ static tm_status launch_t(tm_ctx* ctx, const DslashCall& c, const void* gauge, c
     return TM_OK;
 }
 
-template <typename S>
+template <typename S, int R>
 static tm_status launch16(tm_ctx* ctx, const DslashCall& c, const void* gauge, cudaStream_t st) {
     DslashArgs<float> A;
     A.in = c.in; A.x = c.x; A.out = c.out; A.gauge = gauge;
@@ -809,8 +829,9 @@ static tm_status launch16(tm_ctx* ctx, const DslashCall& c, const void* gauge, c
     const int grid = tiles * A.nb;
     // <PIPE = 2, MINB = 5>: links staged by cp.async, 96 registers, 20 warps/SM.  Measured at 32^3x64 (fp16 XPAY,
     // same box): 66.7 us against 69.8 us for register-loaded links <0, 6> and 67.5 us for <2, 6>.
-    if (c.dagger) dslash16_kernel<S, 1, 2, 5><<<grid, block, 0, st>>>(A);
-    else          dslash16_kernel<S, 0, 2, 5><<<grid, block, 0, st>>>(A);
+    // reconstruct-18: the same kernel without the row-2 rebuild (9 x 4-byte link chunks, 36 KB of slots per CTA)
+    if (c.dagger) dslash16_kernel<S, 1, 2, 5, R><<<grid, block, 0, st>>>(A);
+    else          dslash16_kernel<S, 0, 2, 5, R><<<grid, block, 0, st>>>(A);
     TM_LAUNCH_CHECK(ctx, "dslash16_kernel");
     if (c.red_op != RED_NONE) TM_TRY(tm_reduce_finish(ctx, (unsigned)tiles, c.red_op, c.guard, st));
     return TM_OK;
@@ -823,9 +844,9 @@ tm_status tm_dslash_launch(tm_ctx* ctx, const DslashCall& c, tm_prec prec, tm_re
     switch (prec) {
         case TM_F64:  return r12 ? launch_t<double, 12>(ctx, c, gauge, st) : launch_t<double, 18>(ctx, c, gauge, st);
         case TM_F32:  return r12 ? launch32(ctx, c, gauge, st) : launch_t<float, 18>(ctx, c, gauge, st);
-        case TM_F16:  return r12 ? launch16<__half>(ctx, c, gauge, st) : launch_t<__half, 18>(ctx, c, gauge, st);
-        case TM_BF16: return r12 ? launch16<__nv_bfloat16>(ctx, c, gauge, st)
-                                 : launch_t<__nv_bfloat16, 18>(ctx, c, gauge, st);
+        case TM_F16:  return r12 ? launch16<__half, 12>(ctx, c, gauge, st) : launch16<__half, 18>(ctx, c, gauge, st);
+        case TM_BF16: return r12 ? launch16<__nv_bfloat16, 12>(ctx, c, gauge, st)
+                                 : launch16<__nv_bfloat16, 18>(ctx, c, gauge, st);
     }
     return tm_fail(ctx, TM_EPREC, "tm_dslash: unknown precision");
 }
