@@ -72,8 +72,11 @@ const char* tm_last_error(const tm_ctx* ctx);
  *                         split-fp32 operands, hi*hi + lo*hi + hi*lo: same 1e-5 bound) and a forward-only s-family
  *                         derivative (whole-vector calls; never the automatic choice: measured slower than 2);
  *                         2 and 3 need Lx <= 32 and fall back to 1 otherwise
+ *   TM_OPT_POISON         debugging aid (compute-sanitizer's initcheck is not available everywhere): 1 = every workspace
+ *                         the context allocates from now on starts as 0xFF bytes, i.e. NaN in all four storage
+ *                         precisions, so that a read of never-written workspace memory reaches the results
  * TM_EARG for an unknown option or value. */
-typedef enum { TM_OPT_GROUP = 0, TM_OPT_CONTRACT_PATH = 1 } tm_option;
+typedef enum { TM_OPT_GROUP = 0, TM_OPT_CONTRACT_PATH = 1, TM_OPT_POISON = 2 } tm_option;
 tm_status tm_set_option(tm_ctx* ctx, tm_option opt, int value);
 
 /* d_U: device, canonical complex128 [V][4][3][3].  Copied into the context (fp64 master) asynchronously on stream;

@@ -106,6 +106,10 @@ extern "C" tm_status tm_set_option(tm_ctx* c, tm_option opt, int value) {
             if (value < 0 || value > 3) return tm_fail(c, TM_EARG, "tm_set_option: TM_OPT_CONTRACT_PATH must be 0..3");
             c->opt_contract = value;
             return TM_OK;
+        case TM_OPT_POISON:
+            if (value != 0 && value != 1) return tm_fail(c, TM_EARG, "tm_set_option: TM_OPT_POISON must be 0 or 1");
+            c->opt_poison = value;
+            return TM_OK;
     }
     return tm_fail(c, TM_EARG, "tm_set_option: unknown option");
 }
@@ -155,6 +159,10 @@ tm_status tm_ws(tm_ctx* c, int slot, size_t bytes, void** out) {
         cudaError_t e = cudaMalloc(&c->scratch[slot], bytes);
         if (e != cudaSuccess) { cudaGetLastError(); c->scratch[slot] = nullptr; return tm_fail(c, TM_EALLOC, "workspace: out of device memory"); }
         c->scratch_bytes[slot] = bytes;
+        // TM_OPT_POISON: fresh workspaces start as NaN in every storage precision (0xFF bytes), so a kernel that reads
+        // workspace memory nothing has written yet shows up in the results instead of seeing the driver's zero pages
+        if (c->opt_poison && cudaMemset(c->scratch[slot], 0xFF, bytes) != cudaSuccess)
+            return tm_cuda_fail(c, cudaGetLastError(), "workspace poison");
     }
     *out = c->scratch[slot];
     return TM_OK;
