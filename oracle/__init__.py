@@ -253,3 +253,52 @@ def loops_time_diluted(eta, U, kappa, mu, rho, momenta, tb=-1, max_iter=10000):
         worst = max(worst, tr)
         out[:, :, t0] = plain_loops_project(e, s, U, mom, tb, t0, t0 + 1)[:, :, t0]
     return out, worst
+
+
+# ---------------------------------------------------------------------------- hopping parameter expansion (row f4)
+def apply_AinvH(v, U, kappa, mu, tb=-1) -> np.ndarray:
+    """One factor of the expansion: A^-1 H v with A = 1 + 2 i kappa mu g5, H = A - M (reading 23)."""
+    v, p_v = _c(v)
+    U, p_U = _c(U)
+    out = np.empty_like(v)
+    lib().orc_apply_AinvH(out.ctypes.data_as(ctypes.c_void_p), p_v, p_U, _dims(dims_of(v)), ctypes.c_int(tb),
+                          ctypes.c_double(kappa), ctypes.c_double(mu))
+    return out
+
+
+def hpe_exact(U, kappa, mu, momenta, tb=-1, order_local=4, order_deriv=2) -> np.ndarray:
+    """Exact part sum_x e^{ipx} tr[X_i sum_{k<n_i} ((A^-1 H)^k A^-1)(x,x)] per timeslice, [80, nmom, T], by brute force
+    over all 12 V unit vectors (small lattices only)."""
+    U, p_U = _c(U)
+    T, lz, ly, lx = U.shape[:4]
+    mom = np.ascontiguousarray(momenta, dtype=np.int32).reshape(-1, 3)
+    out = np.zeros((80, len(mom), T), dtype=np.complex128)
+    lib().orc_hpe_exact(out.ctypes.data_as(ctypes.c_void_p), p_U, _dims((lx, ly, lz, T)), ctypes.c_int(tb),
+                        ctypes.c_double(kappa), ctypes.c_double(mu), ctypes.c_int(order_local), ctypes.c_int(order_deriv),
+                        mom.ctypes.data_as(ctypes.c_void_p), ctypes.c_int(len(mom)))
+    return out
+
+
+def hpe_orders(order: int):
+    """Reading 23: the ultra-local insertions are expanded to `order` (<= 4), the one-derivative ones to min(order, 2)
+    (their order-3 term closes four-link loops and is not site-independent)."""
+    if order < 0 or order > 4:
+        raise ValueError("HPE order must be 0..4")
+    return order, min(order, 2)
+
+
+def loops_hpe(eta, s, U, kappa, mu, momenta, tb=-1, order=4, exact=None) -> np.ndarray:
+    """HPE-improved plain loops of one (noise vector, solution) pair, step by step (reading 23):
+    remainder eta^dag X_i (A^-1 H)^{n_i} s, projected per timeslice, plus the exact part.  [80, nmom, T].
+    exact: the (source-independent) exact part if already computed."""
+    n_loc, n_der = hpe_orders(order)
+    mom = np.ascontiguousarray(momenta, dtype=np.int32).reshape(-1, 3)
+    v = {0: np.ascontiguousarray(s)}
+    for k in range(1, max(n_loc, n_der) + 1):
+        v[k] = apply_AinvH(v[k - 1], U, kappa, mu, tb)
+    out = np.empty((80, len(mom), eta.shape[0]), dtype=np.complex128)
+    out[:16] = plain_loops_project(eta, v[n_loc], U, mom, tb)[:16]
+    out[16:] = plain_loops_project(eta, v[n_der], U, mom, tb)[16:]
+    if exact is None:
+        exact = hpe_exact(U, kappa, mu, mom, tb, n_loc, n_der)
+    return out + exact

@@ -25,6 +25,8 @@
  *                               transform, cut in p^2               -> orc_loops_project
  *   sec 2.2  PAPER.md:88, 92    time-dilution: sources on one timeslice, "contract a single
  *                               time slice"                         -> orc_time_dilute, orc_plain_loops_project
+ *   sec 2.3  PAPER.md:92        Hopping Parameter Expansion [7]: M^-1 = sum_{k<n} (A^-1 H)^k A^-1 + (A^-1 H)^n M^-1
+ *                                                                   -> orc_apply_AinvH, orc_hpe_exact
  *
  * Pins (tests/test_oracle_*.py, all -m "not gpu"): gamma algebra; gamma5-
  * hermiticity; free-field plane waves vs the momentum-space closed form;
@@ -32,7 +34,9 @@
  * loops vs traces of dense inverses; summation by parts; numpy.fft cross-check
  * of the projection; TSM identity; Fig. 2's 13-source example of the binary
  * storage; time dilution: exact spin-colour-site dilution of one timeslice vs the
- * trace of the dense inverse, dense-D_m einsum, linearity in t0.  No function here
+ * trace of the dense inverse, dense-D_m einsum, linearity in t0; HPE: A^-1 H against the
+ * dense matrices, the expansion identity and the exact part against traces of dense
+ * matrices on 2^4, the closed forms of the exact part on 4^4.  No function here
  * is "parity unpinned".
  *
  * Conventions (readings 1-7,15,16): dims = {Lx,Ly,Lz,T}; site index
@@ -499,6 +503,108 @@ void orc_time_dilute(cplx *out, const cplx *eta, const int *dims, int t0)
     const long V3 = (long)dims[0] * dims[1] * dims[2], V = V3 * dims[3];
     for (long j = 0; j < V * 12; j++) out[j] = 0;
     for (long j = 0; j < V3 * 12; j++) out[(long)t0 * V3 * 12 + j] = eta[(long)t0 * V3 * 12 + j];
+}
+
+/* ------------------------------------------------------- hopping parameter expansion (row f4) */
+/* PAPER.md:92 "... variance reduction methods, namely the TSM, the one-end trick ..., time-dilution and the Hopping
+ * Parameter Expansion (HPE) [7]" + DESIGN.md reading 23.  Split M = A - H with the site-local A = 1 + 2 i kappa mu g5
+ * and the hopping part H = A - M (= kappa * sum of the eight hops).  For every n >= 0, exactly,
+ *     M^-1 = sum_{k<n} (A^-1 H)^k A^-1  +  (A^-1 H)^n M^-1 .
+ * The loop tr[X M^-1] is the sum of an exact part (first sum: no noise) and a remainder estimated stochastically with
+ * the same solution s = M^-1 eta:  eta^dag X (A^-1 H)^n s.
+ *
+ * orc_apply_AinvH: out = A^-1 (A in - M in), one factor of the expansion, from the definition H = A - M;
+ * A^-1 = (1 - 2 i kappa mu g5) / (1 + 4 kappa^2 mu^2) because g5^2 = 1. */
+void orc_apply_AinvH(cplx *out, const cplx *in, const cplx *U, const int *dims, int tb, double kappa, double mu)
+{
+    const long V = (long)dims[0] * dims[1] * dims[2] * dims[3];
+    cplx g5[4][4];
+    gamma_mat(4, g5);
+    const double a = 2.0 * kappa * mu;
+    cplx *Min = malloc(V * 12 * sizeof(cplx));
+    orc_apply_M(Min, in, U, dims, tb, kappa, mu, 0);
+    for (long x = 0; x < V; x++)
+        for (int c = 0; c < 3; c++) {
+            cplx w[4];                          /* w = A in - M in at this site and colour */
+            for (int s = 0; s < 4; s++) {
+                cplx g5in = 0;
+                for (int s2 = 0; s2 < 4; s2++) g5in += g5[s][s2] * in[x * 12 + s2 * 3 + c];
+                w[s] = in[x * 12 + s * 3 + c] + I * a * g5in - Min[x * 12 + s * 3 + c];
+            }
+            for (int s = 0; s < 4; s++) {
+                cplx g5w = 0;
+                for (int s2 = 0; s2 < 4; s2++) g5w += g5[s][s2] * w[s2];
+                out[x * 12 + s * 3 + c] = (w[s] - I * a * g5w) / (1.0 + a * a);
+            }
+        }
+    free(Min);
+}
+
+/* Exact part of the expansion, by brute force (column j of the operator from the unit vector e_j, for all 12 V of them):
+ *     out[(i*nmom + q)*T + t] = sum_{x in t} exp(+2 pi i p_q.x/L) tr_{spin,colour}[ ( X_i S_i )(x,x) ],
+ *     S_i = sum_{k < n_i} (A^-1 H)^k A^-1,   n_i = order_local for the ultra-local X_i = Gamma_n (i < 16),
+ *                                            n_i = order_deriv for X_{16+16m+n} = Gamma_n D_m.
+ * O(V^2): for the small lattices of the tests only. */
+void orc_hpe_exact(cplx *out, const cplx *U, const int *dims, int tb, double kappa, double mu,
+                   int order_local, int order_deriv, const int *momenta, int nmom)
+{
+    const int Lx = dims[0], Ly = dims[1], Lz = dims[2], T = dims[3];
+    const long V = (long)Lx * Ly * Lz * T;
+    const double a = 2.0 * kappa * mu;
+    const int nmax = order_local > order_deriv ? order_local : order_deriv;
+    cplx G[16][4][4], g5[4][4];
+    for (int n = 0; n < 16; n++) Gamma_mat(n, G[n]);
+    gamma_mat(4, g5);
+    cplx *site = calloc(V * 80, sizeof(cplx));          /* tr[(X_i S_i)(x,x)] for every site x */
+    cplx *w = malloc(V * 12 * sizeof(cplx)), *w2 = malloc(V * 12 * sizeof(cplx));
+    cplx *Sl = malloc(V * 12 * sizeof(cplx)), *Sd = malloc(V * 12 * sizeof(cplx));
+    for (long x0 = 0; x0 < V; x0++)
+        for (int j = 0; j < 12; j++) {
+            /* w = A^-1 e_j (k = 0), then w <- A^-1 H w; Sl, Sd = the partial sums applied to e_j */
+            for (long i = 0; i < V * 12; i++) { w[i] = 0; Sl[i] = 0; Sd[i] = 0; }
+            const int sp = j / 3, c = j % 3;
+            for (int s = 0; s < 4; s++) w[x0 * 12 + s * 3 + c] = ((s == sp ? 1.0 : 0.0) - I * a * g5[s][sp]) / (1.0 + a * a);
+            for (int k = 0; k < nmax; k++) {
+                if (k < order_local) for (long i = 0; i < V * 12; i++) Sl[i] += w[i];
+                if (k < order_deriv) for (long i = 0; i < V * 12; i++) Sd[i] += w[i];
+                if (k + 1 < nmax) {
+                    orc_apply_AinvH(w2, w, U, dims, tb, kappa, mu);
+                    memcpy(w, w2, V * 12 * sizeof(cplx));
+                }
+            }
+            /* diagonal entry (x0, j) of X_i S_i: component j at site x0 of X_i applied to the column */
+            for (int n = 0; n < 16; n++) {
+                cplx acc = 0;
+                for (int s2 = 0; s2 < 4; s2++) acc += G[n][sp][s2] * Sl[x0 * 12 + s2 * 3 + c];
+                site[x0 * 80 + n] += acc;
+            }
+            for (int m = 0; m < 4; m++) {
+                cplx d[12];
+                cov_deriv_site(d, Sd, U, dims, tb, x0, m);
+                for (int n = 0; n < 16; n++) {
+                    cplx acc = 0;
+                    for (int s2 = 0; s2 < 4; s2++) acc += G[n][sp][s2] * d[s2 * 3 + c];
+                    site[x0 * 80 + 16 + 16 * m + n] += acc;
+                }
+            }
+        }
+    for (int q = 0; q < nmom; q++)
+        for (int t = 0; t < T; t++) {
+            cplx acc[80];
+            memset(acc, 0, sizeof(acc));
+            for (int z = 0; z < Lz; z++)
+                for (int y = 0; y < Ly; y++)
+                    for (int x = 0; x < Lx; x++) {
+                        const double ph = 2.0 * M_PI * ((double)momenta[q * 3 + 0] * x / Lx
+                                                        + (double)momenta[q * 3 + 1] * y / Ly
+                                                        + (double)momenta[q * 3 + 2] * z / Lz);
+                        const cplx e = cos(ph) + I * sin(ph);
+                        const cplx *lx = site + ((((long)t * Lz + z) * Ly + y) * Lx + x) * 80;
+                        for (int i = 0; i < 80; i++) acc[i] += e * lx[i];
+                    }
+            for (int i = 0; i < 80; i++) out[((long)i * nmom + q) * T + t] = acc[i];
+        }
+    free(site); free(w); free(w2); free(Sl); free(Sd);
 }
 
 /* sec 2.1 + reading 14:
