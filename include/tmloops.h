@@ -224,6 +224,26 @@ tm_status loop_plain_project_timeslice(tm_ctx* ctx, void* d_out, const void* d_a
 tm_status tsm_estimate_time_diluted(tm_ctx* ctx, void* d_out, void* d_per_source, const tsm_params* params,
                                     tsm_info* info, void* stream);
 
+/* Row f4 of SURVEY.md sec 8, second half -- Hopping Parameter Expansion ("... time-dilution and the Hopping
+ * Parameter Expansion (HPE) [7], and all the possible combinations of these"; reading 23).
+ * With A = 1 + 2 i kappa mu g5 and H = A - M (kappa times the hopping term):
+ *   M^-1 = sum_{k<n} (A^-1 H)^k A^-1 + (A^-1 H)^n M^-1   for every n,
+ * so the plain loop estimator splits into an exact part and a remainder estimated with the same solution:
+ *   d_out[(i*nmom + k)*T + t] = sum_{x,y,z} exp(+2 pi i p_k.x / L) eta(x,t)^dag X_i ((A^-1 H)^{n_i} s)(x,t) + E_i(p_k),
+ *   X_n = G_n (n < 16): n_i = order;  X_{16+16m+n} = G_n D_m: n_i = min(order, 2);  order = 0..4 (0: the plain estimator);
+ *   E_i = the site- and gauge-independent trace of X_i sum_{k<n_i} (A^-1 H)^k A^-1 (closed forms, nonzero at p = 0 only).
+ * loop_hpe_project: one (eta, s) pair, device canonical complex128 spinors; d_out: device complex128 [80][nmom][T].
+ * tsm_estimate_hpe: the TSM estimator of these loops (whole-volume Z4 sources, solved 8 per launch; LP for all n_lp
+ *   sources, HP as well for the first n_hp): d_out = (1/n_lp) sum_r l_r^LP + (1/n_hp) sum_{r<n_hp} (l_r^HP - l_r^LP),
+ *   complex128 [80][nmom][T]; d_per_source: optional (NULL ok) [n_lp + n_hp][80][nmom][T]; params as for tsm_estimate
+ *   (d_solutions is not used).  TM_ENOCONV if any solve missed its rho (outputs still filled); synchronises the stream.
+ * TM_EDIM if order > 0 and an extent is < 4 (paths of fewer than 4 hops would close around the torus), TM_EARG for an
+ * order outside 0..4. */
+tm_status loop_hpe_project(tm_ctx* ctx, void* d_out, const void* d_eta, const void* d_s, double kappa, double mu,
+                           const int* h_momenta, int nmom, int order, tm_prec acc, void* stream);
+tm_status tsm_estimate_hpe(tm_ctx* ctx, void* d_out, void* d_per_source, const tsm_params* params, int order,
+                           tsm_info* info, void* stream);
+
 /* sec 2.1.1 (Fig. 2): binary storage of partial sums, on the device, in momentum space.
  * File k = 0, 1, 2, ... (the paper's File.2^k) holds the SUM of the per-source arrays of the 2^k sources
  * r = 2^k - 1 ... 2^(k+1) - 2, so n sources need loop_binary_nfiles(n) = ceil(log2(n + 1)) arrays instead of n.

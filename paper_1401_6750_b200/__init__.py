@@ -38,6 +38,7 @@ EXPORTS = [
     "loop_plain_project_timeslice", "tsm_estimate_time_diluted", "tm_launch_count", "tm_set_option", "tsm_partial_sums", "tsm_combine_sums",
     "tm_fma_peak",
     "loop_binary_nfiles", "loop_binary_accumulate", "loop_binary_recover", "tsm_estimate_binary",
+    "loop_hpe_project", "tsm_estimate_hpe",
 ]
 
 
@@ -113,6 +114,8 @@ def load_library():
     L.tsm_estimate_host.argtypes = [vp, vp, vp, ctypes.POINTER(tsm_params), ctypes.POINTER(tsm_info), vp]
     L.loop_plain_project_timeslice.argtypes = [vp, vp, vp, vp, ctypes.POINTER(ci), ci, ci, ci, vp]
     L.tsm_estimate_time_diluted.argtypes = [vp, vp, vp, ctypes.POINTER(tsm_params), ctypes.POINTER(tsm_info), vp]
+    L.loop_hpe_project.argtypes = [vp, vp, vp, vp, cd, cd, ctypes.POINTER(ci), ci, ci, ci, vp]
+    L.tsm_estimate_hpe.argtypes = [vp, vp, vp, ctypes.POINTER(tsm_params), ci, ctypes.POINTER(tsm_info), vp]
     L.tsm_partial_sums_host.argtypes = [vp, vp, vp, ctypes.POINTER(tsm_params), ctypes.POINTER(tsm_info), vp]
     L.loop_binary_nfiles.argtypes = [ci]
     L.loop_binary_nfiles.restype = ci
@@ -443,6 +446,38 @@ class TmContext:
         info = tsm_info()
         st = self.lib.tsm_estimate_time_diluted(self.h, out.data_ptr(), ps.data_ptr() if ps is not None else None,
                                                 ctypes.byref(P), ctypes.byref(info), _stream())
+        self._check(st, allow=() if raise_on_noconv else (TM_ENOCONV,))
+        return out, ps, self._tsm_info(info, st)
+
+    # ------------------------------------------------------------------ hopping parameter expansion (row f4)
+    def loop_hpe_project(self, eta, s, kappa, mu, momenta, order=4, acc=TM_F64):
+        """HPE-improved plain loops of one (eta, s) pair (reading 23), complex128 [80, nmom, T]."""
+        torch = _torch()
+        eta = self._dev(eta, torch.complex128)
+        s = self._dev(s, torch.complex128)
+        mom = np.ascontiguousarray(momenta, dtype=np.int32).reshape(-1, 3)
+        out = torch.empty((80, len(mom), self.T), dtype=torch.complex128, device=self.tdev)
+        self._check(self.lib.loop_hpe_project(
+            self.h, out.data_ptr(), eta.data_ptr(), s.data_ptr(), float(kappa), float(mu),
+            mom.ctypes.data_as(ctypes.POINTER(ctypes.c_int)), len(mom), int(order), int(acc), _stream()))
+        return out
+
+    def tsm_estimate_hpe(self, n_lp, n_hp, kappa, mu, momenta, lp, hp, order=4, acc_lp=TM_F32, acc_hp=TM_F64,
+                         z4=None, seed=0, per_source=False, raise_on_noconv=True, src_first=0, src_stride=1):
+        """TSM estimate of the HPE-improved plain loops: (out [80,nmom,T], per_source | None, info)."""
+        torch = _torch()
+        d_z4 = None
+        if z4 is not None:
+            z4 = self._dev(z4, torch.uint8)
+            assert z4.numel() == n_lp * 3 * self.V
+            d_z4 = z4.data_ptr()
+        P, mom = self._tsm_params(n_lp, n_hp, kappa, mu, momenta, lp, hp, acc_lp, acc_hp, d_z4, seed, src_first, src_stride)
+        shape = (80, len(mom), self.T)
+        out = torch.empty(shape, dtype=torch.complex128, device=self.tdev)
+        ps = torch.empty((n_lp + n_hp,) + shape, dtype=torch.complex128, device=self.tdev) if per_source else None
+        info = tsm_info()
+        st = self.lib.tsm_estimate_hpe(self.h, out.data_ptr(), ps.data_ptr() if ps is not None else None,
+                                       ctypes.byref(P), int(order), ctypes.byref(info), _stream())
         self._check(st, allow=() if raise_on_noconv else (TM_ENOCONV,))
         return out, ps, self._tsm_info(info, st)
 

@@ -122,7 +122,8 @@ enum {
     WS_CT_S, WS_CT_ETA, WS_CT_PLANES, WS_CT_OUT,                // contraction
     WS_TSM_ACC, WS_TSM_ETA32, WS_TSM_ETA64, WS_TSM_S32, WS_TSM_S64, WS_TSM_Z4, WS_TSM_KEEP,
     WS_API_A, WS_API_B, WS_API_C,
-    WS_TD_ACC, WS_TD_PRIM                                       // time dilution (dilution.cu)
+    WS_TD_ACC, WS_TD_PRIM,                                      // time dilution (dilution.cu), HPE (hpe.cu)
+    WS_HPE_A, WS_HPE_B, WS_HPE_C, WS_HPE_TAB                   // HPE: hopping-term ping-pong vectors, tables
 };
 tm_status tm_ws(tm_ctx* c, int slot, size_t bytes, void** out);     // api.cu
 tm_status tm_lane_use(tm_ctx* c, int lane);                          // api.cu: make `lane` the active one
