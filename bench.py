@@ -480,6 +480,18 @@ def run_b200(args, cfg):
     ms_per_step = float(ms.item()) / args.steps
     value = n_lp_job / (ms_per_step * 1e-3)
 
+    if args.step_only:
+        # the launch-list capture under profiles/ wraps this mode: warm-up + timed steps, nothing else
+        if rank == 0:
+            print(json.dumps({"metric": "tsm_sources_per_sec", "value": value, "unit": "sources/s", "n_gpus": world,
+                              "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step, "step_only": True,
+                              "config": workload_config(cfg, args), "clocks": clocks, "gpu_launches": int(launches),
+                              "extras": {k: float(np.mean([i[k] for i in infos])) for k in ("ms_lp_solve", "ms_hp_solve", "ms_contract")}}))
+        ctx.close()
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
     # ---- end to end through host buffers (pinned): gauge + noise H2D, estimate D2H, every step
     U_host = torch.empty(U.shape, dtype=U.dtype).pin_memory()
     U_host.copy_(U)
@@ -648,6 +660,9 @@ def main():
     ap.add_argument("--n-lp", type=int, default=None, help="override N_LP (debugging; invalidates the headline)")
     ap.add_argument("--n-hp", type=int, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--step-only", action="store_true",
+                    help="warm-up + timed TSM steps only (no end-to-end leg, rooflines, sweep or CPU baseline): the command of "
+                         "the ncu launch list under profiles/")
     ap.add_argument("--no-c5-sweep", action="store_true")
     ap.add_argument("--lp-delta", type=float, default=None, help="reliable-update trigger of the LP solves (tuning)")
     ap.add_argument("--hp-delta", type=float, default=None, help="reliable-update trigger of the HP solves (tuning)")

@@ -82,7 +82,13 @@ tm_status tm_set_option(tm_ctx* ctx, tm_option opt, int value);
 /* d_U: device, canonical complex128 [V][4][3][3].  Copied into the context (fp64 master) asynchronously on stream;
  * previously built reduced-precision copies are marked stale and repacked on their next use.
  * tm_load_gauge_host: the same from HOST memory (pinned for a truly asynchronous copy); the buffer must stay valid
- * until the stream has passed the call. */
+ * until the stream has passed the call.
+ * Streams: every call is stream-ordered on the stream it is given.  The context's lazily built state is ordered across
+ * streams by events: a call on another stream than the one that uploaded the master or packed a reduced-precision copy
+ * waits (on the device) for that upload / pack before using it, and a new upload waits for the packs of the previous
+ * master.  What the library cannot know is which kernels of OTHER streams still read the previous gauge field or a
+ * workspace: load a new gauge field, and share one context between streams, only at points where the caller has
+ * ordered those streams itself (one context per stream is the simple rule; tsm_estimate's own lanes are ordered inside). */
 tm_status tm_load_gauge(tm_ctx* ctx, const void* d_U, void* stream);
 tm_status tm_load_gauge_host(tm_ctx* ctx, const void* h_U, void* stream);
 

@@ -126,6 +126,10 @@ extern "C" tm_status tm_destroy(tm_ctx* c) {
     cudaDeviceSynchronize();
     drop_gauge_copies(c);
     if (c->d_Ucanon) cudaFree(c->d_Ucanon);
+    if (c->master_ev) cudaEventDestroy(c->master_ev);
+    for (int p = 0; p < 4; p++)
+        for (int r = 0; r < 2; r++)
+            if (c->gauge_ev[p][r]) cudaEventDestroy(c->gauge_ev[p][r]);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     lane_park(c, &c->lanes[c->cur_lane]);
     for (int l = 0; l < TM_NLANES; l++) {
@@ -178,7 +182,14 @@ static tm_status load_gauge_impl(tm_ctx* c, const void* U, cudaMemcpyKind kind, 
         if (e != cudaSuccess) { cudaGetLastError(); c->d_Ucanon = nullptr; return tm_fail(c, TM_EALLOC, "tm_load_gauge: out of device memory"); }
     }
     memset(c->gauge_valid, 0, sizeof(c->gauge_valid));
+    // packs of the previous master that were enqueued on other streams must have read it before it is overwritten
+    for (int p = 0; p < 4; p++)
+        for (int r = 0; r < 2; r++)
+            if (c->gauge_ev[p][r] && c->gauge_st[p][r] != st) TM_CUDA(c, cudaStreamWaitEvent(st, c->gauge_ev[p][r], 0));
     TM_CUDA(c, cudaMemcpyAsync(c->d_Ucanon, U, bytes, kind, st));
+    if (!c->master_ev) TM_CUDA(c, cudaEventCreateWithFlags(&c->master_ev, cudaEventDisableTiming));
+    TM_CUDA(c, cudaEventRecord(c->master_ev, st));
+    c->master_st = st;
     return TM_OK;
 }
 

@@ -63,6 +63,10 @@ struct tm_ctx {
     void* d_Ucanon;                 // fp64 master, canonical [V][4][3][3] complex128
     void* gauge[4][2];              // [prec][recon==12] internal copies, built lazily
     int gauge_valid[4][2];          // 0: allocated but stale (a new master was loaded) -> repacked on next use
+    // cross-stream ordering of the lazily built gauge state: the event recorded after the master upload / after each
+    // pack, and the stream it was recorded on; a call on another stream waits on the event before it touches the data
+    cudaEvent_t master_ev, gauge_ev[4][2];
+    cudaStream_t master_st, gauge_st[4][2];
     cudaStream_t copy_stream;       // host -> device prefetch of the packed noise (tsm_estimate_host), created on first use
     // reduction scratch
     double* d_partials;             // per-block partial sums

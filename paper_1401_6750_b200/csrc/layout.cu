@@ -52,6 +52,8 @@ tm_status tm_get_gauge(tm_ctx* ctx, tm_prec prec, tm_recon recon, cudaStream_t s
     const int r = (recon == TM_R12) ? 1 : 0;
     void** slot = &ctx->gauge[prec][r];
     if (!*slot || !ctx->gauge_valid[prec][r]) {
+        // the master may have been uploaded on another stream
+        if (ctx->master_ev && ctx->master_st != st) TM_CUDA(ctx, cudaStreamWaitEvent(st, ctx->master_ev, 0));
         tm_status s = TM_OK;
         switch (prec) {
             case TM_F64:  s = r ? gauge_pack_t<double, 12>(ctx, slot, st) : gauge_pack_t<double, 18>(ctx, slot, st); break;
@@ -61,6 +63,12 @@ tm_status tm_get_gauge(tm_ctx* ctx, tm_prec prec, tm_recon recon, cudaStream_t s
         }
         TM_TRY(s);
         ctx->gauge_valid[prec][r] = 1;
+        if (!ctx->gauge_ev[prec][r]) TM_CUDA(ctx, cudaEventCreateWithFlags(&ctx->gauge_ev[prec][r], cudaEventDisableTiming));
+        TM_CUDA(ctx, cudaEventRecord(ctx->gauge_ev[prec][r], st));
+        ctx->gauge_st[prec][r] = st;
+    } else if (ctx->gauge_ev[prec][r] && ctx->gauge_st[prec][r] != st) {
+        // packed on another stream: order this stream after the pack (a no-op once the pack has finished)
+        TM_CUDA(ctx, cudaStreamWaitEvent(st, ctx->gauge_ev[prec][r], 0));
     }
     *out = *slot;
     return TM_OK;

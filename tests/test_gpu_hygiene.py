@@ -141,3 +141,38 @@ def test_grouped_two_lane_runs_repeat_bit_identically():
                 first = got
             else:
                 assert np.array_equal(got[0], first[0]) and np.array_equal(got[1], first[1]), rep
+
+
+def test_gauge_state_is_ordered_across_streams(orc):
+    """The master gauge field is uploaded on one stream, the reduced-precision copy packed on a second and reused on a
+    third, with no host synchronisation in between: the context's events must order them (include/tmloops.h,
+    "Streams")."""
+    import torch
+    t = tm()
+    c = inputs.CONFIGS["c2"]
+    dims = c["dims"]
+    from paper_1401_6750_b200 import inputs_torch
+    dev = torch.device("cuda", 0)
+    U = inputs_torch.gauge_field(dims, c["eps"], c["seed"], dev)
+    U2 = inputs_torch.gauge_field(dims, c["eps"], c["seed"] + 1, dev)
+    psi = inputs_torch.z4_source(dims, 3, 0, dev)
+    torch.cuda.synchronize()
+    s1, s2, s3 = torch.cuda.Stream(), torch.cuda.Stream(), torch.cuda.Stream()
+    with t.TmContext(dims, -1) as ctx:
+        got = {}
+        for name, field in (("first", U), ("second", U2)):          # the second upload overwrites a master in use
+            with torch.cuda.stream(s1):
+                ctx.tm_load_gauge(field)
+            with torch.cuda.stream(s2):
+                a = ctx.apply_M(psi, c["kappa"], c["mu"], t.TM_F32, 12)
+            with torch.cuda.stream(s3):
+                b = ctx.apply_M(psi, c["kappa"], c["mu"], t.TM_F32, 12)
+                d = ctx.apply_M(psi, c["kappa"], c["mu"], t.TM_F64, 18)
+            torch.cuda.synchronize()
+            got[name] = (to_np(a), to_np(b), to_np(d))
+        for name, field in (("first", U), ("second", U2)):
+            ref = orc.apply_M(to_np(psi), to_np(field), c["kappa"], c["mu"], -1)
+            a, b, d = got[name]
+            assert np.array_equal(a, b)
+            assert np.linalg.norm(a - ref) <= 1e-6 * np.linalg.norm(ref), name
+            assert np.linalg.norm(d - ref) <= 1e-13 * np.linalg.norm(ref), name

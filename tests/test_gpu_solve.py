@@ -90,3 +90,62 @@ def test_solve_edge_cases(orc, c1):
         ctx.tm_load_gauge(U)
         s, info = ctx.tm_cg_solve(eta, C1["kappa"], -C1["mu"], "f32", "f64", 12, 1e-9, 2000)
         assert orc.true_residual(to_np(s), eta, U, C1["kappa"], -C1["mu"], +1) <= 1e-9
+
+
+HARD = dict(dims=(16, 16, 16, 32), tb=1, eps=0.1, seed=3, kappa=0.126, mu=0.004)
+
+
+def test_solve_hard_operator_16bit_reliable_updates(orc):
+    """A badly conditioned operator at 16^3x32 (smooth gauge field, periodic time boundary, kappa next to the free
+    critical value 1/8: the smallest singular value of M is ~ 2 kappa mu): 16-bit sloppy storage must survive several
+    reliable updates -- fp16 ~100 iterations / 5 updates, bf16 ~700 iterations with the forced update every 100
+    iterations -- and the mixed fp32/fp64 solve ~160 iterations.  True residuals are evaluated by the oracle."""
+    import torch
+    t = tm()
+    from paper_1401_6750_b200 import inputs_torch
+    H = HARD
+    dev = torch.device("cuda", 0)
+    U = inputs_torch.gauge_field(H["dims"], H["eps"], H["seed"], dev)
+    eta = inputs_torch.z4_source(H["dims"], 2, 0, dev)
+    U_np, eta_np = to_np(U), to_np(eta)
+    with t.TmContext(H["dims"], H["tb"]) as ctx:
+        ctx.tm_load_gauge(U)
+        seen = {}
+        for sloppy, outer, rho in (("f16", "f32", 1e-5), ("bf16", "f32", 1e-5), ("f32", "f64", 1e-8)):
+            s, info = ctx.tm_cg_solve(eta, H["kappa"], H["mu"], sloppy, outer, 12, rho, 20000, 0.1)
+            tr = orc.true_residual(to_np(s), eta_np, U_np, H["kappa"], H["mu"], H["tb"])
+            assert tr <= rho, (sloppy, tr)
+            assert abs(tr - info["true_resid"]) <= 0.05 * rho
+            seen[sloppy] = info
+        assert seen["f16"]["iters"] >= 60 and seen["f16"]["reliable_updates"] >= 4
+        assert seen["bf16"]["iters"] >= 200 and seen["bf16"]["reliable_updates"] >= 6      # forced updates every 100
+        assert seen["f32"]["iters"] >= 100 and seen["f32"]["reliable_updates"] >= 6
+        # fp16 storage has no exponent range for a 1e-8 residual (unscaled vectors underflow): the solver must say so
+        # (TM_ENOCONV via the stagnation rule, outputs filled) instead of iterating to max_iter or returning garbage
+        s, info = ctx.tm_cg_solve(eta, H["kappa"], H["mu"], "f16", "f64", 12, 1e-8, 20000, 0.1, raise_on_noconv=False)
+        assert info["status"] == t.TM_ENOCONV and info["iters"] < 2000
+        tr = orc.true_residual(to_np(s), eta_np, U_np, H["kappa"], H["mu"], H["tb"])
+        assert abs(tr - info["true_resid"]) <= 0.05 * max(tr, 1e-8) and tr < 1e-3
+
+
+def test_grouped_hard_solves_pause_at_different_iterations():
+    """Eight sources of the hard operator solved in one group with bf16 storage: they pause for reliable updates and
+    finish at different iterations; every per-source array must still be bit-identical to one source per launch."""
+    import torch
+    t = tm()
+    from paper_1401_6750_b200 import inputs_torch
+    H = HARD
+    dev = torch.device("cuda", 0)
+    U = inputs_torch.gauge_field(H["dims"], H["eps"], H["seed"], dev)
+    mom = inputs.momentum_list(1)
+    lp = dict(sloppy="bf16", outer="f32", recon=12, rho=1e-4, max_iter=20000, delta=0.1)
+    hp = dict(sloppy="f32", outer="f64", recon=12, rho=1e-8, max_iter=20000, delta=0.1)
+    with t.TmContext(H["dims"], H["tb"]) as ctx:
+        ctx.tm_load_gauge(U)
+        out_g, ps_g, info_g = ctx.tsm_estimate(8, 2, H["kappa"], H["mu"], mom, lp, hp, t.TM_F32, t.TM_F64, seed=7, per_source=True)
+        ctx.tm_set_option(t.TM_OPT_GROUP, 1)
+        out_1, ps_1, info_1 = ctx.tsm_estimate(8, 2, H["kappa"], H["mu"], mom, lp, hp, t.TM_F32, t.TM_F64, seed=7, per_source=True)
+        ctx.tm_set_option(t.TM_OPT_GROUP, 0)
+        assert np.array_equal(to_np(ps_g), to_np(ps_1))
+        assert info_g["iters_lp"] == info_1["iters_lp"] and info_g["iters_hp"] == info_1["iters_hp"]
+        assert info_g["iters_lp"] >= 8 * 30 and info_g["worst_resid_lp"] <= lp["rho"] and info_g["worst_resid_hp"] <= hp["rho"]
