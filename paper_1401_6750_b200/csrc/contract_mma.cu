@@ -1,5 +1,5 @@
 // contract_mma.cu -- fused contraction + projection, site stage and x/y-DFT, third implementation (fp32, Lx <= 32,
-// whole-vector launches; TM_OPT_CONTRACT_PATH 3, the automatic choice when usable).
+// whole-vector launches; TM_OPT_CONTRACT_PATH 3; measured slower than contract_tma.cu, so never the automatic choice).
 //
 // Same mathematics as contract_xy_kernel in contract.cu and the same
 // TMA operand staging as contract_tma.cu.  contract_tma.cu is bound by how well two lock-stepped producer warps per

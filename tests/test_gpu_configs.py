@@ -86,16 +86,16 @@ def test_c3_small_tsm_run(orc):
         lp = dict(sloppy="bf16", outer="f32", recon=12, rho=1e-2, max_iter=2000, delta=0.01)
         hp = dict(sloppy="f32", outer="f64", recon=12, rho=1e-8, max_iter=5000, delta=0.01)
         out, ps, info = ctx.tsm_estimate(n_lp, n_hp, c["kappa"], c["mu"], mom, lp, hp, t.TM_F32, t.TM_F64,
-                                         seed=c["src_seed"], per_source=True)
+                                         seed=c["src_seed"], per_source=True, solutions=True)
+        sol = info["solutions"]                     # the run's own solutions: [n_lp + n_hp, T, Lz, Ly, Lx, 4, 3]
         assert info["worst_resid_lp"] <= 1e-2 and info["worst_resid_hp"] <= 1e-8
         out, ps = to_np(out), to_np(ps)
         assert rel_l2(out, orc.tsm_combine(ps[:n_lp], ps[n_lp:])) <= 1e-12
         from paper_1401_6750_b200 import inputs_torch
         for r in (0, n_hp - 1):
             eta = inputs_torch.z4_source(c["dims"], c["src_seed"], r, dev)
-            # the GPU's own HP solution: residual by the oracle, loops of that solution by the oracle
-            s, _ = ctx.tm_cg_solve(eta, c["kappa"], c["mu"], **hp)
-            s_h, eta_h = to_np(s), to_np(eta)
+            # the run's own HP solution of this source (d_solutions): residual by the oracle, loops of that solution by the oracle
+            s_h, eta_h = to_np(sol[n_lp + r]), to_np(eta)
             assert orc.true_residual(s_h, eta_h, U_h, c["kappa"], c["mu"], -1) <= 1e-8
             for ts in (0, 47):
                 ref = orc.loops_project(s_h, eta_h, U_h, c["kappa"], c["mu"], mom, -1, ts, ts + 1)[..., ts]
