@@ -652,7 +652,7 @@ def main():
                     help="N > 1: shard the one (N_LP, N_HP) workload over the ranks (strong) or run N times the workload (weak)")
     ap.add_argument("--what", default="step", choices=["step", "dslash", "dslash_group", "contract", "blas", "solve"],
                     help="step: the bench line; otherwise run one kernel family a few times (ncu captures)")
-    ap.add_argument("--contract-path", type=int, default=0, choices=[0, 1, 2, 3],
+    ap.add_argument("--contract-path", type=int, default=0, choices=[0, 1, 2, 3, 4],
                     help="TM_OPT_CONTRACT_PATH of the fp32 contraction (0 = automatic, see include/tmloops.h)")
     ap.add_argument("--prec", default="f16", help="--what != step: storage precision (contract: f32 | f64)")
     ap.add_argument("--recon", type=int, default=12)

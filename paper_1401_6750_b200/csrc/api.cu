@@ -103,7 +103,7 @@ extern "C" tm_status tm_set_option(tm_ctx* c, tm_option opt, int value) {
             c->opt_group = value;
             return TM_OK;
         case TM_OPT_CONTRACT_PATH:
-            if (value < 0 || value > 3) return tm_fail(c, TM_EARG, "tm_set_option: TM_OPT_CONTRACT_PATH must be 0..3");
+            if (value < 0 || value > 4) return tm_fail(c, TM_EARG, "tm_set_option: TM_OPT_CONTRACT_PATH must be 0..4");
             c->opt_contract = value;
             return TM_OK;
         case TM_OPT_POISON:

@@ -34,6 +34,8 @@ struct TmaContractArgs {
     Geom g;
     float tb;
     int t_first;           // first timeslice of the launch
+    float wf[7][6];        // folded x-stage (LX > 0): c1, s1, c2, s2, c3, s3 at x = j + 1, j < LX / 4 - 1 (kernel
+                           // parameters live in the constant bank: FFMA2 takes them as uniform-register operands)
 };
 
 // shared-memory plan (bytes), every TMA destination 128-byte aligned
@@ -94,6 +96,23 @@ __device__ __forceinline__ void lds_link(const float4* blk, int Xh, int seg0, in
 // row blocks of one input stage, in the order the loader fills them
 enum { ROW_C = 0, ROW_YP, ROW_YM, ROW_ZP, ROW_ZM, ROW_TP, ROW_TM };
 
+// Folded x-stage (compile-time LX = Lx, a multiple of 4).  cos / sin(2 pi m x / L), m <= 3, take the same absolute
+// values on the four sites {j, L - j, L/2 - j, L/2 + j}, so the consumers first form the four sign combinations of a
+// group (8 adds) and then need 7 weighted accumulations per group instead of 28: 15 packed operations per 4 sites.  The
+// producers store site x at row-buffer column fold_col(x): group j occupies columns 4j .. 4j + 3 (two 16-byte reads);
+// group 0 holds the self-mirrored sites 0, L/2 and L/4, 3L/4, whose weights are 0 and +-1.
+template <int LX> __device__ __forceinline__ int fold_col(int x) {
+    if (x == 0) return 0;
+    if (x == LX / 2) return 1;
+    if (x == LX / 4) return 2;
+    if (x == 3 * LX / 4) return 3;
+    if (x < LX / 4) return 4 * x;
+    if (x < LX / 2) return 4 * (LX / 2 - x) + 2;
+    if (x < 3 * LX / 4) return 4 * (x - LX / 2) + 3;
+    return 4 * (LX - x) + 1;
+}
+__device__ __forceinline__ T2 sub2(T2 a, T2 b) { T2 d; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+
 struct TxShared {             // resolved shared-memory pointers of the CTA
     unsigned char* in;        // [TX_NSI] input stages
     T2* cbuf;                 // [TX_NSC][160][CT_BSC]
@@ -105,6 +124,7 @@ struct TxShared {             // resolved shared-memory pointers of the CTA
 // producer warp: fixed derivative job (fam, mu) for every row of the plane, plus the rotating d = 0 jobs.
 // One copy of the code for all directions (the direction only selects loop-invariant shared-memory
 // offsets), so the 8 producer warps share the instruction cache.
+template <int LX>
 __device__ __forceinline__ void producer_rows(const TxShared& sh, const TxPlan& P, const Geom& g, int z, int t,
                                               int warp, int lane, float tb) {
     const int Xh = g.Xh;
@@ -127,6 +147,9 @@ __device__ __forceinline__ void producer_rows(const TxShared& sh, const TxPlan& 
     const int nbf_blk = fam_off + rf * P.row + ((1 - p) * 6) * Xh * 16;
     const int nbb_blk = fam_off + rb * P.row + ((1 - p) * 6) * Xh * 16;
     const int seg = Xh * 16;
+    // row-buffer column of this lane's site for x = 2 idx (+ 1): the site column itself, or its folded position
+    const int col_e = LX > 0 ? fold_col<(LX > 0 ? LX : 4)>(2 * idx) : lane;
+    const int col_o = LX > 0 ? fold_col<(LX > 0 ? LX : 4)>(2 * idx + 1) : lane;
     for (int y = 0; y < g.X1; y++) {
         const int si = y % TX_NSI, sc = y % TX_NSC;
         const unsigned char* stage = sh.in + (size_t)si * P.stage;
@@ -135,6 +158,7 @@ __device__ __forceinline__ void producer_rows(const TxShared& sh, const TxPlan& 
         if (y >= TX_NSC) named_bar_sync(1 + TX_NSC + sc, TX_NCOMP);
         if (active) {
             const int xo = (p ^ (y + z + t)) & 1;                 // x = 2 idx + xo
+            const int col = xo ? col_o : col_e;
             const int idx_f = mu == 0 ? (xo ? idx_up : idx) : idx;
             const int idx_b = mu == 0 ? (xo ? idx : idx_dn) : idx;
             T2 sv[12];
@@ -176,7 +200,7 @@ __device__ __forceinline__ void producer_rows(const TxShared& sh, const TxPlan& 
                 }
                 lds_link(reinterpret_cast<const float4*>(stage + ub_blk + idx_b * 16), Xh, 0, 0, U);
                 su3_macc<1, 1, float>(U, nb, psi);
-                outer_store<float>(sv, psi, rowbuf, fam * 5 + 1 + mu, lane);
+                outer_store<float>(sv, psi, rowbuf, fam * 5 + 1 + mu, col);
             }
             {
                 // this warp's quarter of a d = 0 job: column bb = mu of C_{fam,0}[a][bb] = sum_c conj(s_ac) f_{bb,c}
@@ -207,7 +231,7 @@ __device__ __forceinline__ void producer_rows(const TxShared& sh, const TxPlan& 
 #pragma unroll
                     for (int a = 0; a < 4; a++) acc[a] = P2<float>::fma_s(-sim[a], ip, acc[a]);
                 }
-                T2* out = rowbuf + (size_t)(fam * 5 * 16 + bb) * CT_BSC + lane;
+                T2* out = rowbuf + (size_t)(fam * 5 * 16 + bb) * CT_BSC + col;
 #pragma unroll
                 for (int a = 0; a < 4; a++) out[(size_t)(a * 4) * CT_BSC] = acc[a];
             }
@@ -218,7 +242,7 @@ __device__ __forceinline__ void producer_rows(const TxShared& sh, const TxPlan& 
     }
 }
 
-template <int PRUNE>
+template <int PRUNE, int LX>
 __global__ void __launch_bounds__(TX_NTHREADS, 1)
 contract_xy_tma_kernel(const __grid_constant__ CUtensorMap tm_s, const __grid_constant__ CUtensorMap tm_e,
                        const __grid_constant__ CUtensorMap tm_gf, const __grid_constant__ CUtensorMap tm_gb,
@@ -306,7 +330,7 @@ contract_xy_tma_kernel(const __grid_constant__ CUtensorMap tm_s, const __grid_co
         }
     } else if (warp < TX_NP) {
         // ================================================================ producers
-        producer_rows(sh, P, g, z, t, warp, lane, A.tb);
+        producer_rows<LX>(sh, P, g, z, t, warp, lane, A.tb);
     } else {
         // ================================================================ consumers
         typedef P2<float> PP;
@@ -322,15 +346,44 @@ contract_xy_tma_kernel(const __grid_constant__ CUtensorMap tm_s, const __grid_co
 #pragma unroll
             for (int m = 0; m < 3; m++) { ac[m] = PP::make(0.f, 0.f); as[m] = PP::make(0.f, 0.f); }
             named_bar_sync(1 + sc, TX_NCOMP);
-#pragma unroll 4
-            for (int l = 0; l < g.X0; l++) {
-                const T2 val = v[l];
-                const float* wl = w + l * 8;
-                a0 = PP::add(a0, val);
+            if (LX > 0) {
+                // folded x-stage: see fold_col
+                const ulonglong2* v4 = reinterpret_cast<const ulonglong2*>(v);
+                {
+                    const ulonglong2 q0 = v4[0], q1 = v4[1];       // C(0), C(L/2); C(L/4), C(3L/4)
+                    const T2 Pp = PP::add(q0.x, q0.y), Mm = sub2(q0.x, q0.y);
+                    const T2 Ee = PP::add(q1.x, q1.y), Oo = sub2(q1.x, q1.y);
+                    a0 = PP::add(Pp, Ee);
+                    ac[1] = sub2(Pp, Ee);
+                    ac[0] = Mm; ac[2] = Mm;
+                    as[0] = Oo; as[2] = sub2(as[2], Oo);
+                }
 #pragma unroll
-                for (int m = 0; m < 3; m++) {
-                    ac[m] = PP::fma_s(wl[2 * m + 1], val, ac[m]);
-                    as[m] = PP::fma_s(wl[2 * m + 2], val, as[m]);
+                for (int j = 1; j < (LX > 0 ? LX / 4 : 1); j++) {
+                    const ulonglong2 q0 = v4[2 * j], q1 = v4[2 * j + 1];   // C(j), C(L-j); C(L/2-j), C(L/2+j)
+                    const T2 E1 = PP::add(q0.x, q0.y), O1 = sub2(q0.x, q0.y);
+                    const T2 E2 = PP::add(q1.x, q1.y), O2 = sub2(q1.y, q1.x);
+                    const T2 Pp = PP::add(E1, E2), Mm = sub2(E1, E2), Rr = PP::add(O1, O2), Ss = sub2(O1, O2);
+                    const float* wj = A.wf[j - 1];
+                    a0 = PP::add(a0, Pp);
+                    ac[0] = PP::fma_s(wj[0], Mm, ac[0]);
+                    as[0] = PP::fma_s(wj[1], Ss, as[0]);
+                    ac[1] = PP::fma_s(wj[2], Pp, ac[1]);
+                    as[1] = PP::fma_s(wj[3], Rr, as[1]);
+                    ac[2] = PP::fma_s(wj[4], Mm, ac[2]);
+                    as[2] = PP::fma_s(wj[5], Ss, as[2]);
+                }
+            } else {
+#pragma unroll 4
+                for (int l = 0; l < g.X0; l++) {
+                    const T2 val = v[l];
+                    const float* wl = w + l * 8;
+                    a0 = PP::add(a0, val);
+#pragma unroll
+                    for (int m = 0; m < 3; m++) {
+                        ac[m] = PP::fma_s(wl[2 * m + 1], val, ac[m]);
+                        as[m] = PP::fma_s(wl[2 * m + 2], val, as[m]);
+                    }
                 }
             }
             if (y + TX_NSC < g.X1) named_bar_arrive(1 + TX_NSC + sc, TX_NCOMP);
@@ -399,13 +452,29 @@ tm_status tm_contract_xy_tma(tm_ctx* ctx, void* qbuf, const void* d_s, const voi
     A.t_first = t_first;
     const TxPlan P = tx_plan(ctx->X[0], ctx->X[1]);
     const unsigned grid = (unsigned)(ctx->X[2] * nt);
+    // folded x-stage for the extents the configurations use (any multiple of 4 would do); other extents take the
+    // plain weighted sum over the row
+    const int L = ctx->X[0];
+    const int lx = (ctx->opt_contract != 4 && (L == 32 || L == 24 || L == 16)) ? L : 0;
+    memset(A.wf, 0, sizeof(A.wf));
+    for (int j = 1; lx && j < lx / 4; j++)
+        for (int m = 1; m < 4; m++) {
+            const double th = 2.0 * M_PI * (double)((m * j) % lx) / (double)lx;      // exact argument reduction
+            A.wf[j - 1][2 * m - 2] = (float)cos(th);
+            A.wf[j - 1][2 * m - 1] = (float)sin(th);
+        }
+#define TX_LAUNCH(PR, LXV)                                                                                              \
+    do {                                                                                                                \
+        TM_CUDA(ctx, cudaFuncSetAttribute(contract_xy_tma_kernel<PR, LXV>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
+                                          P.total));                                                                    \
+        contract_xy_tma_kernel<PR, LXV><<<grid, TX_NTHREADS, P.total, st>>>(ms, me, mgf, mgb, A);                       \
+    } while (0)
     if (prune) {
-        TM_CUDA(ctx, cudaFuncSetAttribute(contract_xy_tma_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, P.total));
-        contract_xy_tma_kernel<1><<<grid, TX_NTHREADS, P.total, st>>>(ms, me, mgf, mgb, A);
+        if (lx == 32) TX_LAUNCH(1, 32); else if (lx == 24) TX_LAUNCH(1, 24); else if (lx == 16) TX_LAUNCH(1, 16); else TX_LAUNCH(1, 0);
     } else {
-        TM_CUDA(ctx, cudaFuncSetAttribute(contract_xy_tma_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, P.total));
-        contract_xy_tma_kernel<0><<<grid, TX_NTHREADS, P.total, st>>>(ms, me, mgf, mgb, A);
+        if (lx == 32) TX_LAUNCH(0, 32); else if (lx == 24) TX_LAUNCH(0, 24); else if (lx == 16) TX_LAUNCH(0, 16); else TX_LAUNCH(0, 0);
     }
+#undef TX_LAUNCH
     TM_LAUNCH_CHECK(ctx, "contract_xy_tma_kernel");
     return TM_OK;
 }
