@@ -493,15 +493,18 @@ tm_status tm_contract_internal(tm_ctx* ctx, void* d_out, const void* d_s, const 
     A.g = tm_geom(ctx);
     A.tb = (double)ctx->tb;
     A.t_first = t_first;
-    // the forward-only s family of contract_mma.cu needs timeslice t - 1 in the assembly: whole-vector launches only
-    // (measured at c4, profiles/r02_contract_paths.md: 0.98 ms against 0.93 ms for contract_tma.cu although it issues
-    // 40 % fewer FFMA2 -- both are bound by shared-memory operand traffic + fp32 pipe time, which add up -- so it is
-    // not the automatic choice)
-    const bool half0 = acc == TM_F32 && nt == ctx->X[3] && ctx->opt_contract == 3 && tm_contract_mma_usable(ctx);
+    // The forward-only s family (half0: the backward half of the s-family derivative is the shifted conjugate transpose
+    // of the forward half and is restored by contract_assemble_kernel from the same sums) needs timeslice t - 1 in the
+    // assembly: whole-vector launches only.  contract_tma.cu uses it except under TM_OPT_CONTRACT_PATH 4; contract_mma.cu
+    // always (measured at c4, profiles/r02_contract_paths.md: slower than contract_tma.cu although it issues fewer
+    // FFMA2, so it is not the automatic choice).
+    const bool whole = nt == ctx->X[3];
+    const bool mma = acc == TM_F32 && whole && ctx->opt_contract == 3 && tm_contract_mma_usable(ctx);
+    const bool tma = acc == TM_F32 && !mma && ctx->opt_contract != 1 && tm_contract_tma_usable(ctx);
+    const bool half0 = mma || (tma && whole && ctx->opt_contract != 4);
     if (acc == TM_F64) TM_TRY((launch_xy<double, 18>(ctx, A, prune, nt, st)));
-    else if (half0) TM_TRY(tm_contract_xy_mma(ctx, qbuf, d_s, d_eta, gauge, A.wx, A.wy, prune, t_first, nt, st));
-    else if (ctx->opt_contract != 1 && tm_contract_tma_usable(ctx))
-        TM_TRY(tm_contract_xy_tma(ctx, qbuf, d_s, d_eta, gauge, A.wx, A.wy, prune, t_first, nt, st));
+    else if (mma) TM_TRY(tm_contract_xy_mma(ctx, qbuf, d_s, d_eta, gauge, A.wx, A.wy, prune, t_first, nt, st));
+    else if (tma) TM_TRY(tm_contract_xy_tma(ctx, qbuf, d_s, d_eta, gauge, A.wx, A.wy, prune, half0 ? 1 : 0, t_first, nt, st));
     else TM_TRY((launch_xy<float, 12>(ctx, A, prune, nt, st)));
 
     AssembleArgs B;

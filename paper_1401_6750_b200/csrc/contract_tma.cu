@@ -124,7 +124,7 @@ struct TxShared {             // resolved shared-memory pointers of the CTA
 // producer warp: fixed derivative job (fam, mu) for every row of the plane, plus the rotating d = 0 jobs.
 // One copy of the code for all directions (the direction only selects loop-invariant shared-memory
 // offsets), so the 8 producer warps share the instruction cache.
-template <int LX>
+template <int LX, int HALF0>
 __device__ __forceinline__ void producer_rows(const TxShared& sh, const TxPlan& P, const Geom& g, int z, int t,
                                               int warp, int lane, float tb) {
     const int Xh = g.Xh;
@@ -187,53 +187,62 @@ __device__ __forceinline__ void producer_rows(const TxShared& sh, const TxPlan& 
                 }
                 lds_link(reinterpret_cast<const float4*>(stage + off_uf), Xh, 0, 0, U);
                 su3_macc<0, 0, float>(U, nb, psi);
-                const unsigned char* nbk = stage + nbb_blk + idx_b * 16;
+                // HALF0: the s family keeps only the forward half F_mu; contract_assemble_kernel restores the backward
+                // half from the same sums (it is the shifted conjugate transpose of the forward half)
+                if (!(HALF0 && fam == 0)) {
+                    const unsigned char* nbk = stage + nbb_blk + idx_b * 16;
 #pragma unroll
-                for (int k = 0; k < 6; k++) {
-                    const float4 f = *reinterpret_cast<const float4*>(nbk + k * seg);
-                    nb[2 * k] = P2<float>::make(f.x, f.y);
-                    nb[2 * k + 1] = P2<float>::make(f.z, f.w);
-                }
-                if (sgn_b != 1.f) {
+                    for (int k = 0; k < 6; k++) {
+                        const float4 f = *reinterpret_cast<const float4*>(nbk + k * seg);
+                        nb[2 * k] = P2<float>::make(f.x, f.y);
+                        nb[2 * k + 1] = P2<float>::make(f.z, f.w);
+                    }
+                    if (sgn_b != 1.f) {
 #pragma unroll
-                    for (int i = 0; i < 12; i++) nb[i] = P2<float>::mul_s(sgn_b, nb[i]);
+                        for (int i = 0; i < 12; i++) nb[i] = P2<float>::mul_s(sgn_b, nb[i]);
+                    }
+                    lds_link(reinterpret_cast<const float4*>(stage + ub_blk + idx_b * 16), Xh, 0, 0, U);
+                    su3_macc<1, 1, float>(U, nb, psi);
                 }
-                lds_link(reinterpret_cast<const float4*>(stage + ub_blk + idx_b * 16), Xh, 0, 0, U);
-                su3_macc<1, 1, float>(U, nb, psi);
                 outer_store<float>(sv, psi, rowbuf, fam * 5 + 1 + mu, col);
             }
-            {
-                // this warp's quarter of a d = 0 job: column bb = mu of C_{fam,0}[a][bb] = sum_c conj(s_ac) f_{bb,c}
-                // (splitting the two light jobs 8 ways keeps the producer warps in step)
-                const int bb = mu;
-                T2 f3[3];
-                if (fam == 0) {
+            // this warp's share of the two d = 0 jobs: column bb = mu of C_{fd,0}[a][bb] = sum_c conj(s_ac) f_{bb,c}
+            // (splitting the two light jobs keeps the producer warps in step: every warp one column of its own family,
+            // or with HALF0 the four s-family warps, which skip the backward half, one column of each family)
+            if (!HALF0 || fam == 0) {
 #pragma unroll
-                    for (int c = 0; c < 3; c++) f3[c] = bb == 0 ? sv[c] : bb == 1 ? sv[3 + c] : bb == 2 ? sv[6 + c] : sv[9 + c];
-                } else {
-                    const int k0 = (6 * bb) >> 2;
-                    const float4 f0 = *reinterpret_cast<const float4*>(stage + off_ev + k0 * seg);
-                    const float4 f1 = *reinterpret_cast<const float4*>(stage + off_ev + (k0 + 1) * seg);
-                    if (bb & 1) { f3[0] = P2<float>::make(f0.z, f0.w); f3[1] = P2<float>::make(f1.x, f1.y); f3[2] = P2<float>::make(f1.z, f1.w); }
-                    else        { f3[0] = P2<float>::make(f0.x, f0.y); f3[1] = P2<float>::make(f0.z, f0.w); f3[2] = P2<float>::make(f1.x, f1.y); }
+                for (int ff = 0; ff < (HALF0 ? 2 : 1); ff++) {
+                    const int fd = HALF0 ? ff : fam;
+                    const int bb = mu;
+                    T2 f3[3];
+                    if (fd == 0) {
+#pragma unroll
+                        for (int c = 0; c < 3; c++) f3[c] = bb == 0 ? sv[c] : bb == 1 ? sv[3 + c] : bb == 2 ? sv[6 + c] : sv[9 + c];
+                    } else {
+                        const int k0 = (6 * bb) >> 2;
+                        const float4 f0 = *reinterpret_cast<const float4*>(stage + off_ev + k0 * seg);
+                        const float4 f1 = *reinterpret_cast<const float4*>(stage + off_ev + (k0 + 1) * seg);
+                        if (bb & 1) { f3[0] = P2<float>::make(f0.z, f0.w); f3[1] = P2<float>::make(f1.x, f1.y); f3[2] = P2<float>::make(f1.z, f1.w); }
+                        else        { f3[0] = P2<float>::make(f0.x, f0.y); f3[1] = P2<float>::make(f0.z, f0.w); f3[2] = P2<float>::make(f1.x, f1.y); }
+                    }
+                    T2 acc[4];
+#pragma unroll
+                    for (int a = 0; a < 4; a++) acc[a] = P2<float>::make(0.f, 0.f);
+#pragma unroll
+                    for (int c = 0; c < 3; c++) {
+                        const T2 ip = times_i<float>(f3[c]);
+                        float sre[4], sim[4];
+#pragma unroll
+                        for (int a = 0; a < 4; a++) { P2<float>::get(sv[a * 3 + c], sre[a], sim[a]); }
+#pragma unroll
+                        for (int a = 0; a < 4; a++) acc[a] = P2<float>::fma_s(sre[a], f3[c], acc[a]);
+#pragma unroll
+                        for (int a = 0; a < 4; a++) acc[a] = P2<float>::fma_s(-sim[a], ip, acc[a]);
+                    }
+                    T2* out = rowbuf + (size_t)(fd * 5 * 16 + bb) * CT_BSC + col;
+#pragma unroll
+                    for (int a = 0; a < 4; a++) out[(size_t)(a * 4) * CT_BSC] = acc[a];
                 }
-                T2 acc[4];
-#pragma unroll
-                for (int a = 0; a < 4; a++) acc[a] = P2<float>::make(0.f, 0.f);
-#pragma unroll
-                for (int c = 0; c < 3; c++) {
-                    const T2 ip = times_i<float>(f3[c]);
-                    float sre[4], sim[4];
-#pragma unroll
-                    for (int a = 0; a < 4; a++) { P2<float>::get(sv[a * 3 + c], sre[a], sim[a]); }
-#pragma unroll
-                    for (int a = 0; a < 4; a++) acc[a] = P2<float>::fma_s(sre[a], f3[c], acc[a]);
-#pragma unroll
-                    for (int a = 0; a < 4; a++) acc[a] = P2<float>::fma_s(-sim[a], ip, acc[a]);
-                }
-                T2* out = rowbuf + (size_t)(fam * 5 * 16 + bb) * CT_BSC + col;
-#pragma unroll
-                for (int a = 0; a < 4; a++) out[(size_t)(a * 4) * CT_BSC] = acc[a];
             }
         }
         __syncwarp();
@@ -242,7 +251,7 @@ __device__ __forceinline__ void producer_rows(const TxShared& sh, const TxPlan& 
     }
 }
 
-template <int PRUNE, int LX>
+template <int PRUNE, int LX, int HALF0>
 __global__ void __launch_bounds__(TX_NTHREADS, 1)
 contract_xy_tma_kernel(const __grid_constant__ CUtensorMap tm_s, const __grid_constant__ CUtensorMap tm_e,
                        const __grid_constant__ CUtensorMap tm_gf, const __grid_constant__ CUtensorMap tm_gb,
@@ -330,7 +339,7 @@ contract_xy_tma_kernel(const __grid_constant__ CUtensorMap tm_s, const __grid_co
         }
     } else if (warp < TX_NP) {
         // ================================================================ producers
-        producer_rows<LX>(sh, P, g, z, t, warp, lane, A.tb);
+        producer_rows<LX, HALF0>(sh, P, g, z, t, warp, lane, A.tb);
     } else {
         // ================================================================ consumers
         typedef P2<float> PP;
@@ -426,7 +435,7 @@ bool tm_contract_tma_usable(const tm_ctx* ctx) {
 
 // s, eta: fp32 full-lattice internal fields; gauge: fp32 reconstruct-12 internal copy; wx, wy: float tables
 tm_status tm_contract_xy_tma(tm_ctx* ctx, void* qbuf, const void* d_s, const void* d_eta, const void* gauge,
-                             const void* wx, const void* wy, int prune, int t_first, int nt, cudaStream_t st) {
+                             const void* wx, const void* wy, int prune, int half0, int t_first, int nt, cudaStream_t st) {
     const int Xh = ctx->Xh;
     const cuuint64_t Vh = ctx->Vh;
     CUtensorMap ms, me, mgf, mgb;
@@ -465,9 +474,15 @@ tm_status tm_contract_xy_tma(tm_ctx* ctx, void* qbuf, const void* d_s, const voi
         }
 #define TX_LAUNCH(PR, LXV)                                                                                              \
     do {                                                                                                                \
-        TM_CUDA(ctx, cudaFuncSetAttribute(contract_xy_tma_kernel<PR, LXV>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
-                                          P.total));                                                                    \
-        contract_xy_tma_kernel<PR, LXV><<<grid, TX_NTHREADS, P.total, st>>>(ms, me, mgf, mgb, A);                       \
+        if (half0) {                                                                                                    \
+            TM_CUDA(ctx, cudaFuncSetAttribute(contract_xy_tma_kernel<PR, LXV, 1>,                                       \
+                                              cudaFuncAttributeMaxDynamicSharedMemorySize, P.total));                   \
+            contract_xy_tma_kernel<PR, LXV, 1><<<grid, TX_NTHREADS, P.total, st>>>(ms, me, mgf, mgb, A);                \
+        } else {                                                                                                        \
+            TM_CUDA(ctx, cudaFuncSetAttribute(contract_xy_tma_kernel<PR, LXV, 0>,                                       \
+                                              cudaFuncAttributeMaxDynamicSharedMemorySize, P.total));                   \
+            contract_xy_tma_kernel<PR, LXV, 0><<<grid, TX_NTHREADS, P.total, st>>>(ms, me, mgf, mgb, A);                \
+        }                                                                                                               \
     } while (0)
     if (prune) {
         if (lx == 32) TX_LAUNCH(1, 32); else if (lx == 24) TX_LAUNCH(1, 24); else if (lx == 16) TX_LAUNCH(1, 16); else TX_LAUNCH(1, 0);

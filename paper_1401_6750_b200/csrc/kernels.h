@@ -89,8 +89,9 @@ tm_status tm_contract_internal(tm_ctx* ctx, void* d_out, const void* d_s, const 
                                cudaStream_t st, int t_first = 0, int nt = 0 /* 0: all timeslices */);
 // contract_tma.cu: TMA-staged fast path of the site + x/y-DFT stage (fp32, Lx <= 32)
 bool tm_contract_tma_usable(const tm_ctx* ctx);
+// half0: the s-family derivative slots receive only the forward half F_mu (AssembleArgs::half0 restores the rest)
 tm_status tm_contract_xy_tma(tm_ctx* ctx, void* qbuf, const void* d_s, const void* d_eta, const void* gauge,
-                             const void* wx, const void* wy, int prune, int t_first, int nt, cudaStream_t st);
+                             const void* wx, const void* wy, int prune, int half0, int t_first, int nt, cudaStream_t st);
 // contract_mma.cu: the same with the x-stage DFT on the tensor cores (mma.sync tf32, split-fp32 operands)
 bool tm_contract_mma_usable(const tm_ctx* ctx);
 tm_status tm_contract_xy_mma(tm_ctx* ctx, void* qbuf, const void* d_s, const void* d_eta, const void* gauge,
