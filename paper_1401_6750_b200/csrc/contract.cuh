@@ -39,6 +39,13 @@ template <> struct P2<float> {
     }
     static __device__ __forceinline__ T add(T a, T b) { T d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
     static __device__ __forceinline__ T mul_s(float s, T b) { T d; const T ss = make(s, s); asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(ss), "l"(b)); return d; }
+    // c + s * (i b) = (c.re - s b.im, c.im + s b.re): two scalar FFMA on the halves of the pairs -- the same fp32-pipe
+    // time as one FFMA2, and no (-im, re) pair has to be built first (a negation and a register move per operand)
+    static __device__ __forceinline__ T fma_si(float s, T b, T c) {
+        float br, bi, cr, ci;
+        get(b, br, bi); get(c, cr, ci);
+        return make(fmaf(-s, bi, cr), fmaf(s, br, ci));
+    }
 };
 template <> struct P2<double> {
     typedef double2 T;
@@ -47,6 +54,7 @@ template <> struct P2<double> {
     static __device__ __forceinline__ T fma_s(double s, T b, T c) { return make_double2(fma(s, b.x, c.x), fma(s, b.y, c.y)); }
     static __device__ __forceinline__ T add(T a, T b) { return make_double2(a.x + b.x, a.y + b.y); }
     static __device__ __forceinline__ T mul_s(double s, T b) { return make_double2(s * b.x, s * b.y); }
+    static __device__ __forceinline__ T fma_si(double s, T b, T c) { return make_double2(fma(-s, b.y, c.x), fma(s, b.x, c.y)); }
 };
 // i * v = (-im, re)
 template <typename F> __device__ __forceinline__ typename P2<F>::T times_i(typename P2<F>::T v) {
@@ -63,9 +71,6 @@ __device__ __forceinline__ void su3_macc(const F* U, const typename P2<F>::T* in
     typedef typename P2<F>::T T;
 #pragma unroll
     for (int b = 0; b < 3; b++) {
-        T ib[4];
-#pragma unroll
-        for (int sp = 0; sp < 4; sp++) ib[sp] = times_i<F>(in[sp * 3 + b]);
         F ur[3], ui[3];
 #pragma unroll
         for (int a = 0; a < 3; a++) {
@@ -81,7 +86,7 @@ __device__ __forceinline__ void su3_macc(const F* U, const typename P2<F>::T* in
 #pragma unroll
         for (int a = 0; a < 3; a++)
 #pragma unroll
-            for (int sp = 0; sp < 4; sp++) out[sp * 3 + a] = P2<F>::fma_s(ui[a], ib[sp], out[sp * 3 + a]);
+            for (int sp = 0; sp < 4; sp++) out[sp * 3 + a] = P2<F>::fma_si(ui[a], in[sp * 3 + b], out[sp * 3 + a]);
     }
 }
 
@@ -108,11 +113,8 @@ __device__ __forceinline__ void outer_store(const typename P2<F>::T* sv, const t
 #pragma unroll
     for (int c = 0; c < 3; c++) {
         F sre[4], sim[4];
-        T ip[4];
 #pragma unroll
         for (int a = 0; a < 4; a++) { P2<F>::get(sv[a * 3 + c], sre[a], sim[a]); sim[a] = -sim[a]; }
-#pragma unroll
-        for (int bb = 0; bb < 4; bb++) ip[bb] = times_i<F>(psi[bb * 3 + c]);
         // conj(s) psi = s.re * psi - s.im * (i psi)
 #pragma unroll
         for (int a = 0; a < 4; a++)
@@ -121,7 +123,7 @@ __device__ __forceinline__ void outer_store(const typename P2<F>::T* sv, const t
 #pragma unroll
         for (int a = 0; a < 4; a++)
 #pragma unroll
-            for (int bb = 0; bb < 4; bb++) acc[a * 4 + bb] = P2<F>::fma_s(sim[a], ip[bb], acc[a * 4 + bb]);
+            for (int bb = 0; bb < 4; bb++) acc[a * 4 + bb] = P2<F>::fma_si(sim[a], psi[bb * 3 + c], acc[a * 4 + bb]);
     }
     T* out = rowbuf + (size_t)(slot * 16) * CT_BSC + lane;
 #pragma unroll

@@ -18,10 +18,9 @@
 #include "contract.cuh"
 #include "tma.cuh"
 
-#define TX_NP 8
-#define TX_NTHREADS ((TX_NP + CT_NC + 1) * 32)
-#define TX_NCOMP ((TX_NP + CT_NC) * 32)       // threads taking part in the row-buffer barriers
-#define TX_NSI 2                               // input stages
+// NP producer warps (one (fam, mu) derivative job each), then CT_NC consumer warps and the loader warp
+#define TX_NTHREADS(NP) (((NP) + CT_NC + 1) * 32)
+#define TX_NCOMP(NP) (((NP) + CT_NC) * 32)    // threads taking part in the row-buffer barriers
 #define TX_NSC 2                               // row-buffer stages
 #ifndef TX_PF
 #define TX_PF 1000                                // L2 prefetch distance in rows
@@ -40,21 +39,25 @@ struct TmaContractArgs {
 
 // shared-memory plan (bytes), every TMA destination 128-byte aligned
 struct TxPlan {
+    int nsi;               // input stages: 2, or 3 when the s family needs no backward rows (HALF0)
+    int nrow_s;            // staged spinor rows of the s family: 7, or 4 with HALF0 (centre, y+1, z+1, t+1)
     int seg;               // bytes of one segment: Xh float4
     int row;               // one spinor row block: 12 segments, padded to 128
     int gf, gb;            // forward-link block (24 segments), one backward-link block (6 segments)
-    int stage;             // one input stage: 14 rows + gf + 3 gb
+    int stage;             // one input stage: (nrow_s + 7) rows + gf + 3 gb
     int off_c, off_wx, off_wy, off_bar, total;
 };
 __host__ __device__ inline int tx_pad128(int b) { return (b + 127) & ~127; }
-__host__ __device__ inline TxPlan tx_plan(int Lx, int Ly) {
+__host__ __device__ inline TxPlan tx_plan(int Lx, int Ly, int half0) {
     TxPlan P;
+    P.nsi = half0 ? 3 : 2;
+    P.nrow_s = half0 ? 4 : 7;
     P.seg = (Lx / 2) * 16;
     P.row = tx_pad128(12 * P.seg);
     P.gf = tx_pad128(24 * P.seg);
     P.gb = tx_pad128(6 * P.seg);
-    P.stage = 14 * P.row + P.gf + 3 * P.gb;
-    P.off_c = TX_NSI * P.stage;
+    P.stage = (P.nrow_s + 7) * P.row + P.gf + 3 * P.gb;
+    P.off_c = P.nsi * P.stage;
     P.off_wx = P.off_c + TX_NSC * CT_NCC * CT_BSC * 8;
     P.off_wy = P.off_wx + 2 * 32 * 8 * 4;
     P.off_bar = tx_pad128(P.off_wy + Ly * 8 * 4);
@@ -114,7 +117,7 @@ template <int LX> __device__ __forceinline__ int fold_col(int x) {
 __device__ __forceinline__ T2 sub2(T2 a, T2 b) { T2 d; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
 
 struct TxShared {             // resolved shared-memory pointers of the CTA
-    unsigned char* in;        // [TX_NSI] input stages
+    unsigned char* in;        // [P.nsi] input stages
     T2* cbuf;                 // [TX_NSC][160][CT_BSC]
     float* swx;               // [2 row parities][32 columns][8]
     float* swy;               // [Ly][8]
@@ -134,16 +137,19 @@ __device__ __forceinline__ void producer_rows(const TxShared& sh, const TxPlan& 
     const float sgn_f = (mu == 3 && t + 1 == g.X3) ? tb : 1.f;
     const float sgn_b = (mu == 3 && t == 0) ? tb : 1.f;
     // byte offsets inside an input stage (float4 index = segment * Xh + idx)
-    const int fam_off = fam ? 7 * P.row : 0;
-    const int rf = mu == 0 ? ROW_C : mu == 1 ? ROW_YP : mu == 2 ? ROW_ZP : ROW_TP;
+    constexpr int NSI = HALF0 ? 3 : 2;
+    // rows of a stage: the s family (7 rows in the order of the enum, or with HALF0 centre, y+1, z+1, t+1), then eta (7)
+    const int fam_off = fam ? P.nrow_s * P.row : 0;
+    const int rf = mu == 0 ? ROW_C : (HALF0 && fam == 0) ? mu : mu == 1 ? ROW_YP : mu == 2 ? ROW_ZP : ROW_TP;
     const int rb = mu == 0 ? ROW_C : mu == 1 ? ROW_YM : mu == 2 ? ROW_ZM : ROW_TM;
     const int idx_up = idx + 1 == Xh ? 0 : idx + 1, idx_dn = idx == 0 ? Xh - 1 : idx - 1;
+    const int gbase = (P.nrow_s + 7) * P.row;
     const int off_sv = ((p * 6) * Xh + idx) * 16;                                   // centre s
-    const int off_ev = 7 * P.row + off_sv;                                          // centre eta
-    const int off_uf = 14 * P.row + (((p * 4 + mu) * 3) * Xh + idx) * 16;           // U_mu(x)
+    const int off_ev = P.nrow_s * P.row + off_sv;                                   // centre eta
+    const int off_uf = gbase + (((p * 4 + mu) * 3) * Xh + idx) * 16;                // U_mu(x)
     // backward link U_mu(x - mu): mu = 0 from the row's own forward block, else from the staged neighbour row
-    const int ub_blk = mu == 0 ? 14 * P.row + (((1 - p) * 4) * 3) * Xh * 16
-                               : 14 * P.row + P.gf + (mu - 1) * P.gb + ((1 - p) * 3) * Xh * 16;
+    const int ub_blk = mu == 0 ? gbase + (((1 - p) * 4) * 3) * Xh * 16
+                               : gbase + P.gf + (mu - 1) * P.gb + ((1 - p) * 3) * Xh * 16;
     const int nbf_blk = fam_off + rf * P.row + ((1 - p) * 6) * Xh * 16;
     const int nbb_blk = fam_off + rb * P.row + ((1 - p) * 6) * Xh * 16;
     const int seg = Xh * 16;
@@ -151,11 +157,11 @@ __device__ __forceinline__ void producer_rows(const TxShared& sh, const TxPlan& 
     const int col_e = LX > 0 ? fold_col<(LX > 0 ? LX : 4)>(2 * idx) : lane;
     const int col_o = LX > 0 ? fold_col<(LX > 0 ? LX : 4)>(2 * idx + 1) : lane;
     for (int y = 0; y < g.X1; y++) {
-        const int si = y % TX_NSI, sc = y % TX_NSC;
+        const int si = y % NSI, sc = y % TX_NSC;
         const unsigned char* stage = sh.in + (size_t)si * P.stage;
         T2* rowbuf = sh.cbuf + (size_t)sc * CT_NCC * CT_BSC;
-        mbar_wait(sh.bar_full + 8 * si, (y / TX_NSI) & 1);
-        if (y >= TX_NSC) named_bar_sync(1 + TX_NSC + sc, TX_NCOMP);
+        mbar_wait(sh.bar_full + 8 * si, (y / NSI) & 1);
+        if (y >= TX_NSC) named_bar_sync(1 + TX_NSC + sc, TX_NCOMP(8));
         if (active) {
             const int xo = (p ^ (y + z + t)) & 1;                 // x = 2 idx + xo
             const int col = xo ? col_o : col_e;
@@ -214,30 +220,27 @@ __device__ __forceinline__ void producer_rows(const TxShared& sh, const TxPlan& 
                 for (int ff = 0; ff < (HALF0 ? 2 : 1); ff++) {
                     const int fd = HALF0 ? ff : fam;
                     const int bb = mu;
+                    // spin component bb of the centre row of family fd, straight from the stage (complex number j sits
+                    // in half j & 1 of segment j >> 1): no run-time selection among the registers of sv
+                    const unsigned char* cb = stage + (fd ? off_ev : off_sv);
                     T2 f3[3];
-                    if (fd == 0) {
 #pragma unroll
-                        for (int c = 0; c < 3; c++) f3[c] = bb == 0 ? sv[c] : bb == 1 ? sv[3 + c] : bb == 2 ? sv[6 + c] : sv[9 + c];
-                    } else {
-                        const int k0 = (6 * bb) >> 2;
-                        const float4 f0 = *reinterpret_cast<const float4*>(stage + off_ev + k0 * seg);
-                        const float4 f1 = *reinterpret_cast<const float4*>(stage + off_ev + (k0 + 1) * seg);
-                        if (bb & 1) { f3[0] = P2<float>::make(f0.z, f0.w); f3[1] = P2<float>::make(f1.x, f1.y); f3[2] = P2<float>::make(f1.z, f1.w); }
-                        else        { f3[0] = P2<float>::make(f0.x, f0.y); f3[1] = P2<float>::make(f0.z, f0.w); f3[2] = P2<float>::make(f1.x, f1.y); }
+                    for (int c = 0; c < 3; c++) {
+                        const int j = 3 * bb + c;
+                        f3[c] = *reinterpret_cast<const T2*>(cb + (j >> 1) * seg + (j & 1) * 8);
                     }
                     T2 acc[4];
 #pragma unroll
                     for (int a = 0; a < 4; a++) acc[a] = P2<float>::make(0.f, 0.f);
 #pragma unroll
                     for (int c = 0; c < 3; c++) {
-                        const T2 ip = times_i<float>(f3[c]);
                         float sre[4], sim[4];
 #pragma unroll
                         for (int a = 0; a < 4; a++) { P2<float>::get(sv[a * 3 + c], sre[a], sim[a]); }
 #pragma unroll
                         for (int a = 0; a < 4; a++) acc[a] = P2<float>::fma_s(sre[a], f3[c], acc[a]);
 #pragma unroll
-                        for (int a = 0; a < 4; a++) acc[a] = P2<float>::fma_s(-sim[a], ip, acc[a]);
+                        for (int a = 0; a < 4; a++) acc[a] = P2<float>::fma_si(-sim[a], f3[c], acc[a]);
                     }
                     T2* out = rowbuf + (size_t)(fd * 5 * 16 + bb) * CT_BSC + col;
 #pragma unroll
@@ -247,33 +250,34 @@ __device__ __forceinline__ void producer_rows(const TxShared& sh, const TxPlan& 
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(sh.bar_empty + 8 * si);        // this warp is done reading the input stage
-        named_bar_arrive(1 + sc, TX_NCOMP);
+        named_bar_arrive(1 + sc, TX_NCOMP(8));
     }
 }
 
-template <int PRUNE, int LX, int HALF0>
-__global__ void __launch_bounds__(TX_NTHREADS, 1)
+template <int PRUNE, int LX, int HALF0, int NP>
+__global__ void __launch_bounds__(TX_NTHREADS(NP), 1)
 contract_xy_tma_kernel(const __grid_constant__ CUtensorMap tm_s, const __grid_constant__ CUtensorMap tm_e,
                        const __grid_constant__ CUtensorMap tm_gf, const __grid_constant__ CUtensorMap tm_gb,
                        TmaContractArgs A) {
     constexpr int NQ = QLayout<PRUNE>::NQ;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     const Geom& g = A.g;
-    const TxPlan P = tx_plan(g.X0, g.X1);
+    constexpr int NSI = HALF0 ? 3 : 2;
+    const TxPlan P = tx_plan(g.X0, g.X1, HALF0);
     TxShared sh;
     sh.in = smem_raw;
     sh.cbuf = reinterpret_cast<T2*>(smem_raw + P.off_c);
     sh.swx = reinterpret_cast<float*>(smem_raw + P.off_wx);
     sh.swy = reinterpret_cast<float*>(smem_raw + P.off_wy);
     sh.bar_full = smem_u32(smem_raw + P.off_bar);
-    sh.bar_empty = sh.bar_full + 8 * TX_NSI;
+    sh.bar_empty = sh.bar_full + 8 * NSI;
     const int zt = blockIdx.x + A.t_first * g.X2;
     const int z = zt % g.X2, t = zt / g.X2;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int Xh = g.Xh;
 
     // x-weight tables in column order: column l <-> x = 2 (l % Xh) + ((l / Xh) ^ row parity)
-    for (int i = threadIdx.x; i < 2 * 32 * 8; i += TX_NTHREADS) {
+    for (int i = threadIdx.x; i < 2 * 32 * 8; i += TX_NTHREADS(NP)) {
         const int rp = i >> 8, l = (i >> 3) & 31, k = i & 7;
         float w = 0.f;
         if (l < g.X0) {
@@ -282,17 +286,17 @@ contract_xy_tma_kernel(const __grid_constant__ CUtensorMap tm_s, const __grid_co
         }
         sh.swx[i] = w;
     }
-    for (int i = threadIdx.x; i < g.X1 * 8; i += TX_NTHREADS) sh.swy[i] = A.wy[i];
+    for (int i = threadIdx.x; i < g.X1 * 8; i += TX_NTHREADS(NP)) sh.swy[i] = A.wy[i];
     if (threadIdx.x == 0) {
-        for (int s = 0; s < TX_NSI; s++) {
+        for (int s = 0; s < NSI; s++) {
             mbar_init(sh.bar_full + 8 * s, 1);
-            mbar_init(sh.bar_empty + 8 * s, TX_NP);
+            mbar_init(sh.bar_empty + 8 * s, NP);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
 
-    if (warp == TX_NP + CT_NC) {
+    if (warp == NP + CT_NC) {
         // ================================================================ loader
         if (lane == 0) {
             asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_s) : "memory");
@@ -302,23 +306,27 @@ contract_xy_tma_kernel(const __grid_constant__ CUtensorMap tm_s, const __grid_co
             const unsigned in0 = smem_u32(sh.in);
             const int zp = z + 1 == g.X2 ? 0 : z + 1, zm = z == 0 ? g.X2 - 1 : z - 1;
             const int tp = t + 1 == g.X3 ? 0 : t + 1, tm = t == 0 ? g.X3 - 1 : t - 1;
-            const unsigned bytes = (unsigned)(14 * 12 + 24 + 18) * (unsigned)P.seg;
+            const unsigned bytes = (unsigned)((P.nrow_s + 7) * 12 + 24 + 18) * (unsigned)P.seg;
             for (int y = 0; y < g.X1; y++) {
-                const int si = y % TX_NSI;
+                const int si = y % NSI;
                 const unsigned full = sh.bar_full + 8 * si;
-                if (y >= TX_NSI) mbar_wait(sh.bar_empty + 8 * si, ((y / TX_NSI) - 1) & 1);
+                if (y >= NSI) mbar_wait(sh.bar_empty + 8 * si, ((y / NSI) - 1) & 1);
                 mbar_expect_tx(full, bytes);
                 const int yp = y + 1 == g.X1 ? 0 : y + 1, ym = y == 0 ? g.X1 - 1 : y - 1;
                 // float coordinate of the first site of row (yy, zz, tt) inside a parity block: 4 * (lex / 2)
                 auto c0 = [&](int yy, int zz, int tt) { return 2 * (((tt * g.X2 + zz) * g.X1 + yy) * g.X0); };
                 const int rc[7] = {c0(y, z, t), c0(yp, z, t), c0(ym, z, t), c0(y, zp, t), c0(y, zm, t), c0(y, z, tp), c0(y, z, tm)};
                 const unsigned st0 = in0 + (unsigned)si * (unsigned)P.stage;
+                if (HALF0) {        // s family: centre and forward rows only
 #pragma unroll
-                for (int r = 0; r < 7; r++) {
-                    tma_load_2d(st0 + (unsigned)(r * P.row), &tm_s, full, rc[r], 0);
-                    tma_load_2d(st0 + (unsigned)((7 + r) * P.row), &tm_e, full, rc[r], 0);
+                    for (int r = 0; r < 4; r++) tma_load_2d(st0 + (unsigned)(r * P.row), &tm_s, full, rc[r == 0 ? 0 : 2 * r - 1], 0);
+                } else {
+#pragma unroll
+                    for (int r = 0; r < 7; r++) tma_load_2d(st0 + (unsigned)(r * P.row), &tm_s, full, rc[r], 0);
                 }
-                const unsigned gbase = st0 + (unsigned)(14 * P.row);
+#pragma unroll
+                for (int r = 0; r < 7; r++) tma_load_2d(st0 + (unsigned)((P.nrow_s + r) * P.row), &tm_e, full, rc[r], 0);
+                const unsigned gbase = st0 + (unsigned)((P.nrow_s + 7) * P.row);
                 tma_load_4d(gbase, &tm_gf, full, rc[0], 0, 0, 0);
                 tma_load_4d(gbase + (unsigned)P.gf, &tm_gb, full, rc[2], 0, 1, 0);
                 tma_load_4d(gbase + (unsigned)(P.gf + P.gb), &tm_gb, full, rc[4], 0, 2, 0);
@@ -337,13 +345,13 @@ contract_xy_tma_kernel(const __grid_constant__ CUtensorMap tm_s, const __grid_co
                 }
             }
         }
-    } else if (warp < TX_NP) {
+    } else if (warp < NP) {
         // ================================================================ producers
         producer_rows<LX, HALF0>(sh, P, g, z, t, warp, lane, A.tb);
     } else {
         // ================================================================ consumers
         typedef P2<float> PP;
-        const int cc = threadIdx.x - TX_NP * 32;        // 0..159
+        const int cc = threadIdx.x - NP * 32;           // 0..159
         T2 Q[NQ];
 #pragma unroll
         for (int q = 0; q < NQ; q++) Q[q] = PP::make(0.f, 0.f);
@@ -354,7 +362,7 @@ contract_xy_tma_kernel(const __grid_constant__ CUtensorMap tm_s, const __grid_co
             T2 a0 = PP::make(0.f, 0.f), ac[3], as[3];
 #pragma unroll
             for (int m = 0; m < 3; m++) { ac[m] = PP::make(0.f, 0.f); as[m] = PP::make(0.f, 0.f); }
-            named_bar_sync(1 + sc, TX_NCOMP);
+            named_bar_sync(1 + sc, TX_NCOMP(NP));
             if (LX > 0) {
                 // folded x-stage: see fold_col
                 const ulonglong2* v4 = reinterpret_cast<const ulonglong2*>(v);
@@ -395,7 +403,7 @@ contract_xy_tma_kernel(const __grid_constant__ CUtensorMap tm_s, const __grid_co
                     }
                 }
             }
-            if (y + TX_NSC < g.X1) named_bar_arrive(1 + TX_NSC + sc, TX_NCOMP);
+            if (y + TX_NSC < g.X1) named_bar_arrive(1 + TX_NSC + sc, TX_NCOMP(NP));
             const float* wl = sh.swy + y * 8;
             float cy[4], sy[4];
             cy[0] = 1.f; sy[0] = 0.f;
@@ -428,8 +436,8 @@ contract_xy_tma_kernel(const __grid_constant__ CUtensorMap tm_s, const __grid_co
 bool tm_contract_tma_usable(const tm_ctx* ctx) {
     if (ctx->X[0] > 32) return false;
     if (4 * ctx->Vh >= (size_t)1 << 31) return false;             // TMA coordinates are int32
-    const TxPlan P = tx_plan(ctx->X[0], ctx->X[1]);
-    if (P.total > 227 * 1024) return false;
+    const TxPlan P = tx_plan(ctx->X[0], ctx->X[1], 0);       // the larger of the two plans
+    if (P.total > 227 * 1024 || tx_plan(ctx->X[0], ctx->X[1], 1).total > 227 * 1024) return false;
     return get_encode_fn() != nullptr;
 }
 
@@ -459,7 +467,7 @@ tm_status tm_contract_xy_tma(tm_ctx* ctx, void* qbuf, const void* d_s, const voi
     A.g = tm_geom(ctx);
     A.tb = (float)ctx->tb;
     A.t_first = t_first;
-    const TxPlan P = tx_plan(ctx->X[0], ctx->X[1]);
+    const TxPlan P = tx_plan(ctx->X[0], ctx->X[1], half0);
     const unsigned grid = (unsigned)(ctx->X[2] * nt);
     // folded x-stage for the extents the configurations use (any multiple of 4 would do); other extents take the
     // plain weighted sum over the row
@@ -472,17 +480,16 @@ tm_status tm_contract_xy_tma(tm_ctx* ctx, void* qbuf, const void* d_s, const voi
             A.wf[j - 1][2 * m - 2] = (float)cos(th);
             A.wf[j - 1][2 * m - 1] = (float)sin(th);
         }
+#define TX_LAUNCH1(PR, LXV, H0, NPV)                                                                                    \
+    do {                                                                                                                \
+        TM_CUDA(ctx, cudaFuncSetAttribute(contract_xy_tma_kernel<PR, LXV, H0, NPV>,                                     \
+                                          cudaFuncAttributeMaxDynamicSharedMemorySize, P.total));                       \
+        contract_xy_tma_kernel<PR, LXV, H0, NPV><<<grid, TX_NTHREADS(NPV), P.total, st>>>(ms, me, mgf, mgb, A);         \
+    } while (0)
 #define TX_LAUNCH(PR, LXV)                                                                                              \
     do {                                                                                                                \
-        if (half0) {                                                                                                    \
-            TM_CUDA(ctx, cudaFuncSetAttribute(contract_xy_tma_kernel<PR, LXV, 1>,                                       \
-                                              cudaFuncAttributeMaxDynamicSharedMemorySize, P.total));                   \
-            contract_xy_tma_kernel<PR, LXV, 1><<<grid, TX_NTHREADS, P.total, st>>>(ms, me, mgf, mgb, A);                \
-        } else {                                                                                                        \
-            TM_CUDA(ctx, cudaFuncSetAttribute(contract_xy_tma_kernel<PR, LXV, 0>,                                       \
-                                              cudaFuncAttributeMaxDynamicSharedMemorySize, P.total));                   \
-            contract_xy_tma_kernel<PR, LXV, 0><<<grid, TX_NTHREADS, P.total, st>>>(ms, me, mgf, mgb, A);                \
-        }                                                                                                               \
+        if (half0) TX_LAUNCH1(PR, LXV, 1, 8);                                                                           \
+        else TX_LAUNCH1(PR, LXV, 0, 8);                                                                                 \
     } while (0)
     if (prune) {
         if (lx == 32) TX_LAUNCH(1, 32); else if (lx == 24) TX_LAUNCH(1, 24); else if (lx == 16) TX_LAUNCH(1, 16); else TX_LAUNCH(1, 0);
@@ -490,6 +497,7 @@ tm_status tm_contract_xy_tma(tm_ctx* ctx, void* qbuf, const void* d_s, const voi
         if (lx == 32) TX_LAUNCH(0, 32); else if (lx == 24) TX_LAUNCH(0, 24); else if (lx == 16) TX_LAUNCH(0, 16); else TX_LAUNCH(0, 0);
     }
 #undef TX_LAUNCH
+#undef TX_LAUNCH1
     TM_LAUNCH_CHECK(ctx, "contract_xy_tma_kernel");
     return TM_OK;
 }
