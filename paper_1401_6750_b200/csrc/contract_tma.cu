@@ -128,9 +128,11 @@ struct TxShared {             // resolved shared-memory pointers of the CTA
 // One copy of the code for all directions (the direction only selects loop-invariant shared-memory
 // offsets), so the 8 producer warps share the instruction cache.
 template <int LX, int HALF0>
-__device__ __forceinline__ void producer_rows(const TxShared& sh, const TxPlan& P, const Geom& g, int z, int t,
+__device__ __forceinline__ void producer_rows(const TxShared& sh, const TxPlan& Prt, const Geom& g, int z, int t,
                                               int warp, int lane, float tb) {
-    const int Xh = g.Xh;
+    // with a compile-time row length every stage offset below is an immediate of its LDS (no address arithmetic)
+    const int Xh = LX > 0 ? LX / 2 : g.Xh;
+    const TxPlan P = LX > 0 ? tx_plan(LX, 2, HALF0) : Prt;        // the fields used here depend on Lx and HALF0 only
     const int fam = warp >> 2, mu = warp & 3;
     const int p = lane / Xh, idx = lane - p * Xh;
     const bool active = lane < g.X0;
@@ -310,7 +312,7 @@ contract_xy_tma_kernel(const __grid_constant__ CUtensorMap tm_s, const __grid_co
             for (int y = 0; y < g.X1; y++) {
                 const int si = y % NSI;
                 const unsigned full = sh.bar_full + 8 * si;
-                if (y >= NSI) mbar_wait(sh.bar_empty + 8 * si, ((y / NSI) - 1) & 1);
+                if (y >= NSI) mbar_wait_relaxed(sh.bar_empty + 8 * si, ((y / NSI) - 1) & 1);
                 mbar_expect_tx(full, bytes);
                 const int yp = y + 1 == g.X1 ? 0 : y + 1, ym = y == 0 ? g.X1 - 1 : y - 1;
                 // float coordinate of the first site of row (yy, zz, tt) inside a parity block: 4 * (lex / 2)
