@@ -238,8 +238,12 @@ __global__ void __launch_bounds__(CT_THREADS) contract_zsum_kernel(AssembleArgs 
 __global__ void __launch_bounds__(CT_THREADS) contract_assemble_kernel(AssembleArgs A) {
     __shared__ double zre[CT_THREADS], zim[CT_THREADS];
     __shared__ double zre_tm[32], zim_tm[32];               // half0: the t-derivative slot of the s family at t - 1
+    // every thread reads its own row of the Gamma table: from __constant__ memory that serialises in the constant
+    // cache (16 distinct addresses per warp and access), so the table is staged in shared memory once per CTA
+    __shared__ GammaTable sg;
     const int k = blockIdx.x, t = blockIdx.y + A.t_first;
     const int jr = threadIdx.x;
+    if (jr < (int)(sizeof(GammaTable) / 4)) reinterpret_cast<int*>(&sg)[jr] = reinterpret_cast<const int*>(&c_gamma)[jr];
     const int px = A.mom[3 * k], py = A.mom[3 * k + 1], pz = A.mom[3 * k + 2];
     const int m = abs(px), n = abs(py), l = abs(pz);
     const double sx = px < 0 ? -1.0 : 1.0, sy = py < 0 ? -1.0 : 1.0, sz = pz < 0 ? -1.0 : 1.0;
@@ -281,8 +285,8 @@ __global__ void __launch_bounds__(CT_THREADS) contract_assemble_kernel(AssembleA
         double l0r = 0, l0i = 0, l1r = 0, l1i = 0;
 #pragma unroll
         for (int a = 0; a < 4; a++) {
-            const int bcol = c_gamma.perm[nG][a];
-            const double pr = c_gamma.phre[nG][a], pi = c_gamma.phim[nG][a];
+            const int bcol = sg.perm[nG][a];
+            const double pr = sg.phre[nG][a], pi = sg.phim[nG][a];
             {   // s family: raw complex value = (Z[re comp]) + i (Z[im comp]) with each Z complex
                 const int j = (d * 32) + (a * 4 + bcol) * 2;
                 double rr = zre[j] - zim[j + 1], ri = zim[j] + zre[j + 1];
