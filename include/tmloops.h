@@ -68,12 +68,13 @@ const char* tm_last_error(const tm_ctx* ctx);
  *                         fit the device memory), or 1 | 2 | 4 | 8
  *   TM_OPT_CONTRACT_PATH  site + x/y-DFT stage of the contraction: 0 = automatic (fastest usable), 1 = generic kernel
  *                         (read-only-cache loads; any Lx, fp64), 2 = TMA-staged fp32 kernel with the DFT on the fp32 pipe
- *                         (x-stage folded over the sites {x, L-x, L/2-x, L/2+x} where Lx is 16, 24 or 32),
- *                         3 = TMA-staged fp32 kernel with the x-stage of the DFT on the tensor cores (tf32 MMAs on
- *                         split-fp32 operands, hi*hi + lo*hi + hi*lo: same 1e-5 bound) and a forward-only s-family
- *                         derivative (whole-vector calls; never the automatic choice: measured slower than 2);
- *                         4 = kernel 2 with the plain (unfolded) weighted sum over x; 2, 3 and 4 need Lx <= 32 and fall
- *                         back to 1 otherwise
+ *                         (x-stage folded over the sites {x, L-x, L/2-x, L/2+x} where Lx is 16, 24 or 32; whole-vector
+ *                         calls keep only the forward half of the s-family derivative and restore the rest in the
+ *                         assembly), 3 = TMA-staged fp32 kernel with the x-stage of the DFT on the tensor cores (tf32
+ *                         MMAs on split-fp32 operands, hi*hi + lo*hi + hi*lo: same 1e-5 bound; whole-vector calls; never
+ *                         the automatic choice: measured slower than 2), 4 = kernel 2 without the fold and with both
+ *                         halves of every derivative (the plain form; what single-timeslice calls of 2 also use for the
+ *                         derivative); 2, 3 and 4 need Lx <= 32 and fall back to 1 otherwise
  *   TM_OPT_POISON         debugging aid (compute-sanitizer's initcheck is not available everywhere): 1 = every workspace
  *                         the context allocates from now on starts as 0xFF bytes, i.e. NaN in all four storage
  *                         precisions, so that a read of never-written workspace memory reaches the results

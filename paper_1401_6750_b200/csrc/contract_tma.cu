@@ -1,20 +1,35 @@
 // contract_tma.cu -- TMA-staged fast path of the fused contraction + projection kernel (fp32, Lx <= 32).
 //
 // Same mathematics and the same output (qbuf) as contract_xy_kernel in contract.cu (SURVEY.md sec 8
-// rows a6-a8); what changes is how operands reach the SM.  One CTA per (z,t)
-// plane, 14 warps:
-//   warp 13      loader: one thread issues, per y-row, 18 TMA tensor copies (cp.async.bulk.tensor) that
-//                land the 7 rows of s and eta the row needs (centre, y+-1, z+-1, t+-1), the row's 4
+// rows a6-a8); what changes is how operands reach the SM and how much arithmetic is
+// left per site.  One CTA per (z,t) plane, 14 warps:
+//   warp 13      loader: one thread issues, per y-row, the TMA tensor copies (cp.async.bulk.tensor) that
+//                land the rows of s and eta the row needs (centre, y+-1, z+-1, t+-1), the row's 4
 //                forward links and the 3 backward links of the y-1, z-1, t-1 rows in shared memory,
-//                completion signalled on an mbarrier (2-stage ring)
-//   warps 0..7   producers, one fixed (fam, mu) derivative job each (+ the rotating d = 0 jobs): operands
-//                come from shared memory with compile-time offsets (no global address arithmetic, no
-//                long-scoreboard stalls), FFMA2 complex arithmetic, 16 complex outer-product values per
-//                site -> row buffer
+//                completion signalled on an mbarrier (ring of 2 stages, or 3 with HALF0)
+//   warps 0..7   producers, one fixed (fam, mu) derivative job each (+ a share of the d = 0 jobs): operands
+//                come from shared memory at compile-time offsets (no global address arithmetic, no
+//                long-scoreboard stalls), 16 complex outer-product values per site -> row buffer
 //   warps 8..12  consumers: thread = complex component; x-sum with 7 real weights, y-stage accumulators
 // Lane l of a producer handles the site of parity p = l / Xh with in-row half index idx = l % Xh
 // (x = 2 idx + (p ^ row parity)), so that every shared-memory operand read is a contiguous run of
-// 16-byte vectors; the consumers use the correspondingly permuted x-weight table.
+// 16-byte vectors.
+//
+// The kernel is bound by instruction issue (ncu: no pipe above 55 %, issue slots the scarce resource; an FFMA2
+// costs one slot but two fp32-pipe cycles), so round 2 removed instructions (profiles/r02_contract_f32.md):
+//   * LX > 0 (Lx = 16, 24, 32): folded x-stage -- the consumers combine the four sites {x, L-x, L/2-x, L/2+x}, on which
+//     every cos / sin weight has the same absolute value, before weighting (15 packed operations per 4 sites instead
+//     of 28); the weights are kernel parameters (constant bank -> uniform-register operands of FFMA2, no
+//     shared-memory weight table); the producers store site x at the folded column fold_col(x);
+//   * HALF0 (whole-vector launches): the s-family derivative slots receive only the forward half
+//     F_mu = s^dag (x) U_mu(x) s(x + mu); the backward half is its shifted conjugate transpose and is restored by
+//     contract_assemble_kernel from the same sums.  The s-family warps then do the d = 0 columns of both families, the
+//     three backward rows of s are not staged (3 input stages fit), -14 % fp32 work;
+//   * complex multiplies as one FFMA2 (real coefficient, broadcast scalar) + two scalar FFMA (imaginary coefficient):
+//     no (-im, re) operand pair has to be built (P2::fma_si);
+//   * d = 0 columns read straight from the stage instead of selected among registers at run time.
+// TM_OPT_CONTRACT_PATH 4 launches the kernel without the first two (LX = 0, HALF0 = 0): the reference the tests
+// compare with, and the only form a single-timeslice launch can take for HALF0 (it needs timeslice t - 1).
 #include "contract.cuh"
 #include "tma.cuh"
 
