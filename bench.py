@@ -480,6 +480,24 @@ def run_b200(args, cfg):
     ms_per_step = float(ms.item()) / args.steps
     value = n_lp_job / (ms_per_step * 1e-3)
 
+    # Where the step goes.  On one lane (the automatic choice when sources are solved 8 per launch) the phases of a step
+    # follow one another on one stream and their event times add up to the step, so the breakdown comes from the timed
+    # steps themselves; a run that used two lanes (overlapping phase times) gets one more, untimed, step on one lane.
+    breakdown = None
+    if not args.step_only:
+        if all(i["lanes"] == 1 for i in infos):
+            binfo = {k: float(np.mean([i[k] for i in infos])) for k in ("ms_total", "ms_lp_solve", "ms_hp_solve", "ms_contract")}
+            src = "mean over the timed steps (one lane)"
+        else:
+            ctx.tm_set_option(tmod.TM_OPT_LANES, 1)
+            _, binfo = step()
+            torch.cuda.synchronize()
+            ctx.tm_set_option(tmod.TM_OPT_LANES, 0)
+            src = "one more, untimed, step on one lane (the timed steps ran two lanes, whose phase times overlap)"
+        breakdown = {"lanes": 1, "ms_step": binfo["ms_total"], "ms_lp_solves": binfo["ms_lp_solve"],
+                     "ms_hp_solves": binfo["ms_hp_solve"], "ms_contraction_noise_accumulate": binfo["ms_contract"],
+                     "source": src}
+
     if args.step_only:
         # the launch-list capture under profiles/ wraps this mode: warm-up + timed steps, nothing else
         if rank == 0:
@@ -610,6 +628,8 @@ def run_b200(args, cfg):
         "ms_lp_solve": float(np.mean([i["ms_lp_solve"] for i in infos])),
         "ms_hp_solve": float(np.mean([i["ms_hp_solve"] for i in infos])),
         "ms_contract_and_rest": float(np.mean([i["ms_contract"] for i in infos])),
+        "lanes": int(infos[0]["lanes"]),
+        "one_lane_breakdown": breakdown,
         "worst_resid_lp": max(i["worst_resid_lp"] for i in infos),
         "worst_resid_hp": max(i["worst_resid_hp"] for i in infos),
         "fp32_fma_peak_tflops": {"ffma": ctx.tm_fma_peak(0, 8192), "ffma2": ctx.tm_fma_peak(1, 8192)},

@@ -78,8 +78,13 @@ const char* tm_last_error(const tm_ctx* ctx);
  *   TM_OPT_POISON         debugging aid (compute-sanitizer's initcheck is not available everywhere): 1 = every workspace
  *                         the context allocates from now on starts as 0xFF bytes, i.e. NaN in all four storage
  *                         precisions, so that a read of never-written workspace memory reaches the results
+ *   TM_OPT_LANES          jobs in flight in tsm_estimate*, each on a lane of its own (stream + workspaces): 0 = automatic
+ *                         (one when the sources are solved 8 per launch -- such kernels fill the GPU --, else two), 1, 2.
+ *                         On one lane the solve / contraction phases follow one another on one stream and the phase
+ *                         times of tsm_info add up to the total; estimates of one and two lanes differ only by the order
+ *                         of the fp64 accumulation
  * TM_EARG for an unknown option or value. */
-typedef enum { TM_OPT_GROUP = 0, TM_OPT_CONTRACT_PATH = 1, TM_OPT_POISON = 2 } tm_option;
+typedef enum { TM_OPT_GROUP = 0, TM_OPT_CONTRACT_PATH = 1, TM_OPT_POISON = 2, TM_OPT_LANES = 3 } tm_option;
 tm_status tm_set_option(tm_ctx* ctx, tm_option opt, int value);
 
 /* d_U: device, canonical complex128 [V][4][3][3].  Copied into the context (fp64 master) asynchronously on stream;
@@ -187,7 +192,9 @@ typedef struct { int n_lp, n_hp; tm_solve_params lp, hp; double kappa, mu;
                  const unsigned char* d_z4; unsigned long long seed;
                  int src_first, src_stride; void* d_solutions; } tsm_params;
 typedef struct { double ms_total, ms_lp_solve, ms_hp_solve, ms_contract; long iters_lp, iters_hp;
-                 double worst_resid_lp, worst_resid_hp; int launches; } tsm_info;
+                 double worst_resid_lp, worst_resid_hp; int launches; int lanes; } tsm_info;
+/* tsm_info: ms_* are device times (CUDA events); with lanes = 1 the three phase times add up to ms_total, with two lanes
+ * the solve times of the lanes overlap and their sums are halved; lanes = jobs that were in flight (TM_OPT_LANES). */
 /* d_out: device complex128 [2][80][nmom][T]; d_per_source: optional (NULL ok) device complex128
  * [n_lp + n_hp][2][80][nmom][T] receiving every per-source array (LP first, then HP).
  * TM_ENOCONV if any solve missed its rho (outputs still filled). */

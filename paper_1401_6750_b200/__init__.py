@@ -25,7 +25,7 @@ TM_OK, TM_EARG, TM_EDIM, TM_EPREC, TM_ECUDA, TM_ENOCONV, TM_EALLOC = range(7)
 TM_F64, TM_F32, TM_F16, TM_BF16 = range(4)
 TM_R18, TM_R12 = 18, 12
 TM_OP_HOP, TM_OP_HOP_TWINV, TM_OP_XPAY, TM_OP_M_FULL, TM_OP_MHAT = range(5)
-TM_OPT_GROUP, TM_OPT_CONTRACT_PATH, TM_OPT_POISON = range(3)
+TM_OPT_GROUP, TM_OPT_CONTRACT_PATH, TM_OPT_POISON, TM_OPT_LANES = range(4)
 PREC = {"f64": TM_F64, "f32": TM_F32, "f16": TM_F16, "bf16": TM_BF16}
 PREC_BYTES = {TM_F64: 8, TM_F32: 4, TM_F16: 2, TM_BF16: 2}
 
@@ -73,7 +73,7 @@ class tsm_info(ctypes.Structure):
                 ("ms_hp_solve", ctypes.c_double), ("ms_contract", ctypes.c_double),
                 ("iters_lp", ctypes.c_long), ("iters_hp", ctypes.c_long),
                 ("worst_resid_lp", ctypes.c_double), ("worst_resid_hp", ctypes.c_double),
-                ("launches", ctypes.c_int)]
+                ("launches", ctypes.c_int), ("lanes", ctypes.c_int)]
 
 
 _lib = None
@@ -206,7 +206,7 @@ class TmContext:
         return int(self.lib.tm_launch_count(self.h))
 
     def tm_set_option(self, opt: int, value: int):
-        """TM_OPT_GROUP (0 = automatic | 1 | 2 | 4 | 8), TM_OPT_CONTRACT_PATH (0 = automatic | 1 | 2 | 3) or TM_OPT_POISON (0 | 1); see tmloops.h."""
+        """TM_OPT_GROUP (0 = automatic | 1 | 2 | 4 | 8), TM_OPT_CONTRACT_PATH (0 = automatic | 1 .. 4), TM_OPT_POISON (0 | 1) or TM_OPT_LANES (0 = automatic | 1 | 2); see tmloops.h."""
         self._check(self.lib.tm_set_option(self.h, int(opt), int(value)))
 
     def tm_fma_peak(self, mode: int = 1, iters: int = 4096) -> float:
@@ -376,7 +376,7 @@ class TmContext:
     @staticmethod
     def _tsm_info(info, st):
         return dict(ms_total=info.ms_total, ms_lp_solve=info.ms_lp_solve, ms_hp_solve=info.ms_hp_solve,
-                    ms_contract=info.ms_contract, iters_lp=info.iters_lp, iters_hp=info.iters_hp,
+                    ms_contract=info.ms_contract, iters_lp=info.iters_lp, iters_hp=info.iters_hp, lanes=info.lanes,
                     worst_resid_lp=info.worst_resid_lp, worst_resid_hp=info.worst_resid_hp,
                     launches=info.launches, status=st)
 

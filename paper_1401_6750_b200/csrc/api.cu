@@ -106,6 +106,10 @@ extern "C" tm_status tm_set_option(tm_ctx* c, tm_option opt, int value) {
             if (value < 0 || value > 4) return tm_fail(c, TM_EARG, "tm_set_option: TM_OPT_CONTRACT_PATH must be 0..4");
             c->opt_contract = value;
             return TM_OK;
+        case TM_OPT_LANES:
+            if (value < 0 || value > TM_NLANES) return tm_fail(c, TM_EARG, "tm_set_option: TM_OPT_LANES must be 0 (automatic), 1 or 2");
+            c->opt_lanes = value;
+            return TM_OK;
         case TM_OPT_POISON:
             if (value != 0 && value != 1) return tm_fail(c, TM_EARG, "tm_set_option: TM_OPT_POISON must be 0 or 1");
             c->opt_poison = value;

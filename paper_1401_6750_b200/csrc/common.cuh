@@ -88,6 +88,7 @@ struct tm_ctx {
     TmLane lanes[TM_NLANES];        // parked state of the inactive lanes (the active one lives in the fields above)
     cudaStream_t lane_stream;       // stream owned by the active lane (0 for lane 0)
     int opt_group;                  // TM_OPT_GROUP: 0 = automatic | 1 | 2 | 4 | 8 sources per solve
+    int opt_lanes;                  // TM_OPT_LANES: 0 = automatic | 1 | 2 jobs in flight
     int opt_poison;                 // TM_OPT_POISON: fill newly allocated workspaces with 0xFF bytes (NaN)
     int opt_contract;               // TM_OPT_CONTRACT_PATH: 0 = automatic | 1 generic | 2 TMA + fp32-pipe DFT | 3 TMA + tensor-core DFT (contract_mma.cu)
 };

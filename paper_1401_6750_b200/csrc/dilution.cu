@@ -173,6 +173,7 @@ extern "C" tm_status tsm_estimate_time_diluted(tm_ctx* ctx, void* d_out, void* d
         info->iters_lp = it_lp; info->iters_hp = it_hp;
         info->worst_resid_lp = worst_lp; info->worst_resid_hp = worst_hp;
         info->launches = (int)(ctx->launches - launches0);
+        info->lanes = 1;
     }
     if (noconv) {
         snprintf(ctx->err, sizeof(ctx->err), "tsm_estimate_time_diluted: %d solve(s) missed their rho (worst LP %g, HP %g)",

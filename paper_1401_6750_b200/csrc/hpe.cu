@@ -321,6 +321,7 @@ extern "C" tm_status tsm_estimate_hpe(tm_ctx* ctx, void* d_out, void* d_per_sour
         info->iters_lp = it_lp; info->iters_hp = it_hp;
         info->worst_resid_lp = worst_lp; info->worst_resid_hp = worst_hp;
         info->launches = (int)(ctx->launches - launches0);
+        info->lanes = 1;
     }
     if (noconv) {
         snprintf(ctx->err, sizeof(ctx->err), "tsm_estimate_hpe: %d solve(s) missed their rho (worst LP %g, HP %g)",

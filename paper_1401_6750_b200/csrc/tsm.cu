@@ -361,7 +361,11 @@ static tm_status tsm_core(tm_ctx* ctx, void* d_out, void* d_per_source, const ts
         while (2 * R.group <= gsz && 2 * R.group <= TM_MAXNB) R.group *= 2;
     }
     // the binary-storage files are shared accumulators: one lane keeps their additions ordered
-    const int NL = (d_files_lp || d_files_corr || P->n_lp + P->n_hp < 2) ? 1 : TM_NLANES;
+    // TM_OPT_LANES, else automatic: kernels that cover 8 sources fill the GPU by themselves, a second job in flight then
+    // only adds cache pressure (measured at c4, three A/B pairs on one box: 2089-2129 ms per step on one lane against
+    // 2104-2131 ms on two); smaller groups (memory-bound choice, ragged runs) keep two lanes to cover launch gaps
+    int NL = ctx->opt_lanes ? ctx->opt_lanes : (R.group >= 8 ? 1 : TM_NLANES);
+    if (d_files_lp || d_files_corr || P->n_lp + P->n_hp < 2) NL = 1;
     if (d_files_lp) TM_CUDA(ctx, cudaMemsetAsync(d_files_lp, 0, (size_t)loop_binary_nfiles(P->n_lp) * R.nr * sizeof(double), st));
     if (d_files_corr && P->n_hp) {
         TM_CUDA(ctx, cudaMemsetAsync(d_files_corr, 0, (size_t)loop_binary_nfiles(P->n_hp) * R.nr * sizeof(double), st));
@@ -422,6 +426,7 @@ static tm_status tsm_core(tm_ctx* ctx, void* d_out, void* d_per_source, const ts
         info->iters_lp = R.it_lp; info->iters_hp = R.it_hp;
         info->worst_resid_lp = R.worst_lp; info->worst_resid_hp = R.worst_hp;
         info->launches = (int)(ctx->launches - launches0);
+        info->lanes = NL;
     }
     if (R.noconv) {
         snprintf(ctx->err, sizeof(ctx->err), "tsm_estimate: %d solve(s) missed their rho (worst LP %g, HP %g)",

@@ -93,7 +93,7 @@ def test_contract_c4_sampled_timeslices(orc, c4, acc, tol):
 
 
 def test_tsm_c4_grouped_launches(orc, c4):
-    """The launch configuration bench.py times: sources solved 8 per launch on two lanes.  Per-source arrays must be
+    """The launch configuration bench.py times: sources solved 8 per launch (one lane).  Per-source arrays must be
     bit-identical to the one-source-per-launch path, and a grouped solution must pass the oracle's residual check."""
     t, ctx, U_h, eta = c4
     mom = inputs.momentum_list(9)

@@ -133,6 +133,7 @@ def test_grouped_two_lane_runs_repeat_bit_identically():
     mom = inputs.momentum_list(2)
     with t.TmContext(dims, -1) as ctx:
         ctx.tm_load_gauge(U)
+        ctx.tm_set_option(t.TM_OPT_LANES, 2)        # automatic would run groups of 8 on one lane
         first = None
         for rep in range(20):
             out, ps, _ = ctx.tsm_estimate(19, 11, C1["kappa"], C1["mu"], mom, LP, HP, t.TM_F32, t.TM_F64, seed=9, per_source=True)

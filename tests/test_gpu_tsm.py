@@ -128,6 +128,34 @@ def test_tsm_grouped_solves_equal_single_source_solves(setup):
             assert rel_l2(to_np(out_p), to_np(out_s)) <= 1e-13        # lanes sum the sources in another order
 
 
+def test_tsm_one_lane_equals_two_lanes(setup):
+    """TM_OPT_LANES: one job in flight and two give the same per-source arrays bit for bit and the same estimate up to
+    the order of the fp64 accumulation; on one lane the phase times add up to the total; automatic = one lane when the
+    sources are solved 8 per launch, two for smaller groups."""
+    t = tm()
+    dims, U, mom = setup
+    k, mu = C1["kappa"], C1["mu"]
+    with t.TmContext(dims, -1) as ctx:
+        ctx.tm_load_gauge(U)
+        with pytest.raises(t.TmError):
+            ctx.tm_set_option(t.TM_OPT_LANES, 3)
+        ctx.tm_set_option(t.TM_OPT_LANES, 2)
+        out2, ps2, info2 = ctx.tsm_estimate(19, 5, k, mu, mom, LP, HP, t.TM_F32, t.TM_F64, seed=3, per_source=True)
+        ctx.tm_set_option(t.TM_OPT_LANES, 1)
+        out1, ps1, info1 = ctx.tsm_estimate(19, 5, k, mu, mom, LP, HP, t.TM_F32, t.TM_F64, seed=3, per_source=True)
+        ctx.tm_set_option(t.TM_OPT_LANES, 0)
+        assert info2["lanes"] == 2 and info1["lanes"] == 1
+        assert ctx.tsm_estimate(9, 2, k, mu, mom, LP, HP, t.TM_F32, t.TM_F64, seed=3)[2]["lanes"] == 1
+        ctx.tm_set_option(t.TM_OPT_GROUP, 4)
+        assert ctx.tsm_estimate(9, 2, k, mu, mom, LP, HP, t.TM_F32, t.TM_F64, seed=3)[2]["lanes"] == 2
+        ctx.tm_set_option(t.TM_OPT_GROUP, 0)
+        assert np.array_equal(to_np(ps1), to_np(ps2))
+        assert rel_l2(to_np(out1), to_np(out2)) <= 1e-13
+        assert info1["iters_lp"] == info2["iters_lp"] and info1["iters_hp"] == info2["iters_hp"]
+        parts = info1["ms_lp_solve"] + info1["ms_hp_solve"] + info1["ms_contract"]
+        assert abs(parts - info1["ms_total"]) <= 1e-6 * info1["ms_total"] and info1["ms_contract"] > 0
+
+
 def test_tsm_run_solutions_checked_by_oracle(orc, setup):
     """SURVEY.md sec 8 c.3 steps (1), (2) done ON the run: tsm_estimate hands back its own solutions (d_solutions) and
     the oracle evaluates, for EVERY source of a group of 8 plus a ragged tail (and both passes), the true residual
