@@ -608,14 +608,14 @@ __device__ __forceinline__ void hop32(const float* in, const float* gauge, size_
     for (int c = 0; c < 3; c++) {
         const c2 p0 = p[c], p1 = p[3 + c], p2 = p[6 + c], p3 = p[9 + c];
         if (MU == 0) {          // (-i psi3, -i psi2)
-            u[c] = P2<float>::fma_s(-SGN, times_i<float>(p3), p0);
-            u[3 + c] = P2<float>::fma_s(-SGN, times_i<float>(p2), p1);
+            u[c] = P2<float>::fma_si(-SGN, p3, p0);
+            u[3 + c] = P2<float>::fma_si(-SGN, p2, p1);
         } else if (MU == 1) {   // (-psi3, psi2)
             u[c] = P2<float>::fma_s(-SGN, p3, p0);
             u[3 + c] = P2<float>::fma_s(SGN, p2, p1);
         } else if (MU == 2) {   // (-i psi2, i psi3)
-            u[c] = P2<float>::fma_s(-SGN, times_i<float>(p2), p0);
-            u[3 + c] = P2<float>::fma_s(SGN, times_i<float>(p3), p1);
+            u[c] = P2<float>::fma_si(-SGN, p2, p0);
+            u[3 + c] = P2<float>::fma_si(SGN, p3, p1);
         } else {                // (psi2, psi3)
             u[c] = P2<float>::fma_s(SGN, p2, p0);
             u[3 + c] = P2<float>::fma_s(SGN, p3, p1);
@@ -631,7 +631,6 @@ __device__ __forceinline__ void hop32(const float* in, const float* gauge, size_
     for (int i = 0; i < 6; i++) v[i] = P2<float>::make(0.f, 0.f);
 #pragma unroll
     for (int b = 0; b < 3; b++) {
-        const c2 ib0 = times_i<float>(u[b]), ib1 = times_i<float>(u[3 + b]);
         float ur[3], ui[3];
 #pragma unroll
         for (int a = 0; a < 3; a++) {
@@ -645,8 +644,8 @@ __device__ __forceinline__ void hop32(const float* in, const float* gauge, size_
         }
 #pragma unroll
         for (int a = 0; a < 3; a++) {
-            v[a] = P2<float>::fma_s(ui[a], ib0, v[a]);
-            v[3 + a] = P2<float>::fma_s(ui[a], ib1, v[3 + a]);
+            v[a] = P2<float>::fma_si(ui[a], u[b], v[a]);
+            v[3 + a] = P2<float>::fma_si(ui[a], u[3 + b], v[3 + a]);
         }
     }
     // acc_up += v ; acc_low += s B_mu^dag v
@@ -656,14 +655,14 @@ __device__ __forceinline__ void hop32(const float* in, const float* gauge, size_
         acc[c] = P2<float>::add(acc[c], v0);
         acc[3 + c] = P2<float>::add(acc[3 + c], v1);
         if (MU == 0) {          // (i v1, i v0)
-            acc[6 + c] = P2<float>::fma_s(SGN, times_i<float>(v1), acc[6 + c]);
-            acc[9 + c] = P2<float>::fma_s(SGN, times_i<float>(v0), acc[9 + c]);
+            acc[6 + c] = P2<float>::fma_si(SGN, v1, acc[6 + c]);
+            acc[9 + c] = P2<float>::fma_si(SGN, v0, acc[9 + c]);
         } else if (MU == 1) {   // (v1, -v0)
             acc[6 + c] = P2<float>::fma_s(SGN, v1, acc[6 + c]);
             acc[9 + c] = P2<float>::fma_s(-SGN, v0, acc[9 + c]);
         } else if (MU == 2) {   // (i v0, -i v1)
-            acc[6 + c] = P2<float>::fma_s(SGN, times_i<float>(v0), acc[6 + c]);
-            acc[9 + c] = P2<float>::fma_s(-SGN, times_i<float>(v1), acc[9 + c]);
+            acc[6 + c] = P2<float>::fma_si(SGN, v0, acc[6 + c]);
+            acc[9 + c] = P2<float>::fma_si(-SGN, v1, acc[9 + c]);
         } else {                // (v0, v1)
             acc[6 + c] = P2<float>::fma_s(SGN, v0, acc[6 + c]);
             acc[9 + c] = P2<float>::fma_s(SGN, v1, acc[9 + c]);
