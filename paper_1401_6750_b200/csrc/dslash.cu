@@ -573,10 +573,13 @@ __device__ __forceinline__ void hop32(const float* in, const float* gauge, size_
     constexpr float SGN = (float)((FWD ? -1 : 1) * (DAGGER ? -1 : 1));      // forward: (1 - g), backward: (1 + g)
     c2 p[12];
     {
-        const float4* f = reinterpret_cast<const float4*>(in) + h_nb;
+        // 32-bit element indices (24 * Vh < 2^31 for every supported lattice): one IMAD.WIDE per load instead of a
+        // 64-bit add
+        const float4* f = reinterpret_cast<const float4*>(in);
+        const unsigned hn = (unsigned)h_nb, vh = (unsigned)Vh;
 #pragma unroll
         for (int k = 0; k < 6; k++) {
-            const float4 q = __ldg(f + (size_t)k * Vh);
+            const float4 q = __ldg(f + (hn + (unsigned)k * vh));
             p[2 * k] = P2<float>::make(q.x, q.y);
             p[2 * k + 1] = P2<float>::make(q.z, q.w);
         }
@@ -585,10 +588,11 @@ __device__ __forceinline__ void hop32(const float* in, const float* gauge, size_
     {
         const size_t hl = FWD ? h_out : h_nb;
         const int pl = FWD ? par_out : 1 - par_out;
-        const float4* g = reinterpret_cast<const float4*>(gauge) + ((size_t)(pl * 4 + MU) * 3 * Vh + hl);
+        const float4* g = reinterpret_cast<const float4*>(gauge);
+        const unsigned gi = (unsigned)(pl * 4 + MU) * 3u * (unsigned)Vh + (unsigned)hl;
 #pragma unroll
         for (int k = 0; k < 3; k++) {
-            const float4 q = __ldcs(g + (size_t)k * Vh);
+            const float4 q = __ldcs(g + (gi + (unsigned)k * (unsigned)Vh));
             U[4 * k] = q.x; U[4 * k + 1] = q.y; U[4 * k + 2] = q.z; U[4 * k + 3] = q.w;
         }
 #pragma unroll
