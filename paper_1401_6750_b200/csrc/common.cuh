@@ -343,11 +343,31 @@ struct Geom {
     int Xh;                // Lx/2
     int Vh;
     int s1, s2, s3;        // half-index strides of y, z, t:  Xh, Xh*Ly, Xh*Ly*Lz
+    int sh0, sh1, sh2;     // log2 of Xh, Ly, Lz when all three are powers of two, else sh0 = -1
 };
+// half index -> (xh, y, z, t): shifts and masks where the extents allow (three integer divisions otherwise)
+__host__ __device__ __forceinline__ void site_coords(const Geom& g, int h, int& xh, int& y, int& z, int& t) {
+    if (g.sh0 >= 0) {
+        xh = h & (g.Xh - 1);
+        int q = h >> g.sh0;
+        y = q & (g.X1 - 1); q >>= g.sh1;
+        z = q & (g.X2 - 1);
+        t = q >> g.sh2;
+    } else {
+        xh = h % g.Xh;
+        int q = h / g.Xh;
+        y = q % g.X1; q /= g.X1;
+        z = q % g.X2;
+        t = q / g.X2;
+    }
+}
 static inline Geom tm_geom(const tm_ctx* c) {
     Geom g;
     g.X0 = c->X[0]; g.X1 = c->X[1]; g.X2 = c->X[2]; g.X3 = c->X[3];
     g.Xh = c->Xh; g.Vh = (int)c->Vh;
     g.s1 = g.Xh; g.s2 = g.Xh * g.X1; g.s3 = g.Xh * g.X1 * g.X2;
+    auto lg = [](int v) { int l = 0; while ((1 << l) < v) l++; return (1 << l) == v ? l : -1; };
+    g.sh0 = lg(g.Xh); g.sh1 = lg(g.X1); g.sh2 = lg(g.X2);
+    if (g.sh0 < 0 || g.sh1 < 0 || g.sh2 < 0) g.sh0 = g.sh1 = g.sh2 = -1;
     return g;
 }

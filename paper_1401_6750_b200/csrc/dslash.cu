@@ -121,11 +121,8 @@ __global__ void __launch_bounds__(128) dslash_kernel(DslashArgs<typename Prec<S>
     const int h = bx * blockDim.x + threadIdx.x;
     double nrm = 0.0;
     if (h < g.Vh) {
-        const int xh = h % g.Xh;
-        int q = h / g.Xh;
-        const int y = q % g.X1; q /= g.X1;
-        const int z = q % g.X2;
-        const int t = q / g.X2;
+        int xh, y, z, t;
+        site_coords(g, h, xh, y, z, t);
         const int odd = (y + z + t + A.parity) & 1;     // x = 2*xh + odd
         const S* in = (const S*)A.in;
         const S* gauge = (const S*)A.gauge;
@@ -452,11 +449,8 @@ __global__ void __launch_bounds__(128, MINB) dslash16_kernel(DslashArgs<float> A
     const int h = bx * blockDim.x + threadIdx.x;
     double nrm = 0.0;
     if (h < g.Vh) {
-        const int xh = h % g.Xh;
-        int q = h / g.Xh;
-        const int y = q % g.X1; q /= g.X1;
-        const int z = q % g.X2;
-        const int t = q / g.X2;
+        int xh, y, z, t;
+        site_coords(g, h, xh, y, z, t);
         const int odd = (y + z + t + A.parity) & 1;
         const S* in = (const S*)A.in;
         const S* gauge = (const S*)A.gauge;
@@ -689,11 +683,8 @@ __global__ void __launch_bounds__(128, 4) dslash32_kernel(DslashArgs<float> A) {
     const int h = bx * blockDim.x + threadIdx.x;
     double nrm = 0.0;
     if (h < g.Vh) {
-        const int xh = h % g.Xh;
-        int q = h / g.Xh;
-        const int y = q % g.X1; q /= g.X1;
-        const int z = q % g.X2;
-        const int t = q / g.X2;
+        int xh, y, z, t;
+        site_coords(g, h, xh, y, z, t);
         const int odd = (y + z + t + A.parity) & 1;
         const float* in = (const float*)A.in;
         const float* gauge = (const float*)A.gauge;
