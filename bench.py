@@ -395,6 +395,8 @@ def profile_mode(args, cfg):
     Vh = inputs.volume(dims) // 2
     if args.what in ("dslash", "dslash_group"):
         nb = GROUP if args.what == "dslash_group" else 1
+        if nb > 1 and args.recon != 12:
+            raise SystemExit("bench.py --what dslash_group: tm_dslash_multi (the solver's grouped launch) is reconstruct-12 only")
         ms = time_dslash(ctx, tmod, torch, args.prec, args.recon, kappa, mu, args.napp, nb)
         nbytes = (nb * (48 + 24) + 8 * args.recon) * PREC_BYTES[args.prec] * Vh
         print("dslash %s r%d XPAY, %d source(s) per launch: %.1f us/launch, %.0f GB/s (spinors per source, links once per launch)"
