@@ -181,9 +181,10 @@ def test_contract_single_timeslice(orc, acc):
     ((24, 4, 4, 2), 1),      # c3 row shape
 ])
 def test_contract_fp32_paths(orc, path, dims, tb):
-    """The three implementations of the fp32 site + x/y-DFT stage (TM_OPT_CONTRACT_PATH: generic kernel, TMA-staged with
-    the DFT on the fp32 pipe, TMA-staged with the DFT on the tensor cores as split-fp32 tf32 MMAs) each against the
-    oracle at the north_star bound, for the pruned (p^2 <= 9) and the unpruned accumulator sets."""
+    """The implementations of the fp32 site + x/y-DFT stage (TM_OPT_CONTRACT_PATH: 1 generic kernel, 2 TMA-staged with the
+    folded DFT on the fp32 pipe and the forward-only s family, 3 TMA-staged with the DFT on the tensor cores as split-fp32
+    tf32 MMAs, 4 TMA-staged plain: no fold, both halves of every derivative) each against the oracle at the north_star
+    bound, for the pruned (p^2 <= 9) and the unpruned accumulator sets; Lx = 16, 24, 32 take the folded kernels."""
     t = tm()
     U, s, eta = case(dims, 0.25, 31)
     k, mu = 0.1563, 0.0055
