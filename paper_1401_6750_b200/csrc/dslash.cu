@@ -38,6 +38,7 @@ template <typename F> struct DslashArgs {
                        // so that the second reader of every link finds it in L2
     size_t fstride;    // bytes of one parity vector; source 1's operands sit mul_* vectors behind source 0's
     int mul_in, mul_x, mul_out;
+    int ns;            // dslash16_group_kernel: sources handled one after the other by a CTA (divides nb)
 };
 
 // u (2 spins x 3 colours complex = 12 reals) = psi_up + s * B_mu psi_low
@@ -388,7 +389,8 @@ __device__ __forceinline__ void reconstruct16(const float* v, float* acc) {
 }
 
 template <int MU, int FWD, int DAGGER, typename S, int R>
-__device__ __forceinline__ void compute16(const unsigned* p, const unsigned* Uin, float bsign, bool wrap, float* acc) {
+__device__ __forceinline__ void compute16(const unsigned* p, const unsigned* Uin, float bsign, bool wrap, float* acc,
+                                          unsigned* row2 = nullptr /* R == 12: receives the rebuilt third row */) {
     typedef typename Pk<S>::V2 V2;
     constexpr int SGN = (FWD ? -1 : 1) * (DAGGER ? -1 : 1);       // forward: (1 - g), backward: (1 + g)
     unsigned U[9], u[6];
@@ -415,6 +417,7 @@ __device__ __forceinline__ void compute16(const unsigned* p, const unsigned* Uin
         nim = Pk<S>::template fma<1, 0, 0>(U[j], U[3 + i], nim);
         U[6 + c] = as_u(Pk<S>::make(re, nim));
     }
+    if (R == 12 && row2) { row2[0] = U[6]; row2[1] = U[7]; row2[2] = U[8]; }
     // v = U u (or U^dag u) accumulated straight into the upper components of acc; the lower components
     // get s B_mu^dag v from the increment (new - old)
     float v[12];
@@ -432,6 +435,51 @@ __device__ __forceinline__ void compute16(const unsigned* p, const unsigned* Uin
             v[sp * 6 + 2 * a + 1] = im;
         }
     reconstruct16<MU, SGN>(v, acc);
+}
+
+// epilogue of the 16-bit kernels for one site: res = c * acc (+ x | + A x), optional A^-1, store, optional |res|^2
+template <typename S>
+__device__ __forceinline__ void dslash16_epilogue(const DslashArgs<float>& A, const S* xop, S* out, const Geom& g, int h,
+                                                  float* acc, double& nrm) {
+    // epilogue: res = c * acc (+ x | + A x), optional A^-1, store, optional norm
+    const float cf = A.c, a = A.a;
+    if (A.xmode) {
+        float xv[24];
+        load_spinor<S>(xop, g.Vh, h, xv);
+        if (A.xmode == 2) {
+#pragma unroll
+            for (int i = 0; i < 12; i += 2) {
+                float t0 = xv[i]; t0 -= a * xv[i + 1];              acc[i] = fmaf(cf, acc[i], t0);
+                float t1 = xv[i + 1]; t1 += a * xv[i];              acc[i + 1] = fmaf(cf, acc[i + 1], t1);
+                float t2 = xv[12 + i]; t2 += a * xv[12 + i + 1];    acc[12 + i] = fmaf(cf, acc[12 + i], t2);
+                float t3 = xv[12 + i + 1]; t3 -= a * xv[12 + i];    acc[12 + i + 1] = fmaf(cf, acc[12 + i + 1], t3);
+            }
+        } else {
+#pragma unroll
+            for (int i = 0; i < 24; i++) acc[i] = fmaf(cf, acc[i], xv[i]);
+        }
+    } else {
+#pragma unroll
+        for (int i = 0; i < 24; i++) acc[i] *= cf;
+    }
+    if (A.post) {
+        const float n = 1.f / (1.f + a * a);
+#pragma unroll
+        for (int i = 0; i < 12; i += 2) {
+            const float ur = acc[i], ui = acc[i + 1], lr = acc[12 + i], li = acc[12 + i + 1];
+            acc[i] = n * (ur + a * ui);
+            acc[i + 1] = n * (ui - a * ur);
+            acc[12 + i] = n * (lr - a * li);
+            acc[12 + i + 1] = n * (li + a * lr);
+        }
+    }
+    store_spinor<S>(out, g.Vh, h, acc);
+    if (A.red_op != RED_NONE) {
+        float n2 = 0.f;      // 24 terms in fp32, then fp64 across sites
+#pragma unroll
+        for (int i = 0; i < 24; i++) n2 = fmaf(acc[i], acc[i], n2);
+        nrm = (double)n2;
+    }
 }
 
 template <typename S, int DAGGER, int PIPE, int MINB, int R>
@@ -511,47 +559,124 @@ __global__ void __launch_bounds__(128, MINB) dslash16_kernel(DslashArgs<float> A
             load16<3, 1, S, R>(in, gauge, Vh, par, h, tp, pa, ua); compute16<3, 1, DAGGER, S, R>(pa, ua, A.tb, wp, acc);
             load16<3, 0, S, R>(in, gauge, Vh, par, h, tm, pa, ua); compute16<3, 0, DAGGER, S, R>(pa, ua, A.tb, wm, acc);
         }
-        // epilogue: res = c * acc (+ x | + A x), optional A^-1, store, optional norm
-        const float cf = A.c, a = A.a;
-        if (A.xmode) {
-            float xv[24];
-            load_spinor<S>((const S*)A.x, g.Vh, h, xv);
-            if (A.xmode == 2) {
-#pragma unroll
-                for (int i = 0; i < 12; i += 2) {
-                    float t0 = xv[i]; t0 -= a * xv[i + 1];              acc[i] = fmaf(cf, acc[i], t0);
-                    float t1 = xv[i + 1]; t1 += a * xv[i];              acc[i + 1] = fmaf(cf, acc[i + 1], t1);
-                    float t2 = xv[12 + i]; t2 += a * xv[12 + i + 1];    acc[12 + i] = fmaf(cf, acc[12 + i], t2);
-                    float t3 = xv[12 + i + 1]; t3 -= a * xv[12 + i];    acc[12 + i + 1] = fmaf(cf, acc[12 + i + 1], t3);
-                }
-            } else {
-#pragma unroll
-                for (int i = 0; i < 24; i++) acc[i] = fmaf(cf, acc[i], xv[i]);
-            }
-        } else {
-#pragma unroll
-            for (int i = 0; i < 24; i++) acc[i] *= cf;
-        }
-        if (A.post) {
-            const float n = 1.f / (1.f + a * a);
-#pragma unroll
-            for (int i = 0; i < 12; i += 2) {
-                const float ur = acc[i], ui = acc[i + 1], lr = acc[12 + i], li = acc[12 + i + 1];
-                acc[i] = n * (ur + a * ui);
-                acc[i + 1] = n * (ui - a * ur);
-                acc[12 + i] = n * (lr - a * li);
-                acc[12 + i + 1] = n * (li + a * lr);
-            }
-        }
-        store_spinor<S>((S*)A.out, g.Vh, h, acc);
-        if (A.red_op != RED_NONE) {
-            float n2 = 0.f;      // 24 terms in fp32, then fp64 across sites
-#pragma unroll
-            for (int i = 0; i < 24; i++) n2 = fmaf(acc[i], acc[i], n2);
-            nrm = (double)n2;
-        }
+        dslash16_epilogue<S>(A, (const S*)A.x, (S*)A.out, g, h, acc, nrm);
     }
     if (A.red_op != RED_NONE) block_partial_at(nrm, A.partials, bx, sm);
+}
+
+// -----------------------------------------------------------------------------------------------------
+// Grouped launches (tm_dslash_multi, the solver's launch shape): one CTA applies the stencil to the same 128 sites
+// of `ns` sources, one after the other.  What depends only on the sites is then done once per CTA instead of once
+// per source: the site / neighbour / link index arithmetic, the 24 cp.async of the links, and the rebuild of the
+// third link row -- the first source that runs writes the rebuilt rows next to the staged ones (thread-private
+// slots: no barrier), the others read complete links.  Same arithmetic in the same order per source: results are
+// bit-identical to one source per CTA.  (reconstruct-12 only.)
+#define D16G_CH 4            // 8-byte chunks per hop and thread: rows 0, 1 as staged (3) + two thirds of the rebuilt row 2;
+                             // its last complex number sits in a 4-byte array of its own: 36 KB of slots per CTA, so that
+                             // 5 CTAs stay below the 196 KB shared-memory carve-out (at 228 KB the 28 KB left for L1 cost 21 %)
+
+template <typename S, int DAGGER, int FIRST>
+__device__ __forceinline__ void hops16_group(const S* in, size_t Vh, uint2* sl, unsigned* sl1, const int* nbr, float tb, bool wp,
+                                             bool wm, float* acc) {
+    constexpr int LS = D16G_CH * 128;
+    unsigned pa[12], pb[12], ua[9], row2[3];
+    auto link = [&](int j) {
+        const uint2* s = sl + j * LS;
+        const uint2 q0 = s[0], q1 = s[128], q2 = s[256];
+        ua[0] = q0.x; ua[1] = q0.y; ua[2] = q1.x; ua[3] = q1.y; ua[4] = q2.x; ua[5] = q2.y;
+        if (!FIRST) { const uint2 q3 = s[384]; ua[6] = q3.x; ua[7] = q3.y; ua[8] = sl1[j * 128]; }
+    };
+    auto keep = [&](int j) {
+        if (FIRST) { sl[j * LS + 384] = make_uint2(row2[0], row2[1]); sl1[j * 128] = row2[2]; }
+    };
+#define D16G_HOP(J, MU, FWD, PBUF, BS, WR)                                                                    \
+    do {                                                                                                       \
+        if (FIRST) cp_wait<7 - (J)>();                                                                         \
+        link(J);                                                                                               \
+        if (FIRST) { compute16<MU, FWD, DAGGER, S, 12>(PBUF, ua, BS, WR, acc, row2); keep(J); }                 \
+        else compute16<MU, FWD, DAGGER, S, 18>(PBUF, ua, BS, WR, acc);                                         \
+    } while (0)
+    load_spinor16<S>(in, Vh, nbr[0], pa);
+    load_spinor16<S>(in, Vh, nbr[1], pb);
+    D16G_HOP(0, 0, 1, pa, 1.f, false);
+    load_spinor16<S>(in, Vh, nbr[2], pa);
+    D16G_HOP(1, 0, 0, pb, 1.f, false);
+    load_spinor16<S>(in, Vh, nbr[3], pb);
+    D16G_HOP(2, 1, 1, pa, 1.f, false);
+    load_spinor16<S>(in, Vh, nbr[4], pa);
+    D16G_HOP(3, 1, 0, pb, 1.f, false);
+    load_spinor16<S>(in, Vh, nbr[5], pb);
+    D16G_HOP(4, 2, 1, pa, 1.f, false);
+    load_spinor16<S>(in, Vh, nbr[6], pa);
+    D16G_HOP(5, 2, 0, pb, 1.f, false);
+    load_spinor16<S>(in, Vh, nbr[7], pb);
+    D16G_HOP(6, 3, 1, pa, tb, wp);
+    D16G_HOP(7, 3, 0, pb, tb, wm);
+#undef D16G_HOP
+}
+
+template <typename S, int DAGGER, int MINB>
+__global__ void __launch_bounds__(128, MINB) dslash16_group_kernel(DslashArgs<float> A) {
+    __shared__ double sm[32];
+    __shared__ uint2 smg[8 * D16G_CH * 128];
+    __shared__ unsigned smg1[8 * 128];
+    // CTA index = (tile, group of ns sources): the nb / ns CTAs of a tile are neighbours, so the links they all stage
+    // cross HBM once (L2); ns and nb are powers of two
+    const int ns = A.ns, ng = A.nb / ns;
+    const int bx = blockIdx.x / ng, src0 = (blockIdx.x - bx * ng) * ns;
+    const Geom& g = A.g;
+    const int h = bx * blockDim.x + threadIdx.x;
+    const bool live = h < g.Vh;
+    const S* gauge = (const S*)A.gauge;
+    const size_t Vh = g.Vh;
+    const int par = A.parity;
+    uint2* sl = smg + threadIdx.x;
+    unsigned* sl1 = smg1 + threadIdx.x;
+    int nbr[8];
+    bool wp = false, wm = false;
+    if (live) {
+        int xh, y, z, t;
+        site_coords(g, h, xh, y, z, t);
+        const int odd = (y + z + t + par) & 1;
+        const int row = h - xh;
+        nbr[0] = row + (odd ? (xh + 1 == g.Xh ? 0 : xh + 1) : xh);
+        nbr[1] = row + (odd ? xh : (xh == 0 ? g.Xh - 1 : xh - 1));
+        nbr[2] = (y + 1 == g.X1) ? h - (g.X1 - 1) * g.s1 : h + g.s1;
+        nbr[3] = (y == 0) ? h + (g.X1 - 1) * g.s1 : h - g.s1;
+        nbr[4] = (z + 1 == g.X2) ? h - (g.X2 - 1) * g.s2 : h + g.s2;
+        nbr[5] = (z == 0) ? h + (g.X2 - 1) * g.s2 : h - g.s2;
+        wp = (t + 1 == g.X3); wm = (t == 0);
+        nbr[6] = wp ? h - (g.X3 - 1) * g.s3 : h + g.s3;
+        nbr[7] = wm ? h + (g.X3 - 1) * g.s3 : h - g.s3;
+        constexpr int LS = D16G_CH * 128;
+        stage_link16<0, 1, S, 12>(gauge, Vh, par, h, nbr[0], sl + 0 * LS);
+        stage_link16<0, 0, S, 12>(gauge, Vh, par, h, nbr[1], sl + 1 * LS);
+        stage_link16<1, 1, S, 12>(gauge, Vh, par, h, nbr[2], sl + 2 * LS);
+        stage_link16<1, 0, S, 12>(gauge, Vh, par, h, nbr[3], sl + 3 * LS);
+        stage_link16<2, 1, S, 12>(gauge, Vh, par, h, nbr[4], sl + 4 * LS);
+        stage_link16<2, 0, S, 12>(gauge, Vh, par, h, nbr[5], sl + 5 * LS);
+        stage_link16<3, 1, S, 12>(gauge, Vh, par, h, nbr[6], sl + 6 * LS);
+        stage_link16<3, 0, S, 12>(gauge, Vh, par, h, nbr[7], sl + 7 * LS);
+    }
+    bool first = true;                         // no source has used (and completed) the staged links yet
+    for (int si = 0; si < ns; si++) {
+        const int src = src0 + si;
+        if (guard_skip(A.sc + src, A.guard)) continue;            // uniform over the CTA
+        const S* in = (const S*)((const char*)A.in + (size_t)src * A.mul_in * A.fstride);
+        S* out = (S*)((char*)A.out + (size_t)src * A.mul_out * A.fstride);
+        const S* xop = A.x ? (const S*)((const char*)A.x + (size_t)src * A.mul_x * A.fstride) : nullptr;
+        double nrm = 0.0;
+        if (live) {
+            float acc[24];
+#pragma unroll
+            for (int i = 0; i < 24; i++) acc[i] = 0.f;
+            if (first) hops16_group<S, DAGGER, 1>(in, Vh, sl, sl1, nbr, A.tb, wp, wm, acc);
+            else       hops16_group<S, DAGGER, 0>(in, Vh, sl, sl1, nbr, A.tb, wp, wm, acc);
+            dslash16_epilogue<S>(A, xop, out, g, h, acc, nrm);
+        }
+        first = false;
+        if (A.red_op != RED_NONE) block_partial_at(nrm, A.partials + (size_t)src * TM_PSTRIDE, bx, sm);
+    }
 }
 
 // =====================================================================================================
@@ -824,6 +949,19 @@ static tm_status launch16(tm_ctx* ctx, const DslashCall& c, const void* gauge, c
     // <PIPE = 2, MINB = 5>: links staged by cp.async, 96 registers, 20 warps/SM.  Measured at 32^3x64 (fp16 XPAY,
     // same box): 66.7 us against 69.8 us for register-loaded links <0, 6> and 67.5 us for <2, 6>.
     // reconstruct-18: the same kernel without the row-2 rebuild (9 x 4-byte link chunks, 36 KB of slots per CTA)
+    A.ns = 1;
+    if (R == 12 && A.nb > 1 && std::is_same<S, __half>::value) {
+        // grouped launch: one CTA per tile of 128 sites does all nb sources, which then share the index arithmetic, the
+        // link staging and the row-2 rebuilds.  Measured at 32^3x64, 8 sources, fp16 (same box): 430.8 us with one
+        // source per CTA (dslash16_kernel, CTAs of a tile adjacent) -> 412.4 us with 4 sources per CTA -> 392.5 us
+        // with 8.  bf16 gains nothing (488.5 against 493.7 us) and stays on dslash16_kernel.
+        A.ns = A.nb;
+        if (c.dagger) dslash16_group_kernel<S, 1, 5><<<tiles, block, 0, st>>>(A);
+        else          dslash16_group_kernel<S, 0, 5><<<tiles, block, 0, st>>>(A);
+        TM_LAUNCH_CHECK(ctx, "dslash16_group_kernel");
+        if (c.red_op != RED_NONE) TM_TRY(tm_reduce_finish(ctx, (unsigned)tiles, c.red_op, c.guard, st));
+        return TM_OK;
+    }
     if (c.dagger) dslash16_kernel<S, 1, 2, 5, R><<<grid, block, 0, st>>>(A);
     else          dslash16_kernel<S, 0, 2, 5, R><<<grid, block, 0, st>>>(A);
     TM_LAUNCH_CHECK(ctx, "dslash16_kernel");
