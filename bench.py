@@ -585,16 +585,17 @@ def run_b200(args, cfg):
     single = ds[sl + "_r12"]
     traffic1, traffic1_src = ncu_traffic("r02_dslash16_f16.md", "dslash.cu")
     roofline = {
-        "bound": "hbm", "kernel": "dslash16_kernel<%s> reconstruct-12 XPAY (second half of Mhat), %d sources per launch "
-                                  "(the launch shape of the timed step)" % (sl, GROUP),
+        "bound": "hbm", "kernel": "%s<%s> reconstruct-12 XPAY (second half of Mhat), %d sources per launch "
+                                  "(the launch shape of the timed step)"
+                                  % ("dslash16_group_kernel" if sl == "f16" else "dslash16_kernel", sl, GROUP),
         "achieved": must_move / (t_g * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
         "frac": must_move / (t_g * 1e-3) / 1e9 / peak, "traffic": traffic, "traffic_source": traffic_src,
         "peak_source": peak_src, "algorithmic_bytes_per_launch": must_move,
         "us_per_launch": t_g * 1e3, "us_per_source": t_g * 1e3 / GROUP,
         "how": "CUDA events around 60 back-to-back launches on the current stream, 4 rotating buffer sets of 8 sources",
-        "note": "8 sources share every link through L2, so the launch moves 0.5x the bytes of 8 single-source launches and "
-                "is bound by instruction issue and board power, not by HBM (DESIGN.md sec 6); per source it is faster than "
-                "the single-source launch below",
+        "note": "one CTA per 128 sites does the 8 sources one after the other (links staged and rebuilt once), so the "
+                "launch moves 0.5x the bytes of 8 single-source launches and is bound by instruction issue and board power, "
+                "not by HBM (DESIGN.md sec 6); per source it is faster than the single-source launch below",
         "single_source_equivalent_GBps": GROUP * dslash_bytes_per_site(sl, 12, True) * Vh / (t_g * 1e-3) / 1e9,
         "single_source_launch": {"us": single["us"], "achieved": single["GBps"], "frac": single["GBps"] / peak,
                                  "algorithmic_bytes_per_launch": dslash_bytes_per_site(sl, 12, True) * Vh,
