@@ -670,6 +670,12 @@ __global__ void __launch_bounds__(128, MINB) dslash16_group_kernel(DslashArgs<fl
             float acc[24];
 #pragma unroll
             for (int i = 0; i < 24; i++) acc[i] = 0.f;
+            if (A.xmode) {          // the epilogue's x operand is a load nothing hides (no registers to issue it early): pull it into L2
+                                    // now (392.5 -> 376.5 us per 8-source launch; prefetching the next source's first neighbours too: no gain)
+                const uint4* xf = reinterpret_cast<const uint4*>(xop) + h;
+#pragma unroll
+                for (int k = 0; k < 3; k++) asm volatile("prefetch.global.L2 [%0];" ::"l"(xf + (size_t)k * Vh));
+            }
             if (first) hops16_group<S, DAGGER, 1>(in, Vh, sl, sl1, nbr, A.tb, wp, wm, acc);
             else       hops16_group<S, DAGGER, 0>(in, Vh, sl, sl1, nbr, A.tb, wp, wm, acc);
             dslash16_epilogue<S>(A, xop, out, g, h, acc, nrm);
