@@ -517,6 +517,11 @@ __global__ void __launch_bounds__(128, MINB) dslash16_kernel(DslashArgs<float> A
         const int tp = wp ? h - (g.X3 - 1) * g.s3 : h + g.s3;
         const int tm = wm ? h + (g.X3 - 1) * g.s3 : h - g.s3;
         const int par = A.parity;
+        if (A.xmode) {              // the epilogue's x operand: into L2 now (see dslash16_group_kernel)
+            const uint4* xf = reinterpret_cast<const uint4*>(A.x) + h;
+#pragma unroll
+            for (int k = 0; k < 3; k++) asm volatile("prefetch.global.L2 [%0];" ::"l"(xf + (size_t)k * Vh));
+        }
         unsigned pa[12], ua[R / 2];
         constexpr int LS = LinkSlot<R>::NCH * 128;             // slots of one hop
         if (PIPE == 2) {
@@ -823,6 +828,12 @@ __global__ void __launch_bounds__(128, 4) dslash32_kernel(DslashArgs<float> A) {
         c2 acc[12];
 #pragma unroll
         for (int i = 0; i < 12; i++) acc[i] = P2<float>::make(0.f, 0.f);
+        if (A.xmode && A.nb > 1) {  // the epilogue's x operand: into L2 now (see dslash16_group_kernel); grouped launches only:
+                                    // 697.4 -> 674.5 us per 8 sources, but 113.0 -> 114.5 us for one source per launch
+            const float4* xf = reinterpret_cast<const float4*>(A.x) + h;
+#pragma unroll
+            for (int k = 0; k < 6; k++) asm volatile("prefetch.global.L2 [%0];" ::"l"(xf + (size_t)k * Vh));
+        }
         const int row = h - xh;
         const int xp = row + (odd ? (xh + 1 == g.Xh ? 0 : xh + 1) : xh);
         const int xm = row + (odd ? xh : (xh == 0 ? g.Xh - 1 : xh - 1));
