@@ -134,36 +134,54 @@ tm_status blas_twist_inv(tm_ctx* ctx, void* dst, const void* src, tm_prec p, dou
     });
 }
 
-// ------------------------------------------------------------------ reliable update, part 1: y += x ; x = 0
-template <typename Sy, typename Sx>
-__global__ void ru_begin_kernel(Sy* __restrict__ y, Sx* __restrict__ x, int Vh, const CgScalars* sc, int y_mul) {
-    sc += blockIdx.y; y = src_vec(y, blockIdx.y * y_mul, Vh); x = src_vec(x, blockIdx.y, Vh);
+// ------------------------------------------------------------------ reliable update, part 1: y += x (+ alpha p) ; x = 0
+template <typename Sy, typename Sx, typename Sp>
+__global__ void ru_begin_kernel(Sy* __restrict__ y, Sx* __restrict__ x, const Sp* __restrict__ p, int Vh, const CgScalars* sc,
+                                int y_mul) {
+    sc += blockIdx.y; y = src_vec(y, blockIdx.y * y_mul, Vh); x = src_vec(x, blockIdx.y, Vh); p = src_vec(p, blockIdx.y, Vh);
     if (guard_skip(sc, GUARD_RU)) return;
     const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= 3L * Vh) return;
     const int g = (int)(i / Vh), h = (int)(i % Vh);
     // y += x ; x = 0, with both vectors possibly "zero by construction" (CgScalars::x_zero / y_zero: then they are
-    // not read, and x is not zero-filled -- RED_RU raises x_zero instead)
-    const bool xz = sc->x_zero != 0, yz = sc->y_zero != 0;
-    if (xz && !yz) return;
-    typename Prec<Sx>::F a[8];
+    // not read, and x is not zero-filled -- RED_RU raises x_zero instead); x_pend: the axpy of the last iteration has
+    // not reached x yet (it rides in the next update_p) and is applied here, in x's precision, before x goes into y
+    const bool xz = sc->x_zero != 0, yz = sc->y_zero != 0, pend = sc->x_pend != 0;
+    if (xz && !pend && !yz) return;
+    typedef typename Prec<Sx>::F FA;
+    FA a[8];
     typename Prec<Sy>::F b[8];
 #pragma unroll
     for (int k = 0; k < 8; k++) { a[k] = 0; b[k] = 0; }
     if (!xz) load8<Sx>(x, Vh, h, g, a);
+    if (pend) {
+        const FA alpha = (FA)sc->alpha;
+        typename Prec<Sp>::F vp[8];
+        load8<Sp>(p, Vh, h, g, vp);
+#pragma unroll
+        for (int k = 0; k < 8; k++) a[k] += alpha * (FA)vp[k];
+    }
     if (!yz) load8<Sy>(y, Vh, h, g, b);
 #pragma unroll
     for (int k = 0; k < 8; k++) b[k] += (typename Prec<Sy>::F)a[k];
     store8<Sy>(y, Vh, h, g, b);
 }
 
-tm_status blas_ru_begin(tm_ctx* ctx, void* y, tm_prec po, void* x, tm_prec pacc, cudaStream_t st, int y_mul) {
+tm_status blas_ru_begin(tm_ctx* ctx, void* y, tm_prec po, void* x, tm_prec pacc, const void* p, tm_prec psl, cudaStream_t st,
+                        int y_mul) {
     const dim3 grid = pair_grid(ctx, items_grid(ctx, 256));
     const int Vh = (int)ctx->Vh;
-    if (po == TM_F64 && pacc == TM_F64) ru_begin_kernel<double, double><<<grid, 256, 0, st>>>((double*)y, (double*)x, Vh, ctx->d_scal, y_mul);
-    else if (po == TM_F64 && pacc == TM_F32) ru_begin_kernel<double, float><<<grid, 256, 0, st>>>((double*)y, (float*)x, Vh, ctx->d_scal, y_mul);
-    else if (po == TM_F32 && pacc == TM_F32) ru_begin_kernel<float, float><<<grid, 256, 0, st>>>((float*)y, (float*)x, Vh, ctx->d_scal, y_mul);
-    else return tm_fail(ctx, TM_EPREC, "ru_begin: unsupported precision pair");
+    const CgScalars* sc = ctx->d_scal;
+#define RUB(SY, SX, SP) ru_begin_kernel<SY, SX, SP><<<grid, 256, 0, st>>>((SY*)y, (SX*)x, (const SP*)p, Vh, sc, y_mul)
+    if (po == TM_F64 && pacc == TM_F64 && psl == TM_F64) RUB(double, double, double);
+    else if (po == TM_F64 && pacc == TM_F32 && psl == TM_F32) RUB(double, float, float);
+    else if (po == TM_F64 && pacc == TM_F32 && psl == TM_F16) RUB(double, float, __half);
+    else if (po == TM_F64 && pacc == TM_F32 && psl == TM_BF16) RUB(double, float, __nv_bfloat16);
+    else if (po == TM_F32 && pacc == TM_F32 && psl == TM_F32) RUB(float, float, float);
+    else if (po == TM_F32 && pacc == TM_F32 && psl == TM_F16) RUB(float, float, __half);
+    else if (po == TM_F32 && pacc == TM_F32 && psl == TM_BF16) RUB(float, float, __nv_bfloat16);
+    else return tm_fail(ctx, TM_EPREC, "ru_begin: unsupported precision triple");
+#undef RUB
     TM_LAUNCH_CHECK(ctx, "ru_begin_kernel");
     return TM_OK;
 }
@@ -274,10 +292,12 @@ static tm_status norm_impl(tm_ctx* ctx, const void* v, tm_prec p, int red_op, in
 tm_status blas_norm(tm_ctx* ctx, const void* v, tm_prec p, int red_op, cudaStream_t st) { return norm_impl(ctx, v, p, red_op, 1, st); }
 tm_status blas_norm_full(tm_ctx* ctx, const void* v, tm_prec p, int red_op, cudaStream_t st) { return norm_impl(ctx, v, p, red_op, 2, st); }
 
-// ------------------------------------------------------------------ x += alpha p ; r -= alpha w ; ||r||^2
+// ------------------------------------------------------------------ r -= alpha w ; ||r||^2
+// (x += alpha p, the other half of the textbook update, is deferred to the next update_p -- which reads p anyway -- or
+//  to ru_begin when the solve pauses first: CgScalars::x_pend.  Same operations on x in the same order, one read of
+//  p per iteration less.)
 template <typename SA, typename SL>
-__global__ void __launch_bounds__(256) update_xr_kernel(SA* __restrict__ x, SA* __restrict__ r,
-                                                        const SL* __restrict__ p, const SL* __restrict__ w,
+__global__ void __launch_bounds__(256) update_xr_kernel(SA* __restrict__ r, const SL* __restrict__ w,
                                                         SL* __restrict__ rs, int Vh, double* partials,
                                                         unsigned int* counter, CgScalars* sc) {
     typedef typename Prec<SA>::F FA;
@@ -286,20 +306,15 @@ __global__ void __launch_bounds__(256) update_xr_kernel(SA* __restrict__ x, SA* 
     {
         const int src = blockIdx.y;
         sc += src; partials += src * TM_PSTRIDE; counter += src;
-        x = src_vec(x, src, Vh); r = src_vec(r, src, Vh); p = src_vec(p, src, Vh); w = src_vec(w, src, Vh); rs = src_vec(rs, src, Vh);
+        r = src_vec(r, src, Vh); w = src_vec(w, src, Vh); rs = src_vec(rs, src, Vh);
     }
     if (guard_skip(sc, GUARD_ITER)) return;
     const FA alpha = (FA)sc->alpha;
-    const bool xz = sc->x_zero != 0;             // first update after a (re)start: x is zero by construction
     double nrm = 0.0;
     for (long i = (long)blockIdx.x * blockDim.x + threadIdx.x; i < 3L * Vh; i += (long)gridDim.x * blockDim.x) {
         const int g = (int)(i / Vh), h = (int)(i % Vh);
-        FA vx[8], vr[8];
-        FL vp[8], vw[8];
-        if (xz) {
-#pragma unroll
-            for (int k = 0; k < 8; k++) vx[k] = 0;
-        } else load8<SA>(x, Vh, h, g, vx);
+        FA vr[8];
+        FL vw[8];
         if (r) load8<SA>(r, Vh, h, g, vr);
         else {                                       // r == NULL: the residual lives in sloppy storage only
             FL vs[8];
@@ -307,15 +322,12 @@ __global__ void __launch_bounds__(256) update_xr_kernel(SA* __restrict__ x, SA* 
 #pragma unroll
             for (int k = 0; k < 8; k++) vr[k] = (FA)vs[k];
         }
-        load8<SL>(p, Vh, h, g, vp);
         load8<SL>(w, Vh, h, g, vw);
 #pragma unroll
         for (int k = 0; k < 8; k++) {
-            vx[k] += alpha * (FA)vp[k];
             vr[k] -= alpha * (FA)vw[k];
             nrm += (double)vr[k] * (double)vr[k];
         }
-        store8<SA>(x, Vh, h, g, vx);
         if (r) store8<SA>(r, Vh, h, g, vr);
         if (!std::is_same<SA, SL>::value) {
             FL vs[8];
@@ -327,38 +339,52 @@ __global__ void __launch_bounds__(256) update_xr_kernel(SA* __restrict__ x, SA* 
     grid_reduce(nrm, partials, counter, sc, RED_RR, sm);
 }
 
-tm_status blas_update_xr(tm_ctx* ctx, void* x, void* r, tm_prec pacc, const void* p, const void* w,
-                         void* rs, tm_prec psl, cudaStream_t st) {
+tm_status blas_update_xr(tm_ctx* ctx, void* r, tm_prec pacc, const void* w, void* rs, tm_prec psl, cudaStream_t st) {
     const dim3 grid = pair_grid(ctx, red_grid(ctx, 3L * ctx->Vh, 256));
     const int Vh = (int)ctx->Vh;
     double* pa = ctx->d_partials; unsigned int* cn = ctx->d_counter; CgScalars* sc = ctx->d_scal;
     if (pacc == TM_F64 && psl == TM_F64)
-        update_xr_kernel<double, double><<<grid, 256, 0, st>>>((double*)x, (double*)r, (const double*)p, (const double*)w, (double*)rs, Vh, pa, cn, sc);
+        update_xr_kernel<double, double><<<grid, 256, 0, st>>>((double*)r, (const double*)w, (double*)rs, Vh, pa, cn, sc);
     else if (pacc == TM_F32 && psl == TM_F32)
-        update_xr_kernel<float, float><<<grid, 256, 0, st>>>((float*)x, (float*)r, (const float*)p, (const float*)w, (float*)rs, Vh, pa, cn, sc);
+        update_xr_kernel<float, float><<<grid, 256, 0, st>>>((float*)r, (const float*)w, (float*)rs, Vh, pa, cn, sc);
     else if (pacc == TM_F32 && psl == TM_F16)
-        update_xr_kernel<float, __half><<<grid, 256, 0, st>>>((float*)x, (float*)r, (const __half*)p, (const __half*)w, (__half*)rs, Vh, pa, cn, sc);
+        update_xr_kernel<float, __half><<<grid, 256, 0, st>>>((float*)r, (const __half*)w, (__half*)rs, Vh, pa, cn, sc);
     else if (pacc == TM_F32 && psl == TM_BF16)
-        update_xr_kernel<float, __nv_bfloat16><<<grid, 256, 0, st>>>((float*)x, (float*)r, (const __nv_bfloat16*)p, (const __nv_bfloat16*)w, (__nv_bfloat16*)rs, Vh, pa, cn, sc);
+        update_xr_kernel<float, __nv_bfloat16><<<grid, 256, 0, st>>>((float*)r, (const __nv_bfloat16*)w, (__nv_bfloat16*)rs, Vh, pa, cn, sc);
     else return tm_fail(ctx, TM_EPREC, "update_xr: unsupported precision pair");
     TM_LAUNCH_CHECK(ctx, "update_xr_kernel");
     return TM_OK;
 }
 
-// ------------------------------------------------------------------ p = z + beta p
-template <typename S>
-__global__ void update_p_kernel(S* __restrict__ p, const S* __restrict__ z, int Vh, const CgScalars* sc) {
+// ------------------------------------------------------------------ x += alpha_old p (if pending) ; p = z + beta p
+template <typename SA, typename S>
+__global__ void update_p_kernel(S* __restrict__ p, const S* __restrict__ z, SA* __restrict__ x, int Vh, const CgScalars* sc) {
     typedef typename Prec<S>::F F;
-    sc += blockIdx.y; p = src_vec(p, blockIdx.y, Vh); z = src_vec(z, blockIdx.y, Vh);
+    typedef typename Prec<SA>::F FA;
+    sc += blockIdx.y; p = src_vec(p, blockIdx.y, Vh); z = src_vec(z, blockIdx.y, Vh); x = src_vec(x, blockIdx.y, Vh);
     if (guard_skip(sc, GUARD_ITER)) return;
     const F beta = (F)sc->beta;
+    // the axpy of the previous iteration (CgScalars::x_pend): alpha is still that iteration's (the next RED_WW replaces
+    // it, and marks x as up to date), p is still its search direction
+    const bool pend = sc->x_pend != 0, xz = sc->x_zero != 0;
+    const FA alpha = (FA)sc->alpha;
     const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= 3L * Vh) return;
     const int g = (int)(i / Vh), h = (int)(i % Vh);
     F vp[8], vz[8];
     load8<S>(z, Vh, h, g, vz);
+    if (beta != F(0) || pend) load8<S>(p, Vh, h, g, vp);
+    if (pend) {
+        FA vx[8];
+        if (xz) {                   // first update after a (re)start: x is zero by construction
+#pragma unroll
+            for (int k = 0; k < 8; k++) vx[k] = 0;
+        } else load8<SA>(x, Vh, h, g, vx);
+#pragma unroll
+        for (int k = 0; k < 8; k++) vx[k] += alpha * (FA)vp[k];
+        store8<SA>(x, Vh, h, g, vx);
+    }
     if (beta != F(0)) {             // beta == 0: first iteration of a solve, p is uninitialised, p = z
-        load8<S>(p, Vh, h, g, vp);
 #pragma unroll
         for (int k = 0; k < 8; k++) vp[k] = vz[k] + beta * vp[k];
     } else {
@@ -368,13 +394,17 @@ __global__ void update_p_kernel(S* __restrict__ p, const S* __restrict__ z, int 
     store8<S>(p, Vh, h, g, vp);
 }
 
-tm_status blas_update_p(tm_ctx* ctx, void* p, const void* z, tm_prec psl, cudaStream_t st) {
-    return dispatch_prec(ctx, psl, [&](auto* t) {
-        typedef TAGTYPE(t) S;
-        update_p_kernel<S><<<pair_grid(ctx, items_grid(ctx, 256)), 256, 0, st>>>((S*)p, (const S*)z, (int)ctx->Vh, ctx->d_scal);
-        TM_LAUNCH_CHECK(ctx, "update_p_kernel");
-        return TM_OK;
-    });
+tm_status blas_update_p(tm_ctx* ctx, void* p, const void* z, tm_prec psl, void* x, tm_prec pacc, cudaStream_t st) {
+    const dim3 grid = pair_grid(ctx, items_grid(ctx, 256));
+    const int Vh = (int)ctx->Vh;
+    const CgScalars* sc = ctx->d_scal;
+    if (pacc == TM_F64 && psl == TM_F64) update_p_kernel<double, double><<<grid, 256, 0, st>>>((double*)p, (const double*)z, (double*)x, Vh, sc);
+    else if (pacc == TM_F32 && psl == TM_F32) update_p_kernel<float, float><<<grid, 256, 0, st>>>((float*)p, (const float*)z, (float*)x, Vh, sc);
+    else if (pacc == TM_F32 && psl == TM_F16) update_p_kernel<float, __half><<<grid, 256, 0, st>>>((__half*)p, (const __half*)z, (float*)x, Vh, sc);
+    else if (pacc == TM_F32 && psl == TM_BF16) update_p_kernel<float, __nv_bfloat16><<<grid, 256, 0, st>>>((__nv_bfloat16*)p, (const __nv_bfloat16*)z, (float*)x, Vh, sc);
+    else return tm_fail(ctx, TM_EPREC, "update_p: unsupported precision pair");
+    TM_LAUNCH_CHECK(ctx, "update_p_kernel");
+    return TM_OK;
 }
 
 // ------------------------------------------------------------------ scalars

@@ -29,6 +29,9 @@ struct CgScalars {
     int n_ru;          // reliable updates so far
     int x_zero;        // x == 0 by construction (start of a solve / after a reliable update): x is neither read nor zero-filled
     int y_zero;        // y == 0 by construction (no reliable update yet): y is not read
+    int x_pend;        // x still lacks alpha * p of the last iteration: that axpy rides in the NEXT update_p (which reads p
+                       // anyway) instead of update_xr, or in ru_begin when the solve pauses first; alpha and p are
+                       // unchanged until then
     int iters_at_ru;   // iteration count at the last reliable update (a reliable update is forced every 100 iterations)
     int stall;         // consecutive reliable updates that did not halve the true residual while far from the target
     int pause_iter[CG_MAX_PAUSES];   // iteration count at each pause (replayed by the host as a launch plan)
@@ -76,9 +79,13 @@ __device__ __forceinline__ double block_sum(double v, double* sm /* >= 32 double
 // what the reduced sum `s` does to the CG state (one thread)
 __device__ __forceinline__ void apply_red_op(CgScalars* sc, int op, double s) {
     switch (op) {
-        case RED_WW: sc->ww = s; sc->alpha = sc->gamma / s; break;
+        case RED_WW:
+            // the update_p that ran just before this Dslash has applied the pending alpha * p to x (with the OLD alpha)
+            if (sc->x_pend) { sc->x_zero = 0; sc->x_pend = 0; }
+            sc->ww = s; sc->alpha = sc->gamma / s;
+            break;
         case RED_RR:
-            sc->rr = s; sc->iters += 1; sc->x_zero = 0;
+            sc->rr = s; sc->iters += 1; sc->x_pend = 1;
             if (!(s > sc->target2) || !(s > sc->ru2) || sc->iters >= sc->max_iter || sc->iters - sc->iters_at_ru >= 100)
                 sc->done = 1;
             break;
@@ -97,7 +104,7 @@ __device__ __forceinline__ void apply_red_op(CgScalars* sc, int op, double s) {
             sc->n_ru += 1;
             sc->rr_true = s;
             sc->iters_at_ru = sc->iters;
-            sc->x_zero = 1; sc->y_zero = 0;      // ru_begin folded x into y
+            sc->x_zero = 1; sc->y_zero = 0; sc->x_pend = 0;      // ru_begin folded x (and the pending alpha p) into y
             if (!(s == s)) sc->done = 3;
             else if (s <= sc->target2) sc->done = 2;
             else if (sc->iters >= sc->max_iter || sc->stall >= 2) sc->done = 3;

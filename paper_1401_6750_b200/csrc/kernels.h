@@ -41,13 +41,14 @@ tm_status blas_norm(tm_ctx* ctx, const void* v, tm_prec p, int red_op, cudaStrea
 // full-lattice norm (2 parities)
 tm_status blas_norm_full(tm_ctx* ctx, const void* v, tm_prec p, int red_op, cudaStream_t st);
 // CG kernels driven by the device-resident state (CgScalars); each runs only in its guard state:
-//   x += alpha p ; r -= alpha w ; ||r||^2 -> RED_RR ; sloppy copy rs of r            (GUARD_ITER)
-tm_status blas_update_xr(tm_ctx* ctx, void* x, void* r, tm_prec pacc, const void* p, const void* w,
-                         void* rs, tm_prec psl, cudaStream_t st);
-//   p = z + beta p  (p = z when beta == 0: first iteration)                                  (GUARD_ITER)
-tm_status blas_update_p(tm_ctx* ctx, void* p, const void* z, tm_prec psl, cudaStream_t st);
-//   y += x ; x = 0                                                                           (GUARD_RU)
-tm_status blas_ru_begin(tm_ctx* ctx, void* y, tm_prec po, void* x, tm_prec pacc, cudaStream_t st, int y_mul = 1);
+//   r -= alpha w ; ||r||^2 -> RED_RR ; sloppy copy rs of r                            (GUARD_ITER)
+//   (the x += alpha p of the same iteration is deferred: CgScalars::x_pend)
+tm_status blas_update_xr(tm_ctx* ctx, void* r, tm_prec pacc, const void* w, void* rs, tm_prec psl, cudaStream_t st);
+//   x += alpha p of the PREVIOUS iteration if pending ; p = z + beta p (p = z when beta == 0: first iteration)  (GUARD_ITER)
+tm_status blas_update_p(tm_ctx* ctx, void* p, const void* z, tm_prec psl, void* x, tm_prec pacc, cudaStream_t st);
+//   y += x (+ the pending alpha p) ; x = 0                                                    (GUARD_RU)
+tm_status blas_ru_begin(tm_ctx* ctx, void* y, tm_prec po, void* x, tm_prec pacc, const void* p, tm_prec psl, cudaStream_t st,
+                        int y_mul = 1);
 //   r = b - m (acc precision) ; rs = b - m (sloppy) ; ||b - m||^2 -> red_op (RED_START: m == NULL,
 //   GUARD_ALWAYS; RED_RU: GUARD_RU)
 tm_status blas_residual(tm_ctx* ctx, void* r, tm_prec pacc, void* rs, tm_prec psl, const void* b, const void* m,

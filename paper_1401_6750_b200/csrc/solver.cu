@@ -45,12 +45,12 @@ static tm_status apply_mhat(tm_ctx* ctx, void* out, const void* in, void* tmp, i
 // Both must be called with the same lane of the context active (tm_lane_use).
 static tm_status job_iteration(tm_ctx* ctx, const SolveJob& J) {
     TM_TRY(apply_mhat(ctx, J.z, J.rs, J.tmp, 1, J.kappa, J.mu, J.ps, J.rc, RED_ZZ, GUARD_ITER, J.st));
-    TM_TRY(blas_update_p(ctx, J.p, J.z, J.ps, J.st));
+    TM_TRY(blas_update_p(ctx, J.p, J.z, J.ps, J.x, J.pa, J.st));
     TM_TRY(apply_mhat(ctx, J.w, J.p, J.tmp, 0, J.kappa, J.mu, J.ps, J.rc, RED_WW, GUARD_ITER, J.st));
-    return blas_update_xr(ctx, J.x, J.r, J.pa, J.p, J.w, J.rs, J.ps, J.st);
+    return blas_update_xr(ctx, J.r, J.pa, J.w, J.rs, J.ps, J.st);
 }
 static tm_status job_update(tm_ctx* ctx, const SolveJob& J) {
-    TM_TRY(blas_ru_begin(ctx, J.y, J.po, J.x, J.pa, J.st, 2));
+    TM_TRY(blas_ru_begin(ctx, J.y, J.po, J.x, J.pa, J.p, J.ps, J.st, 2));
     TM_TRY(apply_mhat(ctx, J.mo, J.y, J.tmpo, 0, J.kappa, J.mu, J.po, J.rc, RED_NONE, GUARD_RU, J.st, 2));
     return blas_residual(ctx, J.r, J.pa, J.rs, J.ps, J.b, J.mo, J.po, RED_RU, GUARD_RU, J.st);
 }
