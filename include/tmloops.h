@@ -153,6 +153,28 @@ tm_status loop_contract_project_fields(tm_ctx* ctx, void* d_out, const void* d_s
                                        double kappa, double mu, const int* h_momenta, int nmom,
                                        tm_prec acc, void* stream);
 
+/* loop_contract_project_fields for callers that cannot allocate (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): same arguments, same result (the generic contraction kernels; fp32 results agree
+ * with the automatic path within the fp32 bound, fp64 within rounding of the DFT weights), but the call performs NO
+ * cudaMalloc / cudaFree / cudaMemcpy or other allocating routine.  Its scratch -- x/y partial sums, z-stage sums, DFT
+ * weight tables, momentum list -- lives in one file-scope device array of loop_contract_static_scratch_bytes() = 16 MiB
+ * that every GPU which loads the library holds until the process exits; the tables are written by a kernel from
+ * kernel arguments.  Limits and rules:
+ *   - the lattice / momentum set must fit: tables + Lz*T*NQ*320*sizeof(acc) + T*NQ*7*320*8 bytes <= 16 MiB, NQ = 29
+ *     (all px^2 + py^2 <= 9) or 49; e.g. 4^3x8 in fp64, 8^3x16 in fp32.  TM_EDIM with the sizes in the message otherwise;
+ *   - nmom <= 128 (TM_EARG otherwise);
+ *   - the packed gauge copy of precision acc is context state, not scratch, and must exist: one call of
+ *     loop_contract_project_fields with the same acc after tm_load_gauge creates it (TM_EARG otherwise);
+ *   - ALL calls on one device share the array (whatever the context): calls that overlap on the GPU, i.e. on different
+ *     streams without ordering, race.  Calls on one stream are safe.  The array keeps the last call's contents; nothing in
+ *     it needs clearing (a call writes every element before reading it);
+ *   - the first call on a device does the one-time set-up (cudaGetSymbolAddress of the array, upload of the 192-byte
+ *     Gamma table into constant memory): do one call before starting a graph capture. */
+tm_status loop_contract_project_fields_static(tm_ctx* ctx, void* d_out, const void* d_s_int, const void* d_eta_int,
+                                              double kappa, double mu, const int* h_momenta, int nmom,
+                                              tm_prec acc, void* stream);
+size_t loop_contract_static_scratch_bytes(void);
+
 /* PAPER.md:88 ("GPU kernels to contract a single time slice or a whole vector", for time-dilution): the same call
  * restricted to ONE timeslice t0 -- 1/T of the work.  d_out keeps the shape [2][80][nmom][T]: column t0 is
  * computed, every other column is set to zero. */

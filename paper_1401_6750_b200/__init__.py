@@ -33,7 +33,7 @@ EXPORTS = [
     "tm_create", "tm_destroy", "tm_last_error", "tm_load_gauge", "tm_field_bytes",
     "tm_field_import", "tm_field_export", "tm_dslash", "tm_dslash_multi", "tm_cg_solve", "loop_contract_project",
     "loop_contract_project_explicit", "loop_contract_project_sym", "loop_contract_project_timeslice",
-    "loop_contract_project_fields",
+    "loop_contract_project_fields", "loop_contract_project_fields_static", "loop_contract_static_scratch_bytes",
     "tsm_estimate", "tsm_estimate_host", "tsm_partial_sums_host", "tm_load_gauge_host",
     "loop_plain_project_timeslice", "tsm_estimate_time_diluted", "tm_launch_count", "tm_set_option", "tsm_partial_sums", "tsm_combine_sums",
     "tm_fma_peak",
@@ -107,6 +107,9 @@ def load_library():
                               ctypes.POINTER(tm_solve_info), vp]
     L.loop_contract_project.argtypes = [vp, vp, vp, vp, cd, cd, ctypes.POINTER(ci), ci, ci, vp]
     L.loop_contract_project_fields.argtypes = [vp, vp, vp, vp, cd, cd, ctypes.POINTER(ci), ci, ci, vp]
+    L.loop_contract_project_fields_static.argtypes = [vp, vp, vp, vp, cd, cd, ctypes.POINTER(ci), ci, ci, vp]
+    L.loop_contract_static_scratch_bytes.restype = ctypes.c_size_t
+    L.loop_contract_static_scratch_bytes.argtypes = []
     L.loop_contract_project_timeslice.argtypes = [vp, vp, vp, vp, cd, cd, ctypes.POINTER(ci), ci, ci, ci, vp]
     L.loop_contract_project_sym.argtypes = [vp, vp, vp, vp, cd, cd, ctypes.POINTER(ci), ci, ci, vp]
     L.loop_contract_project_explicit.argtypes = [vp, vp, vp, cd, cd, ctypes.POINTER(ci), ci, ci, vp]
@@ -319,6 +322,22 @@ class TmContext:
             self.h, out.data_ptr(), s_int.data_ptr(), eta_int.data_ptr(), float(kappa), float(mu),
             mom.ctypes.data_as(ctypes.POINTER(ctypes.c_int)), len(mom), int(acc), _stream()))
         return out
+
+    def loop_contract_project_fields_static(self, s_int, eta_int, kappa, mu, momenta, acc=TM_F32, out=None):
+        """loop_contract_project_fields without any allocation inside the call: scratch in the library's static device
+        array (loop_contract_static_scratch_bytes(); small lattices only; calls on one device must not overlap).  `out`
+        should be passed by callers that must not allocate (the default allocates it with torch)."""
+        torch = _torch()
+        mom = np.ascontiguousarray(momenta, dtype=np.int32).reshape(-1, 3)
+        if out is None:
+            out = torch.empty((2, 80, len(mom), self.T), dtype=torch.complex128, device=self.tdev)
+        self._check(self.lib.loop_contract_project_fields_static(
+            self.h, out.data_ptr(), s_int.data_ptr(), eta_int.data_ptr(), float(kappa), float(mu),
+            mom.ctypes.data_as(ctypes.POINTER(ctypes.c_int)), len(mom), int(acc), _stream()))
+        return out
+
+    def loop_contract_static_scratch_bytes(self):
+        return int(self.lib.loop_contract_static_scratch_bytes())
 
     def loop_contract_project_timeslice(self, s, eta, kappa, mu, momenta, t0, acc=TM_F64):
         """Single-timeslice contraction: column t0 of the [2,80,nmom,T] output, zeros elsewhere."""

@@ -701,3 +701,152 @@ extern "C" tm_status loop_contract_project_timeslice(tm_ctx* ctx, void* d_out, c
     TM_CUDA(ctx, cudaMemsetAsync(d_out, 0, (size_t)160 * nmom * ctx->X[3] * 16, st));
     return tm_contract_internal(ctx, d_out, si, ei, kappa, mu, h_momenta, nmom, acc, st, t0, 1);
 }
+
+// =====================================================================================================
+// loop_contract_project_fields_static: the contraction + projection for callers that cannot allocate
+// (code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc).
+//
+// Same kernels as loop_contract_project_fields on its generic path (contract_xy_kernel, contract_zsum_kernel,
+// contract_assemble_kernel); what differs is where their scratch lives: the x/y partial sums Q, the z-stage sums and the
+// small tables (DFT weights, momentum list, accumulator index) sit in ONE file-scope device array of
+// TM_STATIC_SCRATCH_BYTES instead of context workspaces, and the tables are written by a kernel from values passed as
+// kernel arguments (no cudaMalloc, cudaFree, cudaMemcpy or other allocating call on this path).  Every GPU that loads
+// the library holds the array until the process exits.  All calls, of all contexts, on one device share it: calls
+// that overlap on the GPU (different streams) race.  It keeps the last call's contents; nothing in it has to start at
+// zero (every element a call reads is written by that call first).
+#define TM_STATIC_SCRATCH_BYTES ((size_t)16 << 20)
+#define TM_STATIC_MAX_MOM 128
+static __device__ __align__(256) unsigned char g_static_scratch[TM_STATIC_SCRATCH_BYTES];
+
+struct StaticTablesArgs {
+    int mom[3 * TM_STATIC_MAX_MOM];
+    short qidx[64];
+    int nmom, L[3];
+    unsigned off_wx32, off_wy32, off_wx64, off_wy64, off_wz, off_mom, off_qidx;
+};
+
+// the tables of tm_contract_internal, built on the device: w[x][8] = 1, c1, s1, c2, s2, c3, s3, 0 with
+// c_m + i s_m = exp(2 pi i m x / L) (exact argument reduction, as fill_weights does on the host)
+__global__ void static_tables_kernel(unsigned char* tb, StaticTablesArgs A) {
+    for (int i = threadIdx.x; i < (A.L[0] + A.L[1] + A.L[2]) * 8; i += blockDim.x) {
+        int d = 0, j = i;
+        if (j >= A.L[0] * 8) { j -= A.L[0] * 8; d = 1; }
+        if (d == 1 && j >= A.L[1] * 8) { j -= A.L[1] * 8; d = 2; }
+        const int x = j >> 3, k = j & 7, L = A.L[d];
+        double w = k == 0 ? 1.0 : 0.0;
+        if (k >= 1 && k <= 6) {
+            const int m = (k + 1) >> 1;
+            const double th = 2.0 * (double)((m * x) % L) / (double)L;
+            w = (k & 1) ? cospi(th) : sinpi(th);
+        }
+        if (d == 0) { ((float*)(tb + A.off_wx32))[j] = (float)w; ((double*)(tb + A.off_wx64))[j] = w; }
+        else if (d == 1) { ((float*)(tb + A.off_wy32))[j] = (float)w; ((double*)(tb + A.off_wy64))[j] = w; }
+        else ((double*)(tb + A.off_wz))[j] = w;
+    }
+    for (int i = threadIdx.x; i < 3 * A.nmom; i += blockDim.x) ((int*)(tb + A.off_mom))[i] = A.mom[i];
+    for (int i = threadIdx.x; i < 64; i += blockDim.x) ((short*)(tb + A.off_qidx))[i] = A.qidx[i];
+}
+
+// Device address of g_static_scratch, looked up once per device (in host code the array's name is only a host-side
+// stand-in for the symbol, not a device address) together with the one-time upload of the Gamma table.
+static unsigned char* g_static_ptr[64];
+static tm_status static_setup(tm_ctx* ctx, unsigned char** out) {
+    const int dev = ctx->device;
+    if (dev < 0 || dev >= 64) return tm_fail(ctx, TM_EARG, "loop_contract_project_fields_static: device ordinal above 63");
+    if (!g_static_ptr[dev]) {                                  // ctx->device is current (the caller set it)
+        void* p = nullptr;
+        cudaError_t e = cudaGetSymbolAddress(&p, g_static_scratch);
+        if (e != cudaSuccess || !p) return tm_cuda_fail(ctx, e, "cudaGetSymbolAddress(g_static_scratch)");
+        GammaTable G;
+        build_gamma_table(&G);
+        TM_CUDA(ctx, cudaMemcpyToSymbol(c_gamma, &G, sizeof(G)));   // the same values the allocating path uploads
+        g_static_ptr[dev] = (unsigned char*)p;
+    }
+    *out = g_static_ptr[dev];
+    return TM_OK;
+}
+
+extern "C" size_t loop_contract_static_scratch_bytes(void) { return TM_STATIC_SCRATCH_BYTES; }
+
+extern "C" tm_status loop_contract_project_fields_static(tm_ctx* ctx, void* d_out, const void* d_s_int,
+                                                         const void* d_eta_int, double kappa, double mu,
+                                                         const int* h_momenta, int nmom, tm_prec acc, void* stream) {
+    if (!ctx || !d_out || !d_s_int || !d_eta_int || !h_momenta)
+        return tm_fail(ctx, TM_EARG, "loop_contract_project_fields_static: null argument");
+    if (acc != TM_F64 && acc != TM_F32) return tm_fail(ctx, TM_EPREC, "loop_contract_project_fields_static: acc must be f32 or f64");
+    if (nmom < 1 || nmom > TM_STATIC_MAX_MOM)
+        return tm_fail(ctx, TM_EARG, "loop_contract_project_fields_static: 1 <= nmom <= 128 (the momentum list travels as a kernel argument)");
+    cudaStream_t st = (cudaStream_t)stream;
+    TM_CUDA(ctx, cudaSetDevice(ctx->device));
+    int prune = 1;
+    for (int k = 0; k < nmom; k++) {
+        const int px = h_momenta[3 * k], py = h_momenta[3 * k + 1], pz = h_momenta[3 * k + 2];
+        if (abs(px) > 3 || abs(py) > 3 || abs(pz) > 3)
+            return tm_fail(ctx, TM_EARG, "contract: momentum components must lie in [-3, 3]");
+        if (px * px + py * py > 9) prune = 0;
+    }
+    // layout of the static array: tables | Q[T*Lz][NQ][320] (acc precision) | Z[T][NQ][7][320] (double)
+    const ContractTables L = table_layout(ctx, nmom);
+    const int nq = prune ? 29 : 49;
+    const size_t fsz = acc == TM_F64 ? 8 : 4;
+    const size_t qbytes = ((size_t)ctx->X[2] * ctx->X[3] * nq * CT_THREADS * fsz + 255) & ~(size_t)255;
+    const size_t zbytes = (size_t)ctx->X[3] * nq * 7 * CT_THREADS * sizeof(double);
+    const size_t need = L.total + qbytes + zbytes;
+    if (need > TM_STATIC_SCRATCH_BYTES) {
+        char msg[200];
+        snprintf(msg, sizeof(msg), "loop_contract_project_fields_static: this lattice / momentum set needs %zu bytes of scratch, "
+                 "the static array holds %zu (use loop_contract_project_fields)", need, (size_t)TM_STATIC_SCRATCH_BYTES);
+        return tm_fail(ctx, TM_EDIM, msg);
+    }
+    // the packed gauge copy is context state, not scratch: it must exist already (packing allocates)
+    const tm_recon rc = acc == TM_F64 ? TM_R18 : TM_R12;
+    const int r = rc == TM_R12 ? 1 : 0;
+    if (!ctx->gauge[acc][r] || !ctx->gauge_valid[acc][r])
+        return tm_fail(ctx, TM_EARG, "loop_contract_project_fields_static: no packed gauge copy of this precision yet; one call of "
+                                     "loop_contract_project_fields with the same acc after tm_load_gauge packs it");
+    if (ctx->gauge_ev[acc][r] && ctx->gauge_st[acc][r] != st) TM_CUDA(ctx, cudaStreamWaitEvent(st, ctx->gauge_ev[acc][r], 0));
+    unsigned char* tb = nullptr;
+    TM_TRY(static_setup(ctx, &tb));
+
+    StaticTablesArgs T;
+    memset(&T, 0, sizeof(T));
+    memcpy(T.mom, h_momenta, (size_t)nmom * 12);
+    int nq_chk;
+    tm_contract_qidx(T.qidx, prune, &nq_chk);
+    T.nmom = nmom; T.L[0] = ctx->X[0]; T.L[1] = ctx->X[1]; T.L[2] = ctx->X[2];
+    T.off_wx32 = (unsigned)L.off_wx32; T.off_wy32 = (unsigned)L.off_wy32; T.off_wx64 = (unsigned)L.off_wx64;
+    T.off_wy64 = (unsigned)L.off_wy64; T.off_wz = (unsigned)L.off_wz; T.off_mom = (unsigned)L.off_mom; T.off_qidx = (unsigned)L.off_qidx;
+    static_tables_kernel<<<1, 256, 0, st>>>(tb, T);
+    TM_LAUNCH_CHECK(ctx, "static_tables_kernel");
+
+    void* qbuf = tb + L.total;
+    ContractArgs A;
+    A.s = d_s_int; A.eta = d_eta_int; A.gauge = ctx->gauge[acc][r]; A.qbuf = qbuf;
+    A.wx = tb + (acc == TM_F64 ? L.off_wx64 : L.off_wx32);
+    A.wy = tb + (acc == TM_F64 ? L.off_wy64 : L.off_wy32);
+    A.g = tm_geom(ctx);
+    A.tb = (double)ctx->tb;
+    A.t_first = 0;
+    const int nt = ctx->X[3];
+    if (acc == TM_F64) TM_TRY((launch_xy<double, 18>(ctx, A, prune, nt, st)));
+    else TM_TRY((launch_xy<float, 12>(ctx, A, prune, nt, st)));
+
+    AssembleArgs B;
+    B.qbuf = qbuf; B.out = d_out;
+    B.zbuf = (double*)(tb + L.total + qbytes);
+    B.mom = (const int*)(tb + L.off_mom);
+    B.qidx = (const short*)(tb + L.off_qidx);
+    B.wz = (const double*)(tb + L.off_wz);
+    B.nmom = nmom; B.T = nt; B.Lz = ctx->X[2]; B.NQ = nq; B.t_first = 0;
+    B.twokmu = 2.0 * kappa * mu;
+    B.half0 = 0;
+    B.L[0] = ctx->X[0]; B.L[1] = ctx->X[1]; B.L[2] = ctx->X[2];
+    dim3 zgrid((unsigned)nq, (unsigned)nt);
+    if (acc == TM_F64) contract_zsum_kernel<double><<<zgrid, CT_THREADS, 0, st>>>(B);
+    else contract_zsum_kernel<float><<<zgrid, CT_THREADS, 0, st>>>(B);
+    TM_LAUNCH_CHECK(ctx, "contract_zsum_kernel");
+    dim3 grid((unsigned)nmom, (unsigned)nt);
+    contract_assemble_kernel<<<grid, CT_THREADS, 0, st>>>(B);
+    TM_LAUNCH_CHECK(ctx, "contract_assemble_kernel");
+    return TM_OK;
+}
