@@ -344,8 +344,19 @@ struct Geom {
     int Vh;
     int s1, s2, s3;        // half-index strides of y, z, t:  Xh, Xh*Ly, Xh*Ly*Lz
     int sh0, sh1, sh2;     // log2 of Xh, Ly, Lz when all three are powers of two, else sh0 = -1
+    unsigned dm[3];        // otherwise: division by the invariant integers Xh, Ly, Lz as multiply-high + add + shift
+    int dl[3];             //   q = (umulhi(dm, n) + n) >> dl,  dl = ceil(log2 d),  dm = floor(2^32 (2^dl - d) / d) + 1
 };
-// half index -> (xh, y, z, t): shifts and masks where the extents allow (three integer divisions otherwise)
+// n / d for 0 <= n < 2^31 (Granlund-Montgomery: exact for every 32-bit n in its round-up form; t <= n keeps t + n in 32 bits)
+__host__ __device__ __forceinline__ int fast_div(int n, unsigned m, int l) {
+#ifdef __CUDA_ARCH__
+    return (int)((__umulhi(m, (unsigned)n) + (unsigned)n) >> l);
+#else
+    return (int)(((unsigned)(((unsigned long long)m * (unsigned)n) >> 32) + (unsigned)n) >> l);
+#endif
+}
+// half index -> (xh, y, z, t): shifts and masks where the extents are powers of two, else three divisions by invariant
+// integers (a run-time integer division is ~25 instructions: three of them were 5 % of a Dslash kernel)
 __host__ __device__ __forceinline__ void site_coords(const Geom& g, int h, int& xh, int& y, int& z, int& t) {
     if (g.sh0 >= 0) {
         xh = h & (g.Xh - 1);
@@ -354,11 +365,12 @@ __host__ __device__ __forceinline__ void site_coords(const Geom& g, int h, int& 
         z = q & (g.X2 - 1);
         t = q >> g.sh2;
     } else {
-        xh = h % g.Xh;
-        int q = h / g.Xh;
-        y = q % g.X1; q /= g.X1;
-        z = q % g.X2;
-        t = q / g.X2;
+        int q = fast_div(h, g.dm[0], g.dl[0]);
+        xh = h - q * g.Xh;
+        int q1 = fast_div(q, g.dm[1], g.dl[1]);
+        y = q - q1 * g.X1;
+        t = fast_div(q1, g.dm[2], g.dl[2]);
+        z = q1 - t * g.X2;
     }
 }
 static inline Geom tm_geom(const tm_ctx* c) {
@@ -369,5 +381,12 @@ static inline Geom tm_geom(const tm_ctx* c) {
     auto lg = [](int v) { int l = 0; while ((1 << l) < v) l++; return (1 << l) == v ? l : -1; };
     g.sh0 = lg(g.Xh); g.sh1 = lg(g.X1); g.sh2 = lg(g.X2);
     if (g.sh0 < 0 || g.sh1 < 0 || g.sh2 < 0) g.sh0 = g.sh1 = g.sh2 = -1;
+    const int dv[3] = {g.Xh, g.X1, g.X2};
+    for (int i = 0; i < 3; i++) {
+        int l = 0;
+        while ((1u << l) < (unsigned)dv[i]) l++;
+        g.dl[i] = l;
+        g.dm[i] = (unsigned)((((unsigned long long)1 << 32) * (((unsigned long long)1 << l) - (unsigned)dv[i])) / (unsigned)dv[i]) + 1u;
+    }
     return g;
 }
