@@ -221,9 +221,15 @@ __global__ void __launch_bounds__(CT_THREADS) contract_zsum_kernel(AssembleArgs 
     double acc[7];
 #pragma unroll
     for (int k = 0; k < 7; k++) acc[k] = 0.0;
+    // the 6 weights of a z value from shared memory: as global loads they were 6 of the 7 loads of an iteration and kept
+    // the data loads from overlapping
+    extern __shared__ double swz[];                         // [Lz][8]
+    for (int i = threadIdx.x; i < A.Lz * 8; i += CT_THREADS) swz[i] = A.wz[i];
+    __syncthreads();
+#pragma unroll 4
     for (int z = 0; z < A.Lz; z++) {
         const double v = (double)qb[(size_t)z * A.NQ * CT_THREADS];
-        const double* w = A.wz + z * 8;
+        const double* w = swz + z * 8;
         acc[0] += v;
 #pragma unroll
         for (int k = 1; k < 7; k++) acc[k] += w[k] * v;
@@ -522,8 +528,8 @@ tm_status tm_contract_internal(tm_ctx* ctx, void* d_out, const void* d_s, const 
     B.half0 = half0 ? 1 : 0;
     B.L[0] = ctx->X[0]; B.L[1] = ctx->X[1]; B.L[2] = ctx->X[2];
     dim3 zgrid((unsigned)nq, (unsigned)nt);
-    if (acc == TM_F64) contract_zsum_kernel<double><<<zgrid, CT_THREADS, 0, st>>>(B);
-    else contract_zsum_kernel<float><<<zgrid, CT_THREADS, 0, st>>>(B);
+    if (acc == TM_F64) contract_zsum_kernel<double><<<zgrid, CT_THREADS, (size_t)B.Lz * 64, st>>>(B);
+    else contract_zsum_kernel<float><<<zgrid, CT_THREADS, (size_t)B.Lz * 64, st>>>(B);
     TM_LAUNCH_CHECK(ctx, "contract_zsum_kernel");
     dim3 grid((unsigned)nmom, (unsigned)nt);
     contract_assemble_kernel<<<grid, CT_THREADS, 0, st>>>(B);
@@ -842,8 +848,8 @@ extern "C" tm_status loop_contract_project_fields_static(tm_ctx* ctx, void* d_ou
     B.half0 = 0;
     B.L[0] = ctx->X[0]; B.L[1] = ctx->X[1]; B.L[2] = ctx->X[2];
     dim3 zgrid((unsigned)nq, (unsigned)nt);
-    if (acc == TM_F64) contract_zsum_kernel<double><<<zgrid, CT_THREADS, 0, st>>>(B);
-    else contract_zsum_kernel<float><<<zgrid, CT_THREADS, 0, st>>>(B);
+    if (acc == TM_F64) contract_zsum_kernel<double><<<zgrid, CT_THREADS, (size_t)B.Lz * 64, st>>>(B);
+    else contract_zsum_kernel<float><<<zgrid, CT_THREADS, (size_t)B.Lz * 64, st>>>(B);
     TM_LAUNCH_CHECK(ctx, "contract_zsum_kernel");
     dim3 grid((unsigned)nmom, (unsigned)nt);
     contract_assemble_kernel<<<grid, CT_THREADS, 0, st>>>(B);
