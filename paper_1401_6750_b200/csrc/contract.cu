@@ -211,7 +211,12 @@ struct AssembleArgs {
     int half0;                 // s-family derivative slots hold only the forward half F_mu (contract_mma.cu); every
                                // timeslice must have been summed
     int L[3];                  // Lx, Ly, Lz
+    // by-value copies (constant bank: no dependent global loads at the start of each of the nmom x T small CTAs of the
+    // assembly); mom_v is used when nmom <= AS_MOMV, else the kernel reads A.mom
+    short qidx_v[64];
+    int mom_v[3 * 128];
 };
+#define AS_MOMV 128
 
 // z-stage: every x/y partial sum is read exactly once and reduced against the 7 real z-weights
 template <typename F>
@@ -250,10 +255,11 @@ __global__ void __launch_bounds__(CT_THREADS) contract_assemble_kernel(AssembleA
     const int k = blockIdx.x, t = blockIdx.y + A.t_first;
     const int jr = threadIdx.x;
     if (jr < (int)(sizeof(GammaTable) / 4)) reinterpret_cast<int*>(&sg)[jr] = reinterpret_cast<const int*>(&c_gamma)[jr];
-    const int px = A.mom[3 * k], py = A.mom[3 * k + 1], pz = A.mom[3 * k + 2];
+    const int* momk = A.nmom <= AS_MOMV ? A.mom_v + 3 * k : A.mom + 3 * k;
+    const int px = momk[0], py = momk[1], pz = momk[2];
     const int m = abs(px), n = abs(py), l = abs(pz);
     const double sx = px < 0 ? -1.0 : 1.0, sy = py < 0 ? -1.0 : 1.0, sz = pz < 0 ? -1.0 : 1.0;
-    const short* qi = A.qidx + (m * 4 + n) * 4;
+    const short* qi = A.qidx_v + (m * 4 + n) * 4;
     // Z(tq) = sum over the timeslice of exp(+i p.x) times real component jr
     auto Zof = [&](int tq, double& re, double& im) {
         const double* zb = A.zbuf + (size_t)tq * A.NQ * 7 * CT_THREADS + jr;
@@ -285,7 +291,7 @@ __global__ void __launch_bounds__(CT_THREADS) contract_assemble_kernel(AssembleA
         const double scale = d ? 0.5 : 1.0;
         // half0: C~[a][b](p,t) = F~[a][b](p,t) - e^{i p_mu} conj(F~[b][a](-p,t')), and for real fields Z(-p) = conj(Z(p))
         double phr = 1.0, phi = 0.0;
-        if (A.half0 && d >= 1 && d <= 3) sincospi(2.0 * (double)A.mom[3 * k + d - 1] / (double)A.L[d - 1], &phi, &phr);
+        if (A.half0 && d >= 1 && d <= 3) sincospi(2.0 * (double)momk[d - 1] / (double)A.L[d - 1], &phi, &phr);
         const double* br_ = (d == 4) ? zre_tm - 4 * 32 : zre;
         const double* bi_ = (d == 4) ? zim_tm - 4 * 32 : zim;
         double l0r = 0, l0i = 0, l1r = 0, l1i = 0;
@@ -522,6 +528,9 @@ tm_status tm_contract_internal(tm_ctx* ctx, void* d_out, const void* d_s, const 
     TM_TRY(tm_ws(ctx, WS_CT_OUT, (size_t)ctx->X[3] * nq * 7 * CT_THREADS * sizeof(double), (void**)&B.zbuf));
     B.mom = (const int*)(tb + L.off_mom);
     B.qidx = (const short*)(tb + L.off_qidx);
+    memcpy(B.qidx_v, host.data() + L.off_qidx, sizeof(B.qidx_v));
+    memset(B.mom_v, 0, sizeof(B.mom_v));
+    if (nmom <= AS_MOMV) memcpy(B.mom_v, h_momenta, (size_t)nmom * 12);
     B.wz = (const double*)(tb + L.off_wz);
     B.nmom = nmom; B.T = ctx->X[3]; B.Lz = ctx->X[2]; B.NQ = nq; B.t_first = t_first;
     B.twokmu = 2.0 * kappa * mu;
@@ -842,6 +851,9 @@ extern "C" tm_status loop_contract_project_fields_static(tm_ctx* ctx, void* d_ou
     B.zbuf = (double*)(tb + L.total + qbytes);
     B.mom = (const int*)(tb + L.off_mom);
     B.qidx = (const short*)(tb + L.off_qidx);
+    memcpy(B.qidx_v, T.qidx, sizeof(B.qidx_v));
+    memset(B.mom_v, 0, sizeof(B.mom_v));
+    memcpy(B.mom_v, h_momenta, (size_t)nmom * 12);
     B.wz = (const double*)(tb + L.off_wz);
     B.nmom = nmom; B.T = nt; B.Lz = ctx->X[2]; B.NQ = nq; B.t_first = 0;
     B.twokmu = 2.0 * kappa * mu;
