@@ -58,7 +58,9 @@ def test_static_scratch_contraction_equals_existing_path(acc, dims, tb):
         for j in (0, 1):
             ctx.loop_contract_project_fields_static(ints[j][0], ints[j][1], k, mu, moms[j], P, out=outs[j])
         torch.cuda.synchronize()
-        assert torch.cuda.mem_get_info()[0] == free0
+        # (any workspace the call allocated would take at least one 2 MiB page; 1 MiB of slack keeps unrelated driver
+        # housekeeping from failing the test)
+        assert torch.cuda.mem_get_info()[0] >= free0 - (1 << 20)
         for j in (0, 1):
             got = to_np(outs[j])
             assert np.isfinite(got.view(np.float64)).all()
