@@ -447,8 +447,10 @@ static tm_status launch_xy(tm_ctx* ctx, const ContractArgs& A, int prune, int nt
 
 tm_status tm_contract_internal(tm_ctx* ctx, void* d_out, const void* d_s, const void* d_eta, double kappa,
                                double mu, const int* h_momenta, int nmom, tm_prec acc, cudaStream_t st,
-                               int t_first, int nt) {
+                               int t_first, int nt, int merge) {
     if (nt <= 0) { t_first = 0; nt = ctx->X[3]; }                 // default: every timeslice
+    if (merge && (nt != ctx->X[3] || !tm_contract_merge_ok(ctx, acc)))
+        return tm_fail(ctx, TM_EARG, "contract: merged sources need a whole-vector fp32 call on the TMA path");
     if (t_first < 0 || t_first + nt > ctx->X[3]) return tm_fail(ctx, TM_EARG, "contract: timeslice range outside the lattice");
     if (acc != TM_F64 && acc != TM_F32) return tm_fail(ctx, TM_EPREC, "contract: acc must be f32 or f64");
     if (!h_momenta || nmom < 1) return tm_fail(ctx, TM_EARG, "contract: need at least one momentum");
@@ -520,8 +522,9 @@ tm_status tm_contract_internal(tm_ctx* ctx, void* d_out, const void* d_s, const 
     const bool half0 = mma || (tma && whole && ctx->opt_contract != 4);
     if (acc == TM_F64) TM_TRY((launch_xy<double, 18>(ctx, A, prune, nt, st)));
     else if (mma) TM_TRY(tm_contract_xy_mma(ctx, qbuf, d_s, d_eta, gauge, A.wx, A.wy, prune, t_first, nt, st));
-    else if (tma) TM_TRY(tm_contract_xy_tma(ctx, qbuf, d_s, d_eta, gauge, A.wx, A.wy, prune, half0 ? 1 : 0, t_first, nt, st));
+    else if (tma) TM_TRY(tm_contract_xy_tma(ctx, qbuf, d_s, d_eta, gauge, A.wx, A.wy, prune, half0 ? 1 : 0, t_first, nt, st, merge & 1));
     else TM_TRY((launch_xy<float, 12>(ctx, A, prune, nt, st)));
+    if (merge & 2) return TM_OK;                // the group's last source runs the z-sum and the assembly
 
     AssembleArgs B;
     B.qbuf = qbuf; B.out = d_out;
@@ -544,6 +547,11 @@ tm_status tm_contract_internal(tm_ctx* ctx, void* d_out, const void* d_s, const 
     contract_assemble_kernel<<<grid, CT_THREADS, 0, st>>>(B);
     TM_LAUNCH_CHECK(ctx, "contract_assemble_kernel");
     return TM_OK;
+}
+
+// the path tm_contract_internal takes for a whole-vector call of precision acc is the TMA kernel (what merging needs)
+bool tm_contract_merge_ok(const tm_ctx* ctx, tm_prec acc) {
+    return acc == TM_F32 && ctx->opt_contract != 1 && ctx->opt_contract != 3 && tm_contract_tma_usable(ctx);
 }
 
 extern "C" tm_status loop_contract_project(tm_ctx* ctx, void* d_out, const void* d_s, const void* d_eta,

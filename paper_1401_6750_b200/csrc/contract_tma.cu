@@ -48,6 +48,7 @@ struct TmaContractArgs {
     Geom g;
     float tb;
     int t_first;           // first timeslice of the launch
+    int q_add;             // add this source's partial sums to what qbuf holds (merged LP groups, tsm.cu) instead of overwriting
     float wf[7][6];        // folded x-stage (LX > 0): c1, s1, c2, s2, c3, s3 at x = j + 1, j < LX / 4 - 1 (kernel
                            // parameters live in the constant bank: FFMA2 takes them as uniform-register operands)
 };
@@ -444,6 +445,10 @@ contract_xy_tma_kernel(const __grid_constant__ CUtensorMap tm_s, const __grid_co
                 }
         }
         T2* qb = reinterpret_cast<T2*>((float*)A.qbuf + (size_t)zt * NQ * CT_THREADS) + cc;
+        if (A.q_add) {
+#pragma unroll
+            for (int q = 0; q < NQ; q++) Q[q] = PP::add(Q[q], qb[(size_t)q * CT_NCC]);
+        }
 #pragma unroll
         for (int q = 0; q < NQ; q++) qb[(size_t)q * CT_NCC] = Q[q];
     }
@@ -460,7 +465,8 @@ bool tm_contract_tma_usable(const tm_ctx* ctx) {
 
 // s, eta: fp32 full-lattice internal fields; gauge: fp32 reconstruct-12 internal copy; wx, wy: float tables
 tm_status tm_contract_xy_tma(tm_ctx* ctx, void* qbuf, const void* d_s, const void* d_eta, const void* gauge,
-                             const void* wx, const void* wy, int prune, int half0, int t_first, int nt, cudaStream_t st) {
+                             const void* wx, const void* wy, int prune, int half0, int t_first, int nt, cudaStream_t st,
+                             int q_add) {
     const int Xh = ctx->Xh;
     const cuuint64_t Vh = ctx->Vh;
     CUtensorMap ms, me, mgf, mgb;
@@ -484,6 +490,7 @@ tm_status tm_contract_xy_tma(tm_ctx* ctx, void* qbuf, const void* d_s, const voi
     A.g = tm_geom(ctx);
     A.tb = (float)ctx->tb;
     A.t_first = t_first;
+    A.q_add = q_add;
     const TxPlan P = tx_plan(ctx->X[0], ctx->X[1], half0);
     const unsigned grid = (unsigned)(ctx->X[2] * nt);
     // folded x-stage for the extents the configurations use (any multiple of 4 would do); other extents take the

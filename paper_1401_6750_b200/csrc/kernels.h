@@ -87,12 +87,19 @@ tm_status tm_solve_internal(tm_ctx* ctx, void* d_s, const void* d_eta, double ka
 // s, eta: full-lattice internal fields of precision acc (TM_F32 | TM_F64); out: complex128 [2][80][nmom][T]
 tm_status tm_contract_internal(tm_ctx* ctx, void* d_out, const void* d_s, const void* d_eta,
                                double kappa, double mu, const int* h_momenta, int nmom, tm_prec acc,
-                               cudaStream_t st, int t_first = 0, int nt = 0 /* 0: all timeslices */);
+                               cudaStream_t st, int t_first = 0, int nt = 0 /* 0: all timeslices */,
+                               int merge = 0);
+// merge (whole-vector fp32 calls on the TMA path only: tm_contract_merge_ok): the z-sum and the assembly are linear in
+// the x/y partial sums Q, so sources whose loops are only ever ADDED (LP sources without an HP partner, no per-source
+// output) can share them: bit 0 = add this source's Q to what the workspace holds, bit 1 = stop after the x/y stage
+// (d_out untouched).  A group of n sources calls with merge = 2, 3, ..., 3, 1 and gets the SUM of the n loops in d_out.
+bool tm_contract_merge_ok(const tm_ctx* ctx, tm_prec acc);
 // contract_tma.cu: TMA-staged fast path of the site + x/y-DFT stage (fp32, Lx <= 32)
 bool tm_contract_tma_usable(const tm_ctx* ctx);
 // half0: the s-family derivative slots receive only the forward half F_mu (AssembleArgs::half0 restores the rest)
 tm_status tm_contract_xy_tma(tm_ctx* ctx, void* qbuf, const void* d_s, const void* d_eta, const void* gauge,
-                             const void* wx, const void* wy, int prune, int half0, int t_first, int nt, cudaStream_t st);
+                             const void* wx, const void* wy, int prune, int half0, int t_first, int nt, cudaStream_t st,
+                             int q_add = 0);
 // contract_mma.cu: the same with the x-stage DFT on the tensor cores (mma.sync tf32, split-fp32 operands)
 bool tm_contract_mma_usable(const tm_ctx* ctx);
 tm_status tm_contract_xy_mma(tm_ctx* ctx, void* qbuf, const void* d_s, const void* d_eta, const void* gauge,

@@ -198,6 +198,12 @@ static tm_status job_finish(TsmRun& R, TsmJob& J, int lane) {
     double* A = R.acc[lane];
     const size_t nr = R.nr;
     double *S_lp = A, *S_lpc = A + nr, *S_hp = A + 2 * nr, *tmp = A + 3 * nr;
+    // Merged LP groups: the z-sum, the assembly and the accumulation are linear in the x/y partial sums of the
+    // contraction, so the sources of a group whose loops are only ever added into S_LP (no HP partner, no per-source
+    // output, no binary files) add their partial sums in the contraction's workspace and share ONE z-sum + assembly +
+    // accumulation (fp32 sums of at most 8 sources: inside the fp32-accumulate contract of the LP contraction).
+    const bool merged = !J.pass && J.nb > 1 && J.r >= P->n_hp && !R.d_per_source && !R.d_files_lp && !R.lp_keep
+                        && J.ac == J.po && tm_contract_merge_ok(ctx, J.ac);
     for (int b = 0; b < J.nb; b++) {
         const int r = J.r + b;
         if (J.pass) { R.ms_hp += si[b].ms; R.it_hp += si[b].iters; R.worst_hp = fmax(R.worst_hp, si[b].true_resid); }
@@ -218,6 +224,15 @@ static tm_status job_finish(TsmRun& R, TsmJob& J, int lane) {
             void* ebase;
             TM_TRY(job_noise(R, r, 0, J.ac, st, &ebase));
             eta_c = ebase;
+        }
+        if (merged) {
+            const int last = b == J.nb - 1;
+            TM_TRY(tm_contract_internal(ctx, tmp, s_c, eta_c, P->kappa, P->mu, P->h_momenta, P->nmom, J.ac, st, 0, 0,
+                                        (b > 0 ? 1 : 0) | (last ? 0 : 2)));
+            if (!last) continue;
+            tsm_accumulate_kernel<<<R.agrid, 256, 0, st>>>(S_lp, nullptr, nullptr, tmp, nr);      // the group's sum
+            TM_LAUNCH_CHECK(ctx, "tsm_accumulate_kernel");
+            continue;
         }
         TM_TRY(tm_contract_internal(ctx, tmp, s_c, eta_c, P->kappa, P->mu, P->h_momenta, P->nmom, J.ac, st));
         const int do_hp = r < P->n_hp;

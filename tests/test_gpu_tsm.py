@@ -156,6 +156,30 @@ def test_tsm_one_lane_equals_two_lanes(setup):
         assert abs(parts - info1["ms_total"]) <= 1e-6 * info1["ms_total"] and info1["ms_contract"] > 0
 
 
+def test_tsm_merged_lp_groups(setup):
+    """LP sources without an HP partner and without per-source output share one z-sum + assembly + accumulation per
+    group (their x/y partial sums are added in the contraction's workspace: the later stages are linear).  The estimate
+    must agree with the unmerged path (per_source=True switches merging off) within the fp32-accumulate bound of the LP
+    contraction, per block, for ragged group sizes; with fp64 LP contractions nothing is merged and the two are equal
+    up to the order of the fp64 accumulation."""
+    t = tm()
+    dims, U, mom = setup
+    k, mu = C1["kappa"], C1["mu"]
+    with t.TmContext(dims, -1) as ctx:
+        ctx.tm_load_gauge(U)
+        for n_lp, n_hp in ((27, 3), (16, 0), (11, 8)):
+            out_m, _, info_m = ctx.tsm_estimate(n_lp, n_hp, k, mu, mom, LP, HP, t.TM_F32, t.TM_F64, seed=3)
+            out_u, _, info_u = ctx.tsm_estimate(n_lp, n_hp, k, mu, mom, LP, HP, t.TM_F32, t.TM_F64, seed=3, per_source=True)
+            got, ref = to_np(out_m), to_np(out_u)
+            for f in (0, 1):
+                for sl in (slice(0, 16), slice(16, 80)):
+                    assert rel_l2(got[f, sl], ref[f, sl]) <= 1e-5, (n_lp, n_hp, f, sl)
+            assert info_m["iters_lp"] == info_u["iters_lp"] and info_m["iters_hp"] == info_u["iters_hp"]
+        out_m, _, _ = ctx.tsm_estimate(16, 2, k, mu, mom, LP, HP, t.TM_F64, t.TM_F64, seed=3)
+        out_u, _, _ = ctx.tsm_estimate(16, 2, k, mu, mom, LP, HP, t.TM_F64, t.TM_F64, seed=3, per_source=True)
+        assert rel_l2(to_np(out_m), to_np(out_u)) <= 1e-13
+
+
 def test_tsm_run_solutions_checked_by_oracle(orc, setup):
     """SURVEY.md sec 8 c.3 steps (1), (2) done ON the run: tsm_estimate hands back its own solutions (d_solutions) and
     the oracle evaluates, for EVERY source of a group of 8 plus a ragged tail (and both passes), the true residual
