@@ -175,6 +175,12 @@ def test_tsm_merged_lp_groups(setup):
                 for sl in (slice(0, 16), slice(16, 80)):
                     assert rel_l2(got[f, sl], ref[f, sl]) <= 1e-5, (n_lp, n_hp, f, sl)
             assert info_m["iters_lp"] == info_u["iters_lp"] and info_m["iters_hp"] == info_u["iters_hp"]
+        # two jobs in flight: every lane merges in its own contraction workspace
+        out_1, _, _ = ctx.tsm_estimate(43, 5, k, mu, mom, LP, HP, t.TM_F32, t.TM_F64, seed=3)
+        ctx.tm_set_option(t.TM_OPT_LANES, 2)
+        out_2, _, info_2 = ctx.tsm_estimate(43, 5, k, mu, mom, LP, HP, t.TM_F32, t.TM_F64, seed=3)
+        ctx.tm_set_option(t.TM_OPT_LANES, 0)
+        assert info_2["lanes"] == 2 and rel_l2(to_np(out_2), to_np(out_1)) <= 1e-13
         out_m, _, _ = ctx.tsm_estimate(16, 2, k, mu, mom, LP, HP, t.TM_F64, t.TM_F64, seed=3)
         out_u, _, _ = ctx.tsm_estimate(16, 2, k, mu, mom, LP, HP, t.TM_F64, t.TM_F64, seed=3, per_source=True)
         assert rel_l2(to_np(out_m), to_np(out_u)) <= 1e-13
