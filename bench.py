@@ -41,7 +41,7 @@ sys.path.insert(0, ROOT)
 from paper_1401_6750_b200 import inputs  # noqa: E402
 
 LP = dict(sloppy="f16", outer="f32", recon=12, rho=1e-2, max_iter=2000, delta=0.01)
-HP = dict(sloppy="f32", outer="f64", recon=12, rho=1e-8, max_iter=5000, delta=0.01)
+HP = dict(sloppy="f32", outer="f64", recon=12, rho=1e-8, max_iter=5000, delta=1e-4)     # delta: see DESIGN.md sec 10
 GROUP = 8                       # sources per launch inside tsm_estimate (TM_OPT_GROUP automatic at c4)
 PREC_BYTES = {"f64": 8, "f32": 4, "f16": 2, "bf16": 2}
 
